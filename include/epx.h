@@ -1,0 +1,145 @@
+/*
+ * epx.h -- C-ABI boundary of the B200-native epoch-substitution-model hot path (arxiv 1309.3075).
+ *
+ * What the library computes (citations are PAPER.md lines; "A<n>" are the readings listed in DESIGN.md):
+ *   a1  branch -> ordered (epoch, duration) segments, parent end first        L78 (change-point process), L117 (weights)
+ *   a2  per-epoch eigensystem of a reversible Q (symmetrised Jacobi)          L58 (detailed balance), L80, L314-L316
+ *   a2' Pade [13/13] scaling-and-squaring for an asymmetric Q                 L48 (exp(tQ), Moler & Van Loan)
+ *   a3  segment transition matrices exp(Q_e * r_c * d)                        L58-L60 Eq.(3)
+ *   a4  ordered chain product P_b = prod_k exp(Q_k r_c t_k), parent end first L84-L109 Eq.(5)-(7) (A2)
+ *   a5  Felsenstein pruning of partial likelihoods, post-order                L64-L72 Eq.(4)
+ *   a6  root / category / site-pattern aggregation into log-likelihoods       L72
+ * Every step runs in hand-written sm_100a CUDA kernels; there is no CPU fallback.  fp64 throughout.
+ *
+ * Conventions
+ *   - Time is HEIGHT, measured backwards from the most recent tip (A1).  Epoch e in 0..M-1 covers heights
+ *     [tau[e-1], tau[e]) with tau[-1] = -inf and tau[M-1] = +inf; `tau` holds the M-1 finite boundaries, so
+ *     epoch 0 is the most recent one and the leftmost factor of P_b is the OLDEST epoch on the branch.
+ *   - Matrices are row-major K x K, P[i][j] = Pr(child-end state j | parent-end state i).
+ *   - Every call returns 0 (EPX_OK) or a negative error code; nothing throws, aborts or prints.
+ *     epx_last_error(ctx) is a ctx-owned NUL-terminated message, valid until the next call on that ctx.
+ *   - All `const T*` inputs below are HOST pointers and are copied during the call (caller keeps ownership).
+ *   - Device memory and the stream are OWNED BY THE CALLER and borrowed: the library allocates no device
+ *     memory.  `dev_workspace` must stay alive and untouched while the ctx is bound to it.
+ *   - A ctx is not thread-safe; distinct ctxs are independent.
+ *   - Nothing is cached between compute calls: every epx_update_matrices / epx_*log_likelihood call re-runs
+ *     all of its steps on the device.  Setters only re-upload the array they set.
+ */
+#ifndef EPX_H
+#define EPX_H
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct epx_ctx epx_ctx; /* opaque; created / destroyed by the library */
+
+enum {
+    EPX_OK = 0,
+    EPX_E_ARG = -1,       /* NULL / out-of-range argument */
+    EPX_E_STATE = -2,     /* a required setter or epx_bind has not been called, or wrong mode */
+    EPX_E_TREE = -3,      /* not a strictly bifurcating rooted tree with tips 0..N-1, or a child above its parent */
+    EPX_E_MODEL = -4,     /* Q rows do not sum to 0, negative off-diagonal, freqs not a distribution, reversible flag violated */
+    EPX_E_WORKSPACE = -5, /* workspace too small or misaligned (256 B) */
+    EPX_E_CUDA = -6,      /* a CUDA runtime call failed (message holds cudaGetErrorString) */
+    EPX_E_NUMERIC = -7    /* Jacobi did not converge / non-finite matrix / a site likelihood <= 0 */
+};
+
+/* Limits of this build: 2 <= K <= 64, 1 <= M <= 4096, 1 <= C <= 8, N_tips == 0 or >= 2, L >= 1 when N_tips > 0. */
+
+/* Create a context for K states, M epochs, C rate categories, N_tips tips (0 = branch-list mode: matrices only,
+ * no tree / likelihood; "matrix convolution" workload) and L site patterns on CUDA device `device`. */
+int epx_create(epx_ctx** out, int K, int M, int C, int N_tips, int L, int device);
+void epx_destroy(epx_ctx* ctx);
+
+/* Bytes of device workspace the ctx needs.  Tree mode: valid right after create.  Branch-list mode: after
+ * epx_set_branches (the size depends on n_br). */
+int epx_workspace_bytes(const epx_ctx* ctx, size_t* bytes);
+
+/* Borrow `bytes` of DEVICE memory (256-byte aligned) and a cudaStream_t (may be 0 = legacy default stream; CUDA
+ * graphs are only used with a non-default stream).  All kernels and copies of this ctx are ordered on that stream.
+ * Inputs set before or after bind are uploaded lazily by the next compute call. */
+int epx_bind(epx_ctx* ctx, void* dev_workspace, size_t bytes, void* cuda_stream);
+
+/* ---- model inputs (PAPER.md L46 Q, L58 pi, L72 categories, L78 epochs) ---- */
+/* tau: M-1 finite, strictly increasing boundary heights (NULL allowed iff M == 1). */
+int epx_set_epoch_boundaries(epx_ctx* ctx, const double* tau);
+/* Q: K*K row-major including the diagonal, used as given (not normalised, A7/A8); |sum_j Q_ij| <= 1e-9 max|Q_ii|,
+ * off-diagonals >= 0.  freqs: K, >= 0, sum 1.  reversible = 1 selects the Jacobi path and requires pi_i > 0 and
+ * |pi_i q_ij - pi_j q_ji| <= 1e-9 max|pi q|; 0 selects Pade.  All epochs of a ctx must use the same flag. */
+int epx_set_epoch_model(epx_ctx* ctx, int epoch, const double* Q, const double* freqs, int reversible);
+/* rates: C, >= 0 (the r_c of Eq. 3, A6).  weights: C, >= 0, sum 1. */
+int epx_set_category_rates(epx_ctx* ctx, const double* rates, const double* weights);
+
+/* ---- tree mode (N tips, 2N-1 nodes, bifurcating) ---- */
+/* parent: 2N-1 entries, tips are 0..N-1, the root has -1.  height: 2N-1, height[parent] >= height[child]. */
+int epx_set_tree(epx_ctx* ctx, const int32_t* parent, const double* height);
+/* states: [N][L] row-major; 0..K-1 = observed state, anything else = missing (all-ones tip vector, A10). */
+int epx_set_tip_states(epx_ctx* ctx, const int32_t* states);
+/* wt: L pattern weights (a weight w == the pattern repeated w times), or NULL = all 1. */
+int epx_set_pattern_weights(epx_ctx* ctx, const double* wt);
+/* freqs: K root distribution, or NULL = the freqs of the epoch that contains the root height (A9). */
+int epx_set_root_frequencies(epx_ctx* ctx, const double* freqs);
+
+/* ---- branch-list mode ---- */
+/* n_br branches given by their two end heights, parent_height[b] >= child_height[b]. */
+int epx_set_branches(epx_ctx* ctx, int n_br, const double* child_height, const double* parent_height);
+
+/* ---- compute ---- */
+/* a1..a4, enqueued on the stream, does not synchronise.  Matrix slot = node index (tree mode; the root's slot
+ * holds the identity) or branch index. */
+int epx_update_matrices(epx_ctx* ctx);
+/* a1..a6, enqueued on the stream, does not synchronise (tree mode only). */
+int epx_enqueue_log_likelihood(epx_ctx* ctx);
+/* a1..a6, then synchronises the stream and writes the total log-likelihood to *logL (host). EPX_E_NUMERIC if a
+ * device-side numeric check failed (*logL is still written). */
+int epx_log_likelihood(epx_ctx* ctx, double* logL);
+/* Synchronise and fetch the result of the last enqueue (same checks as epx_log_likelihood). */
+int epx_fetch_log_likelihood(epx_ctx* ctx, double* logL);
+
+/* ---- read-back (each synchronises the stream; results of the LAST compute call) ---- */
+/* Segment list of matrix slot `slot`: *n_seg entries, parent end first; epoch/dur hold at least M entries. */
+int epx_get_segments(epx_ctx* ctx, int slot, int* n_seg, int32_t* epoch, double* dur);
+/* One K*K matrix (host, row-major). */
+int epx_get_matrix(epx_ctx* ctx, int slot, int category, double* out);
+/* Borrowed DEVICE pointer to all matrices, [slot][C][K][K] row-major fp64, valid while bound. */
+int epx_matrices_device(epx_ctx* ctx, const double** dptr);
+/* Partials of `node` as [C][L][K] (host) and the per-pattern power-of-two exponents scale_exp[L]:
+ * true partial = out * 2^scale_exp (A12).  Tips return their 0/1 vectors and zero exponents. */
+int epx_get_partials(epx_ctx* ctx, int node, double* out, int32_t* scale_exp);
+/* Per-pattern log-likelihoods ln l_p (unweighted), L entries (host). */
+int epx_get_site_log_likelihoods(epx_ctx* ctx, double* out);
+
+/* ---- introspection ---- */
+/* Number of kernel launches (graph nodes count individually) the ctx has enqueued since create. */
+int epx_launch_count(const epx_ctx* ctx, long long* n);
+/* Device time in ms of each stage of the LAST compute call is not recorded by the library; time the stream. */
+const char* epx_last_error(const epx_ctx* ctx);
+
+/* Measured fp64 peak on `device`: kind 0 = DFMA (plain FP64 FMA pipe), kind 1 = DMMA (mma.sync m8n8k4 f64).
+ * Runs a register-only kernel for about `ms_target` ms on `cuda_stream` and writes TFLOP/s (2 flop per FMA) to
+ * *tflops (host).  `dev_scratch` is >= 8 bytes of caller-owned DEVICE memory (never written in practice; it keeps the
+ * compiler from deleting the arithmetic).  Synchronises the stream. */
+int epx_measure_fp64_peak(int device, int kind, double ms_target, void* dev_scratch, void* cuda_stream, double* tflops);
+
+/* ---- tuning / test hooks (no effect on results) ---- */
+enum {
+    EPX_OPT_CHAIN_KERNEL = 1, /* 0 auto (default); 1 force the generic shared-memory chain kernel */
+    EPX_OPT_USE_GRAPH = 2,    /* 1 (default) replay the kernel sequence from a CUDA graph on non-default streams; 0 launch directly */
+    EPX_OPT_PRUNE_KERNEL = 3  /* 0 auto (default); 1 force the generic shared-memory pruning kernel */
+};
+int epx_set_option(epx_ctx* ctx, int option, int value);
+/* Device status word of the last compute call (0 = all numeric checks passed); synchronises. */
+int epx_status(epx_ctx* ctx, int* status);
+/* Whole CSR segment list of the last compute call: seg_off[n_slots+1], epoch/dur with capacity `cap` entries. */
+int epx_get_all_segments(epx_ctx* ctx, int32_t* seg_off, int32_t* epoch, double* dur, int cap);
+/* Number of post-order levels of the tree (= pruning launches per likelihood call). */
+int epx_tree_levels(const epx_ctx* ctx, int* n_levels);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* EPX_H */

@@ -1,0 +1,401 @@
+// C-ABI boundary and host orchestration of libepx (include/epx.h).  The host side validates inputs, owns the plan
+// (post-order levels, buffer offsets inside the caller's workspace), uploads inputs, and enqueues the kernels of
+// segmenter.cu / eigen.cu / chain.cu / pade.cu / prune.cu on the caller's stream (replayed from a CUDA graph when the
+// stream is not the legacy default stream).  No arithmetic of the method runs on the host.
+#include "../../include/epx.h"
+#include "epx_internal.h"
+
+#include <algorithm>
+#include <cmath>
+#include <cstdarg>
+#include <cstdio>
+#include <cstring>
+
+namespace {
+
+int fail(epx_ctx* c, int code, const char* fmt, ...) __attribute__((format(printf, 3, 4)));
+int fail(epx_ctx* c, int code, const char* fmt, ...)
+{
+    if (c) {
+        char buf[512];
+        va_list ap;
+        va_start(ap, fmt);
+        vsnprintf(buf, sizeof buf, fmt, ap);
+        va_end(ap);
+        c->err = buf;
+    }
+    return code;
+}
+
+#define CUDA_TRY(c, call)                                                                         \
+    do {                                                                                          \
+        cudaError_t e_ = (call);                                                                  \
+        if (e_ != cudaSuccess) return fail((c), EPX_E_CUDA, "%s: %s", #call, cudaGetErrorString(e_)); \
+    } while (0)
+
+inline size_t align_up(size_t x) { return (x + 255) & ~(size_t)255; }
+
+// Carve the workspace.  With base == nullptr only the total size is computed.
+size_t plan_workspace(const epx_ctx* c, char* base, DevBuffers* d)
+{
+    size_t off = 0;
+    auto take = [&](size_t bytes) -> char* {
+        char* p = base ? base + off : nullptr;
+        off += align_up(bytes ? bytes : 1);
+        return p;
+    };
+    const size_t K = c->K, M = c->M, C = c->C, N = c->N, L = c->L, Kp = c->Kp, S = c->n_slots;
+    DevBuffers t{};
+    t.tau = (double*)take(8 * (M - 1));
+    t.Q = (double*)take(8 * M * K * K);
+    t.freqs = (double*)take(8 * M * K);
+    t.rates = (double*)take(8 * C);
+    t.weights = (double*)take(8 * C);
+    t.root_freqs = (double*)take(8 * K);
+    if (c->tree_mode) {
+        t.parent = (int32_t*)take(4 * S);
+        t.height = (double*)take(8 * S);
+        t.tips = (uint8_t*)take(N * L);
+        t.pattern_wt = (double*)take(8 * L);
+        t.ops = (PruneOp*)take(sizeof(PruneOp) * (N - 1));
+    } else {
+        t.child_h = (double*)take(8 * S);
+        t.parent_h = (double*)take(8 * S);
+    }
+    t.n_seg = (int32_t*)take(4 * S);
+    t.e_hi = (int32_t*)take(4 * S);
+    t.seg_off = (int32_t*)take(4 * (S + 1));
+    t.seg_epoch = (int32_t*)take(4 * S * M);
+    t.seg_dur = (double*)take(8 * S * M);
+    t.order = (int32_t*)take(4 * S);
+    t.lam = (double*)take(8 * M * Kp);
+    t.U = (double*)take(8 * M * Kp * Kp);
+    t.W = (double*)take(8 * M * Kp * Kp);
+    t.sp = (double*)take(8 * M * Kp);
+    t.isp = (double*)take(8 * M * Kp);
+    t.WB = (double*)take(Kp == 64 ? 8 * M * 4096 : 0);
+    t.UTB = (double*)take(Kp == 64 ? 8 * M * 4096 : 0);
+    t.Efull = (double*)take(8 * M * C * K * K);
+    t.P = (double*)take(8 * S * C * K * K);
+    if (c->tree_mode) {
+        t.partials = (double*)take(8 * (N - 1) * C * L * K);
+        t.scale_exp = (int32_t*)take(4 * (N - 1) * L);
+        t.site_lnl = (double*)take(8 * L);
+        t.block_sums = (double*)take(8 * ((L + 255) / 256));
+    }
+    t.lnl = (double*)take(8);
+    t.status = (int32_t*)take(4);
+    if (d) *d = t;
+    return off;
+}
+
+void drop_graphs(epx_ctx* c)
+{
+    if (c->graph_mat) { cudaGraphExecDestroy(c->graph_mat); c->graph_mat = nullptr; }
+    if (c->graph_lik) { cudaGraphExecDestroy(c->graph_lik); c->graph_lik = nullptr; }
+}
+
+// Post-order plan: level(tip) = 0, level(u) = 1 + max(level(children)); ops sorted by level.
+int build_plan(epx_ctx* c)
+{
+    const int n = c->n_nodes, N = c->N;
+    std::vector<int> left(n, -1), right(n, -1), level(n, 0);
+    int root = -1, roots = 0;
+    for (int i = 0; i < n; i++) {
+        int p = c->parent[i];
+        if (p < 0) { root = i; roots++; continue; }
+        if (p >= n || p < N || p == i) return fail(c, EPX_E_TREE, "node %d: parent %d is not an internal node", i, p);
+        if (c->height[p] < c->height[i]) return fail(c, EPX_E_TREE, "node %d is above its parent %d", i, p);
+        if (left[p] < 0) left[p] = i;
+        else if (right[p] < 0) right[p] = i;
+        else return fail(c, EPX_E_TREE, "node %d has more than two children", p);
+    }
+    if (roots != 1) return fail(c, EPX_E_TREE, "%d roots (need exactly one)", roots);
+    for (int i = 0; i < n; i++) {
+        if (!std::isfinite(c->height[i])) return fail(c, EPX_E_TREE, "height[%d] is not finite", i);
+        if (i < N ? (left[i] >= 0) : (right[i] < 0)) return fail(c, EPX_E_TREE, "node %d: not bifurcating / tip with children", i);
+    }
+    // iterative post-order from the root (also proves every node is reachable, i.e. no cycle)
+    std::vector<int> stack{root}, order;
+    order.reserve(n);
+    while (!stack.empty()) {
+        int u = stack.back(); stack.pop_back();
+        order.push_back(u);
+        if (left[u] >= 0) { stack.push_back(left[u]); stack.push_back(right[u]); }
+    }
+    if ((int)order.size() != n) return fail(c, EPX_E_TREE, "tree is not connected (cycle)");
+    int max_level = 0;
+    for (int k = n - 1; k >= 0; k--) {
+        int u = order[k];
+        if (left[u] >= 0) level[u] = 1 + std::max(level[left[u]], level[right[u]]);
+        max_level = std::max(max_level, level[u]);
+    }
+    std::vector<int> internal;
+    for (int i = 0; i < n; i++) if (left[i] >= 0) internal.push_back(i);
+    std::stable_sort(internal.begin(), internal.end(), [&](int a, int b) { return level[a] < level[b]; });
+    c->node_pidx.assign(n, -1);
+    for (size_t k = 0; k < internal.size(); k++) c->node_pidx[internal[k]] = (int)k;
+    c->ops.resize(internal.size());
+    c->level_off.assign(max_level + 1, 0);
+    for (size_t k = 0; k < internal.size(); k++) {
+        int u = internal[k];
+        PruneOp& op = c->ops[k];
+        op.node = u;
+        op.pidx = (int)k;
+        op.child[0] = left[u];
+        op.child[1] = right[u];
+        for (int h = 0; h < 2; h++) {
+            op.child_is_tip[h] = op.child[h] < N;
+            op.cpidx[h] = c->node_pidx[op.child[h]];
+        }
+        c->level_off[level[u]]++;      // count per level (levels 1..max_level)
+    }
+    // level_off[l] currently holds the count of level l (index 0 unused = 0): turn into offsets over levels 1..max
+    std::vector<int> offs(max_level + 1, 0);
+    for (int l = 1; l <= max_level; l++) offs[l] = offs[l - 1] + c->level_off[l];
+    c->level_off = offs;               // ops of level l (1-based) are [offs[l-1], offs[l])
+    c->root = root;
+    return EPX_OK;
+}
+
+}  // namespace
+
+extern "C" {
+
+int epx_create(epx_ctx** out, int K, int M, int C, int N_tips, int L, int device)
+{
+    if (!out) return EPX_E_ARG;
+    *out = nullptr;
+    if (K < 2 || K > EPX_MAX_K || M < 1 || M > EPX_MAX_M || C < 1 || C > EPX_MAX_C) return EPX_E_ARG;
+    if (N_tips != 0 && (N_tips < 2 || L < 1)) return EPX_E_ARG;
+    if (device < 0) return EPX_E_ARG;
+    epx_ctx* c = new (std::nothrow) epx_ctx();
+    if (!c) return EPX_E_ARG;
+    c->K = K; c->M = M; c->C = C; c->N = N_tips; c->L = N_tips ? L : 0; c->device = device;
+    c->Kp = K <= 4 ? K : (K <= 32 ? (K + 7) & ~7 : 64);
+    c->tree_mode = N_tips > 0;
+    c->n_nodes = c->tree_mode ? 2 * N_tips - 1 : 0;
+    c->n_slots = c->n_nodes;
+    c->Q.assign((size_t)M * K * K, 0.0);
+    c->freqs.assign((size_t)M * K, 0.0);
+    c->model_set.assign(M, 0);
+    if (c->tree_mode) {
+        c->pattern_wt.assign(L, 1.0);
+        c->wt_dirty = true;
+        c->reduce_blocks = (L + 255) / 256;
+    }
+    if (M == 1) { c->has_tau = true; }
+    *out = c;
+    return EPX_OK;
+}
+
+void epx_destroy(epx_ctx* c)
+{
+    if (!c) return;
+    drop_graphs(c);
+    delete c;
+}
+
+const char* epx_last_error(const epx_ctx* c) { return c ? c->err.c_str() : "null ctx"; }
+
+int epx_workspace_bytes(const epx_ctx* c, size_t* bytes)
+{
+    if (!c || !bytes) return EPX_E_ARG;
+    if (!c->tree_mode && !c->has_branches) return EPX_E_STATE;
+    *bytes = plan_workspace(c, nullptr, nullptr);
+    return EPX_OK;
+}
+
+int epx_bind(epx_ctx* c, void* ws, size_t bytes, void* stream)
+{
+    if (!c || !ws) return EPX_E_ARG;
+    if (!c->tree_mode && !c->has_branches) return fail(c, EPX_E_STATE, "branch-list mode: call epx_set_branches before epx_bind");
+    if ((uintptr_t)ws & 255) return fail(c, EPX_E_WORKSPACE, "workspace must be 256-byte aligned");
+    size_t need = plan_workspace(c, nullptr, nullptr);
+    if (bytes < need) return fail(c, EPX_E_WORKSPACE, "workspace has %zu bytes, %zu needed", bytes, need);
+    CUDA_TRY(c, cudaSetDevice(c->device));
+    cudaPointerAttributes attr{};
+    CUDA_TRY(c, cudaPointerGetAttributes(&attr, ws));
+    if (attr.type != cudaMemoryTypeDevice && attr.type != cudaMemoryTypeManaged)
+        return fail(c, EPX_E_WORKSPACE, "workspace is not device memory");
+    if (chain_init_attributes() || pade_init_attributes() || eigen_init_attributes() || prune_init_attributes())
+        return fail(c, EPX_E_CUDA, "cudaFuncSetAttribute: %s", cudaGetErrorString(cudaGetLastError()));
+    drop_graphs(c);
+    plan_workspace(c, (char*)ws, &c->d);
+    c->ws = ws; c->ws_bytes = bytes; c->stream = (cudaStream_t)stream; c->bound = true;
+    c->tau_dirty = c->model_dirty = c->rates_dirty = c->tree_dirty = c->branches_dirty = c->tips_dirty = c->wt_dirty =
+        c->rootf_dirty = true;
+    c->have_result = false;
+    return EPX_OK;
+}
+
+int epx_set_option(epx_ctx* c, int option, int value)
+{
+    if (!c) return EPX_E_ARG;
+    switch (option) {
+        case 1: c->chain_kernel = value; break;
+        case 2: c->use_graph = value; break;
+        case 3: c->prune_kernel = value; break;
+        default: return fail(c, EPX_E_ARG, "unknown option %d", option);
+    }
+    drop_graphs(c);
+    return EPX_OK;
+}
+
+int epx_set_epoch_boundaries(epx_ctx* c, const double* tau)
+{
+    if (!c) return EPX_E_ARG;
+    if (c->M == 1) { c->has_tau = true; return EPX_OK; }
+    if (!tau) return fail(c, EPX_E_ARG, "tau is NULL");
+    for (int k = 0; k < c->M - 1; k++) {
+        if (!std::isfinite(tau[k])) return fail(c, EPX_E_ARG, "tau[%d] is not finite", k);
+        if (k && !(tau[k] > tau[k - 1])) return fail(c, EPX_E_ARG, "tau must be strictly increasing (index %d)", k);
+    }
+    c->tau.assign(tau, tau + c->M - 1);
+    c->has_tau = true; c->tau_dirty = true;
+    return EPX_OK;
+}
+
+int epx_set_epoch_model(epx_ctx* c, int epoch, const double* Q, const double* freqs, int reversible)
+{
+    if (!c || !Q || !freqs) return EPX_E_ARG;
+    if (epoch < 0 || epoch >= c->M) return fail(c, EPX_E_ARG, "epoch %d out of range", epoch);
+    const int K = c->K;
+    double maxdiag = 0.0;
+    for (int i = 0; i < K; i++) maxdiag = std::max(maxdiag, std::fabs(Q[i * K + i]));
+    long double fs = 0;
+    for (int i = 0; i < K; i++) {
+        long double s = 0;
+        for (int j = 0; j < K; j++) {
+            double q = Q[i * K + j];
+            if (!std::isfinite(q)) return fail(c, EPX_E_MODEL, "Q[%d][%d] is not finite", i, j);
+            if (i != j && q < 0) return fail(c, EPX_E_MODEL, "Q[%d][%d] < 0", i, j);
+            s += q;
+        }
+        if (std::fabs((double)s) > 1e-9 * maxdiag) return fail(c, EPX_E_MODEL, "row %d of Q sums to %g", i, (double)s);
+        if (!(freqs[i] >= 0)) return fail(c, EPX_E_MODEL, "freqs[%d] < 0 or NaN", i);
+        fs += freqs[i];
+    }
+    if (std::fabs((double)(fs - 1)) > 1e-9) return fail(c, EPX_E_MODEL, "freqs sum to %.12g", (double)fs);
+    if (reversible) {
+        double maxflux = 0.0;
+        for (int i = 0; i < K; i++) {
+            if (!(freqs[i] > 0)) return fail(c, EPX_E_MODEL, "reversible model needs freqs[%d] > 0", i);
+            for (int j = 0; j < K; j++) if (i != j) maxflux = std::max(maxflux, freqs[i] * Q[i * K + j]);
+        }
+        for (int i = 0; i < K; i++)
+            for (int j = i + 1; j < K; j++)
+                if (std::fabs(freqs[i] * Q[i * K + j] - freqs[j] * Q[j * K + i]) > 1e-9 * maxflux)
+                    return fail(c, EPX_E_MODEL, "detailed balance violated at (%d,%d)", i, j);
+    }
+    int flag = reversible ? 1 : 0;
+    if (c->reversible >= 0 && c->reversible != flag) {
+        bool others = false;
+        for (int e = 0; e < c->M; e++) if (e != epoch && c->model_set[e]) others = true;
+        if (others) return fail(c, EPX_E_MODEL, "all epochs of a ctx must share the reversible flag");
+    }
+    if (c->reversible != flag) drop_graphs(c);
+    c->reversible = flag;
+    std::copy(Q, Q + K * K, c->Q.begin() + (size_t)epoch * K * K);
+    std::copy(freqs, freqs + K, c->freqs.begin() + (size_t)epoch * K);
+    c->model_set[epoch] = 1;
+    c->model_dirty = true;
+    return EPX_OK;
+}
+
+int epx_set_category_rates(epx_ctx* c, const double* rates, const double* weights)
+{
+    if (!c || !rates || !weights) return EPX_E_ARG;
+    long double ws = 0;
+    for (int k = 0; k < c->C; k++) {
+        if (!(rates[k] >= 0) || !std::isfinite(rates[k])) return fail(c, EPX_E_ARG, "rates[%d] must be finite and >= 0", k);
+        if (!(weights[k] >= 0)) return fail(c, EPX_E_ARG, "weights[%d] < 0 or NaN", k);
+        ws += weights[k];
+    }
+    if (std::fabs((double)(ws - 1)) > 1e-9) return fail(c, EPX_E_ARG, "category weights sum to %.12g", (double)ws);
+    c->rates.assign(rates, rates + c->C);
+    c->weights.assign(weights, weights + c->C);
+    c->has_rates = true; c->rates_dirty = true;
+    return EPX_OK;
+}
+
+int epx_set_tree(epx_ctx* c, const int32_t* parent, const double* height)
+{
+    if (!c || !parent || !height) return EPX_E_ARG;
+    if (!c->tree_mode) return fail(c, EPX_E_STATE, "ctx is in branch-list mode");
+    std::vector<int32_t> old_parent = c->parent;
+    c->parent.assign(parent, parent + c->n_nodes);
+    c->height.assign(height, height + c->n_nodes);
+    int rc = build_plan(c);
+    if (rc != EPX_OK) { c->has_tree = false; return rc; }
+    if (old_parent != c->parent) drop_graphs(c);      // launch shapes depend on the topology only
+    c->has_tree = true; c->tree_dirty = true;
+    return EPX_OK;
+}
+
+int epx_set_branches(epx_ctx* c, int n_br, const double* child_height, const double* parent_height)
+{
+    if (!c || !child_height || !parent_height || n_br < 1) return EPX_E_ARG;
+    if (c->tree_mode) return fail(c, EPX_E_STATE, "ctx is in tree mode");
+    if (c->bound && n_br != c->n_slots) return fail(c, EPX_E_STATE, "n_br cannot change after epx_bind");
+    for (int b = 0; b < n_br; b++) {
+        if (!std::isfinite(child_height[b]) || !std::isfinite(parent_height[b]) || parent_height[b] < child_height[b])
+            return fail(c, EPX_E_ARG, "branch %d: need finite parent_height >= child_height", b);
+    }
+    c->child_h.assign(child_height, child_height + n_br);
+    c->parent_h.assign(parent_height, parent_height + n_br);
+    c->n_slots = n_br;
+    c->has_branches = true; c->branches_dirty = true;
+    return EPX_OK;
+}
+
+int epx_set_tip_states(epx_ctx* c, const int32_t* states)
+{
+    if (!c || !states) return EPX_E_ARG;
+    if (!c->tree_mode) return fail(c, EPX_E_STATE, "ctx is in branch-list mode");
+    const size_t n = (size_t)c->N * c->L;
+    c->tips.resize(n);
+    const int K = c->K;
+    for (size_t i = 0; i < n; i++) {
+        int32_t s = states[i];
+        c->tips[i] = (s >= 0 && s < K) ? (uint8_t)s : (uint8_t)255;
+    }
+    c->has_tips = true; c->tips_dirty = true;
+    return EPX_OK;
+}
+
+int epx_set_pattern_weights(epx_ctx* c, const double* wt)
+{
+    if (!c) return EPX_E_ARG;
+    if (!c->tree_mode) return fail(c, EPX_E_STATE, "ctx is in branch-list mode");
+    if (wt) {
+        for (int p = 0; p < c->L; p++) if (!std::isfinite(wt[p])) return fail(c, EPX_E_ARG, "wt[%d] is not finite", p);
+        c->pattern_wt.assign(wt, wt + c->L);
+    } else {
+        c->pattern_wt.assign(c->L, 1.0);
+    }
+    c->wt_dirty = true;
+    return EPX_OK;
+}
+
+int epx_set_root_frequencies(epx_ctx* c, const double* freqs)
+{
+    if (!c) return EPX_E_ARG;
+    if (!c->tree_mode) return fail(c, EPX_E_STATE, "ctx is in branch-list mode");
+    bool had = c->has_root_freqs;
+    if (freqs) {
+        long double s = 0;
+        for (int i = 0; i < c->K; i++) { if (!(freqs[i] >= 0)) return fail(c, EPX_E_ARG, "root freqs[%d] < 0 or NaN", i); s += freqs[i]; }
+        if (std::fabs((double)(s - 1)) > 1e-9) return fail(c, EPX_E_ARG, "root freqs sum to %.12g", (double)s);
+        c->root_freqs.assign(freqs, freqs + c->K);
+        c->has_root_freqs = true; c->rootf_dirty = true;
+    } else {
+        c->has_root_freqs = false;
+    }
+    if (had != c->has_root_freqs) drop_graphs(c);
+    return EPX_OK;
+}
+
+}  // extern "C"
+
+#include "api_compute.inc"

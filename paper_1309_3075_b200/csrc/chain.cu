@@ -1,0 +1,344 @@
+// a3 + a4 fused, reversible path: segment exponentials and the ordered matrix-chain convolution
+// (Eq.(3); L84-L109 Eq.(5)-(7), parent end = leftmost factor; L314-L323 App. A).
+//
+// The paper runs two kernels with intermediate buffers in global memory (UpdateTransitionMatrices, then
+// ConvolveTransitionMatrices per boundary).  Here one kernel keeps the whole chain on chip and stays in the
+// eigenbasis across epoch boundaries.  With S_e = Pi_e^{1/2} Q_e Pi_e^{-1/2} = U_e L_e U_e^T and segments
+// s = 1..n (epochs e_1 > e_2 > ... > e_n, durations d_s, category rate r):
+//   P = Pi_{e_1}^{-1/2} [ U_{e_1} D_1 W_{e_1} D_2 W_{e_2} ... D_n U_{e_n}^T ] Pi_{e_n}^{1/2},
+//   D_s = exp(L_{e_s} r d_s),   W_e = U_e^T diag(sqrt(pi_e/pi_{e-1})) U_{e-1}   (prep_kernel)
+// i.e. n dense products per (branch, category) instead of the 3n-1 of exp-then-convolve.  Algebraically identical
+// to Eq. (7); the flop count reported by bench.py is the executed one.
+//
+// Three kernels:
+//   chain_rows_kernel<4>  K == 4: one thread per (slot, category, row) keeps its row of the chain in registers
+//   chain_generic_kernel  any K <= 64: one CTA per (slot, category), operands staged in shared memory, DFMA
+//   chain_dmma64_kernel   32 < K <= 64: one CTA per (slot, 4 categories); 256x64 accumulator in registers,
+//                         mma.sync m8n8k4 f64 (DMMA) tiles, B operands pre-swizzled in fragment order and staged by
+//                         TMA bulk copies (cp.async.bulk + mbarrier) into a double-buffered shared-memory ring
+#include "epx_internal.h"
+
+namespace {
+
+// ------------------------------------------------------------------------------------------------ K == 4
+template <int K>
+__global__ void __launch_bounds__(256) chain_rows_kernel(int n_slots, int C, const int32_t* __restrict__ n_seg,
+    const int32_t* __restrict__ seg_off, const int32_t* __restrict__ seg_epoch, const double* __restrict__ seg_dur,
+    const double* __restrict__ rates, const double* __restrict__ lam, const double* __restrict__ U,
+    const double* __restrict__ W, const double* __restrict__ sp, const double* __restrict__ isp,
+    double* __restrict__ P, int32_t* __restrict__ status)
+{
+    long long idx = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (idx >= (long long)n_slots * C * K) return;
+    const int i = (int)(idx % K);
+    const int c = (int)((idx / K) % C);
+    const int b = (int)(idx / ((long long)K * C));
+    double* out = P + (((size_t)b * C + c) * K + i) * K;
+    const int n = n_seg[b];
+    if (n == 0) {
+#pragma unroll
+        for (int j = 0; j < K; j++) out[j] = (i == j) ? 1.0 : 0.0;
+        return;
+    }
+    const int off = seg_off[b];
+    const double r = rates[c];
+    int e = seg_epoch[off];
+    const double scale_i = isp[e * K + i];
+    double x[K];
+    {
+        const double rd = r * seg_dur[off];
+#pragma unroll
+        for (int k = 0; k < K; k++) x[k] = U[(e * K + i) * K + k] * exp(lam[e * K + k] * rd);
+    }
+    for (int s = 1; s < n; s++) {
+        const double* Wm = W + (size_t)e * K * K;     // boundary between epoch e and e-1
+        e = seg_epoch[off + s];
+        const double rd = r * seg_dur[off + s];
+        double y[K];
+#pragma unroll
+        for (int j = 0; j < K; j++) {
+            double a = 0.0;
+#pragma unroll
+            for (int k = 0; k < K; k++) a = fma(x[k], Wm[k * K + j], a);
+            y[j] = a * exp(lam[e * K + j] * rd);
+        }
+#pragma unroll
+        for (int j = 0; j < K; j++) x[j] = y[j];
+    }
+    bool bad = false;
+#pragma unroll
+    for (int j = 0; j < K; j++) {
+        double a = 0.0;
+#pragma unroll
+        for (int k = 0; k < K; k++) a = fma(x[k], U[(e * K + j) * K + k], a);
+        double v = scale_i * a * sp[e * K + j];
+        bad |= !isfinite(v);
+        out[j] = fmax(v, 0.0);      // reading A18: rounding can leave -1e-17; P is a probability
+    }
+    if (bad) atomicOr(status, EPX_ST_NONFINITE_P);
+}
+
+// ------------------------------------------------------------------------------------------------ any K
+constexpr int GT = 256;
+
+__global__ void __launch_bounds__(GT) chain_generic_kernel(int K, int Kp, int C, const int32_t* __restrict__ order,
+    const int32_t* __restrict__ n_seg, const int32_t* __restrict__ seg_off, const int32_t* __restrict__ seg_epoch,
+    const double* __restrict__ seg_dur, const double* __restrict__ rates, const double* __restrict__ lam,
+    const double* __restrict__ U, const double* __restrict__ W, const double* __restrict__ sp,
+    const double* __restrict__ isp, double* __restrict__ P, int32_t* __restrict__ status)
+{
+    extern __shared__ double sm[];
+    const int ld = Kp + 1;
+    double* X = sm;                       // [Kp][ld]
+    double* Y = X + (size_t)Kp * ld;      // [Kp][ld]
+    double* B = Y + (size_t)Kp * ld;      // [Kp][Kp]  right-hand operand
+    double* D = B + (size_t)Kp * Kp;      // [Kp]
+    const int tid = threadIdx.x;
+    const int b = order[blockIdx.x / C], c = blockIdx.x % C;
+    double* out = P + ((size_t)b * C + c) * K * K;
+    const int n = n_seg[b];
+    if (n == 0) {
+        for (int idx = tid; idx < K * K; idx += GT) out[idx] = (idx / K == idx % K) ? 1.0 : 0.0;
+        return;
+    }
+    const int off = seg_off[b];
+    const double r = rates[c];
+    const int e_hi = seg_epoch[off];
+    int e = e_hi;
+    if (tid < Kp) D[tid] = exp(lam[e * Kp + tid] * r * seg_dur[off]);
+    __syncthreads();
+    for (int idx = tid; idx < Kp * Kp; idx += GT) {
+        int i = idx / Kp, k = idx % Kp;
+        X[i * ld + k] = U[(size_t)e * Kp * Kp + idx] * D[k];
+    }
+    for (int s = 1; s <= n; s++) {
+        const bool last = (s == n);
+        __syncthreads();
+        if (!last) {
+            const double* Wm = W + (size_t)e * Kp * Kp;
+            for (int idx = tid; idx < Kp * Kp; idx += GT) B[idx] = Wm[idx];
+            e = seg_epoch[off + s];
+            if (tid < Kp) D[tid] = exp(lam[e * Kp + tid] * r * seg_dur[off + s]);
+        } else {
+            const double* Ue = U + (size_t)e * Kp * Kp;   // B = U_e^T
+            for (int idx = tid; idx < Kp * Kp; idx += GT) { int j = idx / Kp, k = idx % Kp; B[k * Kp + j] = Ue[idx]; }
+            if (tid < Kp) D[tid] = sp[e * Kp + tid];
+        }
+        __syncthreads();
+        for (int idx = tid; idx < Kp * Kp; idx += GT) {
+            int i = idx / Kp, j = idx % Kp;
+            double a = 0.0;
+            for (int k = 0; k < Kp; k++) a = fma(X[i * ld + k], B[k * Kp + j], a);
+            Y[i * ld + j] = a * D[j];
+        }
+        double* t = X; X = Y; Y = t;
+    }
+    __syncthreads();
+    bool bad = false;
+    for (int idx = tid; idx < K * K; idx += GT) {
+        int i = idx / K, j = idx % K;
+        double v = isp[e_hi * Kp + i] * X[i * ld + j];
+        bad |= !isfinite(v);
+        out[idx] = fmax(v, 0.0);
+    }
+    if (bad) atomicOr(status, EPX_ST_NONFINITE_P);
+}
+
+// ------------------------------------------------------------------------------------------------ 32 < K <= 64, DMMA
+__device__ __forceinline__ void dmma884(double& d0, double& d1, double a, double b)
+{
+    asm volatile("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1}, {%2}, {%3}, {%0,%1};"
+                 : "+d"(d0), "+d"(d1) : "d"(a), "d"(b));
+}
+__device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
+__device__ __forceinline__ void mbar_init(uint64_t* bar, int count)
+{
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(bar)), "r"(count) : "memory");
+}
+__device__ __forceinline__ void mbar_expect_tx(uint64_t* bar, uint32_t bytes)
+{
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(bar)), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void mbar_wait(uint64_t* bar, uint32_t parity)
+{
+    asm volatile(
+        "{\n\t.reg .pred p;\n\t"
+        "WAIT_LOOP:\n\t"
+        "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n\t"
+        "@p bra DONE;\n\t"
+        "bra WAIT_LOOP;\n\t"
+        "DONE:\n\t}" ::"r"(smem_u32(bar)), "r"(parity) : "memory");
+}
+// TMA 1-D bulk copy global -> shared, completion signalled on an mbarrier (SASS: UBLKCP).
+__device__ __forceinline__ void bulk_g2s(void* dst, const void* src, uint32_t bytes, uint64_t* bar)
+{
+    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
+                 ::"r"(smem_u32(dst)), "l"(src), "r"(bytes), "r"(smem_u32(bar)) : "memory");
+}
+
+constexpr int DT = 256;                 // 8 warps: warp w -> category (w>>1), rows 32*(w&1) .. +32
+constexpr int FRAG_DOUBLES = 4096;      // one 64x64 operand in fragment order
+struct DmmaSmem {
+    double B[2][FRAG_DOUBLES];          // TMA destination ring (2 x 32 KB)
+    double D[2][4][64];                 // exp(lambda r d) per stage / category
+    uint64_t bar[2];
+};
+
+__global__ void __launch_bounds__(DT, 1) chain_dmma64_kernel(int K, int C, const int32_t* __restrict__ order,
+    const int32_t* __restrict__ n_seg, const int32_t* __restrict__ seg_off, const int32_t* __restrict__ seg_epoch,
+    const double* __restrict__ seg_dur, const double* __restrict__ rates, const double* __restrict__ lam,
+    const double* __restrict__ WB, const double* __restrict__ UTB, const double* __restrict__ sp,
+    const double* __restrict__ isp, double* __restrict__ P, int32_t* __restrict__ status)
+{
+    extern __shared__ __align__(128) unsigned char smraw[];
+    DmmaSmem& sm = *reinterpret_cast<DmmaSmem*>(smraw);
+    const int tid = threadIdx.x, lane = tid & 31, w = tid >> 5;
+    const int g = lane >> 2, q = lane & 3;
+    const int ncg = (C + 3) >> 2;
+    const int b = order[blockIdx.x / ncg], cg = blockIdx.x % ncg;
+    const int c = cg * 4 + (w >> 1), half = w & 1;
+    const bool active = c < C;
+    const int n = n_seg[b];
+    if (n == 0) {
+        for (int cc = cg * 4; cc < min(C, cg * 4 + 4); cc++) {
+            double* out = P + ((size_t)b * C + cc) * K * K;
+            for (int idx = tid; idx < K * K; idx += DT) out[idx] = (idx / K == idx % K) ? 1.0 : 0.0;
+        }
+        return;
+    }
+    const int off = seg_off[b];
+    const int e_hi = seg_epoch[off], e_lo = seg_epoch[off + n - 1];
+
+    // stage t (0..n-1): B operand = WB[epoch_t] for t < n-1 (boundary epoch_t -> epoch_t - 1), U^T of e_lo for the last
+    auto stage_src = [&](int t) -> const double* {
+        return (t < n - 1) ? WB + (size_t)seg_epoch[off + t] * FRAG_DOUBLES : UTB + (size_t)e_lo * FRAG_DOUBLES;
+    };
+    auto fill_D = [&](int t) {     // one value per thread: category tid>>6, eigen index tid&63
+        int cc = cg * 4 + (tid >> 6), k = tid & 63;
+        double r = cc < C ? rates[cc] : 0.0;
+        sm.D[t & 1][tid >> 6][k] = exp(lam[seg_epoch[off + t] * 64 + k] * (r * seg_dur[off + t]));
+    };
+    if (tid == 0) {
+        mbar_init(&sm.bar[0], 1);
+        mbar_init(&sm.bar[1], 1);
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    }
+    __syncthreads();
+    if (tid == 0) {
+        mbar_expect_tx(&sm.bar[0], FRAG_DOUBLES * 8);
+        bulk_g2s(sm.B[0], stage_src(0), FRAG_DOUBLES * 8, &sm.bar[0]);
+    }
+    fill_D(0);
+
+    // accumulator = the warp's 32x64 slab of the running product, as 4 (m) x 8 (n) C-fragments.
+    // Start: rows of U_{e_hi}; U^T in B-fragment order doubles as U in A-fragment order (same index map).
+    double acc[4][8][2];
+    {
+        const double2* src = reinterpret_cast<const double2*>(UTB + (size_t)e_hi * FRAG_DOUBLES);
+#pragma unroll
+        for (int mt = 0; mt < 4; mt++)
+#pragma unroll
+            for (int kt = 0; kt < 8; kt++) {
+                double2 v = __ldg(&src[(kt * 8 + (4 * half + mt)) * 32 + lane]);
+                acc[mt][kt][0] = v.x;
+                acc[mt][kt][1] = v.y;
+            }
+    }
+    __syncthreads();
+
+    for (int t = 0; t < n; t++) {
+        const int st = t & 1;
+        if (t + 1 < n) {               // prefetch the next stage into the other buffer (freed at the end of t-1)
+            if (tid == 0) {
+                mbar_expect_tx(&sm.bar[st ^ 1], FRAG_DOUBLES * 8);
+                bulk_g2s(sm.B[st ^ 1], stage_src(t + 1), FRAG_DOUBLES * 8, &sm.bar[st ^ 1]);
+            }
+            fill_D(t + 1);
+        }
+        mbar_wait(&sm.bar[st], (t >> 1) & 1);
+        if (active) {
+            const double2* Bs = reinterpret_cast<const double2*>(sm.B[st]);
+            const double2* Ds = reinterpret_cast<const double2*>(sm.D[st][w >> 1]);
+#pragma unroll
+            for (int mp = 0; mp < 2; mp++) {
+                double a[2][8][2];
+#pragma unroll
+                for (int kt = 0; kt < 8; kt++) {
+                    double2 dv = Ds[kt * 4 + q];       // D[8kt + 2q], D[8kt + 2q + 1]
+#pragma unroll
+                    for (int mi = 0; mi < 2; mi++) {
+                        a[mi][kt][0] = acc[2 * mp + mi][kt][0] * dv.x;
+                        a[mi][kt][1] = acc[2 * mp + mi][kt][1] * dv.y;
+                        acc[2 * mp + mi][kt][0] = 0.0;
+                        acc[2 * mp + mi][kt][1] = 0.0;
+                    }
+                }
+#pragma unroll
+                for (int kt = 0; kt < 8; kt++)
+#pragma unroll
+                    for (int nt = 0; nt < 8; nt++) {
+                        double2 bv = Bs[(kt * 8 + nt) * 32 + lane];
+#pragma unroll
+                        for (int mi = 0; mi < 2; mi++) {
+                            dmma884(acc[2 * mp + mi][nt][0], acc[2 * mp + mi][nt][1], a[mi][kt][0], bv.x);
+                            dmma884(acc[2 * mp + mi][nt][0], acc[2 * mp + mi][nt][1], a[mi][kt][1], bv.y);
+                        }
+                    }
+            }
+        }
+        __syncthreads();
+    }
+
+    if (!active) return;
+    double* out = P + ((size_t)b * C + c) * K * K;
+    bool bad = false;
+#pragma unroll
+    for (int mt = 0; mt < 4; mt++) {
+        const int i = 32 * half + 8 * mt + g;
+        if (i >= K) continue;
+        const double si = isp[e_hi * 64 + i];
+#pragma unroll
+        for (int nt = 0; nt < 8; nt++)
+#pragma unroll
+            for (int h = 0; h < 2; h++) {
+                const int j = 8 * nt + 2 * q + h;
+                if (j < K) {
+                    double v = si * acc[mt][nt][h] * sp[e_lo * 64 + j];
+                    bad |= !isfinite(v);
+                    out[(size_t)i * K + j] = fmax(v, 0.0);
+                }
+            }
+    }
+    if (bad) atomicOr(status, EPX_ST_NONFINITE_P);
+}
+
+}  // namespace
+
+int chain_init_attributes()
+{
+    if (cudaFuncSetAttribute(chain_generic_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, 112 * 1024) != cudaSuccess) return -1;
+    if (cudaFuncSetAttribute(chain_dmma64_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(DmmaSmem)) != cudaSuccess) return -1;
+    return 0;
+}
+
+int launch_chain_reversible(const epx_ctx* c, cudaStream_t s)
+{
+    const DevBuffers& d = c->d;
+    const int K = c->K, Kp = c->Kp, C = c->C, n = c->n_slots;
+    if (K == 4) {
+        long long threads = (long long)n * C * 4;
+        int blocks = (int)((threads + 255) / 256);
+        chain_rows_kernel<4><<<blocks, 256, 0, s>>>(n, C, d.n_seg, d.seg_off, d.seg_epoch, d.seg_dur, d.rates, d.lam,
+                                                    d.U, d.W, d.sp, d.isp, d.P, d.status);
+    } else if (Kp == 64 && c->chain_kernel != 1) {
+        int ncg = (C + 3) / 4;
+        chain_dmma64_kernel<<<n * ncg, DT, sizeof(DmmaSmem), s>>>(K, C, d.order, d.n_seg, d.seg_off, d.seg_epoch,
+                                                                 d.seg_dur, d.rates, d.lam, d.WB, d.UTB, d.sp, d.isp,
+                                                                 d.P, d.status);
+    } else {
+        size_t smem = sizeof(double) * (2 * (size_t)Kp * (Kp + 1) + (size_t)Kp * Kp + Kp);
+        chain_generic_kernel<<<n * C, GT, smem, s>>>(K, Kp, C, d.order, d.n_seg, d.seg_off, d.seg_epoch, d.seg_dur,
+                                                     d.rates, d.lam, d.U, d.W, d.sp, d.isp, d.P, d.status);
+    }
+    return cudaGetLastError() == cudaSuccess ? 1 : -1;
+}

@@ -1,0 +1,133 @@
+// Internal declarations shared by the CUDA translation units of libepx (not part of the C ABI).
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+#include <string>
+#include <vector>
+
+#define EPX_MAX_K 64
+#define EPX_MAX_C 8
+#define EPX_MAX_M 4096
+#define EPX_SORT_BINS 64 /* counting-sort bins for n_seg (n_seg >= 63 share the top bin) */
+
+// Device-side status word bits (written by kernels, read back by the *log_likelihood calls).
+enum : int {
+    EPX_ST_JACOBI_NOCONV = 1,
+    EPX_ST_NONFINITE_P = 2,
+    EPX_ST_BAD_SITE = 4,
+    EPX_ST_PADE_SINGULAR = 8,
+};
+
+// One pruning operation: an internal node and its two children (children sorted by label).
+struct PruneOp {
+    int node;
+    int child[2];
+    int child_is_tip[2];
+    int pidx;        // index of `node` in the internal-partials array
+    int cpidx[2];    // same for internal children (unused for tips)
+};
+
+// All device pointers, carved out of the caller's workspace by plan_workspace().
+struct DevBuffers {
+    // inputs
+    double* tau;          // [M-1]
+    double* Q;            // [M][K][K]
+    double* freqs;        // [M][K]
+    double* rates;        // [C]
+    double* weights;      // [C]
+    double* root_freqs;   // [K] (valid iff has_root_freqs)
+    int32_t* parent;      // [n_nodes] tree mode
+    double* height;       // [n_nodes] tree mode
+    double* child_h;      // [n_br] branch-list mode
+    double* parent_h;     // [n_br] branch-list mode
+    uint8_t* tips;        // [N][L]  0..K-1, 255 = missing
+    double* pattern_wt;   // [L]
+    PruneOp* ops;         // [N-1] sorted by level
+    // a1
+    int32_t* n_seg;       // [n_br]
+    int32_t* e_hi;        // [n_br] epoch of the parent end
+    int32_t* seg_off;     // [n_br+1]
+    int32_t* seg_epoch;   // [n_br*M] capacity
+    double* seg_dur;      // [n_br*M] capacity
+    int32_t* order;       // [n_br] slots sorted by n_seg, longest first
+    // a2 (reversible): all with row stride Kp
+    double* lam;          // [M][Kp]
+    double* U;            // [M][Kp][Kp] eigenvectors of S = Pi^1/2 Q Pi^-1/2 (columns), zero padded
+    double* W;            // [M][Kp][Kp] W[e] = U_e^T diag(sqrt(pi_e/pi_{e-1})) U_{e-1}, e >= 1
+    double* sp;           // [M][Kp] sqrt(pi)
+    double* isp;          // [M][Kp] 1/sqrt(pi)
+    double* WB;           // [M][64*64] W in DMMA B-fragment order   (Kp == 64 only)
+    double* UTB;          // [M][64*64] U^T in DMMA B-fragment order == U in A-fragment order (Kp == 64 only)
+    // a2' (asymmetric)
+    double* Efull;        // [M][C][K][K] exp(Q_e r_c (tau_e - tau_{e-1})) for interior epochs 1..M-2
+    // a3/a4 output
+    double* P;            // [n_slots][C][K][K]
+    // a5
+    double* partials;     // [N-1][C][L][K] internal nodes only, in op order
+    int32_t* scale_exp;   // [N-1][L]
+    // a6
+    double* site_lnl;     // [L]
+    double* block_sums;   // [reduce blocks]
+    double* lnl;          // [1]
+    int32_t* status;      // [1]
+};
+
+struct epx_ctx {
+    int K = 0, M = 0, C = 0, N = 0, L = 0, device = 0;
+    int Kp = 0;            // padded K used by the eigen buffers
+    int n_nodes = 0;       // 2N-1 (tree mode)
+    int n_slots = 0;       // matrix slots: n_nodes (tree mode) or n_br
+    bool tree_mode = false;
+    int reversible = -1;   // -1 unset, else the common flag of all epochs
+    int chain_kernel = 0;  // EPX_OPT_CHAIN_KERNEL: 0 auto, 1 force the generic shared-memory kernel
+    int use_graph = 1;     // EPX_OPT_USE_GRAPH
+    int prune_kernel = 0;  // EPX_OPT_PRUNE_KERNEL: 0 auto, 1 force the generic shared-memory kernel
+
+    // host copies of the inputs (uploaded lazily; *_dirty = needs upload)
+    std::vector<double> tau, Q, freqs, rates, weights, root_freqs, height, child_h, parent_h, pattern_wt;
+    std::vector<int32_t> parent;
+    std::vector<uint8_t> tips;
+    std::vector<char> model_set;
+    bool has_tau = false, has_rates = false, has_tree = false, has_branches = false, has_tips = false,
+         has_root_freqs = false;
+    bool tau_dirty = false, model_dirty = false, rates_dirty = false, tree_dirty = false, branches_dirty = false,
+         tips_dirty = false, wt_dirty = false, rootf_dirty = false;
+
+    // plan (host): pruning ops sorted by level
+    std::vector<PruneOp> ops;
+    std::vector<int> level_off;        // ops[level_off[l] .. level_off[l+1]) form level l
+    std::vector<int> node_pidx;        // node -> index in partials (internal) or -1
+    int root = -1;
+    int reduce_blocks = 0;
+
+    // binding
+    void* ws = nullptr;
+    size_t ws_bytes = 0;
+    cudaStream_t stream = nullptr;
+    bool bound = false;
+    DevBuffers d{};
+
+    // CUDA graphs (only with a non-default stream)
+    cudaGraphExec_t graph_mat = nullptr, graph_lik = nullptr;
+    long long graph_mat_nodes = 0, graph_lik_nodes = 0;
+    bool graphs_valid = false;
+
+    long long launches = 0;
+    bool have_result = false;
+    bool have_lik = false;   // the last compute call included a5/a6
+    std::string err;
+};
+
+// ---- kernel launchers (each enqueues on `s`, returns the number of kernels launched, or -1 and sets the CUDA error)
+int launch_segmenter(const epx_ctx* c, cudaStream_t s);
+int launch_eigensystems(const epx_ctx* c, cudaStream_t s);
+int launch_chain_reversible(const epx_ctx* c, cudaStream_t s);
+int launch_pade_chain(const epx_ctx* c, cudaStream_t s);
+int launch_pruning(const epx_ctx* c, cudaStream_t s);
+int launch_root_reduction(const epx_ctx* c, cudaStream_t s);
+size_t pade_smem_bytes(int K);
+int chain_init_attributes();
+int pade_init_attributes();
+int eigen_init_attributes();
+int prune_init_attributes();
+int prune_tile(int K, int C);   // patterns per CTA of the generic pruning kernel

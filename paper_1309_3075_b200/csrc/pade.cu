@@ -1,0 +1,241 @@
+// a2' + a3 + a4, asymmetric path: exp(Q_e r d) by [13/13] Pade scaling-and-squaring, chained per branch
+// (P(t) = exp(tQ), citing Moler & Van Loan for its numerical evaluation; L84-L109 Eq.(5)-(7)).
+// The paper only ever says "eigen decomposition" and is silent on asymmetric Q with complex spectra (reading A13);
+// Pade needs no spectrum.  Textbook method (Higham 2005): A <- A / 2^s with ||A||_1 / 2^s <= theta_13,
+//   U = A [A6 (b13 A6 + b11 A4 + b9 A2) + b7 A6 + b5 A4 + b3 A2 + b1 I]
+//   V =    A6 (b12 A6 + b10 A4 + b8 A2) + b6 A6 + b4 A4 + b2 A2 + b0 I
+//   (V - U) R = (V + U)   (Gauss-Jordan, partial pivoting), then R <- R^2 s times.
+//
+// pade_full_epoch_kernel: one CTA per (interior epoch, category): E = exp(Q_e r_c (tau_e - tau_{e-1})), the factor
+//   every branch that spans the whole epoch uses (a2').
+// pade_chain_kernel: one CTA per (slot, category): first and last segment by Pade, interior segments from the
+//   full-epoch table, product accumulated left to right (parent end first) in shared memory; P written once.
+#include "epx_internal.h"
+
+namespace {
+
+constexpr int PT = 256;
+
+__device__ __forceinline__ void mm(int K, const double* __restrict__ A, const double* __restrict__ B,
+                                   double* __restrict__ Cm)
+{
+    for (int idx = threadIdx.x; idx < K * K; idx += PT) {
+        int i = idx / K, j = idx % K;
+        double a = 0.0;
+        for (int k = 0; k < K; k++) a = fma(A[i * K + k], B[k * K + j], a);
+        Cm[idx] = a;
+    }
+    __syncthreads();
+}
+
+struct PadeBufs {
+    double *A, *A2, *A4, *A6, *T1, *T2, *col;
+    double* red;   // [PT/32 + 2]
+};
+
+// In: b.A holds the (unscaled) matrix.  Returns the buffer (b.T1 or b.T2) that holds exp(A).  All threads call.
+__device__ double* pade13(int K, PadeBufs& b, int32_t* status)
+{
+    const double c[14] = {64764752532480000.0, 32382376266240000.0, 7771770303897600.0, 1187353796428800.0,
+                          129060195264000.0, 10559470521600.0, 670442572800.0, 33522128640.0, 1323241920.0,
+                          40840800.0, 960960.0, 16380.0, 182.0, 1.0};
+    const int tid = threadIdx.x, KK = K * K;
+    // ||A||_1 = max column sum
+    double m = 0.0;
+    for (int j = tid; j < K; j += PT) {
+        double s = 0.0;
+        for (int i = 0; i < K; i++) s += fabs(b.A[i * K + j]);
+        m = fmax(m, s);
+    }
+    for (int o = 16; o > 0; o >>= 1) m = fmax(m, __shfl_xor_sync(0xffffffffu, m, o));
+    if ((tid & 31) == 0) b.red[tid >> 5] = m;
+    __syncthreads();
+    double nrm = 0.0;
+    for (int w = 0; w < PT / 32; w++) nrm = fmax(nrm, b.red[w]);
+    int s = 0;
+    if (nrm > 5.371920351148152) s = max(0, (int)ceil(log2(nrm / 5.371920351148152)));
+    if (!(nrm < 1e300)) { s = 0; if (tid == 0) atomicOr(status, EPX_ST_NONFINITE_P); }
+    const double sc = ldexp(1.0, -s);
+    __syncthreads();
+    for (int idx = tid; idx < KK; idx += PT) b.A[idx] *= sc;
+    __syncthreads();
+    mm(K, b.A, b.A, b.A2);
+    mm(K, b.A2, b.A2, b.A4);
+    mm(K, b.A4, b.A2, b.A6);
+    for (int idx = tid; idx < KK; idx += PT) b.T1[idx] = c[13] * b.A6[idx] + c[11] * b.A4[idx] + c[9] * b.A2[idx];
+    __syncthreads();
+    mm(K, b.A6, b.T1, b.T2);
+    for (int idx = tid; idx < KK; idx += PT) {
+        double d = (idx / K == idx % K) ? c[1] : 0.0;
+        b.T2[idx] += c[7] * b.A6[idx] + c[5] * b.A4[idx] + c[3] * b.A2[idx] + d;
+    }
+    __syncthreads();
+    mm(K, b.A, b.T2, b.T1);                                 // T1 = U
+    for (int idx = tid; idx < KK; idx += PT) b.T2[idx] = c[12] * b.A6[idx] + c[10] * b.A4[idx] + c[8] * b.A2[idx];
+    __syncthreads();
+    mm(K, b.A6, b.T2, b.A);                                 // A = A6 * (...)
+    for (int idx = tid; idx < KK; idx += PT) {
+        double d = (idx / K == idx % K) ? c[0] : 0.0;
+        double v = b.A[idx] + c[6] * b.A6[idx] + c[4] * b.A4[idx] + c[2] * b.A2[idx] + d;   // V
+        double u = b.T1[idx];
+        b.A2[idx] = v - u;                                  // left-hand side
+        b.T1[idx] = v + u;                                  // right-hand side, becomes R
+    }
+    __syncthreads();
+    // Gauss-Jordan with partial pivoting on [A2 | T1]
+    double* Lh = b.A2;
+    double* Rh = b.T1;
+    int* piv = reinterpret_cast<int*>(b.red + PT / 32);
+    for (int k = 0; k < K; k++) {
+        if (tid < 32) {
+            double best = -1.0; int bi = k;
+            for (int i = k + tid; i < K; i += 32) { double v = fabs(Lh[i * K + k]); if (v > best) { best = v; bi = i; } }
+            for (int o = 16; o > 0; o >>= 1) {
+                double ob = __shfl_xor_sync(0xffffffffu, best, o);
+                int oi = __shfl_xor_sync(0xffffffffu, bi, o);
+                if (ob > best || (ob == best && oi < bi)) { best = ob; bi = oi; }
+            }
+            if (tid == 0) {
+                *piv = bi;
+                if (!(best > 0.0)) atomicOr(status, EPX_ST_PADE_SINGULAR);
+            }
+        }
+        __syncthreads();
+        const int p = *piv;
+        if (p != k)
+            for (int j = tid; j < 2 * K; j += PT) {
+                double* Mx = j < K ? Lh : Rh; int jj = j < K ? j : j - K;
+                double t = Mx[k * K + jj]; Mx[k * K + jj] = Mx[p * K + jj]; Mx[p * K + jj] = t;
+            }
+        __syncthreads();
+        const double pinv = 1.0 / Lh[k * K + k];
+        for (int i = tid; i < K; i += PT) b.col[i] = (i == k) ? 0.0 : Lh[i * K + k];
+        __syncthreads();
+        for (int j = tid; j < 2 * K; j += PT) {
+            double* Mx = j < K ? Lh : Rh; int jj = j < K ? j : j - K;
+            Mx[k * K + jj] *= pinv;
+        }
+        __syncthreads();
+        for (int idx = tid; idx < 2 * KK; idx += PT) {
+            int i = idx / (2 * K), j = idx % (2 * K);
+            double* Mx = j < K ? Lh : Rh; int jj = j < K ? j : j - K;
+            Mx[i * K + jj] = fma(-b.col[i], Mx[k * K + jj], Mx[i * K + jj]);
+        }
+        __syncthreads();
+    }
+    double* R = b.T1;
+    double* O = b.T2;
+    for (int q = 0; q < s; q++) {
+        mm(K, R, R, O);
+        double* t = R; R = O; O = t;
+    }
+    return R;
+}
+
+__device__ __forceinline__ void carve(int K, double* sm, PadeBufs& b, double*& acc)
+{
+    const size_t KK = (size_t)K * K;
+    b.A = sm; b.A2 = sm + KK; b.A4 = sm + 2 * KK; b.A6 = sm + 3 * KK; b.T1 = sm + 4 * KK; b.T2 = sm + 5 * KK;
+    acc = sm + 6 * KK;
+    b.col = sm + 7 * KK;
+    b.red = b.col + K;
+}
+
+__global__ void __launch_bounds__(PT) pade_full_epoch_kernel(int K, int M, int C, const double* __restrict__ Q,
+    const double* __restrict__ tau, const double* __restrict__ rates, double* __restrict__ Efull,
+    int32_t* __restrict__ status)
+{
+    extern __shared__ double sm[];
+    PadeBufs b; double* acc;
+    carve(K, sm, b, acc);
+    const int e = 1 + blockIdx.x / C, c = blockIdx.x % C;    // interior epochs 1 .. M-2
+    const double scale = rates[c] * (tau[e] - tau[e - 1]);
+    const double* Qe = Q + (size_t)e * K * K;
+    for (int idx = threadIdx.x; idx < K * K; idx += PT) b.A[idx] = Qe[idx] * scale;
+    __syncthreads();
+    double* R = pade13(K, b, status);
+    double* out = Efull + ((size_t)e * C + c) * K * K;
+    for (int idx = threadIdx.x; idx < K * K; idx += PT) out[idx] = R[idx];
+}
+
+__global__ void __launch_bounds__(PT) pade_chain_kernel(int K, int C, const int32_t* __restrict__ order,
+    const int32_t* __restrict__ n_seg, const int32_t* __restrict__ seg_off, const int32_t* __restrict__ seg_epoch,
+    const double* __restrict__ seg_dur, const double* __restrict__ rates, const double* __restrict__ Q,
+    const double* __restrict__ Efull, double* __restrict__ P, int32_t* __restrict__ status)
+{
+    extern __shared__ double sm[];
+    PadeBufs b; double* acc;
+    carve(K, sm, b, acc);
+    const int tid = threadIdx.x, KK = K * K;
+    const int slot = order[blockIdx.x / C], c = blockIdx.x % C;
+    double* out = P + ((size_t)slot * C + c) * KK;
+    const int n = n_seg[slot];
+    if (n == 0) {
+        for (int idx = tid; idx < KK; idx += PT) out[idx] = (idx / K == idx % K) ? 1.0 : 0.0;
+        return;
+    }
+    const int off = seg_off[slot];
+    const double r = rates[c];
+    double* cur = nullptr;           // running product (nullptr = identity so far)
+    for (int s = 0; s < n; s++) {
+        const int e = seg_epoch[off + s];
+        double* E;
+        if (s > 0 && s < n - 1) {    // the branch spans the whole of epoch e: table lookup
+            const double* src = Efull + ((size_t)e * C + c) * KK;
+            for (int idx = tid; idx < KK; idx += PT) b.T1[idx] = src[idx];
+            __syncthreads();
+            E = b.T1;
+        } else {
+            const double scale = r * seg_dur[off + s];
+            const double* Qe = Q + (size_t)e * KK;
+            for (int idx = tid; idx < KK; idx += PT) b.A[idx] = Qe[idx] * scale;
+            __syncthreads();
+            E = pade13(K, b, status);
+        }
+        if (!cur) {
+            for (int idx = tid; idx < KK; idx += PT) acc[idx] = E[idx];
+            __syncthreads();
+            cur = acc;
+        } else {
+            mm(K, cur, E, b.A);      // b.A is free once E is known; the old product buffer becomes the new b.A
+            double* t = cur; cur = b.A; b.A = t;
+        }
+    }
+    bool bad = false;
+    for (int idx = tid; idx < KK; idx += PT) {
+        double v = cur[idx];
+        bad |= !isfinite(v);
+        out[idx] = fmax(v, 0.0);
+    }
+    if (bad) atomicOr(status, EPX_ST_NONFINITE_P);
+}
+
+}  // namespace
+
+size_t pade_smem_bytes(int K)
+{
+    return sizeof(double) * (7 * (size_t)K * K + K + PT / 32 + 2);
+}
+
+int pade_init_attributes()
+{
+    if (cudaFuncSetAttribute(pade_full_epoch_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024) != cudaSuccess) return -1;
+    if (cudaFuncSetAttribute(pade_chain_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024) != cudaSuccess) return -1;
+    return 0;
+}
+
+int launch_pade_chain(const epx_ctx* c, cudaStream_t s)
+{
+    const DevBuffers& d = c->d;
+    const int K = c->K, C = c->C, M = c->M;
+    const size_t smem = pade_smem_bytes(K);
+    int launched = 0;
+    if (M >= 3) {
+        pade_full_epoch_kernel<<<(M - 2) * C, PT, smem, s>>>(K, M, C, d.Q, d.tau, d.rates, d.Efull, d.status);
+        launched++;
+    }
+    pade_chain_kernel<<<c->n_slots * C, PT, smem, s>>>(K, C, d.order, d.n_seg, d.seg_off, d.seg_epoch, d.seg_dur,
+                                                       d.rates, d.Q, d.Efull, d.P, d.status);
+    launched++;
+    return cudaGetLastError() == cudaSuccess ? launched : -1;
+}

@@ -1,0 +1,142 @@
+// a1: on-device epoch-boundary segmenter (PAPER.md L78 change-point process; L117 per-branch epoch weights).
+//
+// Epoch e covers heights [tau[e-1], tau[e]).  For a branch (h_child, h_parent]:
+//   e_lo = #{k : tau_k <= h_child}     epoch that holds the child end
+//   e_hi = #{k : tau_k <  h_parent}    epoch that holds the parent end        (reading A3)
+// Segments run e_hi, e_hi-1, ..., e_lo (parent end first, Eq. 5-7 / reading A2); every duration is > 0 because
+// tau is strictly increasing and tau[e_hi-1] < h_parent, tau[e_lo] > h_child.  A zero-length branch has no segment.
+//
+// Three kernels: count (binary searches) -> single-CTA scan + counting sort by n_seg (longest first, the launch
+// order of the chain kernels) -> fill (CSR epoch / duration arrays).
+#include "epx_internal.h"
+
+namespace {
+
+__device__ __forceinline__ int count_less(const double* __restrict__ tau, int n, double h, bool or_equal)
+{
+    int lo = 0, hi = n;   // first index whose tau is NOT (< h) / (<= h)
+    while (lo < hi) {
+        int mid = (lo + hi) >> 1;
+        double t = tau[mid];
+        bool in = or_equal ? (t <= h) : (t < h);
+        if (in) lo = mid + 1; else hi = mid;
+    }
+    return lo;
+}
+
+__device__ __forceinline__ void branch_ends(int b, const int32_t* __restrict__ parent, const double* __restrict__ height,
+                                            const double* __restrict__ child_h, const double* __restrict__ parent_h,
+                                            double& hc, double& hp)
+{
+    if (parent) {
+        hc = height[b];
+        int p = parent[b];
+        hp = p < 0 ? hc : height[p];
+    } else {
+        hc = child_h[b];
+        hp = parent_h[b];
+    }
+}
+
+__global__ void seg_count_kernel(int n_br, int M, const double* __restrict__ tau, const int32_t* __restrict__ parent,
+                                 const double* __restrict__ height, const double* __restrict__ child_h,
+                                 const double* __restrict__ parent_h, int32_t* __restrict__ n_seg,
+                                 int32_t* __restrict__ e_hi_out)
+{
+    int b = blockIdx.x * blockDim.x + threadIdx.x;
+    if (b >= n_br) return;
+    double hc, hp;
+    branch_ends(b, parent, height, child_h, parent_h, hc, hp);
+    int e_lo = count_less(tau, M - 1, hc, true);
+    int e_hi = count_less(tau, M - 1, hp, false);
+    e_hi_out[b] = e_hi;
+    n_seg[b] = (hp > hc) ? (e_hi - e_lo + 1) : 0;
+}
+
+// One CTA: exclusive scan of n_seg into seg_off, and a counting sort of the slots by n_seg, longest first.
+__global__ void __launch_bounds__(1024) seg_scan_sort_kernel(int n_br, const int32_t* __restrict__ n_seg,
+                                                             int32_t* __restrict__ seg_off, int32_t* __restrict__ order)
+{
+    __shared__ int warp_tot[32];
+    __shared__ int carry;
+    __shared__ int hist[EPX_SORT_BINS];
+    __shared__ int bin_base[EPX_SORT_BINS];
+    const int tid = threadIdx.x, lane = tid & 31, wid = tid >> 5;
+    if (tid == 0) carry = 0;
+    if (tid < EPX_SORT_BINS) hist[tid] = 0;
+    __syncthreads();
+    for (int base = 0; base < n_br; base += blockDim.x) {
+        int i = base + tid;
+        int v = i < n_br ? n_seg[i] : 0;
+        if (i < n_br) atomicAdd(&hist[min(v, EPX_SORT_BINS - 1)], 1);
+        int x = v;
+        for (int o = 1; o < 32; o <<= 1) {
+            int y = __shfl_up_sync(0xffffffffu, x, o);
+            if (lane >= o) x += y;
+        }
+        if (lane == 31) warp_tot[wid] = x;
+        __syncthreads();
+        if (wid == 0) {
+            int w = warp_tot[lane];
+            for (int o = 1; o < 32; o <<= 1) {
+                int y = __shfl_up_sync(0xffffffffu, w, o);
+                if (lane >= o) w += y;
+            }
+            warp_tot[lane] = w;   // inclusive over warps
+        }
+        __syncthreads();
+        int prefix = carry + (wid ? warp_tot[wid - 1] : 0) + x - v;   // exclusive
+        if (i < n_br) seg_off[i] = prefix;
+        __syncthreads();
+        if (tid == blockDim.x - 1) carry = prefix + v;
+        __syncthreads();
+    }
+    if (tid == 0) {
+        seg_off[n_br] = carry;
+        int acc = 0;
+        for (int k = EPX_SORT_BINS - 1; k >= 0; k--) { bin_base[k] = acc; acc += hist[k]; }
+    }
+    __syncthreads();
+    for (int i = tid; i < n_br; i += blockDim.x) {
+        int k = min(n_seg[i], EPX_SORT_BINS - 1);
+        int pos = atomicAdd(&bin_base[k], 1);
+        order[pos] = i;
+    }
+}
+
+__global__ void seg_fill_kernel(int n_br, int M, const double* __restrict__ tau, const int32_t* __restrict__ parent,
+                                const double* __restrict__ height, const double* __restrict__ child_h,
+                                const double* __restrict__ parent_h, const int32_t* __restrict__ n_seg,
+                                const int32_t* __restrict__ e_hi_in, const int32_t* __restrict__ seg_off,
+                                int32_t* __restrict__ seg_epoch, double* __restrict__ seg_dur)
+{
+    int b = blockIdx.x * blockDim.x + threadIdx.x;
+    if (b >= n_br) return;
+    int n = n_seg[b];
+    if (n == 0) return;
+    double hc, hp;
+    branch_ends(b, parent, height, child_h, parent_h, hc, hp);
+    int e = e_hi_in[b], off = seg_off[b];
+    double upper = hp;
+    for (int i = 0; i < n; i++, e--) {
+        double lower = (i == n - 1) ? hc : tau[e - 1];
+        seg_epoch[off + i] = e;
+        seg_dur[off + i] = upper - lower;
+        upper = lower;
+    }
+}
+
+}  // namespace
+
+int launch_segmenter(const epx_ctx* c, cudaStream_t s)
+{
+    const DevBuffers& d = c->d;
+    int n = c->n_slots;
+    int blocks = (n + 255) / 256;
+    const int32_t* parent = c->tree_mode ? d.parent : nullptr;
+    seg_count_kernel<<<blocks, 256, 0, s>>>(n, c->M, d.tau, parent, d.height, d.child_h, d.parent_h, d.n_seg, d.e_hi);
+    seg_scan_sort_kernel<<<1, 1024, 0, s>>>(n, d.n_seg, d.seg_off, d.order);
+    seg_fill_kernel<<<blocks, 256, 0, s>>>(n, c->M, d.tau, parent, d.height, d.child_h, d.parent_h, d.n_seg, d.e_hi,
+                                           d.seg_off, d.seg_epoch, d.seg_dur);
+    return cudaGetLastError() == cudaSuccess ? 3 : -1;
+}

@@ -1,0 +1,128 @@
+"""CPU-side checks of the C-ABI boundary: libepx.so builds, loads, and exports every symbol include/epx.h declares;
+host-side validation (no kernels are launched, no GPU needed)."""
+import ctypes as ct
+import os
+import re
+
+import numpy as np
+import pytest
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+
+
+@pytest.fixture(scope="module")
+def L():
+    from paper_1309_3075_b200 import build
+    build.build_library()
+    import paper_1309_3075_b200 as epx
+    return epx.lib()
+
+
+def _declared_symbols():
+    src = open(os.path.join(ROOT, "include", "epx.h")).read()
+    src = re.sub(r"/\*.*?\*/", "", src, flags=re.S)
+    return sorted(set(re.findall(r"\b(epx_[a-z0-9_]+)\s*\(", src)))
+
+
+def test_every_declared_symbol_is_exported(L):
+    names = _declared_symbols()
+    assert len(names) >= 25
+    for n in names:
+        assert hasattr(L, n), f"libepx.so does not export {n}"
+
+
+def test_binding_covers_every_symbol(L):
+    import paper_1309_3075_b200 as epx
+    for n in _declared_symbols():
+        short = n[len("epx_"):]
+        assert hasattr(epx.Epx, short) or hasattr(epx, short) or n in ("epx_create", "epx_destroy", "epx_measure_fp64_peak"), n
+
+
+def test_no_torch_types_in_signatures():
+    src = open(os.path.join(ROOT, "include", "epx.h")).read()
+    assert "torch" not in src.lower() and "at::" not in src and "#include <cuda" not in src
+
+
+def test_create_argument_checks(L):
+    import paper_1309_3075_b200 as epx
+    for args in [(1, 1, 1, 2, 1), (65, 1, 1, 2, 1), (4, 0, 1, 2, 1), (4, 1, 9, 2, 1), (4, 1, 1, 1, 1), (4, 1, 1, 2, 0)]:
+        with pytest.raises(epx.EpxError):
+            epx.Epx(*args)
+    c = epx.Epx(4, 2, 2, 3, 5)
+    assert c.workspace_bytes() > 0
+    c.close()
+
+
+def test_host_validation_rules(L):
+    import paper_1309_3075_b200 as epx
+    c = epx.Epx(4, 3, 2, 3, 5)
+    # boundaries: strictly increasing, finite
+    for bad in ([0.5, 0.5], [0.6, 0.5], [0.1, np.inf], [np.nan, 1.0]):
+        with pytest.raises(epx.EpxError) as ei:
+            c.set_epoch_boundaries(bad)
+        assert ei.value.code == epx.EPX_E_ARG
+    c.set_epoch_boundaries([0.1, 0.5])
+    # models
+    pi = np.array([0.1, 0.2, 0.3, 0.4])
+    Q = np.tile(pi, (4, 1)); np.fill_diagonal(Q, 0); np.fill_diagonal(Q, -Q.sum(1))
+    c.set_epoch_model(0, Q, pi, True)
+    Qbad = Q.copy(); Qbad[0, 1] += 1e-3
+    with pytest.raises(epx.EpxError) as ei:
+        c.set_epoch_model(1, Qbad, pi, True)          # row does not sum to 0
+    assert ei.value.code == epx.EPX_E_MODEL
+    Qneg = Q.copy(); Qneg[0, 1] = -0.1; Qneg[0, 0] = -(Qneg[0, 1] + Qneg[0, 2] + Qneg[0, 3])
+    with pytest.raises(epx.EpxError):
+        c.set_epoch_model(1, Qneg, pi, True)
+    Qasym = Q.copy(); Qasym[0, 1] += 0.2; Qasym[0, 0] -= 0.2
+    with pytest.raises(epx.EpxError):
+        c.set_epoch_model(1, Qasym, pi, True)         # detailed balance violated
+    with pytest.raises(epx.EpxError):
+        c.set_epoch_model(1, Qasym, pi, False)        # mixing reversible flags within a ctx
+    with pytest.raises(epx.EpxError):
+        c.set_epoch_model(1, Q, pi * 1.1, True)       # freqs not a distribution
+    with pytest.raises(epx.EpxError):
+        c.set_epoch_model(3, Q, pi, True)             # epoch out of range
+    # category rates
+    with pytest.raises(epx.EpxError):
+        c.set_category_rates([1.0, -1.0], [0.5, 0.5])
+    with pytest.raises(epx.EpxError):
+        c.set_category_rates([1.0, 1.0], [0.5, 0.6])
+    c.set_category_rates([0.5, 1.5], [0.5, 0.5])
+    # trees: N = 3 tips, nodes 0..4
+    good_parent, good_h = [3, 3, 4, 4, -1], [0.0, 0.0, 0.0, 0.3, 1.0]
+    c.set_tree(good_parent, good_h)
+    for parent, h in [([3, 3, 4, 4, 4], good_h),            # no root
+                      ([3, 3, 3, 4, -1], good_h),           # trifurcation
+                      ([3, 3, 4, -1, -1], good_h),          # two roots
+                      ([3, 3, 4, 4, -1], [0, 0, 0, 1.3, 1.0]),  # child above parent
+                      ([1, 3, 4, 4, -1], good_h),           # tip as a parent
+                      ([3, 3, 4, 4, -1], [0, 0, np.nan, 0.3, 1.0])]:
+        with pytest.raises(epx.EpxError) as ei:
+            c.set_tree(parent, h)
+        assert ei.value.code == epx.EPX_E_TREE
+    # compute before bind -> state error, not a crash
+    with pytest.raises(epx.EpxError) as ei:
+        c.log_likelihood()
+    assert ei.value.code == epx.EPX_E_STATE
+    # branch-list setters are refused in tree mode and vice versa
+    with pytest.raises(epx.EpxError):
+        c.set_branches([0.0], [1.0])
+    b = epx.Epx(4, 1, 1, 0, 0)
+    with pytest.raises(epx.EpxError):
+        b.workspace_bytes()                            # needs set_branches first
+    with pytest.raises(epx.EpxError):
+        b.set_branches([0.5], [0.1])                   # parent below child
+    b.set_branches([0.0, 0.1], [1.0, 0.1])
+    assert b.workspace_bytes() > 0
+    with pytest.raises(epx.EpxError):
+        b.set_tree(good_parent, good_h)
+    c.close(); b.close()
+
+
+def test_workspace_scales_with_problem(L):
+    import paper_1309_3075_b200 as epx
+    a = epx.Epx(4, 10, 4, 2000, 10000)
+    need = a.workspace_bytes()
+    partials = 1999 * 4 * 10000 * 4 * 8
+    assert partials < need < partials * 1.2          # the partials buffer dominates (cfg 2: 2.56 GB)
+    a.close()

@@ -1,0 +1,152 @@
+"""GPU parity: the CUDA path (through the C ABI) against the long-double CPU oracle, element by element, on the same
+seeded inputs.  Tolerances (BASELINE.json north_star): 1e-12 absolute on every P entry, 1e-9 relative on the total
+log-likelihood; segment lists must match exactly (epochs) / to 1 ulp (durations)."""
+import numpy as np
+import pytest
+
+import workloads as W
+
+pytestmark = pytest.mark.gpu
+
+P_TOL = 1e-12
+LNL_RTOL = 1e-9
+PARTIAL_RTOL = 1e-10     # per (node, pattern), relative to the largest entry of that vector set
+
+
+@pytest.fixture(scope="module")
+def epx():
+    import torch
+    assert torch.cuda.is_available(), "GPU tests need a CUDA device"
+    import paper_1309_3075_b200 as m
+    m.lib()
+    return m
+
+
+def check_segments(ctx, ref):
+    off, ep, du = ctx.get_all_segments()
+    assert np.array_equal(off, ref["seg_off"])
+    assert np.array_equal(ep, ref["seg_epoch"])
+    rd = ref["seg_dur"]
+    assert np.all(np.abs(du - rd) <= np.spacing(np.abs(rd)))
+    return off
+
+
+def check_matrices(ctx, ref, slots=None):
+    P = ctx.get_all_matrices()
+    Pref = ref["P"]
+    if slots is not None:
+        P = P[slots]
+    err = np.max(np.abs(P.astype(np.longdouble) - Pref))
+    assert err <= P_TOL, f"max |P - P_oracle| = {float(err):.3e}"
+    assert np.all(P >= 0.0)
+    assert np.max(np.abs(P.sum(-1) - 1.0)) < 1e-11
+    return float(err)
+
+
+def check_likelihood(ctx, prob, ref, lnl, partial_nodes=()):
+    ref_lnl = ref["lnl"]
+    assert abs(np.longdouble(lnl) - ref_lnl) <= LNL_RTOL * abs(ref_lnl), (lnl, float(ref_lnl))
+    site = ctx.get_site_log_likelihoods()
+    rs = ref["site_lnl"]
+    assert np.max(np.abs(site.astype(np.longdouble) - rs) / np.abs(rs).clip(1e-300)) <= LNL_RTOL
+    for node in partial_nodes:
+        out, ex = ctx.get_partials(node)
+        got = np.ldexp(out.astype(np.longdouble), ex[None, :, None])
+        want = ref["partials"][node]
+        scale = np.max(want, axis=(0, 2), keepdims=True)
+        assert np.max(np.abs(got - want) / scale) <= PARTIAL_RTOL, f"partials of node {node}"
+
+
+def run_tree(epx, orc, prob, partial_nodes="all", options=()):
+    ctx = epx.from_problem(prob)
+    for o, v in options:
+        ctx.set_option(o, v)
+    lnl = ctx.log_likelihood()
+    want_partials = bool(partial_nodes)
+    ref = orc.evaluate(prob, want_partials=want_partials)
+    check_segments(ctx, ref)
+    check_matrices(ctx, ref)
+    if partial_nodes == "all":
+        partial_nodes = range(prob.n_nodes)
+    check_likelihood(ctx, prob, ref, lnl, partial_nodes or ())
+    assert ctx.status() == 0
+    assert ctx.launch_count() > 0
+    # update_matrices alone reproduces the same matrices
+    ctx.update_matrices()
+    check_matrices(ctx, ref)
+    ctx.close()
+    return lnl, ref
+
+
+# ------------------------------------------------------------------------------------------------ the five configs
+def test_config1_full(epx, orc_ld):
+    run_tree(epx, orc_ld, W.make_config(1))
+
+
+def test_config1_generic_kernels_and_no_graph(epx, orc_ld):
+    prob = W.make_config(1)
+    run_tree(epx, orc_ld, prob, options=[(epx.EPX_OPT_CHAIN_KERNEL, 1), (epx.EPX_OPT_PRUNE_KERNEL, 1)])
+    run_tree(epx, orc_ld, prob, options=[(epx.EPX_OPT_USE_GRAPH, 0)])
+
+
+def test_config2_reduced(epx, orc_ld):
+    # several pattern tiles plus a ragged tail (L = 777 = 3*256 + 9), 10 epochs, dated tips
+    run_tree(epx, orc_ld, W.make_config(2, N=150, L=777))
+
+
+def test_config2_full_size(epx, orc_ld):
+    # the configuration bench.py times; the oracle's naive recursion takes ~1 min here
+    prob = W.make_config(2)
+    run_tree(epx, orc_ld, prob, partial_nodes=())   # oracle partials of every node would be 10 GB; reduced test covers them
+
+
+def test_config3_reduced(epx, orc_ld):
+    prob = W.make_config(3, N=12, L=70)
+    run_tree(epx, orc_ld, prob)
+    run_tree(epx, orc_ld, prob, options=[(epx.EPX_OPT_CHAIN_KERNEL, 1)], partial_nodes=())
+
+
+def test_config3_full_size(epx, orc_ld):
+    prob = W.make_config(3)
+    run_tree(epx, orc_ld, prob, partial_nodes=[prob.N, prob.n_nodes - 1])
+
+
+def test_config4_reduced(epx, orc_ld):
+    run_tree(epx, orc_ld, W.make_config(4, N=60, L=3))
+
+
+def test_config4_full_size(epx, orc_ld):
+    run_tree(epx, orc_ld, W.make_config(4), partial_nodes=[2998, 2000, 1500])
+
+
+def test_config5_reduced_every_branch(epx, orc_ld):
+    prob = W.make_config(5, n_br=300)
+    for kernel in (0, 1):
+        ctx = epx.from_problem(prob)
+        ctx.set_option(epx.EPX_OPT_CHAIN_KERNEL, kernel)
+        ctx.update_matrices()
+        ref = orc_ld.evaluate(prob)
+        check_segments(ctx, ref)
+        check_matrices(ctx, ref)
+        assert ctx.status() == 0
+        ctx.close()
+
+
+def test_config5_full_size_sampled(epx, orc_ld):
+    # full launch configuration (20 000 branches); segments checked for every branch, matrices for a seeded sample
+    # that always includes the longest chains, plus row sums / non-negativity for every matrix
+    prob = W.make_config(5)
+    ctx = epx.from_problem(prob)
+    ctx.update_matrices()
+    off_ref, ep_ref, du_ref = orc_ld.segments(prob.child_height, prob.parent_height, prob.tau)
+    off = check_segments(ctx, {"seg_off": off_ref, "seg_epoch": ep_ref, "seg_dur": du_ref})
+    nseg = np.diff(off)
+    rng = np.random.default_rng(5)
+    sample = np.unique(np.concatenate([np.argsort(nseg)[-8:], np.argsort(nseg)[:4], rng.choice(prob.n_br, 48, replace=False)]))
+    ref = orc_ld.evaluate(prob, branches=sample)
+    P = ctx.get_all_matrices()
+    err = np.max(np.abs(P[sample].astype(np.longdouble) - ref["P"]))
+    assert err <= P_TOL, float(err)
+    assert np.all(P >= 0) and np.max(np.abs(P.sum(-1) - 1.0)) < 1e-11
+    assert ctx.status() == 0
+    ctx.close()
