@@ -125,11 +125,17 @@ const char* epx_last_error(const epx_ctx* ctx);
  * compiler from deleting the arithmetic).  Synchronises the stream. */
 int epx_measure_fp64_peak(int device, int kind, double ms_target, void* dev_scratch, void* cuda_stream, double* tflops);
 
-/* ---- tuning / test hooks (no effect on results) ---- */
+/* ---- tuning / test hooks (options 1-3 have no effect on results) ---- */
 enum {
     EPX_OPT_CHAIN_KERNEL = 1, /* 0 auto (default); 1 force the generic shared-memory chain kernel */
     EPX_OPT_USE_GRAPH = 2,    /* 1 (default) replay the kernel sequence from a CUDA graph on non-default streams; 0 launch directly */
-    EPX_OPT_PRUNE_KERNEL = 3  /* 0 auto (default); 1 force the generic shared-memory pruning kernel */
+    EPX_OPT_PRUNE_KERNEL = 3, /* 0 auto (default); 1 force the generic shared-memory pruning kernel */
+    EPX_OPT_EXP_METHOD = 4    /* a3 method.  1 spectral: Jacobi eigensystem (reversible) / Pade 13 (asymmetric), absolute
+                                 error ~1e-14 per entry.  2 componentwise: shifted non-negative Taylor scaling-and-squaring,
+                                 every entry to a few hundred ulp RELATIVE, ~8 dense products per segment.  0 auto (default):
+                                 2 for tree-mode (likelihood) contexts whose reversible Q have structural zeros (codon
+                                 models: entries of P that vanish like t^2, t^3 decide the likelihood of short branches),
+                                 else 1.  This one DOES change results, within the tolerances above (A21). */
 };
 int epx_set_option(epx_ctx* ctx, int option, int value);
 /* Device status word of the last compute call (0 = all numeric checks passed); synchronises. */

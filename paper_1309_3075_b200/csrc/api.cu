@@ -179,6 +179,7 @@ int epx_create(epx_ctx** out, int K, int M, int C, int N_tips, int L, int device
     c->Q.assign((size_t)M * K * K, 0.0);
     c->freqs.assign((size_t)M * K, 0.0);
     c->model_set.assign(M, 0);
+    c->model_sparse.assign(M, 0);
     if (c->tree_mode) {
         c->pattern_wt.assign(L, 1.0);
         c->wt_dirty = true;
@@ -236,6 +237,7 @@ int epx_set_option(epx_ctx* c, int option, int value)
         case 1: c->chain_kernel = value; break;
         case 2: c->use_graph = value; break;
         case 3: c->prune_kernel = value; break;
+        case 4: if (value < 0 || value > 2) return fail(c, EPX_E_ARG, "exp method %d", value); c->exp_method = value; break;
         default: return fail(c, EPX_E_ARG, "unknown option %d", option);
     }
     drop_graphs(c);
@@ -299,6 +301,14 @@ int epx_set_epoch_model(epx_ctx* c, int epoch, const double* Q, const double* fr
     std::copy(Q, Q + K * K, c->Q.begin() + (size_t)epoch * K * K);
     std::copy(freqs, freqs + K, c->freqs.begin() + (size_t)epoch * K);
     c->model_set[epoch] = 1;
+    {
+        const bool was = c->use_taylor();
+        char sparse = 0;
+        for (int i = 0; i < K; i++)
+            for (int j = 0; j < K; j++) if (i != j && Q[i * K + j] == 0.0) sparse = 1;
+        c->model_sparse[epoch] = sparse;
+        if (was != c->use_taylor()) drop_graphs(c);
+    }
     c->model_dirty = true;
     return EPX_OK;
 }

@@ -82,6 +82,8 @@ struct epx_ctx {
     int chain_kernel = 0;  // EPX_OPT_CHAIN_KERNEL: 0 auto, 1 force the generic shared-memory kernel
     int use_graph = 1;     // EPX_OPT_USE_GRAPH
     int prune_kernel = 0;  // EPX_OPT_PRUNE_KERNEL: 0 auto, 1 force the generic shared-memory kernel
+    int exp_method = 0;    // EPX_OPT_EXP_METHOD: 0 auto, 1 spectral (Jacobi / Pade), 2 componentwise (shifted Taylor)
+    std::vector<char> model_sparse;   // per epoch: Q has a structural zero off the diagonal
 
     // host copies of the inputs (uploaded lazily; *_dirty = needs upload)
     std::vector<double> tau, Q, freqs, rates, weights, root_freqs, height, child_h, parent_h, pattern_wt;
@@ -116,6 +118,17 @@ struct epx_ctx {
     bool have_result = false;
     bool have_lik = false;   // the last compute call included a5/a6
     std::string err;
+
+    // a3 method of the next compute call (reading A21): the componentwise-accurate exponential serves likelihoods
+    // over reversible models with structural zeros (codon models); everything else takes the spectral path.
+    bool use_taylor() const
+    {
+        if (exp_method == 1) return false;
+        if (exp_method == 2) return true;
+        if (!tree_mode || reversible != 1) return false;
+        for (char z : model_sparse) if (z) return true;
+        return false;
+    }
 };
 
 // ---- kernel launchers (each enqueues on `s`, returns the number of kernels launched, or -1 and sets the CUDA error)
@@ -123,6 +136,7 @@ int launch_segmenter(const epx_ctx* c, cudaStream_t s);
 int launch_eigensystems(const epx_ctx* c, cudaStream_t s);
 int launch_chain_reversible(const epx_ctx* c, cudaStream_t s);
 int launch_pade_chain(const epx_ctx* c, cudaStream_t s);
+int launch_taylor_chain(const epx_ctx* c, cudaStream_t s);   // same kernels, shifted non-negative Taylor exponential
 int launch_pruning(const epx_ctx* c, cudaStream_t s);
 int launch_root_reduction(const epx_ctx* c, cudaStream_t s);
 size_t pade_smem_bytes(int K);

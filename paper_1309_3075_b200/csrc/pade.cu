@@ -132,6 +132,73 @@ __device__ double* pade13(int K, PadeBufs& b, int32_t* status)
     return R;
 }
 
+// Componentwise-accurate alternative (reading A21 in DESIGN.md): exp(A) = e^{-mu} exp(A + mu I), mu = max_i |A_ii|.
+// A + mu I is entrywise non-negative, its Taylor series (exp(tQ) = sum_j (tQ)^j / j!) has only
+// non-negative terms, and squaring a non-negative matrix adds non-negative numbers: no cancellation anywhere, so
+// every entry of the result -- including the ones that vanish like t^g for states g substitutions apart -- carries
+// a relative error of a few hundred ulp.  Pade and the eigen path only bound the ABSOLUTE error (~1e-14), which a
+// likelihood over short branches and distant tip states (codon data) amplifies without limit.
+//   M = (A + mu I) / 2^s, ||M||_inf = mu / 2^s <= 1;  degree-16 Taylor by Paterson-Stockmeyer (powers M^2..M^4, three
+//   Horner steps: 6 products);  R = e^{-mu/2^s} * poly(M) (stochastic);  R <- R^2 s times.
+// In: b.A holds A.  Returns the buffer that holds exp(A).  All threads call.
+__device__ double* expm_shifted_taylor(int K, PadeBufs& b, int32_t* status)
+{
+    const double c[17] = {1.0, 1.0, 1.0 / 2, 1.0 / 6, 1.0 / 24, 1.0 / 120, 1.0 / 720, 1.0 / 5040, 1.0 / 40320,
+                          1.0 / 362880, 1.0 / 3628800, 1.0 / 39916800, 1.0 / 479001600, 1.0 / 6227020800.0,
+                          1.0 / 87178291200.0, 1.0 / 1307674368000.0, 1.0 / 20922789888000.0};
+    const int tid = threadIdx.x, KK = K * K;
+    double m = 0.0;
+    for (int i = tid; i < K; i += PT) m = fmax(m, -b.A[i * K + i]);
+    for (int o = 16; o > 0; o >>= 1) m = fmax(m, __shfl_xor_sync(0xffffffffu, m, o));
+    if ((tid & 31) == 0) b.red[tid >> 5] = m;
+    __syncthreads();
+    double mu = 0.0;
+    for (int w = 0; w < PT / 32; w++) mu = fmax(mu, b.red[w]);
+    int s = 0;
+    if (mu > 1.0) s = (int)ceil(log2(mu));
+    if (!(mu < 1e300)) { s = 0; if (tid == 0) atomicOr(status, EPX_ST_NONFINITE_P); }
+    const double sc = ldexp(1.0, -s);
+    __syncthreads();
+    double* M1 = b.A; double* M2 = b.A2; double* M3 = b.A4; double* M4 = b.A6;
+    for (int idx = tid; idx < KK; idx += PT) {
+        double v = M1[idx];
+        if (idx / K == idx % K) v = fmax(v + mu, 0.0);
+        M1[idx] = v * sc;
+    }
+    __syncthreads();
+    mm(K, M1, M1, M2);
+    mm(K, M2, M1, M3);
+    mm(K, M2, M2, M4);
+    auto block = [&](int k, int idx) -> double {   // B_k = c[4k] I + c[4k+1] M + c[4k+2] M^2 + c[4k+3] M^3
+        double d = (idx / K == idx % K) ? c[4 * k] : 0.0;
+        return d + c[4 * k + 1] * M1[idx] + c[4 * k + 2] * M2[idx] + c[4 * k + 3] * M3[idx];
+    };
+    double* R = b.T1;
+    double* O = b.T2;
+    for (int idx = tid; idx < KK; idx += PT) R[idx] = block(3, idx) + c[16] * M4[idx];
+    __syncthreads();
+    for (int k = 2; k >= 0; k--) {
+        mm(K, R, M4, O);
+        for (int idx = tid; idx < KK; idx += PT) O[idx] += block(k, idx);
+        __syncthreads();
+        double* t = R; R = O; O = t;
+    }
+    const double damp = exp(-mu * sc);
+    for (int idx = tid; idx < KK; idx += PT) R[idx] *= damp;
+    __syncthreads();
+    for (int q = 0; q < s; q++) {
+        mm(K, R, R, O);
+        double* t = R; R = O; O = t;
+    }
+    return R;
+}
+
+template <int METHOD>
+__device__ __forceinline__ double* expm_dense(int K, PadeBufs& b, int32_t* status)
+{
+    return METHOD == 0 ? pade13(K, b, status) : expm_shifted_taylor(K, b, status);
+}
+
 __device__ __forceinline__ void carve(int K, double* sm, PadeBufs& b, double*& acc)
 {
     const size_t KK = (size_t)K * K;
@@ -141,6 +208,7 @@ __device__ __forceinline__ void carve(int K, double* sm, PadeBufs& b, double*& a
     b.red = b.col + K;
 }
 
+template <int METHOD>
 __global__ void __launch_bounds__(PT) pade_full_epoch_kernel(int K, int M, int C, const double* __restrict__ Q,
     const double* __restrict__ tau, const double* __restrict__ rates, double* __restrict__ Efull,
     int32_t* __restrict__ status)
@@ -153,11 +221,12 @@ __global__ void __launch_bounds__(PT) pade_full_epoch_kernel(int K, int M, int C
     const double* Qe = Q + (size_t)e * K * K;
     for (int idx = threadIdx.x; idx < K * K; idx += PT) b.A[idx] = Qe[idx] * scale;
     __syncthreads();
-    double* R = pade13(K, b, status);
+    double* R = expm_dense<METHOD>(K, b, status);
     double* out = Efull + ((size_t)e * C + c) * K * K;
     for (int idx = threadIdx.x; idx < K * K; idx += PT) out[idx] = R[idx];
 }
 
+template <int METHOD>
 __global__ void __launch_bounds__(PT) pade_chain_kernel(int K, int C, const int32_t* __restrict__ order,
     const int32_t* __restrict__ n_seg, const int32_t* __restrict__ seg_off, const int32_t* __restrict__ seg_epoch,
     const double* __restrict__ seg_dur, const double* __restrict__ rates, const double* __restrict__ Q,
@@ -190,7 +259,7 @@ __global__ void __launch_bounds__(PT) pade_chain_kernel(int K, int C, const int3
             const double* Qe = Q + (size_t)e * KK;
             for (int idx = tid; idx < KK; idx += PT) b.A[idx] = Qe[idx] * scale;
             __syncthreads();
-            E = pade13(K, b, status);
+            E = expm_dense<METHOD>(K, b, status);
         }
         if (!cur) {
             for (int idx = tid; idx < KK; idx += PT) acc[idx] = E[idx];
@@ -219,23 +288,29 @@ size_t pade_smem_bytes(int K)
 
 int pade_init_attributes()
 {
-    if (cudaFuncSetAttribute(pade_full_epoch_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024) != cudaSuccess) return -1;
-    if (cudaFuncSetAttribute(pade_chain_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024) != cudaSuccess) return -1;
+    if (cudaFuncSetAttribute(pade_full_epoch_kernel<0>, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024) != cudaSuccess) return -1;
+    if (cudaFuncSetAttribute(pade_chain_kernel<0>, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024) != cudaSuccess) return -1;
+    if (cudaFuncSetAttribute(pade_full_epoch_kernel<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024) != cudaSuccess) return -1;
+    if (cudaFuncSetAttribute(pade_chain_kernel<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024) != cudaSuccess) return -1;
     return 0;
 }
 
-int launch_pade_chain(const epx_ctx* c, cudaStream_t s)
+template <int METHOD>
+static int launch_dense(const epx_ctx* c, cudaStream_t s)
 {
     const DevBuffers& d = c->d;
     const int K = c->K, C = c->C, M = c->M;
     const size_t smem = pade_smem_bytes(K);
     int launched = 0;
     if (M >= 3) {
-        pade_full_epoch_kernel<<<(M - 2) * C, PT, smem, s>>>(K, M, C, d.Q, d.tau, d.rates, d.Efull, d.status);
+        pade_full_epoch_kernel<METHOD><<<(M - 2) * C, PT, smem, s>>>(K, M, C, d.Q, d.tau, d.rates, d.Efull, d.status);
         launched++;
     }
-    pade_chain_kernel<<<c->n_slots * C, PT, smem, s>>>(K, C, d.order, d.n_seg, d.seg_off, d.seg_epoch, d.seg_dur,
+    pade_chain_kernel<METHOD><<<c->n_slots * C, PT, smem, s>>>(K, C, d.order, d.n_seg, d.seg_off, d.seg_epoch, d.seg_dur,
                                                        d.rates, d.Q, d.Efull, d.P, d.status);
     launched++;
     return cudaGetLastError() == cudaSuccess ? launched : -1;
 }
+
+int launch_pade_chain(const epx_ctx* c, cudaStream_t s) { return launch_dense<0>(c, s); }
+int launch_taylor_chain(const epx_ctx* c, cudaStream_t s) { return launch_dense<1>(c, s); }
