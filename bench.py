@@ -1,0 +1,386 @@
+#!/usr/bin/env python
+"""bench.py -- throughput of the epoch-substitution-model hot path on B200 (one JSON line on stdout, rank 0).
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl cuda|reference]
+    python -m torch.distributed.run --nnodes=1 --nproc-per-node N --master-addr 127.0.0.1 --master-port P \
+        bench.py --gpus N --steps K --warmup W
+
+A STEP is one pass of the whole hot path (segmenter, eigensystems, segment exponentials +
+chain convolution, pruning, root reduction) over BASELINE.json config 2 (`configs[1]`: HKY, 10 epochs, 2 000 tips,
+10 000 site patterns, 4 rate categories), seeded synthetic input.  BASELINE.json's metric has two halves:
+  * "pruning partials GB/s"     -> the headline `value`: algorithmic bytes of a5+a6
+                                   divided by the time of the WHOLE step;
+  * "epoch branch matrices/s"   -> the `matrices` object: config 5 (61-state convolution microbenchmark, a1..a4), the
+                                   largest single-GPU matrix workload, with its own (FP64 ALU) roofline.
+Multi-GPU: the path does not shard (replicas only) -- every rank runs an independent replica
+of the same problem, no data-path collective; value = N x units / max-over-ranks time ("weak" scaling).
+
+`--impl reference` times the CPU oracle (oracle/, as it stands, long-double build, OpenMP) on a bounded sample of the same
+workload on the box's host cores; rank 0 only.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import sys
+import threading
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+import workloads as W  # noqa: E402  (input generators only; shared with the oracle, holds no arithmetic of the method)
+
+METRIC = "pruning partials GB/s (fp64) over the whole a1..a6 log-likelihood step; epoch branch matrices/s in `matrices`"
+UNIT = "GB/s"
+
+
+# ---------------------------------------------------------------------------------------------- algorithmic work
+def pruning_bytes(prob) -> dict:
+    """Algorithmic HBM bytes of a5: every internal node writes its partials [C][L][K] f64 and its
+    scale exponents [L] i32, reads per child either partials + exponents (internal child) or one byte per pattern
+    (tip child), and the two children's C K x K matrices; a6 re-reads the root partials + exponents, reads the
+    pattern weights and writes the site log-likelihoods."""
+    K, C, L, N = prob.K, prob.C, prob.L, prob.N
+    part = C * L * K * 8
+    n_int = N - 1
+    is_child_internal = np.zeros(2 * N - 1, dtype=bool)
+    is_child_internal[N:] = True
+    par = np.asarray(prob.parent)
+    children = np.nonzero(par >= 0)[0]
+    n_int_children = int(np.sum(children >= N))
+    n_tip_children = int(np.sum(children < N))
+    a5 = n_int * (part + 4 * L + 2 * C * K * K * 8) + n_int_children * (part + 4 * L) + n_tip_children * L
+    a6 = part + 4 * L + 8 * L + 8 * L
+    flops = n_int * C * L * (4 * K * K + K)
+    return {"a5": a5, "a6": a6, "flops": flops}
+
+
+def chain_flops(K: int, C: int, n_seg: np.ndarray) -> dict:
+    """Executed useful flops of the eigenbasis chain (one K^3 product per segment and category, K not padded) and the
+    straightforward exp-then-convolve count of SURVEY.md 8(d) for context."""
+    nseg = n_seg.astype(np.int64)
+    executed = int(nseg.sum()) * C * 2 * K ** 3
+    straightforward = int((2 * nseg - (nseg > 0)).sum()) * C * 2 * K ** 3
+    return {"executed": executed, "straightforward": straightforward}
+
+
+def n_segments(prob) -> np.ndarray:
+    """Segment count per matrix slot from the inputs (host integer arithmetic for the flop count only)."""
+    ch, ph = prob.branch_heights()
+    tau = np.asarray(prob.tau)
+    e_lo = np.searchsorted(tau, ch, side="right")
+    e_hi = np.searchsorted(tau, ph, side="left")
+    return np.where(ph > ch, e_hi - e_lo + 1, 0)
+
+
+# ---------------------------------------------------------------------------------------------- clocks
+class ClockSampler:
+    """Samples SM clock, power and clock-event reasons of one GPU through NVML while the timed regions run."""
+    REASONS = {0x4: "sw_power_cap", 0x8: "hw_slowdown", 0x20: "sw_thermal_slowdown", 0x40: "hw_thermal_slowdown",
+               0x80: "hw_power_brake_slowdown", 0x2: "applications_clocks_setting", 0x10: "sync_boost"}
+
+    def __init__(self, index: int, period_s: float = 0.02):
+        self.samples, self.reason_bits, self.power = [], 0, []
+        self.period, self._stop, self._thr, self.h, self.max_mhz = period_s, threading.Event(), None, None, None
+        try:
+            import pynvml
+            pynvml.nvmlInit()
+            self.nv = pynvml
+            self.h = pynvml.nvmlDeviceGetHandleByIndex(index)
+            self.max_mhz = int(pynvml.nvmlDeviceGetMaxClockInfo(self.h, pynvml.NVML_CLOCK_SM))
+        except Exception as e:  # NVML missing: the JSON line says so instead of inventing clocks
+            self.err = repr(e)
+
+    def _loop(self):
+        nv = self.nv
+        while not self._stop.is_set():
+            try:
+                self.samples.append(int(nv.nvmlDeviceGetClockInfo(self.h, nv.NVML_CLOCK_SM)))
+                try:
+                    bits = nv.nvmlDeviceGetCurrentClocksEventReasons(self.h)
+                except Exception:
+                    bits = nv.nvmlDeviceGetCurrentClocksThrottleReasons(self.h)
+                self.reason_bits |= int(bits)
+                self.power.append(nv.nvmlDeviceGetPowerUsage(self.h) / 1000.0)
+            except Exception:
+                pass
+            self._stop.wait(self.period)
+
+    def start(self):
+        if self.h is not None:
+            self._thr = threading.Thread(target=self._loop, daemon=True)
+            self._thr.start()
+
+    def stop(self) -> dict:
+        if self._thr is None:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvml unavailable"]}
+        self._stop.set()
+        self._thr.join()
+        reasons = [name for bit, name in self.REASONS.items() if self.reason_bits & bit]
+        return {"sm_mhz": float(np.median(self.samples)) if self.samples else None, "sm_max_mhz": self.max_mhz,
+                "reasons": reasons, "samples": len(self.samples),
+                "power_w_max": max(self.power) if self.power else None}
+
+
+# ---------------------------------------------------------------------------------------------- reference arm
+def oracle_sample_problem(prob, L_s: int):
+    """The same workload restricted to its first L_s site patterns (full tree, every branch matrix)."""
+    import copy
+    q = copy.copy(prob)
+    q.L = L_s
+    q.tip_states = np.ascontiguousarray(prob.tip_states[:, :L_s])
+    q.pattern_weights = np.ascontiguousarray(prob.pattern_weights[:L_s])
+    return q
+
+
+def time_oracle(prob, target_s: float, steps: int = 1, warmup: int = 0):
+    """Time the oracle's evaluate() on a pattern sample sized (from a 32-pattern probe) to ~target_s per step.
+    The long-double build is timed: the oracle does no rescaling (reading A12), so its double build
+    underflows on a 2000-tip tree (site likelihoods ~1e-1200) and cannot run this workload."""
+    import oracle
+    orc = oracle.Oracle("ld")
+    cores = int(os.environ.get("OMP_NUM_THREADS", 0)) or len(os.sched_getaffinity(0))
+    probe = oracle_sample_problem(prob, min(32, prob.L))
+    t0 = time.perf_counter()
+    orc.evaluate(probe)
+    t_probe = time.perf_counter() - t0
+    L_s = int(min(prob.L, max(32, 32 * target_s / max(t_probe, 1e-6))))
+    sample = oracle_sample_problem(prob, L_s)
+    for _ in range(warmup):
+        orc.evaluate(sample)
+    times = []
+    for _ in range(steps):
+        t0 = time.perf_counter()
+        out = orc.evaluate(sample)
+        times.append(time.perf_counter() - t0)
+    nbytes = pruning_bytes(sample)
+    sec = float(np.mean(times))
+    return {"value": (nbytes["a5"] + nbytes["a6"]) / sec / 1e9, "unit": UNIT, "cores": cores, "kind": "oracle",
+            "sample": f"first {L_s} of {prob.L} site patterns of config 2, full 2000-tip tree, all {prob.n_br} x {prob.C} "
+                      f"branch matrices; oracle long-double build with OpenMP, {sec:.2f} s per pass",
+            "seconds_per_step": sec, "lnl_sample": float(out["lnl"])}
+
+
+def run_reference(args) -> None:
+    if int(os.environ.get("RANK", "0")) != 0:
+        return
+    prob = W.make_config(2)
+    # bounded: (steps + warmup) passes of ~target seconds each, the whole run within a few minutes
+    target = min(10.0, 150.0 / max(1, args.steps + args.warmup))
+    r = time_oracle(prob, target, steps=args.steps, warmup=args.warmup)
+    line = {"impl": "reference", "metric": METRIC, "value": r["value"], "unit": UNIT, "n_gpus": args.gpus,
+            "steps": args.steps, "warmup": args.warmup, "ms_per_step": r["seconds_per_step"] * 1e3,
+            "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "config": {"workload": W.CONFIG_NAMES[2], "K": prob.K, "M": prob.M, "C": prob.C, "N_tips": prob.N,
+                       "L": prob.L, "note": "CPU oracle on a bounded pattern sample; rank 0 only"},
+            "cpu_baseline": {k: r[k] for k in ("value", "unit", "cores", "kind", "sample")},
+            "e2e": {"value": r["value"], "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+            "gpu_launches": 0}
+    print(json.dumps(line), flush=True)
+
+
+# ---------------------------------------------------------------------------------------------- CUDA arm
+def load_peaks():
+    path = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(path):
+        p = json.load(open(path))
+        return float(p["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs)"
+    return 6650.0, "fallback (B200_PROFILING.md)"
+
+
+def bracket(torch, stream, fn, steps):
+    """Device time in ms of `steps` calls of fn(), CUDA events on the launching stream, synchronised on both sides."""
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    stream.synchronize()
+    e0.record(stream)
+    for _ in range(steps):
+        fn()
+    e1.record(stream)
+    stream.synchronize()
+    return e0.elapsed_time(e1)
+
+
+def run_cuda(args) -> None:
+    import torch
+    import torch.distributed as dist
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device -- the hot path has no CPU fallback (use --impl reference for the oracle)")
+    rank, world = int(os.environ.get("RANK", "0")), int(os.environ.get("WORLD_SIZE", "1"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if world > 1:
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+    torch.cuda.set_device(local)
+    from paper_1309_3075_b200 import build as B
+    if rank == 0:
+        B.build_library()
+    if world > 1:
+        dist.barrier()
+    import paper_1309_3075_b200 as epx
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    def max_over_ranks(x: float) -> float:
+        if world == 1:
+            return x
+        t = torch.tensor([x], dtype=torch.float64, device="cuda")
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        return float(t.item())
+
+    K, Wm = args.steps, max(3, args.warmup)
+    prob = W.make_config(2)
+    nb = pruning_bytes(prob)
+    unit_bytes = nb["a5"] + nb["a6"]
+    ctx = epx.from_problem(prob, device=local)
+    ctx.set_option(epx.EPX_OPT_STAGE_EVENTS, 1)
+    stream = ctx.stream
+    lnl = None
+    for _ in range(Wm):
+        lnl = ctx.log_likelihood()
+    assert ctx.status() == 0 and np.isfinite(lnl)
+
+    clocks = ClockSampler(local)
+    clocks.start()
+    # (1) headline: K steps back to back, inputs resident in HBM; every step re-runs a1..a6 (nothing is cached)
+    launches0 = ctx.launch_count()
+    barrier()
+    ms_total = bracket(torch, stream, ctx.enqueue_log_likelihood, K)
+    barrier()
+    gpu_launches = ctx.launch_count() - launches0
+    assert abs(ctx.fetch_log_likelihood() - lnl) <= 1e-12 * abs(lnl)
+    ms_step = max_over_ranks(ms_total / K)
+
+    # (2) roofline of the dominant kernel: the same K steps with the per-stage CUDA events read after every step
+    stage_ms = np.zeros(5)
+    stage_launches = None
+    for _ in range(K):
+        ctx.enqueue_log_likelihood()
+        ms, stage_launches = ctx.get_stage_ms()
+        stage_ms += ms
+    stage_ms /= K
+
+    # (3) end to end through the C ABI with HOST buffers: every setter (host -> device copies) + log_likelihood
+    #     (device -> host read of logL and the status word) inside the timed region
+    def e2e_step():
+        epx.set_problem(ctx, prob)
+        return ctx.log_likelihood()
+    Ke = max(3, min(K, 20))
+    for _ in range(2):
+        e2e_step()
+    barrier()
+    ms_e2e = bracket(torch, stream, e2e_step, Ke) / Ke
+    barrier()
+    ms_e2e = max_over_ranks(ms_e2e)
+    n_nodes = prob.n_nodes
+    h2d = (prob.N * prob.L + 8 * prob.L + 4 * n_nodes + 8 * n_nodes + 32 * (prob.N - 1) + 8 * prob.M * prob.K * prob.K +
+           8 * prob.M * prob.K + 8 * (prob.M - 1) + 16 * prob.C + 8 * prob.K)
+    clk = clocks.stop()
+    levels = ctx.tree_levels()
+    ws_bytes = ctx.workspace_bytes()
+    ctx.close()
+
+    hbm_peak, peak_src = load_peaks()
+    prune_ms = float(stage_ms[3])
+    prune_launches = int(stage_launches[3])
+    roofline = {"bound": "hbm", "kernel": "prune4_kernel<4> (a5; one launch per post-order level, CUDA graph)",
+                "achieved": nb["a5"] / (prune_ms * 1e-3) / 1e9, "peak": hbm_peak, "unit": "GB/s",
+                "frac": nb["a5"] / (prune_ms * 1e-3) / 1e9 / hbm_peak, "traffic": args.traffic,
+                "peak_source": peak_src, "launches_per_step": prune_launches,
+                "algorithmic_bytes_per_launch": nb["a5"] / prune_launches,
+                "avg_launch_ms": prune_ms / prune_launches, "share_of_step": prune_ms / float(stage_ms.sum()),
+                "stage_ms": {n: float(v) for n, v in zip(epx.STAGE_NAMES, stage_ms)}}
+
+    line = {"metric": METRIC, "value": world * unit_bytes / (ms_step * 1e-3) / 1e9, "unit": UNIT, "n_gpus": world,
+            "steps": K, "warmup": Wm, "ms_per_step": ms_step, "higher_is_better": True, "scaling": "weak",
+            "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "config": {"workload": W.CONFIG_NAMES[2], "K": prob.K, "M": prob.M, "C": prob.C, "N_tips": prob.N,
+                       "L": prob.L, "tree_levels": levels, "parallelism": f"replicas x{world} (no collective)",
+                       "l2": f"inputs larger than L2: {ws_bytes / 1e9:.2f} GB workspace, 2.56 GB of partials rewritten "
+                             "every step vs 126 MB L2", "seed": W.config_seed(2)},
+            "roofline": roofline,
+            "e2e": {"value": world * unit_bytes / (ms_e2e * 1e-3) / 1e9, "unit": UNIT, "h2d_bytes_per_step": h2d,
+                    "d2h_bytes_per_step": 12, "ms_per_step": ms_e2e, "steps": Ke,
+                    "what": "all epx_set_* calls from host arrays + epx_log_likelihood (syncs, reads logL + status)"},
+            "gpu_launches": int(gpu_launches), "clocks": clk, "log_likelihood": lnl,
+            "matrices_per_s_cfg2": world * prob.n_br * prob.C / (float(stage_ms[:3].sum()) * 1e-3)}
+
+    if rank == 0 and not args.no_matrices:
+        line["matrices"] = bench_matrices(torch, epx, local, K)
+    if rank == 0 and not args.no_cpu_baseline and world == 1:
+        r = time_oracle(prob, 15.0)
+        line["cpu_baseline"] = {k: r[k] for k in ("value", "unit", "cores", "kind", "sample")}
+    if world > 1:
+        dist.barrier()
+        dist.destroy_process_group()
+    if rank == 0:
+        print(json.dumps(line), flush=True)
+
+
+def bench_matrices(torch, epx, device: int, K: int) -> dict:
+    """Second half of the metric: config 5 (61-state matrix-convolution microbenchmark, a1..a4 only)."""
+    prob = W.make_config(5)
+    nseg = n_segments(prob)
+    fl = chain_flops(prob.K, prob.C, nseg)
+    ctx = epx.from_problem(prob, device=device)
+    ctx.set_option(epx.EPX_OPT_STAGE_EVENTS, 1)
+    steps = max(3, min(K, 10))
+    for _ in range(3):
+        ctx.update_matrices()
+    assert ctx.status() == 0
+    n0 = ctx.launch_count()
+    ms = bracket(torch, ctx.stream, ctx.update_matrices, steps) / steps
+    launches = ctx.launch_count() - n0
+    stage = np.zeros(5)
+    for _ in range(steps):
+        ctx.update_matrices()
+        m, _ = ctx.get_stage_ms()
+        stage += m
+    stage /= steps
+    ctx.close()
+    dfma = epx.measure_fp64_peak(0, 200.0, device)
+    dmma = epx.measure_fp64_peak(1, 200.0, device)
+    chain_ms = float(stage[2])
+    achieved = fl["executed"] / (chain_ms * 1e-3) / 1e12
+    n_mat = prob.n_br * prob.C
+    return {"metric": "epoch branch matrices/s (fp64)", "value": n_mat / (ms * 1e-3), "unit": "matrices/s",
+            "ms_per_step": ms, "steps": steps, "gpu_launches": int(launches),
+            "config": {"workload": W.CONFIG_NAMES[5], "K": prob.K, "M": prob.M, "C": prob.C, "n_br": prob.n_br,
+                       "segments": int(nseg.sum()), "l2": "2.38 GB of P written per step vs 126 MB L2"},
+            "roofline": {"bound": "alu", "kernel": "chain_dmma64_kernel (a3+a4 fused, mma.sync m8n8k4 f64)",
+                         "achieved": achieved, "peak": dmma, "unit": "TFLOP/s", "frac": achieved / dmma,
+                         "traffic": None, "peak_source": "measured in this run by epx_measure_fp64_peak "
+                                                         "(register-only DMMA m8n8k4 loop); DFMA peak beside it",
+                         "peak_dfma": dfma, "frac_of_dfma": achieved / dfma,
+                         "flops_executed_useful": fl["executed"], "flops_straightforward": fl["straightforward"],
+                         "output_GBps": n_mat * prob.K * prob.K * 8 / (chain_ms * 1e-3) / 1e9,
+                         "stage_ms": {n: float(v) for n, v in zip(epx.STAGE_NAMES, stage)}}}
+
+
+def main() -> None:
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=100)
+    ap.add_argument("--warmup", type=int, default=5)
+    ap.add_argument("--impl", choices=["cuda", "reference"], default="cuda")
+    ap.add_argument("--no-matrices", action="store_true", help="skip the config-5 matrices/s leg")
+    ap.add_argument("--no-cpu-baseline", action="store_true", help="skip timing the oracle on the host cores")
+    ap.add_argument("--traffic", type=float, default=None,
+                    help="dram bytes per launch of the dominant kernel from the committed ncu capture (profiles/)")
+    args = ap.parse_args()
+    if args.impl == "reference":
+        if args.steps == 100 and args.warmup == 5:
+            args.steps, args.warmup = 5, 1
+        run_reference(args)
+    else:
+        run_cuda(args)
+
+
+if __name__ == "__main__":
+    main()

@@ -116,8 +116,23 @@ int epx_get_site_log_likelihoods(epx_ctx* ctx, double* out);
 /* ---- introspection ---- */
 /* Number of kernel launches (graph nodes count individually) the ctx has enqueued since create. */
 int epx_launch_count(const epx_ctx* ctx, long long* n);
-/* Device time in ms of each stage of the LAST compute call is not recorded by the library; time the stream. */
 const char* epx_last_error(const epx_ctx* ctx);
+
+/* Stages of a compute call, in enqueue order. */
+enum {
+    EPX_STAGE_SEGMENT = 0, /* a1 */
+    EPX_STAGE_EIGEN = 1,   /* a2 Jacobi + change-of-basis prep (0 launches on the Pade / Taylor paths) */
+    EPX_STAGE_CHAIN = 2,   /* a2' + a3 + a4 */
+    EPX_STAGE_PRUNE = 3,   /* a5, one launch per post-order level */
+    EPX_STAGE_ROOT = 4,    /* a6 */
+    EPX_N_STAGES = 5
+};
+/* With EPX_OPT_STAGE_EVENTS = 1 every compute call records a CUDA event on the stream before the first stage and
+ * after each stage (inside the CUDA graph when one is used).  This call synchronises the stream and writes the device
+ * time of each stage of the LAST compute call to ms[EPX_N_STAGES] and the number of kernels each stage launched to
+ * launches[EPX_N_STAGES] (either may be NULL).  Stages the call did not run report 0 ms / 0 launches.
+ * EPX_E_STATE if the option is off or nothing has run. */
+int epx_get_stage_ms(epx_ctx* ctx, float* ms, int* launches);
 
 /* Measured fp64 peak on `device`: kind 0 = DFMA (plain FP64 FMA pipe), kind 1 = DMMA (mma.sync m8n8k4 f64).
  * Runs a register-only kernel for about `ms_target` ms on `cuda_stream` and writes TFLOP/s (2 flop per FMA) to
@@ -130,12 +145,13 @@ enum {
     EPX_OPT_CHAIN_KERNEL = 1, /* 0 auto (default); 1 force the generic shared-memory chain kernel */
     EPX_OPT_USE_GRAPH = 2,    /* 1 (default) replay the kernel sequence from a CUDA graph on non-default streams; 0 launch directly */
     EPX_OPT_PRUNE_KERNEL = 3, /* 0 auto (default); 1 force the generic shared-memory pruning kernel */
-    EPX_OPT_EXP_METHOD = 4    /* a3 method.  1 spectral: Jacobi eigensystem (reversible) / Pade 13 (asymmetric), absolute
+    EPX_OPT_EXP_METHOD = 4,   /* a3 method.  1 spectral: Jacobi eigensystem (reversible) / Pade 13 (asymmetric), absolute
                                  error ~1e-14 per entry.  2 componentwise: shifted non-negative Taylor scaling-and-squaring,
                                  every entry to a few hundred ulp RELATIVE, ~8 dense products per segment.  0 auto (default):
                                  2 for tree-mode (likelihood) contexts whose reversible Q have structural zeros (codon
                                  models: entries of P that vanish like t^2, t^3 decide the likelihood of short branches),
                                  else 1.  This one DOES change results, within the tolerances above (A21). */
+    EPX_OPT_STAGE_EVENTS = 5  /* 1 record per-stage CUDA events for epx_get_stage_ms; 0 (default) none */
 };
 int epx_set_option(epx_ctx* ctx, int option, int value);
 /* Device status word of the last compute call (0 = all numeric checks passed); synchronises. */

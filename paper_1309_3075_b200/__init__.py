@@ -17,7 +17,8 @@ _HERE = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.path.join(_HERE, "libepx.so")
 
 EPX_OK, EPX_E_ARG, EPX_E_STATE, EPX_E_TREE, EPX_E_MODEL, EPX_E_WORKSPACE, EPX_E_CUDA, EPX_E_NUMERIC = 0, -1, -2, -3, -4, -5, -6, -7
-EPX_OPT_CHAIN_KERNEL, EPX_OPT_USE_GRAPH, EPX_OPT_PRUNE_KERNEL, EPX_OPT_EXP_METHOD = 1, 2, 3, 4
+EPX_OPT_CHAIN_KERNEL, EPX_OPT_USE_GRAPH, EPX_OPT_PRUNE_KERNEL, EPX_OPT_EXP_METHOD, EPX_OPT_STAGE_EVENTS = 1, 2, 3, 4, 5
+STAGE_NAMES = ("segment", "eigen", "chain", "prune", "root")
 
 _lib = None
 
@@ -68,6 +69,7 @@ def lib():
     _sig(L, "epx_get_site_log_likelihoods", i, vp, dp)
     _sig(L, "epx_launch_count", i, vp, ct.POINTER(ct.c_longlong))
     _sig(L, "epx_tree_levels", i, vp, ct.POINTER(i))
+    _sig(L, "epx_get_stage_ms", i, vp, ct.c_void_p, ct.c_void_p)
     _sig(L, "epx_status", i, vp, ct.POINTER(i))
     _sig(L, "epx_set_option", i, vp, i, i)
     _sig(L, "epx_last_error", ct.c_char_p, vp)
@@ -265,6 +267,13 @@ class Epx:
         n = ct.c_longlong()
         self._check(self._L.epx_launch_count(self._ctx, ct.byref(n)))
         return int(n.value)
+
+    def get_stage_ms(self):
+        """(ms[5], launches[5]) of the last compute call's stages (needs EPX_OPT_STAGE_EVENTS = 1); synchronises."""
+        ms = np.zeros(5, dtype=np.float32)
+        ln = np.zeros(5, dtype=np.int32)
+        self._check(self._L.epx_get_stage_ms(self._ctx, _ptr(ms), _ptr(ln)))
+        return ms, ln
 
     def tree_levels(self) -> int:
         n = ct.c_int()

@@ -194,6 +194,7 @@ void epx_destroy(epx_ctx* c)
 {
     if (!c) return;
     drop_graphs(c);
+    for (cudaEvent_t e : c->ev) if (e) cudaEventDestroy(e);
     delete c;
 }
 
@@ -238,6 +239,7 @@ int epx_set_option(epx_ctx* c, int option, int value)
         case 2: c->use_graph = value; break;
         case 3: c->prune_kernel = value; break;
         case 4: if (value < 0 || value > 2) return fail(c, EPX_E_ARG, "exp method %d", value); c->exp_method = value; break;
+        case 5: c->stage_events = value ? 1 : 0; break;
         default: return fail(c, EPX_E_ARG, "unknown option %d", option);
     }
     drop_graphs(c);

@@ -114,6 +114,12 @@ struct epx_ctx {
     long long graph_mat_nodes = 0, graph_lik_nodes = 0;
     bool graphs_valid = false;
 
+    // EPX_OPT_STAGE_EVENTS: ev[0] before the first stage, ev[k+1] after stage k (created lazily, destroyed with the ctx)
+    int stage_events = 0;
+    cudaEvent_t ev[6] = {nullptr, nullptr, nullptr, nullptr, nullptr, nullptr};
+    int stage_launches_mat[5] = {0, 0, 0, 0, 0}, stage_launches_lik[5] = {0, 0, 0, 0, 0};
+    bool capturing = false;   // enqueue_kernels is running under stream capture
+
     long long launches = 0;
     bool have_result = false;
     bool have_lik = false;   // the last compute call included a5/a6
