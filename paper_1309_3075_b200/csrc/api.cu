@@ -55,9 +55,11 @@ size_t plan_workspace(const epx_ctx* c, char* base, DevBuffers* d)
     if (c->tree_mode) {
         t.parent = (int32_t*)take(4 * S);
         t.height = (double*)take(8 * S);
-        t.tips = (uint8_t*)take(N * L);
+        t.tips = (uint8_t*)take(N * (size_t)c->Lp);
         t.pattern_wt = (double*)take(8 * L);
         t.ops = (PruneOp*)take(sizeof(PruneOp) * (N - 1));
+        t.dfs_ops = (DfsOp*)take(sizeof(DfsOp) * (N - 1));
+        t.dfs_pieces = (DfsPiece*)take(sizeof(DfsPiece) * (N - 1));
     } else {
         t.child_h = (double*)take(8 * S);
         t.parent_h = (double*)take(8 * S);
@@ -155,6 +157,115 @@ int build_plan(epx_ctx* c)
     for (int l = 1; l <= max_level; l++) offs[l] = offs[l - 1] + c->level_off[l];
     c->level_off = offs;               // ops of level l (1-based) are [offs[l-1], offs[l])
     c->root = root;
+
+    // Depth-first post-order walk for prune4_dfs_kernel.  Every internal node becomes one DfsOp; the child visited
+    // SECOND hands its result over in registers, the child visited FIRST parks its result in a stack slot.  Visiting
+    // the subtree that needs more slots first (Sethi-Ullman) keeps the stack at <= log2(N) + 1 slots.
+    // One warp walks one piece for one tile of patterns.  With few patterns a single walk of the whole tree leaves the
+    // SMs short of warps, so the tree is cut into independent subtrees (bottom pieces, one launch) and the part above
+    // them (top piece, a second launch that reads the bottom pieces' root partials from HBM).
+    std::vector<int> size(n, 0), need(n, 0);
+    for (int k = n - 1; k >= 0; k--) {
+        int u = order[k];
+        if (left[u] >= 0) size[u] = 1 + size[left[u]] + size[right[u]];
+    }
+    std::vector<char> is_cut(n, 0);           // roots of the bottom pieces
+    std::vector<int> cuts;
+    {
+        const int lanes = c->C <= 1 ? 1 : c->C <= 2 ? 2 : c->C <= 4 ? 4 : 8;
+        const long tiles = (c->L + 32 / lanes - 1) / (32 / lanes);
+        const long want = std::min<long>(64, 4 * ((148L * 16 + tiles - 1) / tiles));   // pieces wanted (1 = no cut)
+        std::vector<int> heap{root};          // max-heap on subtree size
+        auto cmp = [&](int x, int y) { return size[x] < size[y]; };
+        while (want >= 8 && (long)heap.size() + (long)cuts.size() < want) {
+            std::pop_heap(heap.begin(), heap.end(), cmp);
+            int u = heap.back(); heap.pop_back();
+            if (size[u] <= 8) { heap.push_back(u); std::push_heap(heap.begin(), heap.end(), cmp); break; }
+            for (int ch : {left[u], right[u]})
+                if (left[ch] >= 0) {
+                    if (size[ch] <= 8) cuts.push_back(ch);
+                    else { heap.push_back(ch); std::push_heap(heap.begin(), heap.end(), cmp); }
+                }
+            if (heap.empty()) break;
+        }
+        if (!(heap.size() == 1 && heap[0] == root && cuts.empty())) for (int u : heap) cuts.push_back(u);
+        else cuts.push_back(root);
+        std::sort(cuts.begin(), cuts.end(), [&](int x, int y) { return size[x] != size[y] ? size[x] > size[y] : x < y; });
+        for (int u : cuts) is_cut[u] = 1;
+    }
+    const bool has_top = !(cuts.size() == 1 && cuts[0] == root);
+    // kind of a child as seen from the piece being walked: 0 tip, 1 internal (walk into it), 2 root of a bottom piece
+    auto kind = [&](int v, bool top) { return left[v] < 0 ? 0 : (top && is_cut[v]) ? 2 : 1; };
+    for (int pass = 0; pass < 2; pass++) {     // need[] below the cuts, then above them
+        for (int k = n - 1; k >= 0; k--) {
+            int u = order[k];
+            if (left[u] < 0) continue;
+            int ka = kind(left[u], pass == 1), kb = kind(right[u], pass == 1);
+            int na = ka == 1 ? need[left[u]] : 0, nb = kb == 1 ? need[right[u]] : 0;
+            if (pass == 1 && is_cut[u]) continue;             // keep the bottom value
+            if (ka == 1 && kb == 1) need[u] = std::max(std::max(na, nb), std::min(na, nb) + 1);
+            else need[u] = std::max(1, std::max(na, nb));
+        }
+        if (!has_top) break;
+    }
+    struct Frame { int u, first, second, stage, slot; };
+    std::vector<Frame> fr;
+    std::vector<int> free_slots;
+    int high = 0;
+    c->dfs_ops.clear();
+    c->dfs_ops.reserve(internal.size());
+    c->dfs_pieces.clear();
+    auto walk = [&](int piece_root, bool top) {
+        const int begin = (int)c->dfs_ops.size();
+        free_slots.clear();
+        int next_slot = 0;
+        auto push_node = [&](int u) {
+            int a = left[u], b = right[u];
+            bool ia = kind(a, top) == 1, ib = kind(b, top) == 1;
+            // first = the walked child with the larger need (or the leaf when only one child is walked)
+            if ((ia && ib && need[b] > need[a]) || (ia && !ib)) std::swap(a, b);
+            fr.push_back({u, a, b, 0, -1});
+        };
+        push_node(piece_root);
+        while (!fr.empty()) {
+            const size_t topi = fr.size() - 1;
+            Frame f = fr[topi];
+            const int k1 = kind(f.first, top), k2 = kind(f.second, top);
+            if (f.stage == 0) {
+                fr[topi].stage = 1;
+                if (k1 == 1) { push_node(f.first); continue; }
+                f.stage = 1;
+            }
+            if (f.stage == 1) {
+                if (k1 == 1) {     // the op just emitted is `first`: park its result
+                    int s;
+                    if (!free_slots.empty()) { s = free_slots.back(); free_slots.pop_back(); }
+                    else s = next_slot++;
+                    c->dfs_ops.back().code |= (s + 1) << 16;
+                    fr[topi].slot = f.slot = s;
+                }
+                fr[topi].stage = 2;
+                if (k2 == 1) { push_node(f.second); continue; }
+            }
+            DfsOp op{};
+            op.a = f.first; op.b = f.second; op.pidx = c->node_pidx[f.u];
+            const int srcA = k1 == 1 ? f.slot : k1 == 2 ? EPX_DFS_HBM : EPX_DFS_TIP;
+            const int srcB = k2 == 1 ? EPX_DFS_PREV : k2 == 2 ? EPX_DFS_HBM : EPX_DFS_TIP;
+            op.pa = k1 == 2 ? c->node_pidx[f.first] : 0;
+            op.pb = k2 == 2 ? c->node_pidx[f.second] : 0;
+            op.code = (srcA + 3) | ((srcB + 3) << 8);
+            if (f.slot >= 0) free_slots.push_back(f.slot);
+            c->dfs_ops.push_back(op);
+            fr.pop_back();
+        }
+        high = std::max(high, next_slot);
+        c->dfs_pieces.push_back({begin, (int)c->dfs_ops.size()});
+    };
+    for (int u : cuts) walk(u, false);
+    c->dfs_bottom = (int)cuts.size();
+    if (has_top) walk(root, true);
+    c->dfs_depth = std::max(high, 1);
+    if (high > 250) return fail(c, EPX_E_TREE, "tree needs %d pruning stack slots (limit 250)", high);
     return EPX_OK;
 }
 
@@ -181,6 +292,7 @@ int epx_create(epx_ctx** out, int K, int M, int C, int N_tips, int L, int device
     c->model_set.assign(M, 0);
     c->model_sparse.assign(M, 0);
     if (c->tree_mode) {
+        c->Lp = (L + 31) & ~31;
         c->pattern_wt.assign(L, 1.0);
         c->wt_dirty = true;
         c->reduce_blocks = (L + 255) / 256;
@@ -365,12 +477,16 @@ int epx_set_tip_states(epx_ctx* c, const int32_t* states)
 {
     if (!c || !states) return EPX_E_ARG;
     if (!c->tree_mode) return fail(c, EPX_E_STATE, "ctx is in branch-list mode");
-    const size_t n = (size_t)c->N * c->L;
-    c->tips.resize(n);
+    const size_t L = (size_t)c->L, Lp = (size_t)c->Lp;
+    c->tips.assign((size_t)c->N * Lp, (uint8_t)255);
     const int K = c->K;
-    for (size_t i = 0; i < n; i++) {
-        int32_t s = states[i];
-        c->tips[i] = (s >= 0 && s < K) ? (uint8_t)s : (uint8_t)255;
+    for (size_t t = 0; t < (size_t)c->N; t++) {
+        const int32_t* src = states + t * L;
+        uint8_t* dst = c->tips.data() + t * Lp;
+        for (size_t p = 0; p < L; p++) {
+            int32_t s = src[p];
+            dst[p] = (s >= 0 && s < K) ? (uint8_t)s : (uint8_t)255;
+        }
     }
     c->has_tips = true; c->tips_dirty = true;
     return EPX_OK;

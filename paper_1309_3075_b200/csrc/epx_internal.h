@@ -27,6 +27,25 @@ struct PruneOp {
     int cpidx[2];    // same for internal children (unused for tips)
 };
 
+// One operation of the depth-first pruning walk (prune4_dfs_kernel): node = product of its FIRST child (a) and its
+// SECOND child (b).  code = (srcA+3) | (srcB+3) << 8 | (out_slot+1) << 16 with
+//   src: -3 partials of another piece, read from HBM (pa / pb = its index in the partials array)
+//        -2 tip   -1 result of the previous operation, still in registers (second child only)
+//        >= 0 shared-memory stack slot (first child only)
+//   out_slot: -1 = consumed by the next operation or by another launch; else the stack slot the result is parked in.
+struct __align__(16) DfsOp {
+    int32_t a, b;        // child node ids (matrix slot, tip row)
+    int32_t pidx;        // this node's index in the partials array
+    int32_t code;
+    int32_t pa, pb;      // partials index of an HBM-sourced child
+    int32_t pad0, pad1;
+};
+#define EPX_DFS_HBM (-3)
+#define EPX_DFS_TIP (-2)
+#define EPX_DFS_PREV (-1)
+// A piece of the tree walked by one warp per pattern tile: operations [begin, end) of the DfsOp array.
+struct DfsPiece { int32_t begin, end; };
+
 // All device pointers, carved out of the caller's workspace by plan_workspace().
 struct DevBuffers {
     // inputs
@@ -40,9 +59,11 @@ struct DevBuffers {
     double* height;       // [n_nodes] tree mode
     double* child_h;      // [n_br] branch-list mode
     double* parent_h;     // [n_br] branch-list mode
-    uint8_t* tips;        // [N][L]  0..K-1, 255 = missing
+    uint8_t* tips;        // [N][Lp] 0..K-1, 255 = missing; rows padded to Lp = L rounded up to 32
     double* pattern_wt;   // [L]
     PruneOp* ops;         // [N-1] sorted by level
+    DfsOp* dfs_ops;       // [N-1] depth-first post-order (K == 4 pruning walk), piece after piece
+    DfsPiece* dfs_pieces; // [<= N-1] op ranges of the pieces: bottom pieces (largest first), then the top piece
     // a1
     int32_t* n_seg;       // [n_br]
     int32_t* e_hi;        // [n_br] epoch of the parent end
@@ -99,6 +120,11 @@ struct epx_ctx {
     std::vector<PruneOp> ops;
     std::vector<int> level_off;        // ops[level_off[l] .. level_off[l+1]) form level l
     std::vector<int> node_pidx;        // node -> index in partials (internal) or -1
+    std::vector<DfsOp> dfs_ops;        // depth-first post-order walk with its stack-slot allocation
+    std::vector<DfsPiece> dfs_pieces;  // bottom pieces (independent subtrees, largest first), then the top piece if any
+    int dfs_bottom = 0;                // number of bottom pieces (launch 1); the rest (0 or 1) is launch 2
+    int dfs_depth = 0;                 // stack slots the walk needs
+    int Lp = 0;                        // L rounded up to a multiple of 32 (row stride of the tip-state array)
     int root = -1;
     int reduce_blocks = 0;
 
@@ -151,3 +177,10 @@ int pade_init_attributes();
 int eigen_init_attributes();
 int prune_init_attributes();
 int prune_tile(int K, int C);   // patterns per CTA of the generic pruning kernel
+bool prune_uses_dfs(const epx_ctx* c);   // K == 4 depth-first walk: partials are laid out [node][L][C][4]
+// element (category c, pattern p, state i) of a node's partials sits at c * sc + p * sp + i
+inline void partial_strides(const epx_ctx* c, size_t& sc, size_t& sp)
+{
+    if (prune_uses_dfs(c)) { sc = (size_t)c->K; sp = (size_t)c->C * c->K; }
+    else { sc = (size_t)c->L * c->K; sp = (size_t)c->K; }
+}

@@ -8,9 +8,16 @@
 // divided by 2^e with e = floor(log2(max over category and state)), which is exact in binary floating point; the
 // exponents accumulate up the tree and re-enter at the root as e * ln 2.
 //
-//   prune4_kernel<C>   K == 4: one thread per pattern, all C categories in registers; child partials stream as
-//                      256-bit loads (LDG.E.256), fully coalesced ([C][L][4] is pattern-contiguous per category),
-//                      tips are read as one byte per pattern; one 256-bit store per category.  HBM-bound.
+//   prune4_dfs_kernel<G>  K == 4 (default): patterns are independent, so a warp that owns a tile of patterns can walk the
+//                      WHOLE tree by itself, depth first, with no inter-CTA synchronisation and no launch per level.
+//                      One thread per (pattern, category); a child's partial vector is either in registers (the
+//                      operation just finished) or in a per-warp shared-memory stack (<= log2 N + 1 slots, host-planned),
+//                      so partials are never re-read from HBM: each node's [L][C][4] block is written once (256-bit
+//                      streaming stores) and the only reads are tip states and the 4x4 matrices, both staged three
+//                      operations ahead with cp.async.  HBM traffic = the partials written, half the level-by-level
+//                      scheme's.
+//   prune4_kernel<C>   K == 4, EPX_OPT_PRUNE_KERNEL = 2: the level-by-level scheme (one launch per post-order level,
+//                      one thread per pattern, child partials re-read with 256-bit loads); kept for comparison.
 //   prune_generic_kernel  any K <= 64: one CTA per (node, tile of patterns); per category the two K x K matrices
 //                      and the child tiles are staged in shared memory, DFMA mat-vec products.
 //   root_site_kernel / final_sum_kernel  per-pattern ln-likelihood, deterministic two-stage weighted sum.
@@ -37,7 +44,7 @@ __device__ __forceinline__ double pow2_neg(int e) { return __hiloint2double((102
 
 // ------------------------------------------------------------------------------------------------ K == 4
 template <int C>
-__global__ void __launch_bounds__(256) prune4_kernel(const PruneOp* __restrict__ ops, int tiles, int L,
+__global__ void __launch_bounds__(256) prune4_kernel(const PruneOp* __restrict__ ops, int tiles, int L, int Lp,
     const double* __restrict__ P, const uint8_t* __restrict__ tips, double* __restrict__ partials,
     int32_t* __restrict__ scale_exp)
 {
@@ -57,7 +64,7 @@ __global__ void __launch_bounds__(256) prune4_kernel(const PruneOp* __restrict__
 #pragma unroll
     for (int ch = 0; ch < 2; ch++) {
         if (op.child_is_tip[ch]) {
-            const int s = tips[(size_t)op.child[ch] * L + p];
+            const int s = tips[(size_t)op.child[ch] * Lp + p];
 #pragma unroll
             for (int c = 0; c < C; c++)
 #pragma unroll
@@ -97,11 +104,235 @@ __global__ void __launch_bounds__(256) prune4_kernel(const PruneOp* __restrict__
     scale_exp[(size_t)op.pidx * L + p] = ex;
 }
 
+
+// ------------------------------------------------------------------------------------------------ K == 4, depth first
+__device__ __forceinline__ uint32_t smem_addr(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
+__device__ __forceinline__ void cp_async16(void* dst, const void* src)
+{
+    asm volatile("cp.async.ca.shared.global [%0], [%1], 16;" ::"r"(smem_addr(dst)), "l"(src) : "memory");
+}
+__device__ __forceinline__ void cp_async4(void* dst, const void* src)
+{
+    asm volatile("cp.async.ca.shared.global [%0], [%1], 4;" ::"r"(smem_addr(dst)), "l"(src) : "memory");
+}
+__device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
+template <int N>
+__device__ __forceinline__ void cp_async_wait() { asm volatile("cp.async.wait_group %0;" ::"n"(N) : "memory"); }
+
+constexpr int DFS_STAGES = 6;          // matrix staging ring: operation k+5 is in flight while operation k computes
+constexpr int DFS_PSTRIDE = 18;        // doubles per staged 4x4 matrix: 144 B, so the G categories of a warp hit distinct banks
+__host__ __device__ constexpr int dfs_lanes_of(int C) { return C <= 1 ? 1 : C <= 2 ? 2 : C <= 4 ? 4 : 8; }
+__host__ __device__ constexpr int dfs_stage_bytes(int G) { return 2 * G * DFS_PSTRIDE * 8; }
+
+__device__ __forceinline__ void matvec4(const double* __restrict__ Pm, const double (&v)[4], double (&f)[4])
+{
+#pragma unroll
+    for (int i = 0; i < 4; i++) {
+        const double2 r01 = *reinterpret_cast<const double2*>(Pm + i * 4), r23 = *reinterpret_cast<const double2*>(Pm + i * 4 + 2);
+        f[i] = fma(r23.y, v[3], fma(r23.x, v[2], fma(r01.y, v[1], r01.x * v[0])));
+    }
+}
+
+// One warp per (piece of the tree, tile of 32/G patterns); lane = (pattern, category), G = lanes per pattern = C rounded
+// up to a power of 2.  Inputs are fetched long before they are needed, so the walk never waits on HBM:
+//   - operation descriptors and tip states: every 32 operations lane j loads descriptor j of the NEXT block of 32 and
+//     that operation's tip bytes for the warp's patterns into registers; operation k reads them with warp shuffles;
+//   - the children's 4x4 matrices: cp.async into a shared-memory ring, DFS_STAGES - 1 operations ahead.
+// Shared memory per warp: DFS_STAGES x [2 children][G][18] doubles, then the stack [depth][32 lanes][4] doubles +
+// [depth][32] exponents.  A lane only ever touches its own stack column, so the stack needs no synchronisation.
+template <int C>
+__global__ void __launch_bounds__(32) prune4_dfs_kernel(const DfsOp* __restrict__ ops, const DfsPiece* __restrict__ pieces,
+    int tiles, int L, int Lp, int depth, const double* __restrict__ P, const uint8_t* __restrict__ tips,
+    double* __restrict__ partials, int32_t* __restrict__ scale_exp)
+{
+    extern __shared__ __align__(16) unsigned char smraw[];
+    constexpr int G = dfs_lanes_of(C);
+    constexpr int PW = 32 / G;                      // patterns per warp
+    constexpr int TW = (PW + 3) / 4;                // 32-bit words of tip states per child
+    constexpr int SB = dfs_stage_bytes(G);
+    constexpr int NCH = (16 * C + 31) / 32;         // 16-byte chunks of the two children's matrices per lane
+    constexpr unsigned FULL = 0xffffffffu;
+    double* stack = reinterpret_cast<double*>(smraw + DFS_STAGES * SB);
+    int* stack_ex = reinterpret_cast<int*>(stack + (size_t)depth * 128);
+    const int lane = threadIdx.x;
+    const int pl = lane / G, c = lane % G, cc = min(c, C - 1);
+    const int piece = blockIdx.x / tiles, tile = blockIdx.x - piece * tiles;
+    const int p0 = tile * PW, p = p0 + pl;
+    const bool live = p < L && c < C;
+    const DfsPiece pc = pieces[piece];
+    const int n_ops = pc.end - pc.begin;
+    ops += pc.begin;
+
+    // per-lane constants of the matrix copies: chunk ch = lane + 32 q -> (child, category, 16-byte word)
+    int cp_dst[NCH], cp_src[NCH];
+    bool cp_child[NCH], cp_on[NCH];
+#pragma unroll
+    for (int q = 0; q < NCH; q++) {
+        const int ch = lane + 32 * q;
+        cp_on[q] = ch < 16 * C;
+        cp_child[q] = ch >= 8 * C;
+        const int r = ch - (cp_child[q] ? 8 * C : 0), cat = r >> 3, w = r & 7;
+        cp_dst[q] = ((cp_child[q] ? G : 0) + cat) * (DFS_PSTRIDE * 8) + w * 16;
+        cp_src[q] = cat * 16 + w * 2;
+    }
+    const size_t node_stride = (size_t)L * C * 4;   // doubles per node of the partials array
+    double* const out_base = partials + ((size_t)p * C + c) * 4;
+    const unsigned char* const tip_base = tips + p0;
+    const double* const Pm_base = reinterpret_cast<const double*>(smraw) + cc * DFS_PSTRIDE;
+
+    struct Block { int4 d; int2 h; uint32_t ta[TW], tb[TW]; };
+    auto load_block = [&](int base) -> Block {      // lane j: descriptor base + j and its tip states
+        Block b;
+        b.d = make_int4(0, 0, 0, 0);
+        b.h = make_int2(0, 0);
+#pragma unroll
+        for (int w = 0; w < TW; w++) { b.ta[w] = 0xffffffffu; b.tb[w] = 0xffffffffu; }
+        const int k = base + lane;
+        if (k < n_ops) {
+            const int4* src = reinterpret_cast<const int4*>(ops + k);
+            b.d = __ldg(src);
+            const int4 h = __ldg(src + 1);
+            b.h = make_int2(h.x, h.y);
+            if ((b.d.w & 0xff) - 3 == EPX_DFS_TIP) {
+                const uint32_t* t = reinterpret_cast<const uint32_t*>(tip_base + (size_t)b.d.x * Lp);
+#pragma unroll
+                for (int w = 0; w < TW; w++) b.ta[w] = __ldg(t + w);
+            }
+            if (((b.d.w >> 8) & 0xff) - 3 == EPX_DFS_TIP) {
+                const uint32_t* t = reinterpret_cast<const uint32_t*>(tip_base + (size_t)b.d.y * Lp);
+#pragma unroll
+                for (int w = 0; w < TW; w++) b.tb[w] = __ldg(t + w);
+            }
+        }
+        return b;
+    };
+    Block cb = load_block(0), nb = load_block(32);
+
+    // stage the matrices of operation j (j in the current or the next block of 32) into ring buffer `buf`
+    auto issue = [&](int j, int k, int buf) {
+        const bool in_cur = (j >> 5) == (k >> 5);
+        const int na = __shfl_sync(FULL, in_cur ? cb.d.x : nb.d.x, j & 31);
+        const int nbn = __shfl_sync(FULL, in_cur ? cb.d.y : nb.d.y, j & 31);
+        unsigned char* sb = smraw + buf * SB;
+#pragma unroll
+        for (int q = 0; q < NCH; q++)
+            if (cp_on[q]) cp_async16(sb + cp_dst[q], P + (size_t)(cp_child[q] ? nbn : na) * (C * 16) + cp_src[q]);
+    };
+#pragma unroll
+    for (int j = 0; j < DFS_STAGES - 1; j++) {
+        if (j < n_ops) issue(j, 0, j);
+        cp_async_commit();
+    }
+
+    double cur[4] = {1.0, 1.0, 1.0, 1.0};
+    int cur_ex = 0;
+    int buf = 0;
+    for (int k = 0; k < n_ops; k++) {
+        if ((k & 31) == 0 && k > 0) { cb = nb; nb = load_block(k + 32); }
+        __syncwarp();                               // every lane is done reading the buffer the next stage overwrites
+        {
+            int nbuf = buf + DFS_STAGES - 1; if (nbuf >= DFS_STAGES) nbuf -= DFS_STAGES;
+            if (k + DFS_STAGES - 1 < n_ops) issue(k + DFS_STAGES - 1, k, nbuf);
+            cp_async_commit();
+        }
+        const int src_lane = k & 31;
+        const int pidx = __shfl_sync(FULL, cb.d.z, src_lane);
+        const int code = __shfl_sync(FULL, cb.d.w, src_lane);
+        const int srcA = (code & 0xff) - 3, srcB = ((code >> 8) & 0xff) - 3, out_slot = ((code >> 16) & 0xff) - 1;
+
+        // operands that do not need the staged matrices yet
+        double va[4], vb[4];
+        int ex = 0, sa = 255, sbt = 255;
+        if (srcA == EPX_DFS_TIP) {
+#pragma unroll
+            for (int w = 0; w < TW; w++) {
+                const uint32_t wa = __shfl_sync(FULL, cb.ta[w], src_lane);
+                if (TW == 1 || (pl >> 2) == w) sa = (wa >> (8 * (pl & 3))) & 0xff;
+            }
+        } else if (srcA == EPX_DFS_HBM) {
+            const int pa = __shfl_sync(FULL, cb.h.x, src_lane);
+            va[0] = va[1] = va[2] = va[3] = 1.0;
+            if (live) {
+                const double4a v = ld256(out_base + (size_t)pa * node_stride);
+                va[0] = v.x; va[1] = v.y; va[2] = v.z; va[3] = v.w;
+                ex += scale_exp[(size_t)pa * L + p];
+            }
+        } else {
+            const double2* sv = reinterpret_cast<const double2*>(stack + ((size_t)srcA * 32 + lane) * 4);
+            const double2 v01 = sv[0], v23 = sv[1];
+            va[0] = v01.x; va[1] = v01.y; va[2] = v23.x; va[3] = v23.y;
+            ex += stack_ex[srcA * 32 + lane];
+        }
+        if (srcB == EPX_DFS_TIP) {
+#pragma unroll
+            for (int w = 0; w < TW; w++) {
+                const uint32_t wb = __shfl_sync(FULL, cb.tb[w], src_lane);
+                if (TW == 1 || (pl >> 2) == w) sbt = (wb >> (8 * (pl & 3))) & 0xff;
+            }
+        } else if (srcB == EPX_DFS_HBM) {
+            const int pb = __shfl_sync(FULL, cb.h.y, src_lane);
+            vb[0] = vb[1] = vb[2] = vb[3] = 1.0;
+            if (live) {
+                const double4a v = ld256(out_base + (size_t)pb * node_stride);
+                vb[0] = v.x; vb[1] = v.y; vb[2] = v.z; vb[3] = v.w;
+                ex += scale_exp[(size_t)pb * L + p];
+            }
+        } else {
+#pragma unroll
+            for (int i = 0; i < 4; i++) vb[i] = cur[i];
+            ex += cur_ex;
+        }
+
+        cp_async_wait<DFS_STAGES - 1>();            // this lane's copies for operation k have landed ...
+        __syncwarp();                               // ... and so have every other lane's
+        const double* Pa = Pm_base + buf * (SB / 8);
+        const double* Pb = Pa + G * DFS_PSTRIDE;
+        double fa[4], fb[4];
+        if (srcA == EPX_DFS_TIP) {
+#pragma unroll
+            for (int i = 0; i < 4; i++) fa[i] = (sa < 4) ? Pa[i * 4 + sa] : 1.0;
+        } else {
+            matvec4(Pa, va, fa);
+        }
+        if (srcB == EPX_DFS_TIP) {
+#pragma unroll
+            for (int i = 0; i < 4; i++) fb[i] = (sbt < 4) ? Pb[i * 4 + sbt] : 1.0;
+        } else {
+            matvec4(Pb, vb, fb);
+        }
+        // all values are >= 0, so the largest one has the largest high word: an integer max finds its exponent
+        int hmax = 0;
+#pragma unroll
+        for (int i = 0; i < 4; i++) { fa[i] *= fb[i]; hmax = max(hmax, __double2hiint(fa[i])); }
+#pragma unroll
+        for (int o = 1; o < G; o <<= 1) hmax = max(hmax, __shfl_xor_sync(FULL, hmax, o));
+        double sc = 1.0;
+        {
+            const int e = (hmax >> 20) - 1023;      // hmax < 0x7fe00000: finite and far from overflow
+            if (e > -1000 && hmax < 0x7fe00000) { sc = pow2_neg(e); ex += e; }
+        }
+#pragma unroll
+        for (int i = 0; i < 4; i++) cur[i] = fa[i] * sc;
+        cur_ex = ex;
+        if (live) st256(out_base + (size_t)pidx * node_stride, cur[0], cur[1], cur[2], cur[3]);
+        if (live && c == 0) scale_exp[(size_t)pidx * L + p] = ex;
+        if (out_slot >= 0) {
+            double2* sv = reinterpret_cast<double2*>(stack + ((size_t)out_slot * 32 + lane) * 4);
+            sv[0] = make_double2(cur[0], cur[1]);
+            sv[1] = make_double2(cur[2], cur[3]);
+            stack_ex[out_slot * 32 + lane] = ex;
+        }
+        if (++buf == DFS_STAGES) buf = 0;
+    }
+}
+
+size_t dfs_smem(int G, int depth) { return (size_t)DFS_STAGES * dfs_stage_bytes(G) + (size_t)depth * (128 * 8 + 32 * 4); }
+
 // ------------------------------------------------------------------------------------------------ any K
 constexpr int GT = 256;
 
 __global__ void __launch_bounds__(GT) prune_generic_kernel(const PruneOp* __restrict__ ops, int tiles, int tile_p,
-    int K, int C, int L, const double* __restrict__ P, const uint8_t* __restrict__ tips,
+    int K, int C, int L, int Lp, const double* __restrict__ P, const uint8_t* __restrict__ tips,
     double* __restrict__ partials, int32_t* __restrict__ scale_exp)
 {
     extern __shared__ double sm[];
@@ -118,7 +349,7 @@ __global__ void __launch_bounds__(GT) prune_generic_kernel(const PruneOp* __rest
 
     for (int ch = 0; ch < 2; ch++)
         if (op.child_is_tip[ch])
-            for (int p = tid; p < np; p += GT) st[ch * tile_p + p] = tips[(size_t)op.child[ch] * L + p0 + p];
+            for (int p = tid; p < np; p += GT) st[ch * tile_p + p] = tips[(size_t)op.child[ch] * Lp + p0 + p];
 
     for (int c = 0; c < C; c++) {
         __syncthreads();
@@ -180,7 +411,7 @@ __global__ void __launch_bounds__(GT) prune_generic_kernel(const PruneOp* __rest
 }
 
 // ------------------------------------------------------------------------------------------------ a6
-__global__ void __launch_bounds__(256) root_site_kernel(int K, int C, int L, int root_pidx, int root_node,
+__global__ void __launch_bounds__(256) root_site_kernel(int K, int C, int L, size_t sc, size_t sp, int root_pidx, int root_node,
     const double* __restrict__ partials, const int32_t* __restrict__ scale_exp, const double* __restrict__ freqs,
     const int32_t* __restrict__ e_hi, const double* __restrict__ root_freqs, const double* __restrict__ weights,
     const double* __restrict__ pattern_wt, double* __restrict__ site_lnl, double* __restrict__ block_sums,
@@ -194,7 +425,7 @@ __global__ void __launch_bounds__(256) root_site_kernel(int K, int C, int L, int
     if (p < L) {
         double site = 0.0;
         for (int c = 0; c < C; c++) {
-            const double* v = partials + (((size_t)root_pidx * C + c) * L + p) * K;
+            const double* v = partials + (size_t)root_pidx * C * L * K + c * sc + p * sp;
             double s = 0.0;
             for (int i = 0; i < K; i++) s = fma(rf[i], v[i], s);
             site = fma(weights[c], s, site);
@@ -241,7 +472,7 @@ template <int C>
 void launch_prune4(const PruneOp* ops, int nops, int L, const DevBuffers& d, cudaStream_t s)
 {
     const int tiles = (L + 255) / 256;
-    prune4_kernel<C><<<nops * tiles, 256, 0, s>>>(ops, tiles, L, d.P, d.tips, d.partials, d.scale_exp);
+    prune4_kernel<C><<<nops * tiles, 256, 0, s>>>(ops, tiles, L, (L + 31) & ~31, d.P, d.tips, d.partials, d.scale_exp);
 }
 
 }  // namespace
@@ -253,15 +484,63 @@ int prune_tile(int K, int C)
     return t;
 }
 
+template <int C>
+static int dfs_set_attr()
+{
+    return cudaFuncSetAttribute(prune4_dfs_kernel<C>, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024) == cudaSuccess ? 0 : -1;
+}
+
 int prune_init_attributes()
 {
+    if (dfs_set_attr<1>() || dfs_set_attr<2>() || dfs_set_attr<3>() || dfs_set_attr<4>() || dfs_set_attr<5>() ||
+        dfs_set_attr<6>() || dfs_set_attr<7>() || dfs_set_attr<8>()) return -1;
     return cudaFuncSetAttribute(prune_generic_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024) == cudaSuccess ? 0 : -1;
+}
+
+bool prune_uses_dfs(const epx_ctx* c)
+{
+    return c->tree_mode && c->K == 4 && c->prune_kernel == 0 &&
+           dfs_smem(dfs_lanes_of(c->C), c->dfs_depth > 0 ? c->dfs_depth : 1) <= 227 * 1024;
+}
+
+template <int C>
+static void launch_dfs(const epx_ctx* c, int first_piece, int n_pieces, cudaStream_t s)
+{
+    const DevBuffers& d = c->d;
+    constexpr int G = dfs_lanes_of(C);
+    const int tiles = (c->L + 32 / G - 1) / (32 / G);
+    prune4_dfs_kernel<C><<<n_pieces * tiles, 32, dfs_smem(G, c->dfs_depth), s>>>(d.dfs_ops, d.dfs_pieces + first_piece, tiles,
+        c->L, c->Lp, c->dfs_depth, d.P, d.tips, d.partials, d.scale_exp);
+}
+
+// Launch 1: the bottom pieces (independent subtrees); launch 2: the top piece, which reads their roots from HBM.
+static int launch_pruning_dfs(const epx_ctx* c, cudaStream_t s)
+{
+    int launched = 0;
+    const int total = (int)c->dfs_pieces.size();
+    for (int pass = 0; pass < 2; pass++) {
+        const int first = pass == 0 ? 0 : c->dfs_bottom, count = pass == 0 ? c->dfs_bottom : total - c->dfs_bottom;
+        if (count <= 0) continue;
+        switch (c->C) {
+            case 1: launch_dfs<1>(c, first, count, s); break;
+            case 2: launch_dfs<2>(c, first, count, s); break;
+            case 3: launch_dfs<3>(c, first, count, s); break;
+            case 4: launch_dfs<4>(c, first, count, s); break;
+            case 5: launch_dfs<5>(c, first, count, s); break;
+            case 6: launch_dfs<6>(c, first, count, s); break;
+            case 7: launch_dfs<7>(c, first, count, s); break;
+            default: launch_dfs<8>(c, first, count, s); break;
+        }
+        launched++;
+    }
+    return cudaGetLastError() == cudaSuccess ? launched : -1;
 }
 
 int launch_pruning(const epx_ctx* c, cudaStream_t s)
 {
     const DevBuffers& d = c->d;
     const int K = c->K, C = c->C, L = c->L;
+    if (prune_uses_dfs(c)) return launch_pruning_dfs(c, s);
     int launched = 0;
     const int n_levels = (int)c->level_off.size() - 1;
     for (int l = 0; l < n_levels; l++) {
@@ -282,7 +561,7 @@ int launch_pruning(const epx_ctx* c, cudaStream_t s)
         } else {
             const int tile_p = prune_tile(K, C);
             const int tiles = (L + tile_p - 1) / tile_p;
-            prune_generic_kernel<<<nops * tiles, GT, generic_smem(K, C, tile_p), s>>>(ops, tiles, tile_p, K, C, L, d.P,
+            prune_generic_kernel<<<nops * tiles, GT, generic_smem(K, C, tile_p), s>>>(ops, tiles, tile_p, K, C, L, c->Lp, d.P,
                                                                                       d.tips, d.partials, d.scale_exp);
         }
         launched++;
@@ -295,7 +574,9 @@ int launch_root_reduction(const epx_ctx* c, cudaStream_t s)
     const DevBuffers& d = c->d;
     const int blocks = c->reduce_blocks;
     const int root_pidx = c->node_pidx[c->root];
-    root_site_kernel<<<blocks, 256, 0, s>>>(c->K, c->C, c->L, root_pidx, c->root, d.partials, d.scale_exp, d.freqs,
+    size_t sc, sp;
+    partial_strides(c, sc, sp);
+    root_site_kernel<<<blocks, 256, 0, s>>>(c->K, c->C, c->L, sc, sp, root_pidx, c->root, d.partials, d.scale_exp, d.freqs,
                                             d.e_hi, c->has_root_freqs ? d.root_freqs : nullptr, d.weights,
                                             d.pattern_wt, d.site_lnl, d.block_sums, d.status);
     final_sum_kernel<<<1, 256, 0, s>>>(blocks, d.block_sums, d.lnl);

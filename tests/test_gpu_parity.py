@@ -91,8 +91,62 @@ def test_config1_generic_kernels_and_no_graph(epx, orc_ld):
 
 
 def test_config2_reduced(epx, orc_ld):
-    # several pattern tiles plus a ragged tail (L = 777 = 3*256 + 9), 10 epochs, dated tips
-    run_tree(epx, orc_ld, W.make_config(2, N=150, L=777))
+    # several pattern tiles plus a ragged tail (L = 777 = 3*256 + 9 = 97*8 + 1), 10 epochs, dated tips
+    prob = W.make_config(2, N=150, L=777)
+    run_tree(epx, orc_ld, prob)                                                  # depth-first walk (default)
+    run_tree(epx, orc_ld, prob, options=[(epx.EPX_OPT_PRUNE_KERNEL, 2)])         # level-by-level register kernel
+    run_tree(epx, orc_ld, prob, options=[(epx.EPX_OPT_PRUNE_KERNEL, 1)])         # generic shared-memory kernel
+
+
+@pytest.mark.parametrize("C", [1, 2, 3, 5, 8])
+def test_k4_every_category_count(epx, orc_ld, C):
+    # lanes per pattern G = 1, 2, 4, 8, 8 with C < G idle lanes; missing tip states; ragged L
+    import dataclasses
+    prob = W.make_config(2, N=40, L=203)
+    rates, weights = W.models.discrete_gamma(0.5, C)
+    tips = prob.tip_states.copy()
+    tips[::3, ::7] = -1
+    tips[5, :] = 99
+    prob = dataclasses.replace(prob, C=C, rates=rates, weights=weights, tip_states=tips)
+    run_tree(epx, orc_ld, prob)
+    run_tree(epx, orc_ld, prob, options=[(epx.EPX_OPT_PRUNE_KERNEL, 2)], partial_nodes=[prob.n_nodes - 1])
+
+
+def _shaped_tree(shape, N):
+    """parent / height arrays of a caterpillar (ladder) or a perfectly balanced tree on N tips, heights in (0, 1]."""
+    parent = np.full(2 * N - 1, -1, dtype=np.int32)
+    height = np.zeros(2 * N - 1)
+    nxt = N
+    if shape == "caterpillar":
+        cur = 0
+        for t in range(1, N):
+            parent[cur] = parent[t] = nxt
+            height[nxt] = t / (N - 1)
+            cur = nxt
+            nxt += 1
+    else:
+        layer, h = list(range(N)), 0
+        while len(layer) > 1:
+            h += 1
+            new = []
+            for i in range(0, len(layer), 2):
+                parent[layer[i]] = parent[layer[i + 1]] = nxt
+                height[nxt] = h
+                new.append(nxt)
+                nxt += 1
+            layer = new
+        height /= height.max()
+    return parent, height
+
+
+@pytest.mark.parametrize("shape,N", [("caterpillar", 33), ("balanced", 64)])
+def test_k4_extreme_tree_shapes(epx, orc_ld, shape, N):
+    # stack depth 1 (every result handed over in registers) and log2(N) (every slot in use)
+    import dataclasses
+    prob = W.make_config(1, N=N, L=100)
+    parent, height = _shaped_tree(shape, N)
+    prob = dataclasses.replace(prob, parent=parent, height=height)
+    run_tree(epx, orc_ld, prob)
 
 
 def test_config2_full_size(epx, orc_ld):
