@@ -174,7 +174,7 @@ int build_plan(epx_ctx* c)
     {
         const int lanes = c->C <= 1 ? 1 : c->C <= 2 ? 2 : c->C <= 4 ? 4 : 8;
         const long tiles = (c->L + 32 / lanes - 1) / (32 / lanes);
-        const long want = std::min<long>(64, 4 * ((148L * 16 + tiles - 1) / tiles));   // pieces wanted (1 = no cut)
+        const long want = std::min<long>(64, 4 * ((148L * 24 + tiles - 1) / tiles));   // pieces wanted (1 = no cut)
         std::vector<int> heap{root};          // max-heap on subtree size
         auto cmp = [&](int x, int y) { return size[x] < size[y]; };
         while (want >= 8 && (long)heap.size() + (long)cuts.size() < want) {

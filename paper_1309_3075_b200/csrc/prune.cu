@@ -119,8 +119,11 @@ __device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commi
 template <int N>
 __device__ __forceinline__ void cp_async_wait() { asm volatile("cp.async.wait_group %0;" ::"n"(N) : "memory"); }
 
-constexpr int DFS_STAGES = 6;          // matrix staging ring: operation k+5 is in flight while operation k computes
-constexpr int DFS_PSTRIDE = 18;        // doubles per staged 4x4 matrix: 144 B, so the G categories of a warp hit distinct banks
+#ifndef EPX_DFS_STAGES
+#define EPX_DFS_STAGES 5
+#endif
+constexpr int DFS_STAGES = EPX_DFS_STAGES;   // matrix staging ring: operation k+STAGES-1 is in flight while operation k computes
+constexpr int DFS_PSTRIDE = 20;        // doubles per staged 4x4 matrix: 160 B = 40 banks, so 4 categories never share a bank
 __host__ __device__ constexpr int dfs_lanes_of(int C) { return C <= 1 ? 1 : C <= 2 ? 2 : C <= 4 ? 4 : 8; }
 __host__ __device__ constexpr int dfs_stage_bytes(int G) { return 2 * G * DFS_PSTRIDE * 8; }
 
@@ -138,7 +141,7 @@ __device__ __forceinline__ void matvec4(const double* __restrict__ Pm, const dou
 //   - operation descriptors and tip states: every 32 operations lane j loads descriptor j of the NEXT block of 32 and
 //     that operation's tip bytes for the warp's patterns into registers; operation k reads them with warp shuffles;
 //   - the children's 4x4 matrices: cp.async into a shared-memory ring, DFS_STAGES - 1 operations ahead.
-// Shared memory per warp: DFS_STAGES x [2 children][G][18] doubles, then the stack [depth][32 lanes][4] doubles +
+// Shared memory per warp: DFS_STAGES x [2 children][G][20] doubles, then the stack [depth][2 halves][32 lanes] double2 +
 // [depth][32] exponents.  A lane only ever touches its own stack column, so the stack needs no synchronisation.
 template <int C>
 __global__ void __launch_bounds__(32) prune4_dfs_kernel(const DfsOp* __restrict__ ops, const DfsPiece* __restrict__ pieces,
@@ -152,8 +155,8 @@ __global__ void __launch_bounds__(32) prune4_dfs_kernel(const DfsOp* __restrict_
     constexpr int SB = dfs_stage_bytes(G);
     constexpr int NCH = (16 * C + 31) / 32;         // 16-byte chunks of the two children's matrices per lane
     constexpr unsigned FULL = 0xffffffffu;
-    double* stack = reinterpret_cast<double*>(smraw + DFS_STAGES * SB);
-    int* stack_ex = reinterpret_cast<int*>(stack + (size_t)depth * 128);
+    double2* stack = reinterpret_cast<double2*>(smraw + DFS_STAGES * SB);     // [depth][2][32]: conflict-free 128-bit rows
+    int* stack_ex = reinterpret_cast<int*>(stack + (size_t)depth * 64);
     const int lane = threadIdx.x;
     const int pl = lane / G, c = lane % G, cc = min(c, C - 1);
     const int piece = blockIdx.x / tiles, tile = blockIdx.x - piece * tiles;
@@ -175,8 +178,10 @@ __global__ void __launch_bounds__(32) prune4_dfs_kernel(const DfsOp* __restrict_
         cp_dst[q] = ((cp_child[q] ? G : 0) + cat) * (DFS_PSTRIDE * 8) + w * 16;
         cp_src[q] = cat * 16 + w * 2;
     }
-    const size_t node_stride = (size_t)L * C * 4;   // doubles per node of the partials array
-    double* const out_base = partials + ((size_t)p * C + c) * 4;
+    // 32-bit indexing in units of one state vector (32 B): (N-1) L C < 2^32 is checked by prune_uses_dfs
+    const unsigned node_stride = (unsigned)L * C;
+    double4a* const out_base = reinterpret_cast<double4a*>(partials) + ((size_t)p * C + c);
+    int32_t* const exp_base = scale_exp + p;
     const unsigned char* const tip_base = tips + p0;
     const double* const Pm_base = reinterpret_cast<const double*>(smraw) + cc * DFS_PSTRIDE;
 
@@ -253,13 +258,12 @@ __global__ void __launch_bounds__(32) prune4_dfs_kernel(const DfsOp* __restrict_
             const int pa = __shfl_sync(FULL, cb.h.x, src_lane);
             va[0] = va[1] = va[2] = va[3] = 1.0;
             if (live) {
-                const double4a v = ld256(out_base + (size_t)pa * node_stride);
+                const double4a v = ld256(reinterpret_cast<const double*>(out_base + (unsigned)pa * node_stride));
                 va[0] = v.x; va[1] = v.y; va[2] = v.z; va[3] = v.w;
-                ex += scale_exp[(size_t)pa * L + p];
+                ex += exp_base[(unsigned)pa * (unsigned)L];
             }
         } else {
-            const double2* sv = reinterpret_cast<const double2*>(stack + ((size_t)srcA * 32 + lane) * 4);
-            const double2 v01 = sv[0], v23 = sv[1];
+            const double2 v01 = stack[srcA * 64 + lane], v23 = stack[srcA * 64 + 32 + lane];
             va[0] = v01.x; va[1] = v01.y; va[2] = v23.x; va[3] = v23.y;
             ex += stack_ex[srcA * 32 + lane];
         }
@@ -273,13 +277,11 @@ __global__ void __launch_bounds__(32) prune4_dfs_kernel(const DfsOp* __restrict_
             const int pb = __shfl_sync(FULL, cb.h.y, src_lane);
             vb[0] = vb[1] = vb[2] = vb[3] = 1.0;
             if (live) {
-                const double4a v = ld256(out_base + (size_t)pb * node_stride);
+                const double4a v = ld256(reinterpret_cast<const double*>(out_base + (unsigned)pb * node_stride));
                 vb[0] = v.x; vb[1] = v.y; vb[2] = v.z; vb[3] = v.w;
-                ex += scale_exp[(size_t)pb * L + p];
+                ex += exp_base[(unsigned)pb * (unsigned)L];
             }
         } else {
-#pragma unroll
-            for (int i = 0; i < 4; i++) vb[i] = cur[i];
             ex += cur_ex;
         }
 
@@ -297,6 +299,8 @@ __global__ void __launch_bounds__(32) prune4_dfs_kernel(const DfsOp* __restrict_
         if (srcB == EPX_DFS_TIP) {
 #pragma unroll
             for (int i = 0; i < 4; i++) fb[i] = (sbt < 4) ? Pb[i * 4 + sbt] : 1.0;
+        } else if (srcB == EPX_DFS_PREV) {
+            matvec4(Pb, cur, fb);
         } else {
             matvec4(Pb, vb, fb);
         }
@@ -314,12 +318,11 @@ __global__ void __launch_bounds__(32) prune4_dfs_kernel(const DfsOp* __restrict_
 #pragma unroll
         for (int i = 0; i < 4; i++) cur[i] = fa[i] * sc;
         cur_ex = ex;
-        if (live) st256(out_base + (size_t)pidx * node_stride, cur[0], cur[1], cur[2], cur[3]);
-        if (live && c == 0) scale_exp[(size_t)pidx * L + p] = ex;
+        if (live) st256(reinterpret_cast<double*>(out_base + (unsigned)pidx * node_stride), cur[0], cur[1], cur[2], cur[3]);
+        if (live && c == 0) exp_base[(unsigned)pidx * (unsigned)L] = ex;
         if (out_slot >= 0) {
-            double2* sv = reinterpret_cast<double2*>(stack + ((size_t)out_slot * 32 + lane) * 4);
-            sv[0] = make_double2(cur[0], cur[1]);
-            sv[1] = make_double2(cur[2], cur[3]);
+            stack[out_slot * 64 + lane] = make_double2(cur[0], cur[1]);
+            stack[out_slot * 64 + 32 + lane] = make_double2(cur[2], cur[3]);
             stack_ex[out_slot * 32 + lane] = ex;
         }
         if (++buf == DFS_STAGES) buf = 0;
@@ -500,6 +503,7 @@ int prune_init_attributes()
 bool prune_uses_dfs(const epx_ctx* c)
 {
     return c->tree_mode && c->K == 4 && c->prune_kernel == 0 &&
+           (double)(c->N - 1) * c->L * c->C < 4294967296.0 &&
            dfs_smem(dfs_lanes_of(c->C), c->dfs_depth > 0 ? c->dfs_depth : 1) <= 227 * 1024;
 }
 
