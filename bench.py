@@ -35,6 +35,10 @@ if ROOT not in sys.path:
 
 import workloads as W  # noqa: E402  (input generators only; shared with the oracle, holds no arithmetic of the method)
 
+# dram__bytes_read.sum + dram__bytes_write.sum of the pruning launches of one config-2 step, from the committed
+# `ncu --set full` capture (profiles/r1_prune4_dfs_ncu.md): 2561.7 + 23.1 MB (bottom pieces) + 15.9 MB (top piece)
+NCU_TRAFFIC_BYTES_PER_STEP = 2.6007e9
+
 METRIC = "pruning partials GB/s (fp64) over the whole a1..a6 log-likelihood step; epoch branch matrices/s in `matrices`"
 UNIT = "GB/s"
 
@@ -205,6 +209,22 @@ def bracket(torch, stream, fn, steps):
     return e0.elapsed_time(e1)
 
 
+def max_over_ranks(x: float, world: int, device: str = "cuda") -> float:
+    """Max of a per-rank device time over all ranks (the only cross-rank exchange of the bench: replicas only)."""
+    if world == 1:
+        return x
+    import torch
+    import torch.distributed as dist
+    t = torch.tensor([x], dtype=torch.float64, device=device)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return float(t.item())
+
+
+def whole_job_value(unit_bytes: float, ms_step: float, world: int) -> float:
+    """GB/s of `world` independent replicas that each moved `unit_bytes` per step, the slowest taking ms_step."""
+    return world * unit_bytes / (ms_step * 1e-3) / 1e9
+
+
 def run_cuda(args) -> None:
     import torch
     import torch.distributed as dist
@@ -227,13 +247,6 @@ def run_cuda(args) -> None:
             dist.barrier()
         torch.cuda.synchronize()
 
-    def max_over_ranks(x: float) -> float:
-        if world == 1:
-            return x
-        t = torch.tensor([x], dtype=torch.float64, device="cuda")
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        return float(t.item())
-
     K, Wm = args.steps, max(3, args.warmup)
     prob = W.make_config(2)
     nb = pruning_bytes(prob)
@@ -255,7 +268,7 @@ def run_cuda(args) -> None:
     barrier()
     gpu_launches = ctx.launch_count() - launches0
     assert abs(ctx.fetch_log_likelihood() - lnl) <= 1e-12 * abs(lnl)
-    ms_step = max_over_ranks(ms_total / K)
+    ms_step = max_over_ranks(ms_total / K, world)
 
     # (2) roofline of the dominant kernel: the same K steps with the per-stage CUDA events read after every step
     stage_ms = np.zeros(5)
@@ -277,7 +290,7 @@ def run_cuda(args) -> None:
     barrier()
     ms_e2e = bracket(torch, stream, e2e_step, Ke) / Ke
     barrier()
-    ms_e2e = max_over_ranks(ms_e2e)
+    ms_e2e = max_over_ranks(ms_e2e, world)
     n_nodes = prob.n_nodes
     h2d = (prob.N * prob.L + 8 * prob.L + 4 * n_nodes + 8 * n_nodes + 32 * (prob.N - 1) + 8 * prob.M * prob.K * prob.K +
            8 * prob.M * prob.K + 8 * (prob.M - 1) + 16 * prob.C + 8 * prob.K)
@@ -289,15 +302,19 @@ def run_cuda(args) -> None:
     hbm_peak, peak_src = load_peaks()
     prune_ms = float(stage_ms[3])
     prune_launches = int(stage_launches[3])
-    roofline = {"bound": "hbm", "kernel": "prune4_kernel<4> (a5; one launch per post-order level, CUDA graph)",
+    roofline = {"bound": "hbm", "kernel": "prune4_dfs_kernel<4> (a5; depth-first walk, bottom pieces + top piece)",
                 "achieved": nb["a5"] / (prune_ms * 1e-3) / 1e9, "peak": hbm_peak, "unit": "GB/s",
-                "frac": nb["a5"] / (prune_ms * 1e-3) / 1e9 / hbm_peak, "traffic": args.traffic,
+                "frac": nb["a5"] / (prune_ms * 1e-3) / 1e9 / hbm_peak,
+                "traffic": args.traffic if args.traffic is not None else NCU_TRAFFIC_BYTES_PER_STEP / prune_launches,
+                "traffic_note": "dram__bytes_read+write per launch (sum over the step's launches / launches), "
+                                "profiles/r1_prune4_dfs_ncu.md; below the algorithmic bytes because child partials "
+                                "stay in registers / shared memory and are never re-read from HBM",
                 "peak_source": peak_src, "launches_per_step": prune_launches,
                 "algorithmic_bytes_per_launch": nb["a5"] / prune_launches,
                 "avg_launch_ms": prune_ms / prune_launches, "share_of_step": prune_ms / float(stage_ms.sum()),
                 "stage_ms": {n: float(v) for n, v in zip(epx.STAGE_NAMES, stage_ms)}}
 
-    line = {"metric": METRIC, "value": world * unit_bytes / (ms_step * 1e-3) / 1e9, "unit": UNIT, "n_gpus": world,
+    line = {"metric": METRIC, "value": whole_job_value(unit_bytes, ms_step, world), "unit": UNIT, "n_gpus": world,
             "steps": K, "warmup": Wm, "ms_per_step": ms_step, "higher_is_better": True, "scaling": "weak",
             "vs_baseline": None, "dtype": "f64", "data": "synthetic",
             "config": {"workload": W.CONFIG_NAMES[2], "K": prob.K, "M": prob.M, "C": prob.C, "N_tips": prob.N,
@@ -305,7 +322,7 @@ def run_cuda(args) -> None:
                        "l2": f"inputs larger than L2: {ws_bytes / 1e9:.2f} GB workspace, 2.56 GB of partials rewritten "
                              "every step vs 126 MB L2", "seed": W.config_seed(2)},
             "roofline": roofline,
-            "e2e": {"value": world * unit_bytes / (ms_e2e * 1e-3) / 1e9, "unit": UNIT, "h2d_bytes_per_step": h2d,
+            "e2e": {"value": whole_job_value(unit_bytes, ms_e2e, world), "unit": UNIT, "h2d_bytes_per_step": h2d,
                     "d2h_bytes_per_step": 12, "ms_per_step": ms_e2e, "steps": Ke,
                     "what": "all epx_set_* calls from host arrays + epx_log_likelihood (syncs, reads logL + status)"},
             "gpu_launches": int(gpu_launches), "clocks": clk, "log_likelihood": lnl,

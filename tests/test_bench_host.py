@@ -1,0 +1,82 @@
+"""Host-side logic of bench.py (no GPU): the algorithmic byte / flop counts, and the N > 1 path -- replicas only, the one
+cross-rank exchange is a MAX all-reduce of the device time -- on a world_size-2 gloo group."""
+import json
+import os
+import subprocess
+import sys
+
+import numpy as np
+import pytest
+
+import workloads as W
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+
+
+def test_pruning_bytes_formula_matches_a_node_by_node_count():
+    import bench
+    prob = W.make_config(2, N=37, L=123)
+    K, C, L, N = prob.K, prob.C, prob.L, prob.N
+    total = 0
+    for u in range(N, 2 * N - 1):                       # node-by-node restatement of DESIGN.md section 5
+        total += C * L * K * 8 + 4 * L + 2 * C * K * K * 8
+        for ch in np.nonzero(prob.parent == u)[0]:
+            total += L if ch < N else C * L * K * 8 + 4 * L
+    got = bench.pruning_bytes(prob)
+    assert got["a5"] == total
+    assert got["a6"] == C * L * K * 8 + 4 * L + 16 * L
+    assert got["flops"] == (N - 1) * C * L * (4 * K * K + K)
+
+
+def test_config2_algorithmic_bytes_is_the_surveyed_5_2_GB():
+    import bench
+    nb = bench.pruning_bytes(W.make_config(2))
+    assert 5.1e9 < nb["a5"] + nb["a6"] < 5.4e9          # ~5.20 GB
+
+
+def test_segment_counts_and_chain_flops(orc_ld):
+    import bench
+    prob = W.make_config(5, n_br=500)
+    nseg = bench.n_segments(prob)
+    off, _, _ = orc_ld.segments(prob.child_height, prob.parent_height, prob.tau)
+    assert np.array_equal(nseg, np.diff(off))
+    fl = bench.chain_flops(61, 4, nseg)
+    assert fl["executed"] == int(nseg.sum()) * 4 * 2 * 61 ** 3
+    assert fl["straightforward"] > fl["executed"]
+
+
+_WORKER = r"""
+import os, sys
+sys.path.insert(0, sys.argv[1])
+import torch.distributed as dist
+import bench
+rank = int(os.environ["RANK"])
+dist.init_process_group("gloo")
+mine = 1.5 if rank == 0 else 2.25                      # rank 1 is the slow replica
+ms = bench.max_over_ranks(mine, 2, device="cpu")
+val = bench.whole_job_value(1e9, ms, 2)
+print(f"RESULT {rank} {ms} {val}", flush=True)
+dist.destroy_process_group()
+"""
+
+
+def test_replicas_aggregate_with_gloo_world_size_2(tmp_path):
+    script = tmp_path / "worker.py"
+    script.write_text(_WORKER)
+    env = dict(os.environ, MASTER_ADDR="127.0.0.1", MASTER_PORT="29533", WORLD_SIZE="2")
+    procs = [subprocess.Popen([sys.executable, str(script), ROOT], env=dict(env, RANK=str(r)), stdout=subprocess.PIPE,
+                              stderr=subprocess.PIPE, text=True) for r in range(2)]
+    outs = [p.communicate(timeout=120) for p in procs]
+    for p, (o, e) in zip(procs, outs):
+        assert p.returncode == 0, e
+    for o, _ in outs:
+        line = [x for x in o.splitlines() if x.startswith("RESULT")][0].split()
+        assert float(line[2]) == 2.25                                  # max over ranks on every rank
+        assert abs(float(line[3]) - 2 * 1e9 / 2.25e-3 / 1e9) < 1e-9    # 2 replicas / slowest time
+
+
+def test_reference_arm_only_rank0_prints(tmp_path):
+    env = dict(os.environ, RANK="1", WORLD_SIZE="2")
+    r = subprocess.run([sys.executable, os.path.join(ROOT, "bench.py"), "--impl", "reference", "--steps", "1", "--warmup", "0"],
+                       env=env, capture_output=True, text=True, timeout=120)
+    assert r.returncode == 0 and r.stdout.strip() == ""
