@@ -16,7 +16,7 @@ LIB_PATH = os.path.join(_HERE, "libepx.so")
 SOURCES = ["api.cu", "segmenter.cu", "eigen.cu", "chain.cu", "pade.cu", "prune.cu", "peaks.cu"]
 DEPS = ["epx_internal.h", "api_compute.inc", os.path.join("..", "..", "include", "epx.h")]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",
-              "-Xcompiler", "-fPIC"]
+              "-Xcompiler", "-fPIC"] + os.environ.get("EPX_NVCC_EXTRA", "").split()
 
 
 def _nvcc() -> str:

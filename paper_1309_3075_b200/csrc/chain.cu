@@ -273,16 +273,21 @@ __global__ void __launch_bounds__(DT, 1) chain_dmma64_kernel(int K, int C, const
                         acc[2 * mp + mi][kt][1] = 0.0;
                     }
                 }
+                // issue order: four different accumulator tiles between two DMMAs on the same one (DMMA latency)
 #pragma unroll
                 for (int kt = 0; kt < 8; kt++)
 #pragma unroll
-                    for (int nt = 0; nt < 8; nt++) {
-                        double2 bv = Bs[(kt * 8 + nt) * 32 + lane];
+                    for (int np = 0; np < 4; np++) {
+                        const double2 b0 = Bs[(kt * 8 + 2 * np) * 32 + lane], b1 = Bs[(kt * 8 + 2 * np + 1) * 32 + lane];
 #pragma unroll
-                        for (int mi = 0; mi < 2; mi++) {
-                            dmma884(acc[2 * mp + mi][nt][0], acc[2 * mp + mi][nt][1], a[mi][kt][0], bv.x);
-                            dmma884(acc[2 * mp + mi][nt][0], acc[2 * mp + mi][nt][1], a[mi][kt][1], bv.y);
-                        }
+                        for (int h = 0; h < 2; h++)
+#pragma unroll
+                            for (int nn = 0; nn < 2; nn++)
+#pragma unroll
+                                for (int mi = 0; mi < 2; mi++) {
+                                    const double bb = nn ? (h ? b1.y : b1.x) : (h ? b0.y : b0.x);
+                                    dmma884(acc[2 * mp + mi][2 * np + nn][0], acc[2 * mp + mi][2 * np + nn][1], a[mi][kt][h], bb);
+                                }
                     }
             }
         }

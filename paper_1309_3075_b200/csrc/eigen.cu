@@ -9,25 +9,31 @@
 // kernel stay in the eigenbasis across a boundary (one product per segment instead of three), plus copies of W and
 // U^T in DMMA B-fragment order for the 64-wide tensor-core chain kernel.
 #include "epx_internal.h"
+#include <cstdio>
 
 namespace {
 
-constexpr int JT = 256;   // threads per CTA
+constexpr int JT_MAX = 1024;   // threads per CTA for K > 32 (one 2x2 block of S per thread and round); 256 otherwise
 
-__global__ void __launch_bounds__(JT) jacobi_kernel(int K, int Kp, const double* __restrict__ Qall,
-                                                    const double* __restrict__ freqs, double* __restrict__ lam,
-                                                    double* __restrict__ Uout, double* __restrict__ sp_out,
-                                                    double* __restrict__ isp_out, int32_t* __restrict__ status)
+// Two-sided Jacobi, round-robin ordering: in one round the n/2 pivot pairs are disjoint, so S' = J^T S J splits into
+// (n/2)^2 independent 2x2 blocks (rows of pair a, columns of pair b) that each depend on their own four entries and the
+// two rotations only.  One thread per block applies the column and the row rotation in registers: two barriers per round
+// instead of three, and 961 busy threads at K = 61.
+__global__ void __launch_bounds__(JT_MAX) jacobi_kernel(int K, int Kp, const double* __restrict__ Qall,
+                                                        const double* __restrict__ freqs, double* __restrict__ lam,
+                                                        double* __restrict__ Uout, double* __restrict__ sp_out,
+                                                        double* __restrict__ isp_out, int32_t* __restrict__ status)
 {
     extern __shared__ double sm[];
+    const int JT = blockDim.x;
     const int ld = K | 1;                       // odd row stride: column walks are bank-conflict free
     double* S = sm;                             // [K][ld]
     double* V = S + (size_t)K * ld;             // [K][ld]
     double* rc = V + (size_t)K * ld;            // [K/2+1] cos
     double* rs = rc + (K / 2 + 1);              // [K/2+1] sin
-    double* red = rs + (K / 2 + 1);             // [JT/32] reduction scratch
-    int* rp = (int*)(red + JT / 32);            // [K/2+1] p
-    int* rq = rp + (K / 2 + 1);                 // [K/2+1] q
+    double* red = rs + (K / 2 + 1);             // [32] reduction scratch
+    int* rp = (int*)(red + 32);                 // [K/2+1] p
+    int* rq = rp + (K / 2 + 1);                 // [K/2+1] q (>= K: the dummy player of an odd K)
     __shared__ double s_off2, s_tot2;
 
     const int e = blockIdx.x, tid = threadIdx.x;
@@ -63,6 +69,9 @@ __global__ void __launch_bounds__(JT) jacobi_kernel(int K, int Kp, const double*
     const int n = (K + 1) & ~1;          // players (a dummy one if K is odd)
     const int npair = n / 2;
     const double eps = 2.220446049250313e-16;
+    // item -> (pair a, pair b) and (pair, row) maps do not change from round to round
+    const int blk_a = tid / npair, blk_b = tid - blk_a * npair;
+    const int v_k = tid / K, v_i = tid - v_k * K;
     bool converged = false;
     for (int sweep = 0; sweep < 40 && !converged; sweep++) {
         for (int r = 0; r < n - 1; r++) {
@@ -73,46 +82,52 @@ __global__ void __launch_bounds__(JT) jacobi_kernel(int K, int Kp, const double*
                 int p = min(a, b), q = max(a, b);
                 double c = 1.0, s = 0.0;
                 if (q < K) {
-                    double apq = S[p * ld + q];
+                    const double apq = S[p * ld + q];
                     if (fabs(apq) > 1e-300) {
-                        double theta = (S[q * ld + q] - S[p * ld + p]) / (2.0 * apq);
-                        double t = 1.0 / (fabs(theta) + sqrt(theta * theta + 1.0));
-                        if (theta < 0) t = -t;
-                        c = 1.0 / sqrt(t * t + 1.0);
+                        // t = tan of the rotation angle, the root of smaller magnitude of t^2 + 2 theta t - 1 = 0 with
+                        // theta = d / h: t = sgn(d) h / (|d| + sqrt(d^2 + h^2)); one rsqrt per square root, one division
+                        const double d = S[q * ld + q] - S[p * ld + p], h = 2.0 * apq;
+                        const double r2 = fma(d, d, h * h);
+                        const double r = r2 * rsqrt(r2);
+                        const double t = (d < 0 ? -h : h) / (fabs(d) + r);
+                        c = rsqrt(fma(t, t, 1.0));
                         s = t * c;
                     }
-                } else {
-                    p = -1;
                 }
                 rp[tid] = p; rq[tid] = q; rc[tid] = c; rs[tid] = s;
             }
             __syncthreads();
-            // columns: S <- S J, V <- V J
+            // S <- J^T S J, one 2x2 block per item
+            for (int blk = tid; blk < npair * npair; blk += JT) {
+                const int a = blk == tid ? blk_a : blk / npair, b = blk == tid ? blk_b : blk - a * npair;
+                const int pa = rp[a], qa = rq[a], pb = rp[b], qb = rq[b];
+                const double ca = rc[a], sa = rs[a], cb = rc[b], sb = rs[b];
+                const bool ra = qa < K, cbv = qb < K;            // second row / column is a real index
+                double x00 = S[pa * ld + pb];
+                double x01 = cbv ? S[pa * ld + qb] : 0.0;
+                double x10 = ra ? S[qa * ld + pb] : 0.0;
+                double x11 = (ra && cbv) ? S[qa * ld + qb] : 0.0;
+                // columns (pair b)
+                double t00 = cb * x00 - sb * x01, t01 = sb * x00 + cb * x01;
+                double t10 = cb * x10 - sb * x11, t11 = sb * x10 + cb * x11;
+                // rows (pair a)
+                double y00 = ca * t00 - sa * t10, y01 = ca * t01 - sa * t11;
+                double y10 = sa * t00 + ca * t10, y11 = sa * t01 + ca * t11;
+                if (a == b) { y01 = 0.0; y10 = 0.0; }            // the pivot pair is annihilated exactly
+                S[pa * ld + pb] = y00;
+                if (cbv) S[pa * ld + qb] = y01;
+                if (ra) S[qa * ld + pb] = y10;
+                if (ra && cbv) S[qa * ld + qb] = y11;
+            }
+            // V <- V J
             for (int idx = tid; idx < npair * K; idx += JT) {
-                int k = idx / K, i = idx % K, p = rp[k];
-                if (p < 0) continue;
-                int q = rq[k];
-                double c = rc[k], s = rs[k];
-                double x = S[i * ld + p], y = S[i * ld + q];
-                S[i * ld + p] = c * x - s * y;
-                S[i * ld + q] = s * x + c * y;
-                x = V[i * ld + p]; y = V[i * ld + q];
+                const int k = idx == tid ? v_k : idx / K, i = idx == tid ? v_i : idx - k * K, q = rq[k];
+                if (q >= K) continue;
+                const int p = rp[k];
+                const double c = rc[k], s = rs[k];
+                const double x = V[i * ld + p], y = V[i * ld + q];
                 V[i * ld + p] = c * x - s * y;
                 V[i * ld + q] = s * x + c * y;
-            }
-            __syncthreads();
-            // rows: S <- J^T S ; the pivot pair is annihilated exactly
-            for (int idx = tid; idx < npair * K; idx += JT) {
-                int k = idx / K, j = idx % K, p = rp[k];
-                if (p < 0) continue;
-                int q = rq[k];
-                double c = rc[k], s = rs[k];
-                double x = S[p * ld + j], y = S[q * ld + j];
-                double xp = c * x - s * y, yq = s * x + c * y;
-                if (j == q) xp = 0.0;
-                if (j == p) yq = 0.0;
-                S[p * ld + j] = xp;
-                S[q * ld + j] = yq;
             }
             __syncthreads();
         }
@@ -125,6 +140,9 @@ __global__ void __launch_bounds__(JT) jacobi_kernel(int K, int Kp, const double*
         if (tid == 0) s_off2 = t;
         __syncthreads();
         converged = s_off2 <= 0.25 * eps * eps * s_tot2;
+#ifdef EPX_DEBUG_JACOBI
+        if (tid == 0) printf("epoch %d sweep %d off/tot %.3e\n", e, sweep, sqrt(s_off2 / s_tot2));
+#endif
     }
     if (tid == 0 && !(s_off2 <= 1e-28 * s_tot2)) atomicOr(status, EPX_ST_JACOBI_NOCONV);
 
@@ -139,6 +157,8 @@ __global__ void __launch_bounds__(JT) jacobi_kernel(int K, int Kp, const double*
         isp_out[(size_t)e * Kp + i] = i < K ? 1.0 / sqrt(pi[i]) : 0.0;
     }
 }
+
+constexpr int JT = 256;   // threads per CTA of the prep kernels
 
 // W_e[a][b] = sum_k U_e[k][a] * sqrt(pi_e[k] / pi_{e-1}[k]) * U_{e-1}[k][b]   (e >= 1)
 // Fragment order (lane = 4g + q of an m8n8k4 DMMA; the contraction index of k-step (kt,h) at position q is
@@ -177,6 +197,42 @@ __global__ void __launch_bounds__(JT) prep_kernel(int Kp, const double* __restri
     }
 }
 
+
+// 64-padded models: grid (M, 8), CTA (e, y) computes rows 8y .. 8y+7 of W_e and writes W, WB and UTB directly.
+__global__ void __launch_bounds__(JT) prep64_kernel(const double* __restrict__ U, const double* __restrict__ sp,
+                                                    const double* __restrict__ isp, double* __restrict__ W,
+                                                    double* __restrict__ WB, double* __restrict__ UTB)
+{
+    __shared__ double ue[64][8];      // U_e[k][a0 + j] * sqrt(pi_e[k] / pi_{e-1}[k])
+    const int e = blockIdx.x, a0 = blockIdx.y * 8, tid = threadIdx.x;
+    const double* Ue = U + (size_t)e * 4096;
+    const int b = tid & 63, ar = tid >> 6;
+    double acc[2] = {0.0, 0.0};
+    if (e >= 1) {
+        const double* Um = U + (size_t)(e - 1) * 4096;
+        for (int idx = tid; idx < 512; idx += JT) {
+            const int k = idx >> 3, j = idx & 7;
+            ue[k][j] = Ue[k * 64 + a0 + j] * (sp[(size_t)e * 64 + k] * isp[(size_t)(e - 1) * 64 + k]);
+        }
+        __syncthreads();
+#pragma unroll 8
+        for (int k = 0; k < 64; k++) {
+            const double um = Um[k * 64 + b];
+            acc[0] = fma(ue[k][ar], um, acc[0]);
+            acc[1] = fma(ue[k][ar + 4], um, acc[1]);
+        }
+    }
+#pragma unroll
+    for (int h2 = 0; h2 < 2; h2++) {
+        const int a = a0 + ar + 4 * h2;                 // row (contraction index kappa of the B fragment), column b
+        const int kt = a >> 3, q = (a & 7) >> 1, h = a & 1, nt = b >> 3, g = b & 7;
+        const int idx = ((kt * 8 + nt) * 32 + 4 * g + q) * 2 + h;
+        W[(size_t)e * 4096 + a * 64 + b] = acc[h2];
+        WB[(size_t)e * 4096 + idx] = acc[h2];
+        UTB[(size_t)e * 4096 + idx] = Ue[b * 64 + a];   // U^T[a][b]
+    }
+}
+
 }  // namespace
 
 int eigen_init_attributes()
@@ -189,8 +245,9 @@ int launch_eigensystems(const epx_ctx* c, cudaStream_t s)
     const DevBuffers& d = c->d;
     const int K = c->K, Kp = c->Kp;
     const int ld = K | 1;
-    size_t smem = sizeof(double) * (2 * (size_t)K * ld + 2 * (K / 2 + 1) + JT / 32) + sizeof(int) * 2 * (K / 2 + 1);
-    jacobi_kernel<<<c->M, JT, smem, s>>>(K, Kp, d.Q, d.freqs, d.lam, d.U, d.sp, d.isp, d.status);
-    prep_kernel<<<c->M, JT, 0, s>>>(Kp, d.U, d.sp, d.isp, d.W, d.WB, d.UTB);
+    size_t smem = sizeof(double) * (2 * (size_t)K * ld + 2 * (K / 2 + 1) + 32) + sizeof(int) * 2 * (K / 2 + 1);
+    jacobi_kernel<<<c->M, K > 32 ? JT_MAX : 256, smem, s>>>(K, Kp, d.Q, d.freqs, d.lam, d.U, d.sp, d.isp, d.status);
+    if (Kp == 64) prep64_kernel<<<dim3(c->M, 8), JT, 0, s>>>(d.U, d.sp, d.isp, d.W, d.WB, d.UTB);
+    else prep_kernel<<<c->M, JT, 0, s>>>(Kp, d.U, d.sp, d.isp, d.W, d.WB, d.UTB);
     return cudaGetLastError() == cudaSuccess ? 2 : -1;
 }
