@@ -292,7 +292,9 @@ def run_cuda(args) -> None:
     barrier()
     ms_e2e = max_over_ranks(ms_e2e, world)
     n_nodes = prob.n_nodes
-    h2d = (prob.N * prob.L + 8 * prob.L + 4 * n_nodes + 8 * n_nodes + 32 * (prob.N - 1) + 8 * prob.M * prob.K * prob.K +
+    # tip states as bytes (rows padded to 32), pattern weights, parent + height, the two pruning plans (32 B per node each),
+    # models, boundaries, category rates + weights, root frequencies
+    h2d = (prob.N * ((prob.L + 31) // 32 * 32) + 8 * prob.L + 4 * n_nodes + 8 * n_nodes + 64 * (prob.N - 1) + 8 * prob.M * prob.K * prob.K +
            8 * prob.M * prob.K + 8 * (prob.M - 1) + 16 * prob.C + 8 * prob.K)
     clk = clocks.stop()
     levels = ctx.tree_levels()

@@ -152,7 +152,8 @@ enum {
                                  2 for tree-mode (likelihood) contexts whose reversible Q have structural zeros (codon
                                  models: entries of P that vanish like t^2, t^3 decide the likelihood of short branches),
                                  else 1.  This one DOES change results, within the tolerances above (A21). */
-    EPX_OPT_STAGE_EVENTS = 5  /* 1 record per-stage CUDA events for epx_get_stage_ms; 0 (default) none */
+    EPX_OPT_STAGE_EVENTS = 5, /* 1 record per-stage CUDA events for epx_get_stage_ms; 0 (default) none */
+    EPX_OPT_DFS_PPL = 6       /* K == 4 depth-first pruning: site patterns per lane, 1, 2 or 4; 0 (default) auto */
 };
 int epx_set_option(epx_ctx* ctx, int option, int value);
 /* Device status word of the last compute call (0 = all numeric checks passed); synchronises. */

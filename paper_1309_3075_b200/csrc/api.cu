@@ -10,6 +10,7 @@
 #include <cstdarg>
 #include <cstdio>
 #include <cstring>
+#include <thread>
 
 namespace {
 
@@ -172,8 +173,7 @@ int build_plan(epx_ctx* c)
     std::vector<char> is_cut(n, 0);           // roots of the bottom pieces
     std::vector<int> cuts;
     {
-        const int lanes = c->C <= 1 ? 1 : c->C <= 2 ? 2 : c->C <= 4 ? 4 : 8;
-        const long tiles = (c->L + 32 / lanes - 1) / (32 / lanes);
+        const long tiles = dfs_tiles(c);
         const long want = std::min<long>(64, 4 * ((148L * 24 + tiles - 1) / tiles));   // pieces wanted (1 = no cut)
         std::vector<int> heap{root};          // max-heap on subtree size
         auto cmp = [&](int x, int y) { return size[x] < size[y]; };
@@ -307,6 +307,7 @@ void epx_destroy(epx_ctx* c)
     if (!c) return;
     drop_graphs(c);
     for (cudaEvent_t e : c->ev) if (e) cudaEventDestroy(e);
+    if (c->tips) { if (c->tips_pinned) cudaFreeHost(c->tips); else free(c->tips); }
     delete c;
 }
 
@@ -352,6 +353,11 @@ int epx_set_option(epx_ctx* c, int option, int value)
         case 3: c->prune_kernel = value; break;
         case 4: if (value < 0 || value > 2) return fail(c, EPX_E_ARG, "exp method %d", value); c->exp_method = value; break;
         case 5: c->stage_events = value ? 1 : 0; break;
+        case 6:
+            if (value != 0 && value != 1 && value != 2 && value != 4) return fail(c, EPX_E_ARG, "patterns per lane %d", value);
+            c->dfs_ppl = value;
+            if (c->has_tree) { int rc = build_plan(c); if (rc) return rc; c->tree_dirty = true; }
+            break;
         default: return fail(c, EPX_E_ARG, "unknown option %d", option);
     }
     drop_graphs(c);
@@ -477,16 +483,42 @@ int epx_set_tip_states(epx_ctx* c, const int32_t* states)
 {
     if (!c || !states) return EPX_E_ARG;
     if (!c->tree_mode) return fail(c, EPX_E_STATE, "ctx is in branch-list mode");
-    const size_t L = (size_t)c->L, Lp = (size_t)c->Lp;
-    c->tips.assign((size_t)c->N * Lp, (uint8_t)255);
-    const int K = c->K;
-    for (size_t t = 0; t < (size_t)c->N; t++) {
-        const int32_t* src = states + t * L;
-        uint8_t* dst = c->tips.data() + t * Lp;
-        for (size_t p = 0; p < L; p++) {
-            int32_t s = src[p];
-            dst[p] = (s >= 0 && s < K) ? (uint8_t)s : (uint8_t)255;
+    const size_t L = (size_t)c->L, Lp = (size_t)c->Lp, N = (size_t)c->N;
+    if (!c->tips) {
+        // page-locked staging buffer: the upload is then a plain DMA that overlaps the host work of the next setters
+        void* ptr = nullptr;
+        if (cudaSetDevice(c->device) == cudaSuccess && cudaHostAlloc(&ptr, N * Lp, cudaHostAllocDefault) == cudaSuccess) {
+            c->tips = (uint8_t*)ptr; c->tips_pinned = true;
+        } else {
+            cudaGetLastError();
+            c->tips = (uint8_t*)malloc(N * Lp);
+            if (!c->tips) return fail(c, EPX_E_ARG, "out of host memory for %zu tip states", N * Lp);
         }
+    } else if (c->bound) {
+        // an earlier upload may still be reading the staging buffer
+        CUDA_TRY(c, cudaStreamSynchronize(c->stream));
+    }
+    const int K = c->K;
+    uint8_t* const base = c->tips;
+    auto convert_rows = [=](size_t t0, size_t t1) {
+        for (size_t t = t0; t < t1; t++) {
+            const int32_t* src = states + t * L;
+            uint8_t* dst = base + t * Lp;
+            for (size_t p = 0; p < L; p++) {
+                const uint32_t s = (uint32_t)src[p];
+                dst[p] = s < (uint32_t)K ? (uint8_t)s : (uint8_t)255;
+            }
+            for (size_t p = L; p < Lp; p++) dst[p] = 255;
+        }
+    };
+    // integer repacking of the caller's int32 states into bytes, split over host threads (no arithmetic of the method)
+    size_t nthreads = std::min<size_t>(std::min<size_t>(16, std::max(1u, std::thread::hardware_concurrency())), (N * L) >> 20);
+    if (nthreads <= 1) {
+        convert_rows(0, N);
+    } else {
+        std::vector<std::thread> pool;
+        for (size_t w = 0; w < nthreads; w++) pool.emplace_back(convert_rows, N * w / nthreads, N * (w + 1) / nthreads);
+        for (auto& th : pool) th.join();
     }
     c->has_tips = true; c->tips_dirty = true;
     return EPX_OK;

@@ -103,13 +103,15 @@ struct epx_ctx {
     int chain_kernel = 0;  // EPX_OPT_CHAIN_KERNEL: 0 auto, 1 force the generic shared-memory kernel
     int use_graph = 1;     // EPX_OPT_USE_GRAPH
     int prune_kernel = 0;  // EPX_OPT_PRUNE_KERNEL: 0 auto, 1 force the generic shared-memory kernel
+    int dfs_ppl = 0;       // EPX_OPT_DFS_PPL: patterns per lane of the depth-first pruning walk (0 auto, 1, 2, 4)
     int exp_method = 0;    // EPX_OPT_EXP_METHOD: 0 auto, 1 spectral (Jacobi / Pade), 2 componentwise (shifted Taylor)
     std::vector<char> model_sparse;   // per epoch: Q has a structural zero off the diagonal
 
     // host copies of the inputs (uploaded lazily; *_dirty = needs upload)
     std::vector<double> tau, Q, freqs, rates, weights, root_freqs, height, child_h, parent_h, pattern_wt;
     std::vector<int32_t> parent;
-    std::vector<uint8_t> tips;
+    uint8_t* tips = nullptr;           // [N][Lp] host staging of the tip states, page-locked (DMA source); see epx_set_tip_states
+    bool tips_pinned = false;
     std::vector<char> model_set;
     bool has_tau = false, has_rates = false, has_tree = false, has_branches = false, has_tips = false,
          has_root_freqs = false;
@@ -177,6 +179,7 @@ int pade_init_attributes();
 int eigen_init_attributes();
 int prune_init_attributes();
 int prune_tile(int K, int C);   // patterns per CTA of the generic pruning kernel
+int dfs_tiles(const epx_ctx* c);         // warps per piece of the depth-first walk
 bool prune_uses_dfs(const epx_ctx* c);   // K == 4 depth-first walk: partials are laid out [node][L][C][4]
 // element (category c, pattern p, state i) of a node's partials sits at c * sc + p * sp + i
 inline void partial_strides(const epx_ctx* c, size_t& sc, size_t& sp)

@@ -136,32 +136,34 @@ __device__ __forceinline__ void matvec4(const double* __restrict__ Pm, const dou
     }
 }
 
-// One warp per (piece of the tree, tile of 32/G patterns); lane = (pattern, category), G = lanes per pattern = C rounded
-// up to a power of 2.  Inputs are fetched long before they are needed, so the walk never waits on HBM:
+// One warp per (piece of the tree, tile of PPL * 32/G patterns); lane = PPL x (pattern, category), G = lanes per
+// pattern = C rounded up to a power of 2, PPL = patterns per lane (the per-operation overhead -- descriptor decode,
+// staging, branches -- is paid once for PPL state vectors, and the PPL vectors are independent instruction streams).
+// Inputs are fetched long before they are needed, so the walk never waits on HBM:
 //   - operation descriptors and tip states: every 32 operations lane j loads descriptor j of the NEXT block of 32 and
 //     that operation's tip bytes for the warp's patterns into registers; operation k reads them with warp shuffles;
 //   - the children's 4x4 matrices: cp.async into a shared-memory ring, DFS_STAGES - 1 operations ahead.
-// Shared memory per warp: DFS_STAGES x [2 children][G][20] doubles, then the stack [depth][2 halves][32 lanes] double2 +
-// [depth][32] exponents.  A lane only ever touches its own stack column, so the stack needs no synchronisation.
-template <int C>
+// Shared memory per warp: DFS_STAGES x [2 children][G][20] doubles, then the stack [depth][PPL][2 halves][32 lanes]
+// double2 + [depth][PPL][32] exponents.  A lane only ever touches its own stack column: no synchronisation.
+template <int C, int PPL>
 __global__ void __launch_bounds__(32) prune4_dfs_kernel(const DfsOp* __restrict__ ops, const DfsPiece* __restrict__ pieces,
     int tiles, int L, int Lp, int depth, const double* __restrict__ P, const uint8_t* __restrict__ tips,
     double* __restrict__ partials, int32_t* __restrict__ scale_exp)
 {
     extern __shared__ __align__(16) unsigned char smraw[];
     constexpr int G = dfs_lanes_of(C);
-    constexpr int PW = 32 / G;                      // patterns per warp
+    constexpr int PL = 32 / G;                      // patterns per warp and per u
+    constexpr int PW = PPL * PL;                    // patterns per warp
     constexpr int TW = (PW + 3) / 4;                // 32-bit words of tip states per child
     constexpr int SB = dfs_stage_bytes(G);
     constexpr int NCH = (16 * C + 31) / 32;         // 16-byte chunks of the two children's matrices per lane
     constexpr unsigned FULL = 0xffffffffu;
-    double2* stack = reinterpret_cast<double2*>(smraw + DFS_STAGES * SB);     // [depth][2][32]: conflict-free 128-bit rows
-    int* stack_ex = reinterpret_cast<int*>(stack + (size_t)depth * 64);
+    double2* stack = reinterpret_cast<double2*>(smraw + DFS_STAGES * SB);     // [depth][PPL][2][32]: conflict-free rows
+    int* stack_ex = reinterpret_cast<int*>(stack + (size_t)depth * PPL * 64);
     const int lane = threadIdx.x;
     const int pl = lane / G, c = lane % G, cc = min(c, C - 1);
     const int piece = blockIdx.x / tiles, tile = blockIdx.x - piece * tiles;
-    const int p0 = tile * PW, p = p0 + pl;
-    const bool live = p < L && c < C;
+    const int p0 = tile * PW;
     const DfsPiece pc = pieces[piece];
     const int n_ops = pc.end - pc.begin;
     ops += pc.begin;
@@ -180,8 +182,16 @@ __global__ void __launch_bounds__(32) prune4_dfs_kernel(const DfsOp* __restrict_
     }
     // 32-bit indexing in units of one state vector (32 B): (N-1) L C < 2^32 is checked by prune_uses_dfs
     const unsigned node_stride = (unsigned)L * C;
-    double4a* const out_base = reinterpret_cast<double4a*>(partials) + ((size_t)p * C + c);
-    int32_t* const exp_base = scale_exp + p;
+    bool live[PPL];
+    double4a* out_base[PPL];
+    int32_t* exp_base[PPL];
+#pragma unroll
+    for (int u = 0; u < PPL; u++) {
+        const int p = p0 + u * PL + pl;
+        live[u] = p < L && c < C;
+        out_base[u] = reinterpret_cast<double4a*>(partials) + ((size_t)p * C + c);
+        exp_base[u] = scale_exp + p;
+    }
     const unsigned char* const tip_base = tips + p0;
     const double* const Pm_base = reinterpret_cast<const double*>(smraw) + cc * DFS_PSTRIDE;
 
@@ -229,8 +239,19 @@ __global__ void __launch_bounds__(32) prune4_dfs_kernel(const DfsOp* __restrict_
         cp_async_commit();
     }
 
-    double cur[4] = {1.0, 1.0, 1.0, 1.0};
-    int cur_ex = 0;
+    // byte of this lane's pattern u inside the warp's tip words
+    auto tip_of = [&](const uint32_t (&w)[TW], int u) -> int {
+        const int idx = u * PL + pl;
+        uint32_t word = w[0];
+#pragma unroll
+        for (int t = 1; t < TW; t++) if ((idx >> 2) == t) word = w[t];
+        return (word >> (8 * (idx & 3))) & 0xff;
+    };
+
+    double cur[PPL][4];
+    int cur_ex[PPL];
+#pragma unroll
+    for (int u = 0; u < PPL; u++) { cur[u][0] = cur[u][1] = cur[u][2] = cur[u][3] = 1.0; cur_ex[u] = 0; }
     int buf = 0;
     for (int k = 0; k < n_ops; k++) {
         if ((k & 31) == 0 && k > 0) { cb = nb; nb = load_block(k + 32); }
@@ -246,90 +267,91 @@ __global__ void __launch_bounds__(32) prune4_dfs_kernel(const DfsOp* __restrict_
         const int srcA = (code & 0xff) - 3, srcB = ((code >> 8) & 0xff) - 3, out_slot = ((code >> 16) & 0xff) - 1;
 
         // operands that do not need the staged matrices yet
-        double va[4], vb[4];
-        int ex = 0, sa = 255, sbt = 255;
+        uint32_t wa[TW], wb[TW];
+        int pa = 0, pb = 0;
         if (srcA == EPX_DFS_TIP) {
 #pragma unroll
-            for (int w = 0; w < TW; w++) {
-                const uint32_t wa = __shfl_sync(FULL, cb.ta[w], src_lane);
-                if (TW == 1 || (pl >> 2) == w) sa = (wa >> (8 * (pl & 3))) & 0xff;
-            }
+            for (int w = 0; w < TW; w++) wa[w] = __shfl_sync(FULL, cb.ta[w], src_lane);
         } else if (srcA == EPX_DFS_HBM) {
-            const int pa = __shfl_sync(FULL, cb.h.x, src_lane);
-            va[0] = va[1] = va[2] = va[3] = 1.0;
-            if (live) {
-                const double4a v = ld256(reinterpret_cast<const double*>(out_base + (unsigned)pa * node_stride));
-                va[0] = v.x; va[1] = v.y; va[2] = v.z; va[3] = v.w;
-                ex += exp_base[(unsigned)pa * (unsigned)L];
-            }
-        } else {
-            const double2 v01 = stack[srcA * 64 + lane], v23 = stack[srcA * 64 + 32 + lane];
-            va[0] = v01.x; va[1] = v01.y; va[2] = v23.x; va[3] = v23.y;
-            ex += stack_ex[srcA * 32 + lane];
+            pa = __shfl_sync(FULL, cb.h.x, src_lane);
         }
         if (srcB == EPX_DFS_TIP) {
 #pragma unroll
-            for (int w = 0; w < TW; w++) {
-                const uint32_t wb = __shfl_sync(FULL, cb.tb[w], src_lane);
-                if (TW == 1 || (pl >> 2) == w) sbt = (wb >> (8 * (pl & 3))) & 0xff;
-            }
+            for (int w = 0; w < TW; w++) wb[w] = __shfl_sync(FULL, cb.tb[w], src_lane);
         } else if (srcB == EPX_DFS_HBM) {
-            const int pb = __shfl_sync(FULL, cb.h.y, src_lane);
-            vb[0] = vb[1] = vb[2] = vb[3] = 1.0;
-            if (live) {
-                const double4a v = ld256(reinterpret_cast<const double*>(out_base + (unsigned)pb * node_stride));
-                vb[0] = v.x; vb[1] = v.y; vb[2] = v.z; vb[3] = v.w;
-                ex += exp_base[(unsigned)pb * (unsigned)L];
-            }
-        } else {
-            ex += cur_ex;
+            pb = __shfl_sync(FULL, cb.h.y, src_lane);
         }
 
         cp_async_wait<DFS_STAGES - 1>();            // this lane's copies for operation k have landed ...
         __syncwarp();                               // ... and so have every other lane's
         const double* Pa = Pm_base + buf * (SB / 8);
         const double* Pb = Pa + G * DFS_PSTRIDE;
-        double fa[4], fb[4];
-        if (srcA == EPX_DFS_TIP) {
 #pragma unroll
-            for (int i = 0; i < 4; i++) fa[i] = (sa < 4) ? Pa[i * 4 + sa] : 1.0;
-        } else {
-            matvec4(Pa, va, fa);
-        }
-        if (srcB == EPX_DFS_TIP) {
+        for (int u = 0; u < PPL; u++) {
+            double fa[4], fb[4];
+            int ex = 0;
+            if (srcA == EPX_DFS_TIP) {
+                const int sa = tip_of(wa, u);
 #pragma unroll
-            for (int i = 0; i < 4; i++) fb[i] = (sbt < 4) ? Pb[i * 4 + sbt] : 1.0;
-        } else if (srcB == EPX_DFS_PREV) {
-            matvec4(Pb, cur, fb);
-        } else {
-            matvec4(Pb, vb, fb);
-        }
-        // all values are >= 0, so the largest one has the largest high word: an integer max finds its exponent
-        int hmax = 0;
+                for (int i = 0; i < 4; i++) fa[i] = (sa < 4) ? Pa[i * 4 + sa] : 1.0;
+            } else {
+                double va[4] = {1.0, 1.0, 1.0, 1.0};
+                if (srcA == EPX_DFS_HBM) {
+                    if (live[u]) {
+                        const double4a v = ld256(reinterpret_cast<const double*>(out_base[u] + (unsigned)pa * node_stride));
+                        va[0] = v.x; va[1] = v.y; va[2] = v.z; va[3] = v.w;
+                        ex += exp_base[u][(unsigned)pa * (unsigned)L];
+                    }
+                } else {
+                    const double2 v01 = stack[(srcA * PPL + u) * 64 + lane], v23 = stack[(srcA * PPL + u) * 64 + 32 + lane];
+                    va[0] = v01.x; va[1] = v01.y; va[2] = v23.x; va[3] = v23.y;
+                    ex += stack_ex[(srcA * PPL + u) * 32 + lane];
+                }
+                matvec4(Pa, va, fa);
+            }
+            if (srcB == EPX_DFS_TIP) {
+                const int sb2 = tip_of(wb, u);
 #pragma unroll
-        for (int i = 0; i < 4; i++) { fa[i] *= fb[i]; hmax = max(hmax, __double2hiint(fa[i])); }
+                for (int i = 0; i < 4; i++) fb[i] = (sb2 < 4) ? Pb[i * 4 + sb2] : 1.0;
+            } else if (srcB == EPX_DFS_PREV) {
+                ex += cur_ex[u];
+                matvec4(Pb, cur[u], fb);
+            } else {
+                double vb[4] = {1.0, 1.0, 1.0, 1.0};
+                if (live[u]) {
+                    const double4a v = ld256(reinterpret_cast<const double*>(out_base[u] + (unsigned)pb * node_stride));
+                    vb[0] = v.x; vb[1] = v.y; vb[2] = v.z; vb[3] = v.w;
+                    ex += exp_base[u][(unsigned)pb * (unsigned)L];
+                }
+                matvec4(Pb, vb, fb);
+            }
+            // all values are >= 0, so the largest one has the largest high word: an integer max finds its exponent
+            int hmax = 0;
 #pragma unroll
-        for (int o = 1; o < G; o <<= 1) hmax = max(hmax, __shfl_xor_sync(FULL, hmax, o));
-        double sc = 1.0;
-        {
-            const int e = (hmax >> 20) - 1023;      // hmax < 0x7fe00000: finite and far from overflow
-            if (e > -1000 && hmax < 0x7fe00000) { sc = pow2_neg(e); ex += e; }
-        }
+            for (int i = 0; i < 4; i++) { fa[i] *= fb[i]; hmax = max(hmax, __double2hiint(fa[i])); }
 #pragma unroll
-        for (int i = 0; i < 4; i++) cur[i] = fa[i] * sc;
-        cur_ex = ex;
-        if (live) st256(reinterpret_cast<double*>(out_base + (unsigned)pidx * node_stride), cur[0], cur[1], cur[2], cur[3]);
-        if (live && c == 0) exp_base[(unsigned)pidx * (unsigned)L] = ex;
-        if (out_slot >= 0) {
-            stack[out_slot * 64 + lane] = make_double2(cur[0], cur[1]);
-            stack[out_slot * 64 + 32 + lane] = make_double2(cur[2], cur[3]);
-            stack_ex[out_slot * 32 + lane] = ex;
+            for (int o = 1; o < G; o <<= 1) hmax = max(hmax, __shfl_xor_sync(FULL, hmax, o));
+            double sc = 1.0;
+            {
+                const int e = (hmax >> 20) - 1023;      // hmax < 0x7fe00000: finite and far from overflow
+                if (e > -1000 && hmax < 0x7fe00000) { sc = pow2_neg(e); ex += e; }
+            }
+#pragma unroll
+            for (int i = 0; i < 4; i++) cur[u][i] = fa[i] * sc;
+            cur_ex[u] = ex;
+            if (live[u]) st256(reinterpret_cast<double*>(out_base[u] + (unsigned)pidx * node_stride), cur[u][0], cur[u][1], cur[u][2], cur[u][3]);
+            if (live[u] && c == 0) exp_base[u][(unsigned)pidx * (unsigned)L] = ex;
+            if (out_slot >= 0) {
+                stack[(out_slot * PPL + u) * 64 + lane] = make_double2(cur[u][0], cur[u][1]);
+                stack[(out_slot * PPL + u) * 64 + 32 + lane] = make_double2(cur[u][2], cur[u][3]);
+                stack_ex[(out_slot * PPL + u) * 32 + lane] = ex;
+            }
         }
         if (++buf == DFS_STAGES) buf = 0;
     }
 }
 
-size_t dfs_smem(int G, int depth) { return (size_t)DFS_STAGES * dfs_stage_bytes(G) + (size_t)depth * (128 * 8 + 32 * 4); }
+size_t dfs_smem(int G, int depth, int ppl) { return (size_t)DFS_STAGES * dfs_stage_bytes(G) + (size_t)depth * ppl * (128 * 8 + 32 * 4); }
 
 // ------------------------------------------------------------------------------------------------ any K
 constexpr int GT = 256;
@@ -490,7 +512,10 @@ int prune_tile(int K, int C)
 template <int C>
 static int dfs_set_attr()
 {
-    return cudaFuncSetAttribute(prune4_dfs_kernel<C>, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024) == cudaSuccess ? 0 : -1;
+    if (cudaFuncSetAttribute(prune4_dfs_kernel<C, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024) != cudaSuccess) return -1;
+    if (cudaFuncSetAttribute(prune4_dfs_kernel<C, 2>, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024) != cudaSuccess) return -1;
+    if (cudaFuncSetAttribute(prune4_dfs_kernel<C, 4>, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024) != cudaSuccess) return -1;
+    return 0;
 }
 
 int prune_init_attributes()
@@ -500,21 +525,45 @@ int prune_init_attributes()
     return cudaFuncSetAttribute(prune_generic_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024) == cudaSuccess ? 0 : -1;
 }
 
+int dfs_patterns_per_lane(const epx_ctx* c)
+{
+    if (c->dfs_ppl == 1 || c->dfs_ppl == 2 || c->dfs_ppl == 4) return c->dfs_ppl;
+    const int G = dfs_lanes_of(c->C);
+    const long tiles1 = (c->L + 32 / G - 1) / (32 / G);      // warps per piece at one pattern per lane
+    (void)tiles1;
+    return 1;      // measured on config 2: 0.78 ms (1), 0.83 ms (2), 1.09 ms (4) -- resident warps matter more than overhead
+}
+
+int dfs_tiles(const epx_ctx* c)
+{
+    const int pw = dfs_patterns_per_lane(c) * (32 / dfs_lanes_of(c->C));
+    return (c->L + pw - 1) / pw;
+}
+
 bool prune_uses_dfs(const epx_ctx* c)
 {
     return c->tree_mode && c->K == 4 && c->prune_kernel == 0 &&
            (double)(c->N - 1) * c->L * c->C < 4294967296.0 &&
-           dfs_smem(dfs_lanes_of(c->C), c->dfs_depth > 0 ? c->dfs_depth : 1) <= 227 * 1024;
+           dfs_smem(dfs_lanes_of(c->C), c->dfs_depth > 0 ? c->dfs_depth : 1, dfs_patterns_per_lane(c)) <= 227 * 1024;
+}
+
+template <int C, int PPL>
+static void launch_dfs2(const epx_ctx* c, int first_piece, int n_pieces, cudaStream_t s)
+{
+    const DevBuffers& d = c->d;
+    const int tiles = dfs_tiles(c);
+    prune4_dfs_kernel<C, PPL><<<n_pieces * tiles, 32, dfs_smem(dfs_lanes_of(C), c->dfs_depth, PPL), s>>>(d.dfs_ops,
+        d.dfs_pieces + first_piece, tiles, c->L, c->Lp, c->dfs_depth, d.P, d.tips, d.partials, d.scale_exp);
 }
 
 template <int C>
 static void launch_dfs(const epx_ctx* c, int first_piece, int n_pieces, cudaStream_t s)
 {
-    const DevBuffers& d = c->d;
-    constexpr int G = dfs_lanes_of(C);
-    const int tiles = (c->L + 32 / G - 1) / (32 / G);
-    prune4_dfs_kernel<C><<<n_pieces * tiles, 32, dfs_smem(G, c->dfs_depth), s>>>(d.dfs_ops, d.dfs_pieces + first_piece, tiles,
-        c->L, c->Lp, c->dfs_depth, d.P, d.tips, d.partials, d.scale_exp);
+    switch (dfs_patterns_per_lane(c)) {
+        case 1: launch_dfs2<C, 1>(c, first_piece, n_pieces, s); break;
+        case 2: launch_dfs2<C, 2>(c, first_piece, n_pieces, s); break;
+        default: launch_dfs2<C, 4>(c, first_piece, n_pieces, s); break;
+    }
 }
 
 // Launch 1: the bottom pieces (independent subtrees); launch 2: the top piece, which reads their roots from HBM.
