@@ -144,8 +144,10 @@ int epx_measure_fp64_peak(int device, int kind, double ms_target, void* dev_scra
 enum {
     EPX_OPT_CHAIN_KERNEL = 1, /* 0 auto (default); 1 force the generic shared-memory chain kernel */
     EPX_OPT_USE_GRAPH = 2,    /* 1 (default) replay the kernel sequence from a CUDA graph on non-default streams; 0 launch directly */
-    EPX_OPT_PRUNE_KERNEL = 3, /* 0 auto (default: K == 4 walks the tree depth first in one launch); 1 force the generic
-                                 shared-memory level kernel; 2 (K == 4) the level-by-level register kernel */
+    EPX_OPT_PRUNE_KERNEL = 3, /* 0 auto (default: K == 4 walks the tree depth first, partials never re-read from HBM);
+                                 1 force the generic shared-memory level kernel; 2 (K == 4) the level-by-level register
+                                 kernel; 3 (K == 4) the depth-first walk with the 4x4 products on the FP64 tensor pipe
+                                 (mma.sync m8n8k4; measured 5 % slower than 0 on config 2, kept for comparison) */
     EPX_OPT_EXP_METHOD = 4,   /* a3 method.  1 spectral: Jacobi eigensystem (reversible) / Pade 13 (asymmetric), absolute
                                  error ~1e-14 per entry.  2 componentwise: shifted non-negative Taylor scaling-and-squaring,
                                  every entry to a few hundred ulp RELATIVE, ~8 dense products per segment.  0 auto (default):

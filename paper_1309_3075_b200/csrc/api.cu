@@ -350,7 +350,10 @@ int epx_set_option(epx_ctx* c, int option, int value)
     switch (option) {
         case 1: c->chain_kernel = value; break;
         case 2: c->use_graph = value; break;
-        case 3: c->prune_kernel = value; break;
+        case 3:
+            c->prune_kernel = value;
+            if (c->has_tree) { int rc = build_plan(c); if (rc) return rc; c->tree_dirty = true; }   // pieces depend on the kernel's tile
+            break;
         case 4: if (value < 0 || value > 2) return fail(c, EPX_E_ARG, "exp method %d", value); c->exp_method = value; break;
         case 5: c->stage_events = value ? 1 : 0; break;
         case 6:

@@ -351,6 +351,205 @@ __global__ void __launch_bounds__(32) prune4_dfs_kernel(const DfsOp* __restrict_
     }
 }
 
+
+// ------------------------------------------------------------------------------------------------ K == 4, depth first, DMMA
+// Same walk as prune4_dfs_kernel, but the 4x4 matrix-vector products of a warp's 8 patterns x C categories run on the
+// FP64 tensor pipe.  Why: in the scalar kernel every lane needs both children's whole 4x4 matrices in registers (256 B per
+// lane and node); that register fill plus the staging ring saturate the SM's L1 / shared-memory data pipe (ncu:
+// l1tex__data_pipe_lsu_wavefronts = 93 % of the cycles, profiles/r1_prune4_dfs_ncu.md).  mma.sync.m8n8k4.f64 takes ONE double of
+// the matrix and ONE of the vector per lane and does the broadcast inside the tensor core.  Per child and pair of
+// categories (c, c'), transposed so that a lane ends up with one pattern:
+//   A (8x4) = V_c^T resp. V_c'^T : row = pattern, column = child state j
+//   B (4x8) = [P_c^T | 0] resp. [0 | P_c'^T] : row = j, column n = (category n >> 2, parent state i = n & 3)
+//   D (8x8) = A_c B_lo + A_c' B_hi : row = pattern, column = (category, i)     (adding the zero columns is exact)
+// Fragment owners (lane = 4 g + q): A[g][q], B[q][g], D[g][2q], D[g][2q+1] -- lane (g, q) holds, for pattern g, states
+// 2 (q & 1), 2 (q & 1) + 1 of category 2 pr + (q >> 1), and needs, as the next A operand, state q of every category of
+// pattern g.  Every result is therefore written once to a shared-memory slot (stack slot or one of two hand-over slots;
+// XOR-swizzled so both access patterns are bank-conflict free) and once to HBM.  Tips enter as indicator rows (all-ones
+// rows if missing), HBM-sourced children of the top piece as plain loads.  The 4x4 matrices are read straight from
+// global memory (L1-resident: every warp on the SM walks the same nodes), one operation ahead, 4 doubles per lane.
+__device__ __forceinline__ void dmma884(double& d0, double& d1, double a, double b)
+{
+    asm("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1}, {%2}, {%3}, {%0,%1};" : "+d"(d0), "+d"(d1) : "d"(a), "d"(b));
+}
+__host__ __device__ constexpr int mma_cpad(int C) { return C <= 4 ? 4 : 8; }
+__host__ __device__ constexpr int mma_slot_doubles(int C) { return 8 * mma_cpad(C) * 4; }
+// slot element (pattern, category, state): the category's low two bits are XORed with h(pattern & 3), h = {0, 2, 1, 3}
+template <int C>
+__device__ __forceinline__ int slot_addr(int pattern, int cat, int state)
+{
+    const int h = ((pattern & 1) << 1) | ((pattern >> 1) & 1);
+    return pattern * (mma_cpad(C) * 4) + (((cat & ~3) | ((cat & 3) ^ h)) << 2) + state;
+}
+
+template <int C>
+__global__ void __launch_bounds__(32) prune4_mma_kernel(const DfsOp* __restrict__ ops, const DfsPiece* __restrict__ pieces,
+    int tiles, int L, int Lp, int depth, const double* __restrict__ P, const uint8_t* __restrict__ tips,
+    double* __restrict__ partials, int32_t* __restrict__ scale_exp)
+{
+    extern __shared__ __align__(16) unsigned char smraw[];
+    constexpr int NP = (C + 1) / 2;                 // category pairs
+    constexpr int SLOT = mma_slot_doubles(C);
+    constexpr unsigned FULL = 0xffffffffu;
+    double* slots = reinterpret_cast<double*>(smraw);                              // [depth + 2][SLOT]
+    int* slot_ex = reinterpret_cast<int*>(slots + (size_t)(depth + 2) * SLOT);     // [depth + 2][8]
+    const int lane = threadIdx.x, g = lane >> 2, q = lane & 3, hi = g >> 2, sp = q & 1;
+    const double m_lo = hi ? 0.0 : 1.0, m_hi = hi ? 1.0 : 0.0;
+    const int piece = blockIdx.x / tiles, tile = blockIdx.x - piece * tiles;
+    const int p0 = tile * 8;
+    const DfsPiece pc = pieces[piece];
+    const int n_ops = pc.end - pc.begin;
+    ops += pc.begin;
+
+    const unsigned node_stride = (unsigned)L * C * 4;             // doubles per node (< 2^32); node offsets are 32 x 32 -> 64 bit
+    const bool live = p0 + g < L;
+    const double* const inA = partials + ((size_t)(p0 + g) * C) * 4 + q;          // A-operand view: pattern g, state q
+    double* const outD = partials + ((size_t)(p0 + g) * C) * 4 + 2 * sp;          // D view: pattern g, states 2sp, 2sp+1
+    int32_t* const exp_g = scale_exp + p0 + g;
+    int rd_addr[C], wr_addr[NP], pm_off[NP];
+    bool cat_ok[NP];
+#pragma unroll
+    for (int cat = 0; cat < C; cat++) rd_addr[cat] = slot_addr<C>(g, cat, q);
+#pragma unroll
+    for (int pr = 0; pr < NP; pr++) {
+        const int cat_l = 2 * pr + (q >> 1);                      // category this lane's D columns belong to
+        cat_ok[pr] = cat_l < C;
+        wr_addr[pr] = slot_addr<C>(g, min(cat_l, C - 1), 2 * sp);
+        pm_off[pr] = min(2 * pr + hi, C - 1) * 16 + (g & 3) * 4 + q;        // B fragment: P[cat][i = g & 3][j = q]
+    }
+
+    struct Block { int4 d; int2 h; uint32_t ta[2], tb[2]; };
+    auto load_block = [&](int base) -> Block {      // lane j: descriptor base + j and its tip states (8 patterns = 2 words)
+        Block b;
+        b.d = make_int4(0, 0, 0, 0);
+        b.h = make_int2(0, 0);
+        b.ta[0] = b.ta[1] = b.tb[0] = b.tb[1] = 0xffffffffu;
+        const int k = base + lane;
+        if (k < n_ops) {
+            const int4* src = reinterpret_cast<const int4*>(ops + k);
+            b.d = __ldg(src);
+            const int4 h = __ldg(src + 1);
+            b.h = make_int2(h.x, h.y);
+            if ((b.d.w & 0xff) - 3 == EPX_DFS_TIP) {
+                const uint2 t = __ldg(reinterpret_cast<const uint2*>(tips + p0 + (size_t)b.d.x * Lp));
+                b.ta[0] = t.x; b.ta[1] = t.y;
+            }
+            if (((b.d.w >> 8) & 0xff) - 3 == EPX_DFS_TIP) {
+                const uint2 t = __ldg(reinterpret_cast<const uint2*>(tips + p0 + (size_t)b.d.y * Lp));
+                b.tb[0] = t.x; b.tb[1] = t.y;
+            }
+        }
+        return b;
+    };
+    Block cb = load_block(0), nb = load_block(32);
+
+    // B fragments (matrix entries) of operation j, j in the current or the next block of 32
+    auto load_frags = [&](int j, int k, double (&fa)[NP], double (&fb)[NP]) {
+        const bool in_cur = (j >> 5) == (k >> 5);
+        const int na = __shfl_sync(FULL, in_cur ? cb.d.x : nb.d.x, j & 31);
+        const int nbn = __shfl_sync(FULL, in_cur ? cb.d.y : nb.d.y, j & 31);
+        const double* Pa = P + (size_t)na * (C * 16);
+        const double* Pb = P + (size_t)nbn * (C * 16);
+#pragma unroll
+        for (int pr = 0; pr < NP; pr++) { fa[pr] = __ldg(Pa + pm_off[pr]); fb[pr] = __ldg(Pb + pm_off[pr]); }
+    };
+
+    // one child's contribution in D layout: f[pr][e] = state 2sp + e of category 2pr + (q >> 1), pattern g
+    auto child = [&](int src, const double (&bf)[NP], uint32_t t0, uint32_t t1, int hbm_pidx, int prev_slot,
+                     double (&f)[NP][2], int& ex) {
+        double a[C];
+        if (src == EPX_DFS_TIP) {
+            const int s = ((hi ? t1 : t0) >> (8 * (g & 3))) & 0xff;           // tip state of pattern g
+            const double v = s < 4 ? (s == q ? 1.0 : 0.0) : 1.0;
+#pragma unroll
+            for (int cat = 0; cat < C; cat++) a[cat] = v;
+        } else if (src == EPX_DFS_HBM) {
+            const double* base = inA + (unsigned long long)(unsigned)hbm_pidx * node_stride;
+#pragma unroll
+            for (int cat = 0; cat < C; cat++) a[cat] = live ? base[cat * 4] : 1.0;
+            ex += live ? exp_g[(size_t)hbm_pidx * L] : 0;
+        } else {
+            const int sl = src == EPX_DFS_PREV ? prev_slot : src;
+            const double* S = slots + sl * SLOT;
+#pragma unroll
+            for (int cat = 0; cat < C; cat++) a[cat] = S[rd_addr[cat]];
+            ex += slot_ex[sl * 8 + g];
+        }
+#pragma unroll
+        for (int pr = 0; pr < NP; pr++) {
+            const double b_lo = bf[pr] * m_lo, b_hi = bf[pr] * m_hi;      // zero the other category's columns (0 * finite = 0)
+            double d0 = 0.0, d1 = 0.0;
+            dmma884(d0, d1, a[2 * pr], b_lo);
+            if (2 * pr + 1 < C) dmma884(d0, d1, a[2 * pr + 1], b_hi);
+            f[pr][0] = d0; f[pr][1] = d1;
+        }
+    };
+
+    auto step = [&](int k, const double (&pa_cur)[NP], const double (&pb_cur)[NP], double (&pa_nxt)[NP], double (&pb_nxt)[NP]) {
+        if ((k & 31) == 0 && k > 0) { cb = nb; nb = load_block(k + 32); }
+        if (k + 1 < n_ops) load_frags(k + 1, k, pa_nxt, pb_nxt);
+        const int src_lane = k & 31;
+        const int pidx = __shfl_sync(FULL, cb.d.z, src_lane);
+        const int code = __shfl_sync(FULL, cb.d.w, src_lane);
+        const int srcA = (code & 0xff) - 3, srcB = ((code >> 8) & 0xff) - 3, out_slot = ((code >> 16) & 0xff) - 1;
+        uint32_t ta0 = 0, ta1 = 0, tb0 = 0, tb1 = 0;
+        int pa = 0, pb = 0;
+        if (srcA == EPX_DFS_TIP) { ta0 = __shfl_sync(FULL, cb.ta[0], src_lane); ta1 = __shfl_sync(FULL, cb.ta[1], src_lane); }
+        else if (srcA == EPX_DFS_HBM) pa = __shfl_sync(FULL, cb.h.x, src_lane);
+        if (srcB == EPX_DFS_TIP) { tb0 = __shfl_sync(FULL, cb.tb[0], src_lane); tb1 = __shfl_sync(FULL, cb.tb[1], src_lane); }
+        else if (srcB == EPX_DFS_HBM) pb = __shfl_sync(FULL, cb.h.y, src_lane);
+
+        __syncwarp();                               // the slot writes of operation k-1 are visible
+        double fa[NP][2], fb[NP][2];
+        int ex = 0;
+        const int prev_slot = depth + ((k + 1) & 1), my_scratch = depth + (k & 1);
+        child(srcA, pa_cur, ta0, ta1, pa, prev_slot, fa, ex);
+        child(srcB, pb_cur, tb0, tb1, pb, prev_slot, fb, ex);
+
+        // all values are >= 0, so the largest one has the largest high word: an integer max finds its exponent
+        int hmax = 0;
+#pragma unroll
+        for (int pr = 0; pr < NP; pr++) {
+            fa[pr][0] *= fb[pr][0];
+            fa[pr][1] *= fb[pr][1];
+            if (cat_ok[pr]) hmax = max(hmax, max(__double2hiint(fa[pr][0]), __double2hiint(fa[pr][1])));
+        }
+        hmax = max(hmax, __shfl_xor_sync(FULL, hmax, 1));
+        hmax = max(hmax, __shfl_xor_sync(FULL, hmax, 2));
+        double sc = 1.0;
+        {
+            const int e = (hmax >> 20) - 1023;      // hmax < 0x7fe00000: finite and far from overflow
+            if (e > -1000 && hmax < 0x7fe00000) { sc = pow2_neg(e); ex += e; }
+        }
+        const int dst = out_slot >= 0 ? out_slot : my_scratch;
+        double* S = slots + dst * SLOT;
+        double* o = outD + (unsigned long long)(unsigned)pidx * node_stride;
+        __syncwarp();                               // every lane has fetched its operands (dst may be the slot just consumed)
+#pragma unroll
+        for (int pr = 0; pr < NP; pr++) {
+            const double2 v = make_double2(fa[pr][0] * sc, fa[pr][1] * sc);
+            if (cat_ok[pr]) {
+                *reinterpret_cast<double2*>(S + wr_addr[pr]) = v;
+                if (live) *reinterpret_cast<double2*>(o + (2 * pr + (q >> 1)) * 4) = v;
+            }
+        }
+        if (q == 0) {
+            slot_ex[dst * 8 + g] = ex;
+            if (live) exp_g[(size_t)pidx * L] = ex;
+        }
+    };
+    // (unrolling by two with the fragment sets swapping roles was measured slower: 90 registers, 1.00 vs 0.82 ms)
+    double pa_cur[NP], pb_cur[NP], pa_nxt[NP], pb_nxt[NP];
+    load_frags(0, 0, pa_cur, pb_cur);
+    for (int k = 0; k < n_ops; k++) {
+        step(k, pa_cur, pb_cur, pa_nxt, pb_nxt);
+#pragma unroll
+        for (int pr = 0; pr < NP; pr++) { pa_cur[pr] = pa_nxt[pr]; pb_cur[pr] = pb_nxt[pr]; }
+    }
+}
+
+size_t mma_smem(int C, int depth) { return 8 * (size_t)(depth + 2) * mma_slot_doubles(C) + (size_t)(depth + 2) * 32; }
+
 size_t dfs_smem(int G, int depth, int ppl) { return (size_t)DFS_STAGES * dfs_stage_bytes(G) + (size_t)depth * ppl * (128 * 8 + 32 * 4); }
 
 // ------------------------------------------------------------------------------------------------ any K
@@ -512,6 +711,7 @@ int prune_tile(int K, int C)
 template <int C>
 static int dfs_set_attr()
 {
+    if (cudaFuncSetAttribute(prune4_mma_kernel<C>, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024) != cudaSuccess) return -1;
     if (cudaFuncSetAttribute(prune4_dfs_kernel<C, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024) != cudaSuccess) return -1;
     if (cudaFuncSetAttribute(prune4_dfs_kernel<C, 2>, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024) != cudaSuccess) return -1;
     if (cudaFuncSetAttribute(prune4_dfs_kernel<C, 4>, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024) != cudaSuccess) return -1;
@@ -536,15 +736,18 @@ int dfs_patterns_per_lane(const epx_ctx* c)
 
 int dfs_tiles(const epx_ctx* c)
 {
+    if (c->prune_kernel == 3) return (c->L + 7) / 8;          // tensor-core walk: 8 patterns per warp
     const int pw = dfs_patterns_per_lane(c) * (32 / dfs_lanes_of(c->C));
     return (c->L + pw - 1) / pw;
 }
 
 bool prune_uses_dfs(const epx_ctx* c)
 {
-    return c->tree_mode && c->K == 4 && c->prune_kernel == 0 &&
-           (double)(c->N - 1) * c->L * c->C < 4294967296.0 &&
-           dfs_smem(dfs_lanes_of(c->C), c->dfs_depth > 0 ? c->dfs_depth : 1, dfs_patterns_per_lane(c)) <= 227 * 1024;
+    if (!(c->tree_mode && c->K == 4 && (c->prune_kernel == 0 || c->prune_kernel == 3))) return false;
+    const int depth = c->dfs_depth > 0 ? c->dfs_depth : 1;
+    if (c->prune_kernel == 3) return (double)c->L * c->C * 4 < 4294967296.0 && mma_smem(c->C, depth) <= 227 * 1024;
+    if ((double)(c->N - 1) * c->L * c->C >= 4294967296.0) return false;
+    return dfs_smem(dfs_lanes_of(c->C), depth, dfs_patterns_per_lane(c)) <= 227 * 1024;
 }
 
 template <int C, int PPL>
@@ -559,6 +762,13 @@ static void launch_dfs2(const epx_ctx* c, int first_piece, int n_pieces, cudaStr
 template <int C>
 static void launch_dfs(const epx_ctx* c, int first_piece, int n_pieces, cudaStream_t s)
 {
+    if (c->prune_kernel == 3) {
+        const DevBuffers& d = c->d;
+        const int tiles = dfs_tiles(c);
+        prune4_mma_kernel<C><<<n_pieces * tiles, 32, mma_smem(C, c->dfs_depth), s>>>(d.dfs_ops, d.dfs_pieces + first_piece, tiles,
+            c->L, c->Lp, c->dfs_depth, d.P, d.tips, d.partials, d.scale_exp);
+        return;
+    }
     switch (dfs_patterns_per_lane(c)) {
         case 1: launch_dfs2<C, 1>(c, first_piece, n_pieces, s); break;
         case 2: launch_dfs2<C, 2>(c, first_piece, n_pieces, s); break;

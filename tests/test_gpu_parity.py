@@ -94,6 +94,8 @@ def test_config2_reduced(epx, orc_ld):
     # several pattern tiles plus a ragged tail (L = 777 = 3*256 + 9 = 97*8 + 1), 10 epochs, dated tips
     prob = W.make_config(2, N=150, L=777)
     run_tree(epx, orc_ld, prob)                                                  # depth-first walk (default)
+    run_tree(epx, orc_ld, prob, options=[(epx.EPX_OPT_PRUNE_KERNEL, 3)])         # depth-first walk, 4x4 products on the FP64 tensor pipe
+    run_tree(epx, orc_ld, prob, options=[(epx.EPX_OPT_PRUNE_KERNEL, 3), (epx.EPX_OPT_DFS_PPL, 2)])
     run_tree(epx, orc_ld, prob, options=[(epx.EPX_OPT_PRUNE_KERNEL, 2)])         # level-by-level register kernel
     run_tree(epx, orc_ld, prob, options=[(epx.EPX_OPT_PRUNE_KERNEL, 1)])         # generic shared-memory kernel
 
@@ -109,6 +111,7 @@ def test_k4_every_category_count(epx, orc_ld, C):
     tips[5, :] = 99
     prob = dataclasses.replace(prob, C=C, rates=rates, weights=weights, tip_states=tips)
     run_tree(epx, orc_ld, prob)
+    run_tree(epx, orc_ld, prob, options=[(epx.EPX_OPT_PRUNE_KERNEL, 3)])
     run_tree(epx, orc_ld, prob, options=[(epx.EPX_OPT_PRUNE_KERNEL, 2)], partial_nodes=[prob.n_nodes - 1])
 
 
@@ -147,6 +150,7 @@ def test_k4_extreme_tree_shapes(epx, orc_ld, shape, N):
     parent, height = _shaped_tree(shape, N)
     prob = dataclasses.replace(prob, parent=parent, height=height)
     run_tree(epx, orc_ld, prob)
+    run_tree(epx, orc_ld, prob, options=[(epx.EPX_OPT_PRUNE_KERNEL, 3)])
 
 
 def test_config2_full_size(epx, orc_ld):
