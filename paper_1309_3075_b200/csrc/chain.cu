@@ -176,15 +176,17 @@ __device__ __forceinline__ void bulk_g2s(void* dst, const void* src, uint32_t by
                  ::"r"(smem_u32(dst)), "l"(src), "r"(bytes), "r"(smem_u32(bar)) : "memory");
 }
 
-constexpr int DT = 256;                 // 8 warps: warp w -> category (w>>1), rows 32*(w&1) .. +32
+constexpr int CPC = 2;                  // categories per CTA: 2 -> 128 threads, 66 KB, two CTAs per SM overlap each other's
+                                        // prologue (U fragments from L2) and epilogue (P store) with DMMA work
+constexpr int DT = 64 * CPC;            // warp w -> category (w>>1) of the CTA, rows 32*(w&1) .. +32
 constexpr int FRAG_DOUBLES = 4096;      // one 64x64 operand in fragment order
 struct DmmaSmem {
     double B[2][FRAG_DOUBLES];          // TMA destination ring (2 x 32 KB)
-    double D[2][4][64];                 // exp(lambda r d) per stage / category
+    double D[2][CPC][64];               // exp(lambda r d) per stage / category
     uint64_t bar[2];
 };
 
-__global__ void __launch_bounds__(DT, 1) chain_dmma64_kernel(int K, int C, const int32_t* __restrict__ order,
+__global__ void __launch_bounds__(DT, 2) chain_dmma64_kernel(int K, int C, const int32_t* __restrict__ order,
     const int32_t* __restrict__ n_seg, const int32_t* __restrict__ seg_off, const int32_t* __restrict__ seg_epoch,
     const double* __restrict__ seg_dur, const double* __restrict__ rates, const double* __restrict__ lam,
     const double* __restrict__ WB, const double* __restrict__ UTB, const double* __restrict__ sp,
@@ -194,13 +196,13 @@ __global__ void __launch_bounds__(DT, 1) chain_dmma64_kernel(int K, int C, const
     DmmaSmem& sm = *reinterpret_cast<DmmaSmem*>(smraw);
     const int tid = threadIdx.x, lane = tid & 31, w = tid >> 5;
     const int g = lane >> 2, q = lane & 3;
-    const int ncg = (C + 3) >> 2;
+    const int ncg = (C + CPC - 1) / CPC;
     const int b = order[blockIdx.x / ncg], cg = blockIdx.x % ncg;
-    const int c = cg * 4 + (w >> 1), half = w & 1;
+    const int c = cg * CPC + (w >> 1), half = w & 1;
     const bool active = c < C;
     const int n = n_seg[b];
     if (n == 0) {
-        for (int cc = cg * 4; cc < min(C, cg * 4 + 4); cc++) {
+        for (int cc = cg * CPC; cc < min(C, cg * CPC + CPC); cc++) {
             double* out = P + ((size_t)b * C + cc) * K * K;
             for (int idx = tid; idx < K * K; idx += DT) out[idx] = (idx / K == idx % K) ? 1.0 : 0.0;
         }
@@ -214,7 +216,7 @@ __global__ void __launch_bounds__(DT, 1) chain_dmma64_kernel(int K, int C, const
         return (t < n - 1) ? WB + (size_t)seg_epoch[off + t] * FRAG_DOUBLES : UTB + (size_t)e_lo * FRAG_DOUBLES;
     };
     auto fill_D = [&](int t) {     // one value per thread: category tid>>6, eigen index tid&63
-        int cc = cg * 4 + (tid >> 6), k = tid & 63;
+        int cc = cg * CPC + (tid >> 6), k = tid & 63;
         double r = cc < C ? rates[cc] : 0.0;
         sm.D[t & 1][tid >> 6][k] = exp(lam[seg_epoch[off + t] * 64 + k] * (r * seg_dur[off + t]));
     };
@@ -273,21 +275,17 @@ __global__ void __launch_bounds__(DT, 1) chain_dmma64_kernel(int K, int C, const
                         acc[2 * mp + mi][kt][1] = 0.0;
                     }
                 }
-                // issue order: four different accumulator tiles between two DMMAs on the same one (DMMA latency)
 #pragma unroll
                 for (int kt = 0; kt < 8; kt++)
 #pragma unroll
-                    for (int np = 0; np < 4; np++) {
-                        const double2 b0 = Bs[(kt * 8 + 2 * np) * 32 + lane], b1 = Bs[(kt * 8 + 2 * np + 1) * 32 + lane];
+                    for (int nt = 0; nt < 8; nt++) {
+                        const double2 bv = Bs[(kt * 8 + nt) * 32 + lane];
+                        // h outer, mi inner: two other DMMAs sit between the two that update the same accumulator tile
 #pragma unroll
                         for (int h = 0; h < 2; h++)
 #pragma unroll
-                            for (int nn = 0; nn < 2; nn++)
-#pragma unroll
-                                for (int mi = 0; mi < 2; mi++) {
-                                    const double bb = nn ? (h ? b1.y : b1.x) : (h ? b0.y : b0.x);
-                                    dmma884(acc[2 * mp + mi][2 * np + nn][0], acc[2 * mp + mi][2 * np + nn][1], a[mi][kt][h], bb);
-                                }
+                            for (int mi = 0; mi < 2; mi++)
+                                dmma884(acc[2 * mp + mi][nt][0], acc[2 * mp + mi][nt][1], a[mi][kt][h], h ? bv.y : bv.x);
                     }
             }
         }
@@ -336,7 +334,7 @@ int launch_chain_reversible(const epx_ctx* c, cudaStream_t s)
         chain_rows_kernel<4><<<blocks, 256, 0, s>>>(n, C, d.n_seg, d.seg_off, d.seg_epoch, d.seg_dur, d.rates, d.lam,
                                                     d.U, d.W, d.sp, d.isp, d.P, d.status);
     } else if (Kp == 64 && c->chain_kernel != 1) {
-        int ncg = (C + 3) / 4;
+        int ncg = (C + CPC - 1) / CPC;
         chain_dmma64_kernel<<<n * ncg, DT, sizeof(DmmaSmem), s>>>(K, C, d.order, d.n_seg, d.seg_off, d.seg_epoch,
                                                                  d.seg_dur, d.rates, d.lam, d.WB, d.UTB, d.sp, d.isp,
                                                                  d.P, d.status);
