@@ -36,8 +36,8 @@ if ROOT not in sys.path:
 import workloads as W  # noqa: E402  (input generators only; shared with the oracle, holds no arithmetic of the method)
 
 # dram__bytes_read.sum + dram__bytes_write.sum of the pruning launches of one config-2 step, from the committed
-# `ncu --set full` capture (profiles/r1_prune4_dfs_ncu.md): 2561.7 + 23.1 MB (bottom pieces) + 15.9 MB (top piece)
-NCU_TRAFFIC_BYTES_PER_STEP = 2.6007e9
+# `ncu --set full` capture (profiles/r1_prune4_dfs_ncu.md): 2561.8 + 23.1 MB (bottom pieces) + 15.9 MB (top piece)
+NCU_TRAFFIC_BYTES_PER_STEP = 2.6008e9
 
 METRIC = "pruning partials GB/s (fp64) over the whole a1..a6 log-likelihood step; epoch branch matrices/s in `matrices`"
 UNIT = "GB/s"
@@ -373,6 +373,7 @@ def bench_matrices(torch, epx, device: int, K: int) -> dict:
             "config": {"workload": W.CONFIG_NAMES[5], "K": prob.K, "M": prob.M, "C": prob.C, "n_br": prob.n_br,
                        "segments": int(nseg.sum()), "l2": "2.38 GB of P written per step vs 126 MB L2"},
             "roofline": {"bound": "alu", "kernel": "chain_dmma64_kernel (a3+a4 fused, mma.sync m8n8k4 f64)",
+                         "tensor_pipe_active_ncu": 0.795,   # sm__pipe_tensor_subpipe_dmma_cycles_active, profiles/r1_chain_dmma64_ncu.md
                          "achieved": achieved, "peak": dmma, "unit": "TFLOP/s", "frac": achieved / dmma,
                          "traffic": None, "peak_source": "measured in this run by epx_measure_fp64_peak "
                                                          "(register-only DMMA m8n8k4 loop); DFMA peak beside it",
