@@ -10,6 +10,7 @@
 #include <cstdarg>
 #include <cstdio>
 #include <cstring>
+#include <cstdlib>
 #include <thread>
 
 namespace {
@@ -174,7 +175,8 @@ int build_plan(epx_ctx* c)
     std::vector<int> cuts;
     {
         const long tiles = dfs_tiles(c);
-        const long want = std::min<long>(64, 4 * ((148L * 24 + tiles - 1) / tiles));   // pieces wanted (1 = no cut)
+        long want = std::min<long>(64, 4 * ((148L * 24 + tiles - 1) / tiles));   // pieces wanted (1 = no cut)
+        if (getenv("EPX_DFS_WANT")) want = atol(getenv("EPX_DFS_WANT"));
         std::vector<int> heap{root};          // max-heap on subtree size
         auto cmp = [&](int x, int y) { return size[x] < size[y]; };
         while (want >= 8 && (long)heap.size() + (long)cuts.size() < want) {

@@ -120,7 +120,7 @@ template <int N>
 __device__ __forceinline__ void cp_async_wait() { asm volatile("cp.async.wait_group %0;" ::"n"(N) : "memory"); }
 
 #ifndef EPX_DFS_STAGES
-#define EPX_DFS_STAGES 5
+#define EPX_DFS_STAGES 3
 #endif
 constexpr int DFS_STAGES = EPX_DFS_STAGES;   // matrix staging ring: operation k+STAGES-1 is in flight while operation k computes
 constexpr int DFS_PSTRIDE = 20;        // doubles per staged 4x4 matrix: 160 B = 40 banks, so 4 categories never share a bank
@@ -286,65 +286,92 @@ __global__ void __launch_bounds__(32) prune4_dfs_kernel(const DfsOp* __restrict_
         __syncwarp();                               // ... and so have every other lane's
         const double* Pa = Pm_base + buf * (SB / 8);
         const double* Pb = Pa + G * DFS_PSTRIDE;
+        // A matrix is read from shared memory ONCE per operation and serves the lane's PPL patterns from registers: the
+        // register fill of the matrices is what saturates the L1 / shared-memory data pipe (profiles/r1_prune4_dfs_ncu.md)
+        double fa[PPL][4], fb[PPL][4];
+        int ex[PPL];
 #pragma unroll
-        for (int u = 0; u < PPL; u++) {
-            double fa[4], fb[4];
-            int ex = 0;
-            if (srcA == EPX_DFS_TIP) {
+        for (int u = 0; u < PPL; u++) ex[u] = 0;
+        if (srcA == EPX_DFS_TIP) {
+#pragma unroll
+            for (int u = 0; u < PPL; u++) {
                 const int sa = tip_of(wa, u);
 #pragma unroll
-                for (int i = 0; i < 4; i++) fa[i] = (sa < 4) ? Pa[i * 4 + sa] : 1.0;
-            } else {
+                for (int i = 0; i < 4; i++) fa[u][i] = (sa < 4) ? Pa[i * 4 + sa] : 1.0;
+            }
+        } else {
+            double m[16];
+#pragma unroll
+            for (int i = 0; i < 8; i++) { const double2 r = *reinterpret_cast<const double2*>(Pa + 2 * i); m[2 * i] = r.x; m[2 * i + 1] = r.y; }
+#pragma unroll
+            for (int u = 0; u < PPL; u++) {
                 double va[4] = {1.0, 1.0, 1.0, 1.0};
                 if (srcA == EPX_DFS_HBM) {
                     if (live[u]) {
                         const double4a v = ld256(reinterpret_cast<const double*>(out_base[u] + (unsigned)pa * node_stride));
                         va[0] = v.x; va[1] = v.y; va[2] = v.z; va[3] = v.w;
-                        ex += exp_base[u][(unsigned)pa * (unsigned)L];
+                        ex[u] += exp_base[u][(unsigned)pa * (unsigned)L];
                     }
                 } else {
                     const double2 v01 = stack[(srcA * PPL + u) * 64 + lane], v23 = stack[(srcA * PPL + u) * 64 + 32 + lane];
                     va[0] = v01.x; va[1] = v01.y; va[2] = v23.x; va[3] = v23.y;
-                    ex += stack_ex[(srcA * PPL + u) * 32 + lane];
+                    ex[u] += stack_ex[(srcA * PPL + u) * 32 + lane];
                 }
-                matvec4(Pa, va, fa);
+#pragma unroll
+                for (int i = 0; i < 4; i++)
+                    fa[u][i] = fma(m[i * 4 + 3], va[3], fma(m[i * 4 + 2], va[2], fma(m[i * 4 + 1], va[1], m[i * 4] * va[0])));
             }
-            if (srcB == EPX_DFS_TIP) {
+        }
+        if (srcB == EPX_DFS_TIP) {
+#pragma unroll
+            for (int u = 0; u < PPL; u++) {
                 const int sb2 = tip_of(wb, u);
 #pragma unroll
-                for (int i = 0; i < 4; i++) fb[i] = (sb2 < 4) ? Pb[i * 4 + sb2] : 1.0;
-            } else if (srcB == EPX_DFS_PREV) {
-                ex += cur_ex[u];
-                matvec4(Pb, cur[u], fb);
-            } else {
+                for (int i = 0; i < 4; i++) fb[u][i] = (sb2 < 4) ? Pb[i * 4 + sb2] : 1.0;
+            }
+        } else {
+            double m[16];
+#pragma unroll
+            for (int i = 0; i < 8; i++) { const double2 r = *reinterpret_cast<const double2*>(Pb + 2 * i); m[2 * i] = r.x; m[2 * i + 1] = r.y; }
+#pragma unroll
+            for (int u = 0; u < PPL; u++) {
                 double vb[4] = {1.0, 1.0, 1.0, 1.0};
-                if (live[u]) {
+                if (srcB == EPX_DFS_PREV) {
+#pragma unroll
+                    for (int i = 0; i < 4; i++) vb[i] = cur[u][i];
+                    ex[u] += cur_ex[u];
+                } else if (live[u]) {
                     const double4a v = ld256(reinterpret_cast<const double*>(out_base[u] + (unsigned)pb * node_stride));
                     vb[0] = v.x; vb[1] = v.y; vb[2] = v.z; vb[3] = v.w;
-                    ex += exp_base[u][(unsigned)pb * (unsigned)L];
+                    ex[u] += exp_base[u][(unsigned)pb * (unsigned)L];
                 }
-                matvec4(Pb, vb, fb);
+#pragma unroll
+                for (int i = 0; i < 4; i++)
+                    fb[u][i] = fma(m[i * 4 + 3], vb[3], fma(m[i * 4 + 2], vb[2], fma(m[i * 4 + 1], vb[1], m[i * 4] * vb[0])));
             }
+        }
+#pragma unroll
+        for (int u = 0; u < PPL; u++) {
             // all values are >= 0, so the largest one has the largest high word: an integer max finds its exponent
             int hmax = 0;
 #pragma unroll
-            for (int i = 0; i < 4; i++) { fa[i] *= fb[i]; hmax = max(hmax, __double2hiint(fa[i])); }
+            for (int i = 0; i < 4; i++) { fa[u][i] *= fb[u][i]; hmax = max(hmax, __double2hiint(fa[u][i])); }
 #pragma unroll
             for (int o = 1; o < G; o <<= 1) hmax = max(hmax, __shfl_xor_sync(FULL, hmax, o));
             double sc = 1.0;
             {
                 const int e = (hmax >> 20) - 1023;      // hmax < 0x7fe00000: finite and far from overflow
-                if (e > -1000 && hmax < 0x7fe00000) { sc = pow2_neg(e); ex += e; }
+                if (e > -1000 && hmax < 0x7fe00000) { sc = pow2_neg(e); ex[u] += e; }
             }
 #pragma unroll
-            for (int i = 0; i < 4; i++) cur[u][i] = fa[i] * sc;
-            cur_ex[u] = ex;
+            for (int i = 0; i < 4; i++) cur[u][i] = fa[u][i] * sc;
+            cur_ex[u] = ex[u];
             if (live[u]) st256(reinterpret_cast<double*>(out_base[u] + (unsigned)pidx * node_stride), cur[u][0], cur[u][1], cur[u][2], cur[u][3]);
-            if (live[u] && c == 0) exp_base[u][(unsigned)pidx * (unsigned)L] = ex;
+            if (live[u] && c == 0) exp_base[u][(unsigned)pidx * (unsigned)L] = ex[u];
             if (out_slot >= 0) {
                 stack[(out_slot * PPL + u) * 64 + lane] = make_double2(cur[u][0], cur[u][1]);
                 stack[(out_slot * PPL + u) * 64 + 32 + lane] = make_double2(cur[u][2], cur[u][3]);
-                stack_ex[(out_slot * PPL + u) * 32 + lane] = ex;
+                stack_ex[(out_slot * PPL + u) * 32 + lane] = ex[u];
             }
         }
         if (++buf == DFS_STAGES) buf = 0;
@@ -730,8 +757,9 @@ int dfs_patterns_per_lane(const epx_ctx* c)
     if (c->dfs_ppl == 1 || c->dfs_ppl == 2 || c->dfs_ppl == 4) return c->dfs_ppl;
     const int G = dfs_lanes_of(c->C);
     const long tiles1 = (c->L + 32 / G - 1) / (32 / G);      // warps per piece at one pattern per lane
-    (void)tiles1;
-    return 1;      // measured on config 2: 0.78 ms (1), 0.83 ms (2), 1.09 ms (4) -- resident warps matter more than overhead
+    // measured on config 2 (1 250 tiles at one pattern per lane): 0.78 ms (1), 0.66 ms (2), 0.66 ms (4): the matrices are
+    // read from shared memory once per lane and operation, whatever the number of patterns they serve
+    return tiles1 >= 512 ? 2 : 1;
 }
 
 int dfs_tiles(const epx_ctx* c)
