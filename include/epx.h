@@ -121,7 +121,9 @@ const char* epx_last_error(const epx_ctx* ctx);
 /* Stages of a compute call, in enqueue order. */
 enum {
     EPX_STAGE_SEGMENT = 0, /* a1 */
-    EPX_STAGE_EIGEN = 1,   /* a2 Jacobi + change-of-basis prep (0 launches on the Pade / Taylor paths) */
+    EPX_STAGE_EIGEN = 1,   /* a2 Jacobi + change-of-basis prep (0 launches on the Pade / Taylor paths).  When the call is
+                              replayed from a CUDA graph a2 runs as a second branch beside a1 (they are independent) and
+                              this stage's time is only what a1 did not hide */
     EPX_STAGE_CHAIN = 2,   /* a2' + a3 + a4 */
     EPX_STAGE_PRUNE = 3,   /* a5, one launch per post-order level */
     EPX_STAGE_ROOT = 4,    /* a6 */

@@ -147,6 +147,9 @@ struct epx_ctx {
     cudaEvent_t ev[6] = {nullptr, nullptr, nullptr, nullptr, nullptr, nullptr};
     int stage_launches_mat[5] = {0, 0, 0, 0, 0}, stage_launches_lik[5] = {0, 0, 0, 0, 0};
     bool capturing = false;   // enqueue_kernels is running under stream capture
+    // graph mode only: a1 (segmenter) and a2 (eigensystems) are independent and run as two branches of the graph
+    cudaStream_t side = nullptr;
+    cudaEvent_t ev_fork = nullptr, ev_join = nullptr;
 
     long long launches = 0;
     bool have_result = false;

@@ -288,7 +288,7 @@ __global__ void __launch_bounds__(32) prune4_dfs_kernel(const DfsOp* __restrict_
         const double* Pb = Pa + G * DFS_PSTRIDE;
         // A matrix is read from shared memory ONCE per operation and serves the lane's PPL patterns from registers: the
         // register fill of the matrices is what saturates the L1 / shared-memory data pipe (profiles/r1_prune4_dfs_ncu.md)
-        double fa[PPL][4], fb[PPL][4];
+        double fa[PPL][4];       // child A's contribution, then the product with child B's
         int ex[PPL];
 #pragma unroll
         for (int u = 0; u < PPL; u++) ex[u] = 0;
@@ -327,7 +327,7 @@ __global__ void __launch_bounds__(32) prune4_dfs_kernel(const DfsOp* __restrict_
             for (int u = 0; u < PPL; u++) {
                 const int sb2 = tip_of(wb, u);
 #pragma unroll
-                for (int i = 0; i < 4; i++) fb[u][i] = (sb2 < 4) ? Pb[i * 4 + sb2] : 1.0;
+                for (int i = 0; i < 4; i++) fa[u][i] *= (sb2 < 4) ? Pb[i * 4 + sb2] : 1.0;
             }
         } else {
             double m[16];
@@ -347,7 +347,7 @@ __global__ void __launch_bounds__(32) prune4_dfs_kernel(const DfsOp* __restrict_
                 }
 #pragma unroll
                 for (int i = 0; i < 4; i++)
-                    fb[u][i] = fma(m[i * 4 + 3], vb[3], fma(m[i * 4 + 2], vb[2], fma(m[i * 4 + 1], vb[1], m[i * 4] * vb[0])));
+                    fa[u][i] *= fma(m[i * 4 + 3], vb[3], fma(m[i * 4 + 2], vb[2], fma(m[i * 4 + 1], vb[1], m[i * 4] * vb[0])));
             }
         }
 #pragma unroll
@@ -355,7 +355,7 @@ __global__ void __launch_bounds__(32) prune4_dfs_kernel(const DfsOp* __restrict_
             // all values are >= 0, so the largest one has the largest high word: an integer max finds its exponent
             int hmax = 0;
 #pragma unroll
-            for (int i = 0; i < 4; i++) { fa[u][i] *= fb[u][i]; hmax = max(hmax, __double2hiint(fa[u][i])); }
+            for (int i = 0; i < 4; i++) hmax = max(hmax, __double2hiint(fa[u][i]));
 #pragma unroll
             for (int o = 1; o < G; o <<= 1) hmax = max(hmax, __shfl_xor_sync(FULL, hmax, o));
             double sc = 1.0;
