@@ -661,6 +661,124 @@ __global__ void __launch_bounds__(GT) prune_generic_kernel(const PruneOp* __rest
     }
 }
 
+// ------------------------------------------------------------------------------------------------ 32 < K <= 64, DMMA
+// Level kernel for codon-sized models: per (node, tile of 32 patterns) and category, each internal child contributes
+// F[pattern][i] = sum_j V[pattern][j] P[i][j], a 32 x 64 x 64 product.  The scalar kernel reads two shared-memory operands
+// per DFMA and sits at 7 % of the FP64 peak; here the products run on the FP64 tensor pipe (mma.sync.m8n8k4):
+//   A (8x4) = V rows (patterns) x child states j,  B (4x8) = P^T (j x parent states i),  D (8x8) = F tile
+// Warp w of 8: patterns 8 (w & 3) .. +8, parent states 32 (w >> 2) .. +32 (four n-tiles); 16 k-steps.  Shared-memory rows
+// have a stride of 68 doubles (8 banks apart) so the 64-bit fragment loads of a half-warp never collide; the padding
+// columns / rows 61..63 are zero.  Everything after the products (rescaling, stores) is the scalar kernel's code.
+constexpr int MT = 256, M_TP = 32, M_LD = 68;
+
+__global__ void __launch_bounds__(MT) prune64_mma_kernel(const PruneOp* __restrict__ ops, int tiles, int K, int C, int L,
+    int Lp, const double* __restrict__ P, const uint8_t* __restrict__ tips, double* __restrict__ partials,
+    int32_t* __restrict__ scale_exp)
+{
+    extern __shared__ double sm[];
+    double* Pm = sm;                                   // [2][64][68]
+    double* V = Pm + 2 * 64 * M_LD;                    // [2][32][68]
+    double* out = V + 2 * M_TP * M_LD;                 // [C][32][K]
+    double* scl = out + (size_t)C * M_TP * K;          // [32]
+    int* st = reinterpret_cast<int*>(scl + M_TP);      // [2][32] tip states
+    const PruneOp op = ops[blockIdx.x / tiles];
+    const int tid = threadIdx.x, lane = tid & 31, w = tid >> 5, g = lane >> 2, q = lane & 3;
+    const int p0 = (blockIdx.x % tiles) * M_TP;
+    const int np = min(M_TP, L - p0);
+    const int KK = K * K;
+    const int mt = w & 3, nh = w >> 2;
+
+    for (int ch = 0; ch < 2; ch++)
+        if (op.child_is_tip[ch])
+            for (int p = tid; p < M_TP; p += MT) st[ch * M_TP + p] = p < np ? tips[(size_t)op.child[ch] * Lp + p0 + p] : 255;
+
+    for (int c = 0; c < C; c++) {
+        __syncthreads();
+        for (int ch = 0; ch < 2; ch++) {
+            const double* src = P + ((size_t)op.child[ch] * C + c) * KK;
+            for (int idx = tid; idx < 64 * 64; idx += MT) {
+                const int i = idx >> 6, j = idx & 63;
+                Pm[(ch * 64 + i) * M_LD + j] = (i < K && j < K) ? src[i * K + j] : 0.0;
+            }
+            if (!op.child_is_tip[ch]) {
+                const double* cs = partials + (((size_t)op.cpidx[ch] * C + c) * L + p0) * K;
+                for (int idx = tid; idx < M_TP * 64; idx += MT) {
+                    const int p = idx >> 6, j = idx & 63;
+                    V[(ch * M_TP + p) * M_LD + j] = (p < np && j < K) ? cs[p * K + j] : 0.0;
+                }
+            }
+        }
+        __syncthreads();
+        double f[4][2];
+#pragma unroll
+        for (int t = 0; t < 4; t++) f[t][0] = f[t][1] = 1.0;
+        for (int ch = 0; ch < 2; ch++) {
+            const double* Pc = Pm + ch * 64 * M_LD;
+            if (op.child_is_tip[ch]) {
+                const int s = st[ch * M_TP + 8 * mt + g];
+#pragma unroll
+                for (int t = 0; t < 4; t++) {
+                    const int i = 8 * (4 * nh + t) + 2 * q;
+                    f[t][0] *= s < K ? Pc[i * M_LD + s] : 1.0;
+                    f[t][1] *= s < K ? Pc[(i + 1) * M_LD + s] : 1.0;
+                }
+            } else {
+                double acc[4][2];
+#pragma unroll
+                for (int t = 0; t < 4; t++) acc[t][0] = acc[t][1] = 0.0;
+                const double* Arow = V + (ch * M_TP + 8 * mt + g) * M_LD + q;
+                const double* Brow = Pc + (32 * nh + g) * M_LD + q;
+#pragma unroll 4
+                for (int kt = 0; kt < 16; kt++) {
+                    const double a = Arow[4 * kt];
+#pragma unroll
+                    for (int t = 0; t < 4; t++) dmma884(acc[t][0], acc[t][1], a, Brow[8 * t * M_LD + 4 * kt]);
+                }
+#pragma unroll
+                for (int t = 0; t < 4; t++) { f[t][0] *= acc[t][0]; f[t][1] *= acc[t][1]; }
+            }
+        }
+        {
+            const int p = 8 * mt + g;
+#pragma unroll
+            for (int t = 0; t < 4; t++) {
+                const int i = 8 * (4 * nh + t) + 2 * q;
+                if (p < np && i < K) out[((size_t)c * M_TP + p) * K + i] = f[t][0];
+                if (p < np && i + 1 < K) out[((size_t)c * M_TP + p) * K + i + 1] = f[t][1];
+            }
+        }
+    }
+    __syncthreads();
+    // per-pattern maximum over (category, state): 8 lanes per pattern
+    {
+        const int p = tid / 8, sub = tid & 7;
+        double m = 0.0;
+        if (p < np)
+            for (int c = 0; c < C; c++)
+                for (int i = sub; i < K; i += 8) m = fmax(m, out[((size_t)c * M_TP + p) * K + i]);
+        for (int o = 4; o > 0; o >>= 1) m = fmax(m, __shfl_xor_sync(0xffffffffu, m, o));
+        if (p < np && sub == 0) {
+            int ex = 0;
+            for (int ch = 0; ch < 2; ch++)
+                if (!op.child_is_tip[ch]) ex += scale_exp[(size_t)op.cpidx[ch] * L + p0 + p];
+            double sc = 1.0;
+            if (m > 0.0 && m < 1.7e308) {
+                const int e = exponent_of(m);
+                if (e > -1000) { sc = pow2_neg(e); ex += e; }
+            }
+            scl[p] = sc;
+            scale_exp[(size_t)op.pidx * L + p0 + p] = ex;
+        }
+    }
+    __syncthreads();
+    for (int c = 0; c < C; c++) {
+        double* dst = partials + (((size_t)op.pidx * C + c) * L + p0) * K;
+        for (int idx = tid; idx < np * K; idx += MT) dst[idx] = out[(size_t)c * M_TP * K + idx] * scl[idx / K];
+    }
+}
+
+size_t mma64_smem(int K, int C) { return sizeof(double) * (2 * 64 * M_LD + 2 * M_TP * M_LD + (size_t)C * M_TP * K + M_TP) + sizeof(int) * 2 * M_TP; }
+
 // ------------------------------------------------------------------------------------------------ a6
 __global__ void __launch_bounds__(256) root_site_kernel(int K, int C, int L, size_t sc, size_t sp, int root_pidx, int root_node,
     const double* __restrict__ partials, const int32_t* __restrict__ scale_exp, const double* __restrict__ freqs,
@@ -749,6 +867,7 @@ int prune_init_attributes()
 {
     if (dfs_set_attr<1>() || dfs_set_attr<2>() || dfs_set_attr<3>() || dfs_set_attr<4>() || dfs_set_attr<5>() ||
         dfs_set_attr<6>() || dfs_set_attr<7>() || dfs_set_attr<8>()) return -1;
+    if (cudaFuncSetAttribute(prune64_mma_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024) != cudaSuccess) return -1;
     return cudaFuncSetAttribute(prune_generic_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024) == cudaSuccess ? 0 : -1;
 }
 
@@ -849,6 +968,10 @@ int launch_pruning(const epx_ctx* c, cudaStream_t s)
                 case 7: launch_prune4<7>(ops, nops, L, d, s); break;
                 default: launch_prune4<8>(ops, nops, L, d, s); break;
             }
+        } else if (K > 32 && c->prune_kernel != 1 && mma64_smem(K, C) <= 227 * 1024) {
+            const int tiles = (L + M_TP - 1) / M_TP;
+            prune64_mma_kernel<<<nops * tiles, MT, mma64_smem(K, C), s>>>(ops, tiles, K, C, L, c->Lp, d.P, d.tips, d.partials,
+                                                                         d.scale_exp);
         } else {
             const int tile_p = prune_tile(K, C);
             const int tiles = (L + tile_p - 1) / tile_p;
