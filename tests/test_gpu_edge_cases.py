@@ -1,0 +1,160 @@
+"""GPU parity on the degenerate and edge cases of the method (through the C ABI, against the long-double oracle):
+odd state counts on every kernel family, a single epoch, boundaries outside the tree, zero-length branches, all tips
+missing, relabelled trees, an overridden root distribution, and re-evaluation after inputs change (the MCMC use of the
+library: the cached CUDA graph and the dirty-upload logic must not serve stale data)."""
+import dataclasses
+
+import numpy as np
+import pytest
+
+import workloads as W
+from workloads import models, trees
+
+from test_gpu_parity import run_tree, check_matrices, check_segments, P_TOL, LNL_RTOL
+from test_oracle_pins import _small_problem
+
+pytestmark = pytest.mark.gpu
+
+
+@pytest.fixture(scope="module")
+def epx():
+    import torch
+    assert torch.cuda.is_available()
+    import paper_1309_3075_b200 as m
+    m.lib()
+    return m
+
+
+@pytest.mark.parametrize("K,C,L,reversible", [(2, 1, 5, True), (7, 3, 45, True), (24, 2, 33, True), (33, 1, 40, True),
+                                              (40, 3, 45, True), (64, 2, 37, True), (7, 2, 9, False), (20, 1, 3, False)])
+def test_state_counts_across_kernel_families(epx, orc_ld, K, C, L, reversible):
+    # K = 2, 7, 24: generic shared-memory kernels; 33, 40, 64: DMMA chain + DMMA pruning with 31 / 24 / 0 padding columns;
+    # asymmetric: Pade.  L is never a multiple of the pattern tile; some tips are missing.
+    rng = np.random.default_rng(1000 + K)
+    prob = _small_problem(rng, K=K, M=4, C=C, N=9, L=L, reversible=reversible, tip_h=rng.uniform(0, 0.3, 9))
+    tips = prob.tip_states.copy()
+    tips[::2, ::5] = -1
+    prob = dataclasses.replace(prob, tip_states=tips)
+    if not reversible:
+        prob = dataclasses.replace(prob, root_freqs=prob.freqs[-1].copy())
+    run_tree(epx, orc_ld, prob)
+    run_tree(epx, orc_ld, prob, options=[(epx.EPX_OPT_CHAIN_KERNEL, 1), (epx.EPX_OPT_PRUNE_KERNEL, 1)])
+
+
+def test_single_epoch_and_boundaries_outside_the_tree(epx, orc_ld):
+    rng = np.random.default_rng(7)
+    one = _small_problem(rng, K=4, M=1, C=2, N=10, L=50)                    # M = 1: no boundary at all (homogeneous model)
+    lnl_one, _ = run_tree(epx, orc_ld, one)
+    # the same model with two unused boundaries (one below every node, one above the root): same answer (reading A4)
+    three = dataclasses.replace(one, M=3, tau=np.array([-0.5, 2.0]), Q=np.repeat(one.Q, 3, 0), freqs=np.repeat(one.freqs, 3, 0))
+    lnl_three, ref = run_tree(epx, orc_ld, three)
+    assert abs(lnl_one - lnl_three) <= 1e-12 * abs(lnl_one)
+    assert np.all(np.diff(ref["seg_off"]) <= 1)
+
+
+def test_zero_length_branches_and_nodes_on_boundaries(epx, orc_ld):
+    # ((0,1)4, 2)5, 3)6 with node 4, node 5 and tip 2 all at height 0.25 = the first boundary: the branches 4->5 and 2->5
+    # have length zero (no segment, P = I, reading A3) and sit exactly on a boundary
+    rng = np.random.default_rng(8)
+    base = _small_problem(rng, K=4, M=3, C=2, N=4, L=20, tau=[0.25, 0.5])
+    parent = np.array([4, 4, 5, 6, 5, 6, -1], dtype=np.int32)
+    height = np.array([0.0, 0.0, 0.25, 0.0, 0.25, 0.25, 1.0])
+    prob = dataclasses.replace(base, parent=parent, height=height)
+    lnl, ref = run_tree(epx, orc_ld, prob)
+    nseg = np.diff(ref["seg_off"])
+    assert nseg[2] == 0 and nseg[4] == 0 and nseg[6] == 0          # tip 2, node 4, root slot
+    assert nseg[0] == 1 and nseg[5] == 2                           # [0, 0.25) is one epoch; 0.25 -> 1.0 is epochs 2 and 1 (a node ON a boundary starts the older epoch)
+    ctx = epx.from_problem(prob)
+    ctx.update_matrices()
+    assert np.array_equal(ctx.get_matrix(4, 1), np.eye(4))
+    ctx.close()
+
+
+def test_all_tips_missing_gives_zero(epx, orc_ld):
+    prob = W.make_config(2, N=64, L=100)
+    prob = dataclasses.replace(prob, tip_states=np.full_like(prob.tip_states, -1))
+    ctx = epx.from_problem(prob)
+    lnl = ctx.log_likelihood()
+    assert abs(lnl) < 1e-9                              # every site likelihood is 1 (rows of P sum to 1); exercises the rescaling
+    assert ctx.status() == 0
+    ctx.close()
+
+
+def test_relabelled_tree_and_root_override(epx, orc_ld):
+    rng = np.random.default_rng(9)
+    prob = W.make_config(1, N=20, L=64)
+    lnl0, _ = run_tree(epx, orc_ld, prob)
+    parent, height = trees.relabel_internal(rng, prob.parent, prob.height)      # the root is no longer the last node
+    lnl1, _ = run_tree(epx, orc_ld, dataclasses.replace(prob, parent=parent, height=height))
+    assert abs(lnl0 - lnl1) <= 1e-12 * abs(lnl0)
+    rf = rng.dirichlet(np.ones(4))
+    run_tree(epx, orc_ld, dataclasses.replace(prob, root_freqs=rf))
+
+
+def test_reevaluation_after_inputs_change(epx, orc_ld):
+    """One context, many evaluations: heights, models, rates, tips, weights, then the topology change; after each change
+    the result must equal a fresh oracle evaluation (no stale graph, no stale upload)."""
+    rng = np.random.default_rng(10)
+    prob = W.make_config(2, N=60, L=300)
+    ctx = epx.from_problem(prob)
+
+    def check(p):
+        lnl = ctx.log_likelihood()
+        ref = orc_ld.evaluate(p)
+        assert abs(np.longdouble(lnl) - ref["lnl"]) <= LNL_RTOL * abs(ref["lnl"])
+        check_segments(ctx, ref)
+        check_matrices(ctx, ref)
+        assert ctx.status() == 0
+
+    check(prob)
+    # 1. node heights move (same topology: the cached graph is replayed)
+    h = prob.height.copy()
+    internal = h > 0.2
+    h[internal] = 0.2 + (h[internal] - 0.2) * 0.9
+    prob = dataclasses.replace(prob, height=h)
+    ctx.set_tree(prob.parent, prob.height)
+    check(prob)
+    # 2. one epoch's model changes
+    pi = rng.dirichlet(np.full(4, 3.0))
+    Q, F = prob.Q.copy(), prob.freqs.copy()
+    Q[3], F[3] = models.hky(4.2, pi), pi
+    prob = dataclasses.replace(prob, Q=Q, freqs=F)
+    ctx.set_epoch_model(3, Q[3], F[3], True)
+    check(prob)
+    # 3. boundaries and category rates
+    prob = dataclasses.replace(prob, tau=prob.tau * 0.95)
+    ctx.set_epoch_boundaries(prob.tau)
+    rates, weights = models.discrete_gamma(0.9, 4)
+    prob = dataclasses.replace(prob, rates=rates, weights=weights)
+    ctx.set_category_rates(rates, weights)
+    check(prob)
+    # 4. tips and pattern weights
+    tips = prob.tip_states.copy(); tips[:, ::3] = (tips[:, ::3] + 1) % 4
+    wt = rng.poisson(2.0, prob.L) + 1.0
+    prob = dataclasses.replace(prob, tip_states=tips, pattern_weights=wt)
+    ctx.set_tip_states(tips); ctx.set_pattern_weights(wt)
+    check(prob)
+    # 5. a different topology (graph must be rebuilt)
+    parent, height = trees.coalescent(rng, np.sort(rng.uniform(0, 0.2, prob.N)))
+    height = trees.stretch_above(height, 0.2, 1.0)
+    prob = dataclasses.replace(prob, parent=parent, height=height)
+    ctx.set_tree(parent, height)
+    check(prob)
+    ctx.close()
+
+
+def test_stage_events_and_launch_count(epx):
+    prob = W.make_config(1)
+    ctx = epx.from_problem(prob)
+    with pytest.raises(epx.EpxError):
+        ctx.get_stage_ms()                               # option off
+    ctx.set_option(epx.EPX_OPT_STAGE_EVENTS, 1)
+    n0 = ctx.launch_count()
+    ctx.log_likelihood()
+    ms, launches = ctx.get_stage_ms()
+    assert np.all(ms >= 0) and ms[3] > 0 and launches.sum() == ctx.launch_count() - n0
+    assert launches[0] == 3 and launches[4] == 2
+    ctx.update_matrices()
+    ms, launches = ctx.get_stage_ms()
+    assert launches[3] == 0 and launches[4] == 0 and ms[3] == 0
+    ctx.close()
