@@ -88,6 +88,13 @@ int epx_set_root_frequencies(epx_ctx* ctx, const double* freqs);
 /* n_br branches given by their two end heights, parent_height[b] >= child_height[b]. */
 int epx_set_branches(epx_ctx* ctx, int n_br, const double* child_height, const double* parent_height);
 
+/* ---- optional: per-branch rate scalars r_v (relaxed clocks; the rate is constant along a branch) ----
+ * rates: one per matrix slot (tree mode: 2N-1 entries indexed by node, the root's entry is ignored; branch-list mode: n_br
+ * entries), finite and >= 0, or NULL = all 1 (the default).  The effective rate of a segment is r_v * r_c (reading A6), so
+ * P_b = prod_k exp(Q_k r_v r_c t_k); epx_get_segments then reports durations already multiplied by r_v.  Branch-list
+ * mode: call after epx_set_branches. */
+int epx_set_branch_rates(epx_ctx* ctx, const double* rates);
+
 /* ---- compute ---- */
 /* a1..a4, enqueued on the stream, does not synchronise.  Matrix slot = node index (tree mode; the root's slot
  * holds the identity) or branch index. */

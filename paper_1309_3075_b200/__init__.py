@@ -58,6 +58,7 @@ def lib():
     _sig(L, "epx_set_pattern_weights", i, vp, dp)
     _sig(L, "epx_set_root_frequencies", i, vp, dp)
     _sig(L, "epx_set_branches", i, vp, i, dp, dp)
+    _sig(L, "epx_set_branch_rates", i, vp, dp)
     _sig(L, "epx_update_matrices", i, vp)
     _sig(L, "epx_enqueue_log_likelihood", i, vp)
     _sig(L, "epx_log_likelihood", i, vp, ct.POINTER(ct.c_double))
@@ -191,6 +192,11 @@ class Epx:
         assert ch.shape == ph.shape and ch.ndim == 1
         self._check(self._L.epx_set_branches(self._ctx, ch.shape[0], _ptr(ch), _ptr(ph)))
         self.n_slots = ch.shape[0]
+
+    def set_branch_rates(self, rates) -> None:
+        rates = None if rates is None else _f64(rates)
+        assert rates is None or rates.shape == (self.n_slots,)
+        self._check(self._L.epx_set_branch_rates(self._ctx, _ptr(rates)))
 
     def set_option(self, option: int, value: int) -> None:
         self._check(self._L.epx_set_option(self._ctx, option, value))

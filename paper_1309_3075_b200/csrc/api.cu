@@ -66,6 +66,7 @@ size_t plan_workspace(const epx_ctx* c, char* base, DevBuffers* d)
         t.child_h = (double*)take(8 * S);
         t.parent_h = (double*)take(8 * S);
     }
+    t.brate = (double*)take(8 * S);
     t.n_seg = (int32_t*)take(4 * S);
     t.e_hi = (int32_t*)take(4 * S);
     t.seg_off = (int32_t*)take(4 * (S + 1));
@@ -345,7 +346,7 @@ int epx_bind(epx_ctx* c, void* ws, size_t bytes, void* stream)
     plan_workspace(c, (char*)ws, &c->d);
     c->ws = ws; c->ws_bytes = bytes; c->stream = (cudaStream_t)stream; c->bound = true;
     c->tau_dirty = c->model_dirty = c->rates_dirty = c->tree_dirty = c->branches_dirty = c->tips_dirty = c->wt_dirty =
-        c->rootf_dirty = true;
+        c->rootf_dirty = c->brates_dirty = true;
     c->have_result = false;
     return EPX_OK;
 }
@@ -485,6 +486,23 @@ int epx_set_branches(epx_ctx* c, int n_br, const double* child_height, const dou
     c->parent_h.assign(parent_height, parent_height + n_br);
     c->n_slots = n_br;
     c->has_branches = true; c->branches_dirty = true;
+    return EPX_OK;
+}
+
+int epx_set_branch_rates(epx_ctx* c, const double* rates)
+{
+    if (!c) return EPX_E_ARG;
+    const bool had = c->has_brates;
+    if (!rates) {
+        c->has_brates = false;
+    } else {
+        if (!c->tree_mode && !c->has_branches) return fail(c, EPX_E_STATE, "branch-list mode: call epx_set_branches first");
+        for (int b = 0; b < c->n_slots; b++)
+            if (!std::isfinite(rates[b]) || rates[b] < 0) return fail(c, EPX_E_ARG, "branch rate %d must be finite and >= 0", b);
+        c->brates.assign(rates, rates + c->n_slots);
+        c->has_brates = true; c->brates_dirty = true;
+    }
+    if (had != c->has_brates) drop_graphs(c);     // kernel arguments (rate pointer, full-epoch table use) change
     return EPX_OK;
 }
 

@@ -59,6 +59,7 @@ struct DevBuffers {
     double* height;       // [n_nodes] tree mode
     double* child_h;      // [n_br] branch-list mode
     double* parent_h;     // [n_br] branch-list mode
+    double* brate;        // [n_slots] branch rate scalars (valid iff has_brates)
     uint8_t* tips;        // [N][Lp] 0..K-1, 255 = missing; rows padded to Lp = L rounded up to 32
     double* pattern_wt;   // [L]
     PruneOp* ops;         // [N-1] sorted by level
@@ -108,7 +109,8 @@ struct epx_ctx {
     std::vector<char> model_sparse;   // per epoch: Q has a structural zero off the diagonal
 
     // host copies of the inputs (uploaded lazily; *_dirty = needs upload)
-    std::vector<double> tau, Q, freqs, rates, weights, root_freqs, height, child_h, parent_h, pattern_wt;
+    std::vector<double> tau, Q, freqs, rates, weights, root_freqs, height, child_h, parent_h, pattern_wt, brates;
+    bool has_brates = false, brates_dirty = false;
     std::vector<int32_t> parent;
     uint8_t* tips = nullptr;           // [N][Lp] host staging of the tip states, page-locked (DMA source); see epx_set_tip_states
     bool tips_pinned = false;

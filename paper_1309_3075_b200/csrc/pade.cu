@@ -227,7 +227,7 @@ __global__ void __launch_bounds__(PT) pade_full_epoch_kernel(int K, int M, int C
 }
 
 template <int METHOD>
-__global__ void __launch_bounds__(PT) pade_chain_kernel(int K, int C, const int32_t* __restrict__ order,
+__global__ void __launch_bounds__(PT) pade_chain_kernel(int K, int C, int use_table, const int32_t* __restrict__ order,
     const int32_t* __restrict__ n_seg, const int32_t* __restrict__ seg_off, const int32_t* __restrict__ seg_epoch,
     const double* __restrict__ seg_dur, const double* __restrict__ rates, const double* __restrict__ Q,
     const double* __restrict__ Efull, double* __restrict__ P, int32_t* __restrict__ status)
@@ -249,7 +249,7 @@ __global__ void __launch_bounds__(PT) pade_chain_kernel(int K, int C, const int3
     for (int s = 0; s < n; s++) {
         const int e = seg_epoch[off + s];
         double* E;
-        if (s > 0 && s < n - 1) {    // the branch spans the whole of epoch e: table lookup
+        if (use_table && s > 0 && s < n - 1) {    // the branch spans the whole of epoch e at rate r_c: table lookup
             const double* src = Efull + ((size_t)e * C + c) * KK;
             for (int idx = tid; idx < KK; idx += PT) b.T1[idx] = src[idx];
             __syncthreads();
@@ -302,11 +302,12 @@ static int launch_dense(const epx_ctx* c, cudaStream_t s)
     const int K = c->K, C = c->C, M = c->M;
     const size_t smem = pade_smem_bytes(K);
     int launched = 0;
-    if (M >= 3) {
+    const int use_table = c->has_brates ? 0 : 1;     // with branch rates an interior segment lasts r_v * (tau_e - tau_{e-1})
+    if (M >= 3 && use_table) {
         pade_full_epoch_kernel<METHOD><<<(M - 2) * C, PT, smem, s>>>(K, M, C, d.Q, d.tau, d.rates, d.Efull, d.status);
         launched++;
     }
-    pade_chain_kernel<METHOD><<<c->n_slots * C, PT, smem, s>>>(K, C, d.order, d.n_seg, d.seg_off, d.seg_epoch, d.seg_dur,
+    pade_chain_kernel<METHOD><<<c->n_slots * C, PT, smem, s>>>(K, C, use_table, d.order, d.n_seg, d.seg_off, d.seg_epoch, d.seg_dur,
                                                        d.rates, d.Q, d.Efull, d.P, d.status);
     launched++;
     return cudaGetLastError() == cudaSuccess ? launched : -1;

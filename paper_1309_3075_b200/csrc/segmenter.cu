@@ -108,7 +108,8 @@ __global__ void seg_fill_kernel(int n_br, int M, const double* __restrict__ tau,
                                 const double* __restrict__ height, const double* __restrict__ child_h,
                                 const double* __restrict__ parent_h, const int32_t* __restrict__ n_seg,
                                 const int32_t* __restrict__ e_hi_in, const int32_t* __restrict__ seg_off,
-                                int32_t* __restrict__ seg_epoch, double* __restrict__ seg_dur)
+                                const double* __restrict__ brate, int32_t* __restrict__ seg_epoch,
+                                double* __restrict__ seg_dur)
 {
     int b = blockIdx.x * blockDim.x + threadIdx.x;
     if (b >= n_br) return;
@@ -117,11 +118,12 @@ __global__ void seg_fill_kernel(int n_br, int M, const double* __restrict__ tau,
     double hc, hp;
     branch_ends(b, parent, height, child_h, parent_h, hc, hp);
     int e = e_hi_in[b], off = seg_off[b];
+    const double rv = brate ? brate[b] : 1.0;      // branch rate scalar r_v, constant along the branch
     double upper = hp;
     for (int i = 0; i < n; i++, e--) {
         double lower = (i == n - 1) ? hc : tau[e - 1];
         seg_epoch[off + i] = e;
-        seg_dur[off + i] = upper - lower;
+        seg_dur[off + i] = brate ? (upper - lower) * rv : upper - lower;
         upper = lower;
     }
 }
@@ -137,6 +139,6 @@ int launch_segmenter(const epx_ctx* c, cudaStream_t s)
     seg_count_kernel<<<blocks, 256, 0, s>>>(n, c->M, d.tau, parent, d.height, d.child_h, d.parent_h, d.n_seg, d.e_hi);
     seg_scan_sort_kernel<<<1, 1024, 0, s>>>(n, d.n_seg, d.seg_off, d.order);
     seg_fill_kernel<<<blocks, 256, 0, s>>>(n, c->M, d.tau, parent, d.height, d.child_h, d.parent_h, d.n_seg, d.e_hi,
-                                           d.seg_off, d.seg_epoch, d.seg_dur);
+                                           d.seg_off, c->has_brates ? d.brate : nullptr, d.seg_epoch, d.seg_dur);
     return cudaGetLastError() == cudaSuccess ? 3 : -1;
 }

@@ -158,3 +158,52 @@ def test_stage_events_and_launch_count(epx):
     ms, launches = ctx.get_stage_ms()
     assert launches[3] == 0 and launches[4] == 0 and ms[3] == 0
     ctx.close()
+
+
+def _oracle_with_branch_rates(orc, prob, brates):
+    """Oracle evaluation with per-branch rate scalars r_v: the oracle's own routines, fed segment
+    durations multiplied by the branch's rate (effective time r_v * t, reading A6) -- its arithmetic is untouched."""
+    ch, ph = prob.branch_heights()
+    off, ep, du = orc.segments(ch, ph, prob.tau)
+    scaled = du * np.repeat(np.asarray(brates, dtype=np.float64), np.diff(off))
+    P = orc.branch_matrices(prob.Q, prob.rates, off, ep, scaled)
+    out = {"seg_off": off, "seg_epoch": ep, "seg_dur": scaled, "P": P}
+    if prob.N > 0:
+        rf = prob.root_freqs if prob.root_freqs is not None else prob.freqs[orc.epoch_of_parent_end(np.max(prob.height), prob.tau)]
+        out.update(orc.log_likelihood(prob.parent, P, prob.tip_states, rf, prob.weights, prob.pattern_weights))
+    return out
+
+
+@pytest.mark.parametrize("cid,kw", [(2, {"N": 80, "L": 130}), (3, {"N": 8, "L": 20}), (4, {"N": 50, "L": 2}), (5, {"n_br": 120})])
+def test_branch_rates(epx, orc_ld, cid, kw):
+    # every path: K=4 registers, componentwise Taylor (codon likelihood), Pade (the full-epoch table must be bypassed),
+    # eigenbasis DMMA chain (branch list); rates include 0 (P = I) and 1
+    rng = np.random.default_rng(40 + cid)
+    prob = W.make_config(cid, **kw)
+    br = rng.lognormal(0.0, 0.6, prob.n_br)
+    br[1], br[2] = 0.0, 1.0
+    ctx = epx.from_problem(prob)
+    ctx.set_branch_rates(br)
+    ref = _oracle_with_branch_rates(orc_ld, prob, br)
+    if prob.N > 0:
+        lnl = ctx.log_likelihood()
+        assert abs(np.longdouble(lnl) - ref["lnl"]) <= LNL_RTOL * abs(ref["lnl"])
+    else:
+        ctx.update_matrices()
+    off, ep, du = ctx.get_all_segments()
+    assert np.array_equal(off, ref["seg_off"]) and np.array_equal(ep, ref["seg_epoch"])
+    assert np.all(np.abs(du - ref["seg_dur"]) <= 2 * np.spacing(np.abs(ref["seg_dur"])))
+    check_matrices(ctx, ref)
+    assert ctx.status() == 0
+    # back to unit rates: identical to a context that never had them
+    ctx.set_branch_rates(None)
+    ref1 = orc_ld.evaluate(prob)
+    if prob.N > 0:
+        lnl1 = ctx.log_likelihood()
+        assert abs(np.longdouble(lnl1) - ref1["lnl"]) <= LNL_RTOL * abs(ref1["lnl"])
+    else:
+        ctx.update_matrices()
+    check_matrices(ctx, ref1)
+    with pytest.raises(epx.EpxError):
+        ctx.set_branch_rates(np.full(prob.n_br, -1.0))
+    ctx.close()
