@@ -36,8 +36,8 @@ if ROOT not in sys.path:
 import workloads as W  # noqa: E402  (input generators only; shared with the oracle, holds no arithmetic of the method)
 
 # dram__bytes_read.sum + dram__bytes_write.sum of the pruning launches of one config-2 step, from the committed
-# `ncu --set full` capture (profiles/r1_prune4_dfs_ncu.md): 2561.8 + 23.1 MB (bottom pieces) + 15.9 MB (top piece)
-NCU_TRAFFIC_BYTES_PER_STEP = 2.6008e9
+# `ncu --set full` capture (profiles/r1_prune4_dfs_ncu.md): 2550.7 + 22.8 MB (bottom pieces) + 3.8 + 31.8 MB (top piece)
+NCU_TRAFFIC_BYTES_PER_STEP = 2.6091e9
 
 METRIC = "pruning partials GB/s (fp64) over the whole a1..a6 log-likelihood step; epoch branch matrices/s in `matrices`"
 UNIT = "GB/s"
@@ -304,7 +304,7 @@ def run_cuda(args) -> None:
     hbm_peak, peak_src = load_peaks()
     prune_ms = float(stage_ms[3])
     prune_launches = int(stage_launches[3])
-    roofline = {"bound": "hbm", "kernel": "prune4_dfs_kernel<4> (a5; depth-first walk, bottom pieces + top piece)",
+    roofline = {"bound": "hbm", "kernel": "prune4_dfs_kernel<4, 2> (a5; depth-first walk, bottom pieces + top piece)",
                 "achieved": nb["a5"] / (prune_ms * 1e-3) / 1e9, "peak": hbm_peak, "unit": "GB/s",
                 "frac": nb["a5"] / (prune_ms * 1e-3) / 1e9 / hbm_peak,
                 "traffic": args.traffic if args.traffic is not None else NCU_TRAFFIC_BYTES_PER_STEP / prune_launches,
