@@ -107,6 +107,18 @@ int epx_log_likelihood(epx_ctx* ctx, double* logL);
 /* Synchronise and fetch the result of the last enqueue (same checks as epx_log_likelihood). */
 int epx_fetch_log_likelihood(epx_ctx* ctx, double* logL);
 
+/* ---- incremental re-evaluation (an MCMC step re-dispatches only what its proposal
+ * touches) ----
+ * epx_set_node_heights: move `n` nodes (node ids, new heights) without changing the topology; every moved node must stay
+ * between its children and its parent (EPX_E_TREE otherwise, nothing is changed).  Cheaper than epx_set_tree: no plan is
+ * rebuilt, and the moved nodes are remembered.
+ * epx_log_likelihood_incremental: like epx_log_likelihood, but when the device still holds a complete evaluation of the
+ * current inputs and only node heights moved since, it recomputes just the matrices of the moved nodes' branches and of
+ * their children's branches, and the partials of the moved nodes and their ancestors.  The result is bit-identical to a
+ * full evaluation.  In every other situation it is a full evaluation. */
+int epx_set_node_heights(epx_ctx* ctx, int n, const int32_t* nodes, const double* heights);
+int epx_log_likelihood_incremental(epx_ctx* ctx, double* logL);
+
 /* ---- read-back (each synchronises the stream; results of the LAST compute call) ---- */
 /* Segment list of matrix slot `slot`: *n_seg entries, parent end first; epoch/dur hold at least M entries. */
 int epx_get_segments(epx_ctx* ctx, int slot, int* n_seg, int32_t* epoch, double* dur);

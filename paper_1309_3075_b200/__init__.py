@@ -59,6 +59,8 @@ def lib():
     _sig(L, "epx_set_root_frequencies", i, vp, dp)
     _sig(L, "epx_set_branches", i, vp, i, dp, dp)
     _sig(L, "epx_set_branch_rates", i, vp, dp)
+    _sig(L, "epx_set_node_heights", i, vp, i, ip, dp)
+    _sig(L, "epx_log_likelihood_incremental", i, vp, ct.POINTER(ct.c_double))
     _sig(L, "epx_update_matrices", i, vp)
     _sig(L, "epx_enqueue_log_likelihood", i, vp)
     _sig(L, "epx_log_likelihood", i, vp, ct.POINTER(ct.c_double))
@@ -197,6 +199,16 @@ class Epx:
         rates = None if rates is None else _f64(rates)
         assert rates is None or rates.shape == (self.n_slots,)
         self._check(self._L.epx_set_branch_rates(self._ctx, _ptr(rates)))
+
+    def set_node_heights(self, nodes, heights) -> None:
+        nodes, heights = _i32(nodes), _f64(heights)
+        assert nodes.shape == heights.shape and nodes.ndim == 1
+        self._check(self._L.epx_set_node_heights(self._ctx, nodes.shape[0], _ptr(nodes), _ptr(heights)))
+
+    def log_likelihood_incremental(self) -> float:
+        v = ct.c_double()
+        self._check(self._L.epx_log_likelihood_incremental(self._ctx, ct.byref(v)))
+        return v.value
 
     def set_option(self, option: int, value: int) -> None:
         self._check(self._L.epx_set_option(self._ctx, option, value))

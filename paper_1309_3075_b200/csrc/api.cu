@@ -88,6 +88,12 @@ size_t plan_workspace(const epx_ctx* c, char* base, DevBuffers* d)
         t.site_lnl = (double*)take(8 * L);
         t.block_sums = (double*)take(8 * ((L + 255) / 256));
     }
+    t.inc_slots = (int32_t*)take(4 * S);
+    if (c->tree_mode) {
+        t.inc_ops = (DfsOp*)take(sizeof(DfsOp) * (N - 1));
+        t.inc_piece = (DfsPiece*)take(sizeof(DfsPiece));
+        t.inc_pops = (PruneOp*)take(sizeof(PruneOp) * (N - 1));
+    }
     t.lnl = (double*)take(8);
     t.status = (int32_t*)take(4);
     if (d) *d = t;
@@ -96,6 +102,7 @@ size_t plan_workspace(const epx_ctx* c, char* base, DevBuffers* d)
 
 void drop_graphs(epx_ctx* c)
 {
+    c->inc_valid = false;      // whatever invalidates the graphs also invalidates an incremental continuation
     if (c->graph_mat) { cudaGraphExecDestroy(c->graph_mat); c->graph_mat = nullptr; }
     if (c->graph_lik) { cudaGraphExecDestroy(c->graph_lik); c->graph_lik = nullptr; }
 }
@@ -160,6 +167,9 @@ int build_plan(epx_ctx* c)
     for (int l = 1; l <= max_level; l++) offs[l] = offs[l - 1] + c->level_off[l];
     c->level_off = offs;               // ops of level l (1-based) are [offs[l-1], offs[l])
     c->root = root;
+    c->node_level = level;
+    c->node_left = left;
+    c->node_right = right;
 
     // Depth-first post-order walk for prune4_dfs_kernel.  Every internal node becomes one DfsOp; the child visited
     // SECOND hands its result over in registers, the child visited FIRST parks its result in a stack slot.  Visiting
@@ -470,6 +480,32 @@ int epx_set_tree(epx_ctx* c, const int32_t* parent, const double* height)
     if (rc != EPX_OK) { c->has_tree = false; return rc; }
     if (old_parent != c->parent) drop_graphs(c);      // launch shapes depend on the topology only
     c->has_tree = true; c->tree_dirty = true;
+    c->dirty_nodes.clear();
+    return EPX_OK;
+}
+
+int epx_set_node_heights(epx_ctx* c, int n, const int32_t* nodes, const double* heights)
+{
+    if (!c || n < 0 || (n > 0 && (!nodes || !heights))) return EPX_E_ARG;
+    if (!c->tree_mode) return fail(c, EPX_E_STATE, "ctx is in branch-list mode");
+    if (!c->has_tree) return fail(c, EPX_E_STATE, "epx_set_tree has not been called");
+    std::vector<double> old(n);
+    for (int k = 0; k < n; k++) {
+        if (nodes[k] < 0 || nodes[k] >= c->n_nodes) return fail(c, EPX_E_ARG, "node %d out of range", nodes[k]);
+        if (!std::isfinite(heights[k])) return fail(c, EPX_E_ARG, "height of node %d is not finite", nodes[k]);
+    }
+    for (int k = 0; k < n; k++) { old[k] = c->height[nodes[k]]; c->height[nodes[k]] = heights[k]; }
+    for (int k = 0; k < n; k++) {          // the order of parents and children must survive the move
+        const int u = nodes[k], p = c->parent[u];
+        bool ok = p < 0 || c->height[p] >= c->height[u];
+        if (c->node_left[u] >= 0) ok = ok && c->height[u] >= c->height[c->node_left[u]] && c->height[u] >= c->height[c->node_right[u]];
+        if (!ok) {
+            for (int j = n - 1; j >= 0; j--) c->height[nodes[j]] = old[j];
+            return fail(c, EPX_E_TREE, "node %d would leave the interval between its children and its parent", u);
+        }
+    }
+    c->dirty_nodes.insert(c->dirty_nodes.end(), nodes, nodes + n);
+    c->heights_dirty = true;
     return EPX_OK;
 }
 

@@ -22,7 +22,8 @@ namespace {
 
 // ------------------------------------------------------------------------------------------------ K == 4
 template <int K>
-__global__ void __launch_bounds__(256) chain_rows_kernel(int n_slots, int C, const int32_t* __restrict__ n_seg,
+__global__ void __launch_bounds__(256) chain_rows_kernel(int n_slots, int C, const int32_t* __restrict__ list,
+    const int32_t* __restrict__ n_seg,
     const int32_t* __restrict__ seg_off, const int32_t* __restrict__ seg_epoch, const double* __restrict__ seg_dur,
     const double* __restrict__ rates, const double* __restrict__ lam, const double* __restrict__ U,
     const double* __restrict__ W, const double* __restrict__ sp, const double* __restrict__ isp,
@@ -32,7 +33,8 @@ __global__ void __launch_bounds__(256) chain_rows_kernel(int n_slots, int C, con
     if (idx >= (long long)n_slots * C * K) return;
     const int i = (int)(idx % K);
     const int c = (int)((idx / K) % C);
-    const int b = (int)(idx / ((long long)K * C));
+    const int bi = (int)(idx / ((long long)K * C));
+    const int b = list ? list[bi] : bi;            // f1: only the listed slots
     double* out = P + (((size_t)b * C + c) * K + i) * K;
     const int n = n_seg[b];
     if (n == 0) {
@@ -327,20 +329,24 @@ int chain_init_attributes()
 int launch_chain_reversible(const epx_ctx* c, cudaStream_t s)
 {
     const DevBuffers& d = c->d;
-    const int K = c->K, Kp = c->Kp, C = c->C, n = c->n_slots;
+    const int K = c->K, Kp = c->Kp, C = c->C;
+    // f1: an incremental call recomputes only the slots of c->sub_list (any order); a full call all of them, longest first
+    const int n = c->sub_list ? c->sub_count : c->n_slots;
+    const int32_t* order = c->sub_list ? c->sub_list : d.order;
+    if (n == 0) return 0;
     if (K == 4) {
         long long threads = (long long)n * C * 4;
         int blocks = (int)((threads + 255) / 256);
-        chain_rows_kernel<4><<<blocks, 256, 0, s>>>(n, C, d.n_seg, d.seg_off, d.seg_epoch, d.seg_dur, d.rates, d.lam,
-                                                    d.U, d.W, d.sp, d.isp, d.P, d.status);
+        chain_rows_kernel<4><<<blocks, 256, 0, s>>>(n, C, c->sub_list, d.n_seg, d.seg_off, d.seg_epoch, d.seg_dur, d.rates,
+                                                    d.lam, d.U, d.W, d.sp, d.isp, d.P, d.status);
     } else if (Kp == 64 && c->chain_kernel != 1) {
         int ncg = (C + CPC - 1) / CPC;
-        chain_dmma64_kernel<<<n * ncg, DT, sizeof(DmmaSmem), s>>>(K, C, d.order, d.n_seg, d.seg_off, d.seg_epoch,
+        chain_dmma64_kernel<<<n * ncg, DT, sizeof(DmmaSmem), s>>>(K, C, order, d.n_seg, d.seg_off, d.seg_epoch,
                                                                  d.seg_dur, d.rates, d.lam, d.WB, d.UTB, d.sp, d.isp,
                                                                  d.P, d.status);
     } else {
         size_t smem = sizeof(double) * (2 * (size_t)Kp * (Kp + 1) + (size_t)Kp * Kp + Kp);
-        chain_generic_kernel<<<n * C, GT, smem, s>>>(K, Kp, C, d.order, d.n_seg, d.seg_off, d.seg_epoch, d.seg_dur,
+        chain_generic_kernel<<<n * C, GT, smem, s>>>(K, Kp, C, order, d.n_seg, d.seg_off, d.seg_epoch, d.seg_dur,
                                                      d.rates, d.lam, d.U, d.W, d.sp, d.isp, d.P, d.status);
     }
     return cudaGetLastError() == cudaSuccess ? 1 : -1;

@@ -92,6 +92,11 @@ struct DevBuffers {
     double* block_sums;   // [reduce blocks]
     double* lnl;          // [1]
     int32_t* status;      // [1]
+    // f1 incremental re-evaluation (lists rebuilt by every epx_log_likelihood_incremental call)
+    int32_t* inc_slots;   // [n_slots] matrix slots to recompute
+    DfsOp* inc_ops;       // [N-1] K == 4: the dirty nodes as one depth-first piece (children read from HBM or handed over)
+    DfsPiece* inc_piece;  // [1]
+    PruneOp* inc_pops;    // [N-1] other K: the dirty nodes' level-kernel operations, level by level
 };
 
 struct epx_ctx {
@@ -124,6 +129,14 @@ struct epx_ctx {
     std::vector<PruneOp> ops;
     std::vector<int> level_off;        // ops[level_off[l] .. level_off[l+1]) form level l
     std::vector<int> node_pidx;        // node -> index in partials (internal) or -1
+    std::vector<int> node_level;       // post-order level of every node (tips 0)
+    std::vector<int> node_left, node_right;   // children (-1 for tips)
+    // f1: nodes whose height changed since the last evaluation (epx_set_node_heights), and whether the device still
+    // holds a complete evaluation of the current inputs that an incremental call can build on
+    std::vector<int> dirty_nodes;
+    bool inc_valid = false, heights_dirty = false;
+    const int32_t* sub_list = nullptr;  // when set, the chain launchers recompute only these slots ...
+    int sub_count = 0;                  // ... this many
     std::vector<DfsOp> dfs_ops;        // depth-first post-order walk with its stack-slot allocation
     std::vector<DfsPiece> dfs_pieces;  // bottom pieces (independent subtrees, largest first), then the top piece if any
     int dfs_bottom = 0;                // number of bottom pieces (launch 1); the rest (0 or 1) is launch 2
@@ -177,6 +190,7 @@ int launch_chain_reversible(const epx_ctx* c, cudaStream_t s);
 int launch_pade_chain(const epx_ctx* c, cudaStream_t s);
 int launch_taylor_chain(const epx_ctx* c, cudaStream_t s);   // same kernels, shifted non-negative Taylor exponential
 int launch_pruning(const epx_ctx* c, cudaStream_t s);
+int launch_pruning_incremental(const epx_ctx* c, const std::vector<int>& group_off, cudaStream_t s);
 int launch_root_reduction(const epx_ctx* c, cudaStream_t s);
 size_t pade_smem_bytes(int K);
 int chain_init_attributes();

@@ -303,11 +303,14 @@ static int launch_dense(const epx_ctx* c, cudaStream_t s)
     const size_t smem = pade_smem_bytes(K);
     int launched = 0;
     const int use_table = c->has_brates ? 0 : 1;     // with branch rates an interior segment lasts r_v * (tau_e - tau_{e-1})
-    if (M >= 3 && use_table) {
+    const int n = c->sub_list ? c->sub_count : c->n_slots;          // f1: only the listed slots; the full-epoch table
+    const int32_t* order = c->sub_list ? c->sub_list : d.order;      // depends on tau, Q and the rates only and is kept
+    if (n == 0) return 0;
+    if (M >= 3 && use_table && !c->sub_list) {
         pade_full_epoch_kernel<METHOD><<<(M - 2) * C, PT, smem, s>>>(K, M, C, d.Q, d.tau, d.rates, d.Efull, d.status);
         launched++;
     }
-    pade_chain_kernel<METHOD><<<c->n_slots * C, PT, smem, s>>>(K, C, use_table, d.order, d.n_seg, d.seg_off, d.seg_epoch, d.seg_dur,
+    pade_chain_kernel<METHOD><<<n * C, PT, smem, s>>>(K, C, use_table, order, d.n_seg, d.seg_off, d.seg_epoch, d.seg_dur,
                                                        d.rates, d.Q, d.Efull, d.P, d.status);
     launched++;
     return cudaGetLastError() == cudaSuccess ? launched : -1;

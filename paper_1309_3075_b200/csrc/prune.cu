@@ -898,32 +898,46 @@ bool prune_uses_dfs(const epx_ctx* c)
 }
 
 template <int C, int PPL>
-static void launch_dfs2(const epx_ctx* c, int first_piece, int n_pieces, cudaStream_t s)
+static void launch_dfs2(const epx_ctx* c, const DfsOp* ops, const DfsPiece* pieces, int n_pieces, cudaStream_t s)
 {
     const DevBuffers& d = c->d;
     const int pw = PPL * (32 / dfs_lanes_of(C));
     const int tiles = (c->L + pw - 1) / pw;
-    prune4_dfs_kernel<C, PPL><<<n_pieces * tiles, 32, dfs_smem(dfs_lanes_of(C), c->dfs_depth, PPL), s>>>(d.dfs_ops,
-        d.dfs_pieces + first_piece, tiles, c->L, c->Lp, c->dfs_depth, d.P, d.tips, d.partials, d.scale_exp);
+    prune4_dfs_kernel<C, PPL><<<n_pieces * tiles, 32, dfs_smem(dfs_lanes_of(C), c->dfs_depth, PPL), s>>>(ops,
+        pieces, tiles, c->L, c->Lp, c->dfs_depth, d.P, d.tips, d.partials, d.scale_exp);
 }
 
 template <int C>
-static void launch_dfs(const epx_ctx* c, int first_piece, int n_pieces, cudaStream_t s, bool top)
+static void launch_dfs(const epx_ctx* c, const DfsOp* ops, const DfsPiece* pieces, int n_pieces, cudaStream_t s, bool top)
 {
     // the top piece is a few dozen operations whose operands come from HBM: one pattern per lane doubles the warps that
     // hide that latency (measured 41 -> 20 us on config 2)
-    if (top && c->prune_kernel == 0 && c->dfs_ppl == 0) { launch_dfs2<C, 1>(c, first_piece, n_pieces, s); return; }
+    if (top && c->prune_kernel == 0 && c->dfs_ppl == 0) { launch_dfs2<C, 1>(c, ops, pieces, n_pieces, s); return; }
     if (c->prune_kernel == 3) {
         const DevBuffers& d = c->d;
         const int tiles = dfs_tiles(c);
-        prune4_mma_kernel<C><<<n_pieces * tiles, 32, mma_smem(C, c->dfs_depth), s>>>(d.dfs_ops, d.dfs_pieces + first_piece, tiles,
+        prune4_mma_kernel<C><<<n_pieces * tiles, 32, mma_smem(C, c->dfs_depth), s>>>(ops, pieces, tiles,
             c->L, c->Lp, c->dfs_depth, d.P, d.tips, d.partials, d.scale_exp);
         return;
     }
     switch (dfs_patterns_per_lane(c)) {
-        case 1: launch_dfs2<C, 1>(c, first_piece, n_pieces, s); break;
-        case 2: launch_dfs2<C, 2>(c, first_piece, n_pieces, s); break;
-        default: launch_dfs2<C, 4>(c, first_piece, n_pieces, s); break;
+        case 1: launch_dfs2<C, 1>(c, ops, pieces, n_pieces, s); break;
+        case 2: launch_dfs2<C, 2>(c, ops, pieces, n_pieces, s); break;
+        default: launch_dfs2<C, 4>(c, ops, pieces, n_pieces, s); break;
+    }
+}
+
+static void launch_dfs_any(const epx_ctx* c, const DfsOp* ops, const DfsPiece* pieces, int count, cudaStream_t s, bool top)
+{
+    switch (c->C) {
+        case 1: launch_dfs<1>(c, ops, pieces, count, s, top); break;
+        case 2: launch_dfs<2>(c, ops, pieces, count, s, top); break;
+        case 3: launch_dfs<3>(c, ops, pieces, count, s, top); break;
+        case 4: launch_dfs<4>(c, ops, pieces, count, s, top); break;
+        case 5: launch_dfs<5>(c, ops, pieces, count, s, top); break;
+        case 6: launch_dfs<6>(c, ops, pieces, count, s, top); break;
+        case 7: launch_dfs<7>(c, ops, pieces, count, s, top); break;
+        default: launch_dfs<8>(c, ops, pieces, count, s, top); break;
     }
 }
 
@@ -935,54 +949,67 @@ static int launch_pruning_dfs(const epx_ctx* c, cudaStream_t s)
     for (int pass = 0; pass < 2; pass++) {
         const int first = pass == 0 ? 0 : c->dfs_bottom, count = pass == 0 ? c->dfs_bottom : total - c->dfs_bottom;
         if (count <= 0) continue;
-        switch (c->C) {
-            case 1: launch_dfs<1>(c, first, count, s, pass == 1); break;
-            case 2: launch_dfs<2>(c, first, count, s, pass == 1); break;
-            case 3: launch_dfs<3>(c, first, count, s, pass == 1); break;
-            case 4: launch_dfs<4>(c, first, count, s, pass == 1); break;
-            case 5: launch_dfs<5>(c, first, count, s, pass == 1); break;
-            case 6: launch_dfs<6>(c, first, count, s, pass == 1); break;
-            case 7: launch_dfs<7>(c, first, count, s, pass == 1); break;
-            default: launch_dfs<8>(c, first, count, s, pass == 1); break;
-        }
+        launch_dfs_any(c, c->d.dfs_ops, c->d.dfs_pieces + first, count, s, pass == 1);
         launched++;
     }
     return cudaGetLastError() == cudaSuccess ? launched : -1;
 }
 
-int launch_pruning(const epx_ctx* c, cudaStream_t s)
+// one level of the level-by-level kernels: `nops` operations whose children are complete
+static void launch_level(const epx_ctx* c, const PruneOp* ops, int nops, cudaStream_t s)
 {
     const DevBuffers& d = c->d;
     const int K = c->K, C = c->C, L = c->L;
+    if (K == 4 && c->prune_kernel != 1) {
+        switch (C) {
+            case 1: launch_prune4<1>(ops, nops, L, d, s); break;
+            case 2: launch_prune4<2>(ops, nops, L, d, s); break;
+            case 3: launch_prune4<3>(ops, nops, L, d, s); break;
+            case 4: launch_prune4<4>(ops, nops, L, d, s); break;
+            case 5: launch_prune4<5>(ops, nops, L, d, s); break;
+            case 6: launch_prune4<6>(ops, nops, L, d, s); break;
+            case 7: launch_prune4<7>(ops, nops, L, d, s); break;
+            default: launch_prune4<8>(ops, nops, L, d, s); break;
+        }
+    } else if (K > 32 && c->prune_kernel != 1 && mma64_smem(K, C) <= 227 * 1024) {
+        const int tiles = (L + M_TP - 1) / M_TP;
+        prune64_mma_kernel<<<nops * tiles, MT, mma64_smem(K, C), s>>>(ops, tiles, K, C, L, c->Lp, d.P, d.tips, d.partials,
+                                                                     d.scale_exp);
+    } else {
+        const int tile_p = prune_tile(K, C);
+        const int tiles = (L + tile_p - 1) / tile_p;
+        prune_generic_kernel<<<nops * tiles, GT, generic_smem(K, C, tile_p), s>>>(ops, tiles, tile_p, K, C, L, c->Lp, d.P,
+                                                                                  d.tips, d.partials, d.scale_exp);
+    }
+}
+
+int launch_pruning(const epx_ctx* c, cudaStream_t s)
+{
     if (prune_uses_dfs(c)) return launch_pruning_dfs(c, s);
     int launched = 0;
     const int n_levels = (int)c->level_off.size() - 1;
     for (int l = 0; l < n_levels; l++) {
         const int first = c->level_off[l], nops = c->level_off[l + 1] - first;
         if (nops == 0) continue;
-        const PruneOp* ops = d.ops + first;
-        if (K == 4 && c->prune_kernel != 1) {
-            switch (C) {
-                case 1: launch_prune4<1>(ops, nops, L, d, s); break;
-                case 2: launch_prune4<2>(ops, nops, L, d, s); break;
-                case 3: launch_prune4<3>(ops, nops, L, d, s); break;
-                case 4: launch_prune4<4>(ops, nops, L, d, s); break;
-                case 5: launch_prune4<5>(ops, nops, L, d, s); break;
-                case 6: launch_prune4<6>(ops, nops, L, d, s); break;
-                case 7: launch_prune4<7>(ops, nops, L, d, s); break;
-                default: launch_prune4<8>(ops, nops, L, d, s); break;
-            }
-        } else if (K > 32 && c->prune_kernel != 1 && mma64_smem(K, C) <= 227 * 1024) {
-            const int tiles = (L + M_TP - 1) / M_TP;
-            prune64_mma_kernel<<<nops * tiles, MT, mma64_smem(K, C), s>>>(ops, tiles, K, C, L, c->Lp, d.P, d.tips, d.partials,
-                                                                         d.scale_exp);
-        } else {
-            const int tile_p = prune_tile(K, C);
-            const int tiles = (L + tile_p - 1) / tile_p;
-            prune_generic_kernel<<<nops * tiles, GT, generic_smem(K, C, tile_p), s>>>(ops, tiles, tile_p, K, C, L, c->Lp, d.P,
-                                                                                      d.tips, d.partials, d.scale_exp);
-        }
+        launch_level(c, c->d.ops + first, nops, s);
         launched++;
+    }
+    return cudaGetLastError() == cudaSuccess ? launched : -1;
+}
+
+// f1: recompute the partials of the dirty nodes only.  Depth-first layouts: one piece of d.inc_ops (children come from
+// HBM or from the operation before); otherwise d.inc_pops holds the operations level by level, group g = [off[g], off[g+1]).
+int launch_pruning_incremental(const epx_ctx* c, const std::vector<int>& group_off, cudaStream_t s)
+{
+    int launched = 0;
+    if (prune_uses_dfs(c)) {
+        launch_dfs_any(c, c->d.inc_ops, c->d.inc_piece, 1, s, true);
+        launched = 1;
+    } else {
+        for (size_t g = 0; g + 1 < group_off.size(); g++) {
+            launch_level(c, c->d.inc_pops + group_off[g], group_off[g + 1] - group_off[g], s);
+            launched++;
+        }
     }
     return cudaGetLastError() == cudaSuccess ? launched : -1;
 }

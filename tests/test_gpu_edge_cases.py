@@ -207,3 +207,70 @@ def test_branch_rates(epx, orc_ld, cid, kw):
     with pytest.raises(epx.EpxError):
         ctx.set_branch_rates(np.full(prob.n_br, -1.0))
     ctx.close()
+
+
+def _move_nodes(rng, prob, k):
+    """New heights for k random nodes, each strictly inside the interval its children and parent allow."""
+    left, right = trees.children_of(prob.parent)
+    nodes = rng.choice(prob.n_nodes, size=k, replace=False)
+    h = prob.height.copy()
+    out = []
+    for u in nodes:
+        lo = max(h[left[u]], h[right[u]]) if left[u] >= 0 else max(0.0, h[u] - 0.05)
+        hi = h[prob.parent[u]] if prob.parent[u] >= 0 else h[u] * 1.1
+        if left[u] < 0:
+            hi = min(hi, h[u] + 0.05)
+        h[u] = lo + (hi - lo) * rng.uniform(0.05, 0.95)
+        out.append(h[u])
+    return nodes.astype(np.int32), np.array(out), h
+
+
+@pytest.mark.parametrize("cid,kw,opts", [(2, {"N": 120, "L": 333}, ()), (2, {"N": 120, "L": 333}, ((3, 2),)), (1, {}, ()),
+                                         (3, {"N": 10, "L": 40}, ()), (4, {"N": 70, "L": 3}, ())])
+def test_incremental_reevaluation(epx, orc_ld, cid, kw, opts):
+    """f1: after epx_set_node_heights only the touched matrices and the partials above them are recomputed; the result must
+    be BIT-identical to a full evaluation of the same inputs on a fresh context, and match the oracle."""
+    rng = np.random.default_rng(70 + cid)
+    prob = W.make_config(cid, **kw)
+    ctx = epx.from_problem(prob)
+    for o, v in opts:
+        ctx.set_option(o, v)
+    ctx.log_likelihood()
+    for it in range(6):
+        nodes, new_h, h = _move_nodes(rng, prob, 1 if it < 3 else 4)
+        if it == 5:
+            nodes, new_h = np.array([prob.n_nodes - 1], dtype=np.int32), np.array([prob.height.max() * 1.07])   # the root
+            h = prob.height.copy(); h[nodes[0]] = new_h[0]
+        prob = dataclasses.replace(prob, height=h)
+        n0 = ctx.launch_count()
+        ctx.set_node_heights(nodes, new_h)
+        lnl = ctx.log_likelihood_incremental()
+        used = ctx.launch_count() - n0
+        full_cost = 10 if (prob.K == 4 and not opts) else 3 + 2 + 2 + ctx.tree_levels()
+        if prob.K == 4 and not opts:
+            assert used == 3 + 1 + 1 + 2            # segmenter, chain, ONE pruning walk over the dirty path, root
+        else:
+            assert used < full_cost                  # no eigensystems / tables, only the dirty levels
+        fresh = epx.from_problem(prob)
+        for o, v in opts:
+            fresh.set_option(o, v)
+        full = fresh.log_likelihood()
+        assert lnl == full, (it, lnl, full)
+        assert np.array_equal(ctx.get_site_log_likelihoods(), fresh.get_site_log_likelihoods())
+        assert np.array_equal(ctx.get_all_matrices(), fresh.get_all_matrices())
+        for node in (prob.n_nodes - 1, prob.N + 1):
+            a, ea = ctx.get_partials(node); b, eb = fresh.get_partials(node)
+            assert np.array_equal(a, b) and np.array_equal(ea, eb)
+        fresh.close()
+        ref = orc_ld.evaluate(prob)
+        assert abs(np.longdouble(lnl) - ref["lnl"]) <= LNL_RTOL * abs(ref["lnl"])
+        assert ctx.status() == 0
+    # an invalid move is refused and changes nothing
+    with pytest.raises(epx.EpxError) as ei:
+        ctx.set_node_heights(np.array([prob.N], dtype=np.int32), np.array([prob.height.max() * 5]))
+    assert ei.value.code == epx.EPX_E_TREE
+    assert ctx.log_likelihood_incremental() == lnl
+    # any other change falls back to a full evaluation
+    ctx.set_pattern_weights(np.full(prob.L, 2.0))
+    assert abs(ctx.log_likelihood_incremental() - 2.0 * float(orc_ld.evaluate(dataclasses.replace(prob, pattern_weights=np.ones(prob.L)))["lnl"])) <= 1e-9 * abs(2 * lnl)
+    ctx.close()
