@@ -296,6 +296,9 @@ def run_cuda(args) -> None:
     # models, boundaries, category rates + weights, root frequencies
     h2d = (prob.N * ((prob.L + 31) // 32 * 32) + 8 * prob.L + 4 * n_nodes + 8 * n_nodes + 64 * (prob.N - 1) + 8 * prob.M * prob.K * prob.K +
            8 * prob.M * prob.K + 8 * (prob.M - 1) + 16 * prob.C + 8 * prob.K)
+    # (4) SURVEY.md 8(f) f1, reported beside the headline: one MCMC-style move (one random internal node slides between its
+    #     children and its parent) followed by an incremental re-evaluation, host call to host result
+    inc = bench_incremental(torch, epx, ctx, prob, stream)
     clk = clocks.stop()
     levels = ctx.tree_levels()
     ws_bytes = ctx.workspace_bytes()
@@ -330,6 +333,7 @@ def run_cuda(args) -> None:
             "gpu_launches": int(gpu_launches), "clocks": clk, "log_likelihood": lnl,
             "matrices_per_s_cfg2": world * prob.n_br * prob.C / (float(stage_ms[:3].sum()) * 1e-3)}
 
+    line["incremental"] = inc
     if rank == 0 and not args.no_matrices:
         line["matrices"] = bench_matrices(torch, epx, local, K)
     if rank == 0 and not args.no_cpu_baseline and world == 1:
@@ -340,6 +344,43 @@ def run_cuda(args) -> None:
         dist.destroy_process_group()
     if rank == 0:
         print(json.dumps(line), flush=True)
+
+
+def bench_incremental(torch, epx, ctx, prob, stream, moves: int = 64) -> dict:
+    """Average time of epx_set_node_heights (1 node) + epx_log_likelihood_incremental, which synchronises and returns logL."""
+    rng = np.random.default_rng(W.config_seed(2) + 1)
+    par = np.asarray(prob.parent)
+    h = np.asarray(prob.height, dtype=np.float64).copy()
+    kids = [[] for _ in range(prob.n_nodes)]
+    for v, p in enumerate(par):
+        if p >= 0:
+            kids[p].append(v)
+    ctx.set_tree(prob.parent, h)
+    ctx.log_likelihood()
+
+    def one_move():
+        u = int(rng.integers(prob.N, prob.n_nodes))
+        lo = max(h[kids[u][0]], h[kids[u][1]])
+        hi = h[par[u]] if par[u] >= 0 else h[u] * 1.02
+        h[u] = lo + (hi - lo) * rng.uniform(0.1, 0.9)
+        ctx.set_node_heights(np.array([u], dtype=np.int32), np.array([h[u]]))
+        return ctx.log_likelihood_incremental()
+    for _ in range(5):
+        one_move()
+    n0 = ctx.launch_count()
+    t0 = time.perf_counter()
+    ms_dev = bracket(torch, stream, one_move, moves) / moves
+    ms_wall = (time.perf_counter() - t0) / moves * 1e3
+    launches = (ctx.launch_count() - n0) / moves
+    lnl_inc = one_move()
+    ctx.set_tree(prob.parent, h)                      # full evaluation of the same final state: must agree bit for bit
+    lnl_full = ctx.log_likelihood()
+    assert lnl_inc == lnl_full, (lnl_inc, lnl_full)
+    ctx.set_tree(prob.parent, prob.height)
+    ctx.log_likelihood()
+    return {"what": "one random internal node moved (epx_set_node_heights) + epx_log_likelihood_incremental, host call to host "
+                    "result; bit-identical to a full evaluation", "ms_per_move": ms_dev, "ms_per_move_wall": ms_wall,
+            "kernel_launches_per_move": launches, "moves": moves}
 
 
 def bench_matrices(torch, epx, device: int, K: int) -> dict:

@@ -135,6 +135,7 @@ struct epx_ctx {
     // holds a complete evaluation of the current inputs that an incremental call can build on
     std::vector<int> dirty_nodes;
     bool inc_valid = false, heights_dirty = false;
+    bool last_status_ok = false;        // device status word of the last fetched evaluation was 0
     const int32_t* sub_list = nullptr;  // when set, the chain launchers recompute only these slots ...
     int sub_count = 0;                  // ... this many
     std::vector<DfsOp> dfs_ops;        // depth-first post-order walk with its stack-slot allocation

@@ -100,6 +100,12 @@ def test_host_validation_rules(L):
         with pytest.raises(epx.EpxError) as ei:
             c.set_tree(parent, h)
         assert ei.value.code == epx.EPX_E_TREE
+    # moving nodes (f1): a node must stay between its children and its parent; a refused move changes nothing
+    c.set_node_heights([3], [0.5])
+    for nodes, hs in [([3], [1.5]), ([3], [-0.1]), ([4], [0.2]), ([9], [0.1]), ([3], [np.nan])]:
+        with pytest.raises(epx.EpxError):
+            c.set_node_heights(nodes, hs)
+    c.set_node_heights([3, 4], [0.9, 2.0])           # consistent as a set
     # compute before bind -> state error, not a crash
     with pytest.raises(epx.EpxError) as ei:
         c.log_likelihood()
