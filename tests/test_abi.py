@@ -101,6 +101,7 @@ def test_host_validation_rules(L):
             c.set_tree(parent, h)
         assert ei.value.code == epx.EPX_E_TREE
     # moving nodes (f1): a node must stay between its children and its parent; a refused move changes nothing
+    c.set_tree(good_parent, good_h)
     c.set_node_heights([3], [0.5])
     for nodes, hs in [([3], [1.5]), ([3], [-0.1]), ([4], [0.2]), ([9], [0.1]), ([3], [np.nan])]:
         with pytest.raises(epx.EpxError):
