@@ -16,14 +16,42 @@ namespace {
 
 constexpr int PT = 256;
 
+__device__ __forceinline__ void dmma884(double& d0, double& d1, double a, double b)
+{
+    asm("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1}, {%2}, {%3}, {%0,%1};" : "+d"(d0), "+d"(d1) : "d"(a), "d"(b));
+}
+
+// C = A B for dense K x K matrices in shared memory (row stride K).  The K^3 products of the scaling-and-squaring
+// exponentials are where this file spends its time; they run on the FP64 tensor pipe: warp w owns the 8-row tiles w,
+// w + 8, ..., all column tiles of a row tile accumulate in registers, fragments outside the matrix are zero.
 __device__ __forceinline__ void mm(int K, const double* __restrict__ A, const double* __restrict__ B,
                                    double* __restrict__ Cm)
 {
-    for (int idx = threadIdx.x; idx < K * K; idx += PT) {
-        int i = idx / K, j = idx % K;
-        double a = 0.0;
-        for (int k = 0; k < K; k++) a = fma(A[i * K + k], B[k * K + j], a);
-        Cm[idx] = a;
+    const int lane = threadIdx.x & 31, w = threadIdx.x >> 5, g = lane >> 2, q = lane & 3;
+    const int nt_n = (K + 7) >> 3, nk = (K + 3) >> 2;
+    for (int mt = w; mt < nt_n; mt += PT / 32) {
+        const int row = 8 * mt + g;
+        const bool row_ok = row < K;
+        for (int n0 = 0; n0 < nt_n; n0 += 4) {                  // four column tiles at a time: 8 accumulator registers
+            double acc[4][2] = {{0.0, 0.0}, {0.0, 0.0}, {0.0, 0.0}, {0.0, 0.0}};
+            for (int kt = 0; kt < nk; kt++) {
+                const int k = 4 * kt + q;
+                const bool k_ok = k < K;
+                const double a = (row_ok && k_ok) ? A[row * K + k] : 0.0;
+#pragma unroll
+                for (int t = 0; t < 4; t++) {
+                    const int col = 8 * (n0 + t) + g;
+                    const double b = (k_ok && col < K) ? B[k * K + col] : 0.0;
+                    dmma884(acc[t][0], acc[t][1], a, b);
+                }
+            }
+#pragma unroll
+            for (int t = 0; t < 4; t++) {
+                const int col = 8 * (n0 + t) + 2 * q;
+                if (row_ok && col < K) Cm[row * K + col] = acc[t][0];
+                if (row_ok && col + 1 < K) Cm[row * K + col + 1] = acc[t][1];
+            }
+        }
     }
     __syncthreads();
 }
