@@ -168,7 +168,9 @@ enum {
     EPX_OPT_PRUNE_KERNEL = 3, /* 0 auto (default: K == 4 walks the tree depth first, partials never re-read from HBM);
                                  1 force the generic shared-memory level kernel; 2 (K == 4) the level-by-level register
                                  kernel; 3 (K == 4) the depth-first walk with the 4x4 products on the FP64 tensor pipe
-                                 (mma.sync m8n8k4; measured 10 % slower than 0 on config 2, kept for comparison) */
+                                 (mma.sync m8n8k4; measured 10 % slower than 0 on config 2, kept for comparison);
+                                 4 (32 < K <= 64) one CTA per (node, tile) looping over the categories instead of a
+                                 cluster of one CTA per category */
     EPX_OPT_EXP_METHOD = 4,   /* a3 method.  1 spectral: Jacobi eigensystem (reversible) / Pade 13 (asymmetric), absolute
                                  error ~1e-14 per entry.  2 componentwise: shifted non-negative Taylor scaling-and-squaring,
                                  every entry to a few hundred ulp RELATIVE, ~8 dense products per segment.  0 auto (default):

@@ -22,6 +22,7 @@
 //                      and the child tiles are staged in shared memory, DFMA mat-vec products.
 //   root_site_kernel / final_sum_kernel  per-pattern ln-likelihood, deterministic two-stage weighted sum.
 #include "epx_internal.h"
+#include <cooperative_groups.h>
 
 namespace {
 
@@ -777,6 +778,121 @@ __global__ void __launch_bounds__(MT) prune64_mma_kernel(const PruneOp* __restri
     }
 }
 
+// Same products, one CTA per CATEGORY: the C CTAs of a (node, pattern tile) form a thread-block cluster, each stages and
+// multiplies its own category, and the per-pattern maximum over all categories (the rescaling is per (node, pattern),
+// reading A12) is exchanged through distributed shared memory.  C times more CTAs per level and a C times shorter serial
+// path per CTA: the upper levels of a 100-tip codon tree hold one to four nodes.
+__global__ void __launch_bounds__(MT) prune64_cluster_kernel(const PruneOp* __restrict__ ops, int tiles, int K, int C, int L,
+    int Lp, const double* __restrict__ P, const uint8_t* __restrict__ tips, double* __restrict__ partials,
+    int32_t* __restrict__ scale_exp)
+{
+    namespace cg = cooperative_groups;
+    cg::cluster_group cluster = cg::this_cluster();
+    extern __shared__ double sm[];
+    double* Pm = sm;                                   // [64][68]  one child at a time: 68 KB per CTA, three CTAs per SM
+    double* V = Pm + 64 * M_LD;                        // [32][68]
+    double* out = V + M_TP * M_LD;                     // [32][K]
+    double* mx = out + (size_t)M_TP * K;               // [32] this category's per-pattern maximum (read by the cluster)
+    double* scl = mx + M_TP;                           // [32]
+    int* st = reinterpret_cast<int*>(scl + M_TP);      // [32] tip states
+    const int c = (int)cluster.block_rank();
+    const int unit = blockIdx.x / C;
+    const PruneOp op = ops[unit / tiles];
+    const int tid = threadIdx.x, lane = tid & 31, w = tid >> 5, g = lane >> 2, q = lane & 3;
+    const int p0 = (unit % tiles) * M_TP;
+    const int np = min(M_TP, L - p0);
+    const int KK = K * K;
+    const int mt = w & 3, nh = w >> 2;
+
+    double f[4][2];
+#pragma unroll
+    for (int t = 0; t < 4; t++) f[t][0] = f[t][1] = 1.0;
+    for (int ch = 0; ch < 2; ch++) {
+        if (ch) __syncthreads();                       // everyone is done with the first child's operands
+        if (op.child_is_tip[ch])
+            for (int p = tid; p < M_TP; p += MT) st[p] = p < np ? tips[(size_t)op.child[ch] * Lp + p0 + p] : 255;
+        const double* src = P + ((size_t)op.child[ch] * C + c) * KK;
+        for (int idx = tid; idx < 64 * 64; idx += MT) {
+            const int i = idx >> 6, j = idx & 63;
+            Pm[i * M_LD + j] = (i < K && j < K) ? src[i * K + j] : 0.0;
+        }
+        if (!op.child_is_tip[ch]) {
+            const double* cs = partials + (((size_t)op.cpidx[ch] * C + c) * L + p0) * K;
+            for (int idx = tid; idx < M_TP * 64; idx += MT) {
+                const int p = idx >> 6, j = idx & 63;
+                V[p * M_LD + j] = (p < np && j < K) ? cs[p * K + j] : 0.0;
+            }
+        }
+        __syncthreads();
+        if (op.child_is_tip[ch]) {
+            const int s = st[8 * mt + g];
+#pragma unroll
+            for (int t = 0; t < 4; t++) {
+                const int i = 8 * (4 * nh + t) + 2 * q;
+                f[t][0] *= s < K ? Pm[i * M_LD + s] : 1.0;
+                f[t][1] *= s < K ? Pm[(i + 1) * M_LD + s] : 1.0;
+            }
+        } else {
+            double acc[4][2];
+#pragma unroll
+            for (int t = 0; t < 4; t++) acc[t][0] = acc[t][1] = 0.0;
+            const double* Arow = V + (8 * mt + g) * M_LD + q;
+            const double* Brow = Pm + (32 * nh + g) * M_LD + q;
+#pragma unroll 4
+            for (int kt = 0; kt < 16; kt++) {
+                const double a = Arow[4 * kt];
+#pragma unroll
+                for (int t = 0; t < 4; t++) dmma884(acc[t][0], acc[t][1], a, Brow[8 * t * M_LD + 4 * kt]);
+            }
+#pragma unroll
+            for (int t = 0; t < 4; t++) { f[t][0] *= acc[t][0]; f[t][1] *= acc[t][1]; }
+        }
+    }
+    {
+        const int p = 8 * mt + g;
+#pragma unroll
+        for (int t = 0; t < 4; t++) {
+            const int i = 8 * (4 * nh + t) + 2 * q;
+            if (p < np && i < K) out[(size_t)p * K + i] = f[t][0];
+            if (p < np && i + 1 < K) out[(size_t)p * K + i + 1] = f[t][1];
+        }
+    }
+    __syncthreads();
+    {   // this category's per-pattern maximum: 8 lanes per pattern
+        const int p = tid / 8, sub = tid & 7;
+        double m = 0.0;
+        if (p < np)
+            for (int i = sub; i < K; i += 8) m = fmax(m, out[(size_t)p * K + i]);
+        for (int o = 4; o > 0; o >>= 1) m = fmax(m, __shfl_xor_sync(0xffffffffu, m, o));
+        if (sub == 0) mx[p] = p < np ? m : 0.0;
+    }
+    cluster.sync();
+    if (tid < M_TP) {
+        const int p = tid;
+        double m = 0.0;
+        for (int r = 0; r < C; r++) m = fmax(m, cluster.map_shared_rank(mx, r)[p]);
+        double sc = 1.0;
+        int e = 0;
+        if (m > 0.0 && m < 1.7e308) {
+            const int ee = exponent_of(m);
+            if (ee > -1000) { sc = pow2_neg(ee); e = ee; }
+        }
+        scl[p] = sc;
+        if (c == 0 && p < np) {
+            int ex = e;
+            for (int ch = 0; ch < 2; ch++)
+                if (!op.child_is_tip[ch]) ex += scale_exp[(size_t)op.cpidx[ch] * L + p0 + p];
+            scale_exp[(size_t)op.pidx * L + p0 + p] = ex;
+        }
+    }
+    __syncthreads();
+    double* dst = partials + (((size_t)op.pidx * C + c) * L + p0) * K;
+    for (int idx = tid; idx < np * K; idx += MT) dst[idx] = out[idx] * scl[idx / K];
+    cluster.sync();          // nobody leaves while its maxima may still be read
+}
+
+size_t mma64_cluster_smem(int K) { return sizeof(double) * (64 * M_LD + M_TP * M_LD + (size_t)M_TP * K + 2 * M_TP) + sizeof(int) * M_TP; }
+
 size_t mma64_smem(int K, int C) { return sizeof(double) * (2 * 64 * M_LD + 2 * M_TP * M_LD + (size_t)C * M_TP * K + M_TP) + sizeof(int) * 2 * M_TP; }
 
 // ------------------------------------------------------------------------------------------------ a6
@@ -868,6 +984,7 @@ int prune_init_attributes()
     if (dfs_set_attr<1>() || dfs_set_attr<2>() || dfs_set_attr<3>() || dfs_set_attr<4>() || dfs_set_attr<5>() ||
         dfs_set_attr<6>() || dfs_set_attr<7>() || dfs_set_attr<8>()) return -1;
     if (cudaFuncSetAttribute(prune64_mma_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024) != cudaSuccess) return -1;
+    if (cudaFuncSetAttribute(prune64_cluster_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024) != cudaSuccess) return -1;
     return cudaFuncSetAttribute(prune_generic_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024) == cudaSuccess ? 0 : -1;
 }
 
@@ -973,8 +1090,23 @@ static void launch_level(const epx_ctx* c, const PruneOp* ops, int nops, cudaStr
         }
     } else if (K > 32 && c->prune_kernel != 1 && mma64_smem(K, C) <= 227 * 1024) {
         const int tiles = (L + M_TP - 1) / M_TP;
-        prune64_mma_kernel<<<nops * tiles, MT, mma64_smem(K, C), s>>>(ops, tiles, K, C, L, c->Lp, d.P, d.tips, d.partials,
-                                                                     d.scale_exp);
+        if (c->prune_kernel == 0) {              // one CTA per category, clusters of C
+            cudaLaunchConfig_t cfg{};
+            cfg.gridDim = dim3((unsigned)(nops * tiles * C));
+            cfg.blockDim = dim3(MT);
+            cfg.dynamicSmemBytes = mma64_cluster_smem(K);
+            cfg.stream = s;
+            cudaLaunchAttribute attr{};
+            attr.id = cudaLaunchAttributeClusterDimension;
+            attr.val.clusterDim.x = (unsigned)C; attr.val.clusterDim.y = 1; attr.val.clusterDim.z = 1;
+            cfg.attrs = &attr; cfg.numAttrs = 1;
+            const int Lp = c->Lp;
+            cudaLaunchKernelEx(&cfg, prune64_cluster_kernel, ops, tiles, K, C, L, Lp, (const double*)d.P, (const uint8_t*)d.tips,
+                               d.partials, d.scale_exp);
+        } else {
+            prune64_mma_kernel<<<nops * tiles, MT, mma64_smem(K, C), s>>>(ops, tiles, K, C, L, c->Lp, d.P, d.tips, d.partials,
+                                                                         d.scale_exp);
+        }
     } else {
         const int tile_p = prune_tile(K, C);
         const int tiles = (L + tile_p - 1) / tile_p;
