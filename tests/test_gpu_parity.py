@@ -111,6 +111,8 @@ def test_k4_every_category_count(epx, orc_ld, C):
     tips[5, :] = 99
     prob = dataclasses.replace(prob, C=C, rates=rates, weights=weights, tip_states=tips)
     run_tree(epx, orc_ld, prob)
+    for ppl in (2, 4):                                  # 2 / 4 patterns per lane: tiles of 16..128 patterns, ragged tail
+        run_tree(epx, orc_ld, prob, options=[(epx.EPX_OPT_DFS_PPL, ppl)], partial_nodes=[prob.n_nodes - 1, prob.N])
     run_tree(epx, orc_ld, prob, options=[(epx.EPX_OPT_PRUNE_KERNEL, 3)])
     run_tree(epx, orc_ld, prob, options=[(epx.EPX_OPT_PRUNE_KERNEL, 2)], partial_nodes=[prob.n_nodes - 1])
 
