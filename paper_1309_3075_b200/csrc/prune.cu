@@ -895,6 +895,150 @@ size_t mma64_cluster_smem(int K) { return sizeof(double) * (64 * M_LD + M_TP * M
 
 size_t mma64_smem(int K, int C) { return sizeof(double) * (2 * 64 * M_LD + 2 * M_TP * M_LD + (size_t)C * M_TP * K + M_TP) + sizeof(int) * 2 * M_TP; }
 
+// ------------------------------------------------------------------------------------------------ few patterns, K <= 32
+// A discrete trait observed at one site (PAPER.md L224 workload A: K = 7 locations; config 4: K = 24, L = 1): a tree level
+// holds a handful of nodes and the level-by-level kernels are pure launch latency (config 4: 168 levels x 5 us).  The
+// depth-first walk needs no level at all: one warp per (piece of the tree, pattern), lane i = parent state i, the
+// children's vectors in a per-warp shared-memory stack (every result is parked: a dot product needs the whole vector),
+// matrix rows straight from global memory (each lane its own row; the rows of the next operations are pulled into L1 while
+// the current one computes), the per-(node, pattern) maximum by warp shuffles.  Partials keep the generic [node][C][L][K]
+// layout.  The pieces (independent subtrees, then the top piece reading their roots from HBM) are the ones planned for
+// the K = 4 walk.
+constexpr int KD_MAXC = 8;
+
+__device__ __forceinline__ void cp_async8(void* dst, const void* src)
+{
+    asm volatile("cp.async.ca.shared.global [%0], [%1], 8;" ::"r"(smem_addr(dst)), "l"(src) : "memory");
+}
+
+constexpr int KD_STAGES = 3;
+
+__global__ void __launch_bounds__(32) pruneK_dfs_kernel(const DfsOp* __restrict__ ops, const DfsPiece* __restrict__ pieces,
+    int K, int C, int L, int Lp, int depth, const double* __restrict__ P, const uint8_t* __restrict__ tips,
+    double* __restrict__ partials, int32_t* __restrict__ scale_exp)
+{
+    extern __shared__ double kd_sm[];
+    const int CK = C * K, KK = K * K, CKK = C * KK;
+    const int stage_d = 2 * CKK + 2 * CK;                            // doubles per stage: both children's matrices + HBM vectors
+    double* ring = kd_sm;                                            // [KD_STAGES][stage_d]
+    double* slots = ring + (size_t)KD_STAGES * stage_d;              // [depth + 2][C * K]: stack + 2 hand-over slots
+    int* slot_ex = reinterpret_cast<int*>(slots + (size_t)(depth + 2) * CK);    // [depth + 2]
+    const int lane = threadIdx.x, i = min(lane, K - 1);
+    const bool on = lane < K;
+    const int piece = blockIdx.x / L, p = blockIdx.x - piece * L;
+    const DfsPiece pc = pieces[piece];
+    const int n_ops = pc.end - pc.begin;
+    const int4* opv = reinterpret_cast<const int4*>(ops + pc.begin);
+
+    // Everything an operation reads from global memory is fetched ahead of the dependency chain: descriptors four
+    // operations ahead, tip states / exponents of HBM operands two ahead in registers, the children's matrices and the
+    // HBM operands' vectors two ahead with cp.async into a shared-memory ring.
+    auto load_desc = [&](int k, int4& d, int4& h) {
+        d = make_int4(0, 0, 0, 0); h = d;
+        if (k < n_ops) { d = __ldg(opv + 2 * k); h = __ldg(opv + 2 * k + 1); }
+    };
+    auto stage = [&](int k, const int4& d, const int4& h, int& sa, int& sb) {      // sa / sb: tip state, or exponent of an HBM operand
+        sa = sb = 255;
+        if (k < n_ops) {
+            double* st = ring + (size_t)(k % KD_STAGES) * stage_d;
+            const int srcA = (d.w & 0xff) - 3, srcB = ((d.w >> 8) & 0xff) - 3;
+            const double* pa = P + (size_t)d.x * CKK;
+            const double* pb = P + (size_t)d.y * CKK;
+            for (int o = lane; o < CKK; o += 32) { cp_async8(st + o, pa + o); cp_async8(st + CKK + o, pb + o); }
+            if (srcA == EPX_DFS_TIP) sa = tips[(size_t)d.x * Lp + p];
+            if (srcB == EPX_DFS_TIP) sb = tips[(size_t)d.y * Lp + p];
+            if (srcA == EPX_DFS_HBM) {
+                for (int o = lane; o < CK; o += 32)
+                    cp_async8(st + 2 * CKK + o, partials + (((size_t)h.x * C + o / K) * L + p) * K + o % K);
+                sa = scale_exp[(size_t)h.x * L + p];
+            }
+            if (srcB == EPX_DFS_HBM) {
+                for (int o = lane; o < CK; o += 32)
+                    cp_async8(st + 2 * CKK + CK + o, partials + (((size_t)h.y * C + o / K) * L + p) * K + o % K);
+                sb = scale_exp[(size_t)h.y * L + p];
+            }
+        }
+        cp_async_commit();
+    };
+    int4 d0, h0, d1, h1, d2, h2, d3, h3;
+    load_desc(0, d0, h0); load_desc(1, d1, h1); load_desc(2, d2, h2); load_desc(3, d3, h3);
+    int ta0, tb0, ta1, tb1;
+    stage(0, d0, h0, ta0, tb0); stage(1, d1, h1, ta1, tb1);
+    for (int k = 0; k < n_ops; k++) {
+        const int4 d = d0;
+        const int aux[2] = {ta0, tb0};
+        d0 = d1; h0 = h1; d1 = d2; h1 = h2; d2 = d3; h2 = h3;
+        load_desc(k + 4, d3, h3);
+        ta0 = ta1; tb0 = tb1;
+        __syncwarp();                                   // every lane is done with the ring buffer stage k+2 overwrites
+        stage(k + 2, d1, h1, ta1, tb1);
+        const int srcs[2] = {(d.w & 0xff) - 3, ((d.w >> 8) & 0xff) - 3};
+        const int out_slot = ((d.w >> 16) & 0xff) - 1;
+        const int prev_slot = depth + ((k + 1) & 1), dst = out_slot >= 0 ? out_slot : depth + (k & 1);
+        cp_async_wait<2>();
+        __syncwarp();                                   // stage k has landed; the slot written by operation k-1 is visible
+        const double* st = ring + (size_t)(k % KD_STAGES) * stage_d;
+        double f[KD_MAXC];
+#pragma unroll
+        for (int c = 0; c < KD_MAXC; c++) f[c] = 1.0;
+        int ex = 0;
+        for (int ch = 0; ch < 2; ch++) {
+            const int src = srcs[ch];
+            const double* Pm = st + ch * CKK + (size_t)i * K;          // row i of category 0
+            if (src == EPX_DFS_TIP) {
+                const int s = aux[ch];
+#pragma unroll
+                for (int c = 0; c < KD_MAXC; c++)
+                    if (c < C) f[c] *= s < K ? Pm[c * KK + s] : 1.0;
+                continue;
+            }
+            const double* v;
+            if (src == EPX_DFS_HBM) {
+                v = st + 2 * CKK + ch * CK;
+                ex += aux[ch];
+            } else {
+                const int sl = src == EPX_DFS_PREV ? prev_slot : src;
+                v = slots + (size_t)sl * CK;
+                ex += slot_ex[sl];
+            }
+#pragma unroll
+            for (int c = 0; c < KD_MAXC; c++) {
+                if (c >= C) break;
+                const double* row = Pm + c * KK;
+                const double* vc = v + c * K;
+                double acc = 0.0;                      // one chain, j ascending: the level kernels' order, so that an
+                for (int j = 0; j < K; j++) acc = fma(row[j], vc[j], acc);      // incremental re-evaluation is bit-identical
+                f[c] *= acc;
+            }
+        }
+        double m = 0.0;
+#pragma unroll
+        for (int c = 0; c < KD_MAXC; c++)
+            if (c < C && on) m = fmax(m, f[c]);
+        for (int o = 16; o > 0; o >>= 1) m = fmax(m, __shfl_xor_sync(0xffffffffu, m, o));
+        double sc = 1.0;
+        if (m > 0.0 && m < 1.7e308) {
+            const int e = exponent_of(m);
+            if (e > -1000) { sc = pow2_neg(e); ex += e; }
+        }
+        __syncwarp();                                   // every lane has read its operands (dst may be a slot just consumed)
+        double* S = slots + (size_t)dst * CK;
+#pragma unroll
+        for (int c = 0; c < KD_MAXC; c++)
+            if (c < C && on) {
+                const double val = f[c] * sc;
+                S[c * K + lane] = val;
+                partials[(((size_t)d.z * C + c) * L + p) * K + lane] = val;
+            }
+        if (lane == 0) { slot_ex[dst] = ex; scale_exp[(size_t)d.z * L + p] = ex; }
+    }
+}
+
+size_t kdfs_smem(int K, int C, int depth)
+{
+    return sizeof(double) * ((size_t)KD_STAGES * (2 * C * K * K + 2 * C * K) + (size_t)(depth + 2) * C * K) + sizeof(int) * (depth + 4);
+}
+
 // ------------------------------------------------------------------------------------------------ a6
 __global__ void __launch_bounds__(256) root_site_kernel(int K, int C, int L, size_t sc, size_t sp, int root_pidx, int root_node,
     const double* __restrict__ partials, const int32_t* __restrict__ scale_exp, const double* __restrict__ freqs,
@@ -984,6 +1128,7 @@ int prune_init_attributes()
     if (dfs_set_attr<1>() || dfs_set_attr<2>() || dfs_set_attr<3>() || dfs_set_attr<4>() || dfs_set_attr<5>() ||
         dfs_set_attr<6>() || dfs_set_attr<7>() || dfs_set_attr<8>()) return -1;
     if (cudaFuncSetAttribute(prune64_mma_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024) != cudaSuccess) return -1;
+    if (cudaFuncSetAttribute(pruneK_dfs_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, 100 * 1024) != cudaSuccess) return -1;
     if (cudaFuncSetAttribute(prune64_cluster_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024) != cudaSuccess) return -1;
     return cudaFuncSetAttribute(prune_generic_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024) == cudaSuccess ? 0 : -1;
 }
@@ -998,8 +1143,16 @@ int dfs_patterns_per_lane(const epx_ctx* c)
     return tiles1 >= 512 ? 2 : 1;
 }
 
+// walk for few patterns and K <= 32 (pruneK_dfs_kernel); generic partials layout
+bool prune_uses_kdfs(const epx_ctx* c)
+{
+    return c->tree_mode && c->K != 4 && c->K <= 32 && c->C <= KD_MAXC && c->prune_kernel == 0 && (long)c->L * c->C <= 64 &&
+           c->N >= 8 && kdfs_smem(c->K, c->C, c->dfs_depth > 0 ? c->dfs_depth : 1) <= 100 * 1024;
+}
+
 int dfs_tiles(const epx_ctx* c)
 {
+    if (c->K != 4) return c->L;                                // pruneK_dfs_kernel: one warp per pattern
     if (c->prune_kernel == 3) return (c->L + 7) / 8;          // tensor-core walk: 8 patterns per warp
     const int pw = dfs_patterns_per_lane(c) * (32 / dfs_lanes_of(c->C));
     return (c->L + pw - 1) / pw;
@@ -1118,6 +1271,20 @@ static void launch_level(const epx_ctx* c, const PruneOp* ops, int nops, cudaStr
 int launch_pruning(const epx_ctx* c, cudaStream_t s)
 {
     if (prune_uses_dfs(c)) return launch_pruning_dfs(c, s);
+    if (prune_uses_kdfs(c)) {
+        const DevBuffers& d = c->d;
+        const int total = (int)c->dfs_pieces.size();
+        const size_t smem = kdfs_smem(c->K, c->C, c->dfs_depth);
+        int n = 0;
+        for (int pass = 0; pass < 2; pass++) {
+            const int first = pass == 0 ? 0 : c->dfs_bottom, count = pass == 0 ? c->dfs_bottom : total - c->dfs_bottom;
+            if (count <= 0) continue;
+            pruneK_dfs_kernel<<<count * c->L, 32, smem, s>>>(d.dfs_ops, d.dfs_pieces + first, c->K, c->C, c->L, c->Lp, c->dfs_depth,
+                                                           d.P, d.tips, d.partials, d.scale_exp);
+            n++;
+        }
+        return cudaGetLastError() == cudaSuccess ? n : -1;
+    }
     int launched = 0;
     const int n_levels = (int)c->level_off.size() - 1;
     for (int l = 0; l < n_levels; l++) {
