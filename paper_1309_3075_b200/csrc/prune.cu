@@ -581,6 +581,24 @@ size_t mma_smem(int C, int depth) { return 8 * (size_t)(depth + 2) * mma_slot_do
 size_t dfs_smem(int G, int depth, int ppl) { return (size_t)DFS_STAGES * dfs_stage_bytes(G) + (size_t)depth * ppl * (128 * 8 + 32 * 4); }
 
 // ------------------------------------------------------------------------------------------------ any K
+// sum_j row[j] v[j] with four interleaved chains (j mod 4), combined as (a0 + a1) + (a2 + a3).  Shared by the level kernel
+// and the few-pattern walk so that the two produce the same bits (an incremental re-evaluation uses the level kernel).
+__device__ __forceinline__ double dot4(const double* __restrict__ row, const double* __restrict__ v, int K)
+{
+    double a0 = 0.0, a1 = 0.0, a2 = 0.0, a3 = 0.0;
+    int j = 0;
+    for (; j + 4 <= K; j += 4) {
+        a0 = fma(row[j], v[j], a0);
+        a1 = fma(row[j + 1], v[j + 1], a1);
+        a2 = fma(row[j + 2], v[j + 2], a2);
+        a3 = fma(row[j + 3], v[j + 3], a3);
+    }
+    if (j < K) a0 = fma(row[j], v[j], a0);
+    if (j + 1 < K) a1 = fma(row[j + 1], v[j + 1], a1);
+    if (j + 2 < K) a2 = fma(row[j + 2], v[j + 2], a2);
+    return (a0 + a1) + (a2 + a3);
+}
+
 constexpr int GT = 256;
 
 __global__ void __launch_bounds__(GT) prune_generic_kernel(const PruneOp* __restrict__ ops, int tiles, int tile_p,
@@ -625,8 +643,7 @@ __global__ void __launch_bounds__(GT) prune_generic_kernel(const PruneOp* __rest
                     a = s < K ? row[s] : 1.0;
                 } else {
                     const double* v = ch_t + ((size_t)ch * tile_p + p) * K;
-                    a = 0.0;
-                    for (int j = 0; j < K; j++) a = fma(row[j], v[j], a);
+                    a = dot4(row, v, K);
                 }
                 prod *= a;
             }
@@ -944,7 +961,11 @@ __global__ void __launch_bounds__(32) pruneK_dfs_kernel(const DfsOp* __restrict_
             const int srcA = (d.w & 0xff) - 3, srcB = ((d.w >> 8) & 0xff) - 3;
             const double* pa = P + (size_t)d.x * CKK;
             const double* pb = P + (size_t)d.y * CKK;
-            for (int o = lane; o < CKK; o += 32) { cp_async8(st + o, pa + o); cp_async8(st + CKK + o, pb + o); }
+            if ((CKK & 1) == 0) {                        // C K^2 even: 16-byte copies (matrices are 16-byte aligned then)
+                for (int o = 2 * lane; o < CKK; o += 64) { cp_async16(st + o, pa + o); cp_async16(st + CKK + o, pb + o); }
+            } else {
+                for (int o = lane; o < CKK; o += 32) { cp_async8(st + o, pa + o); cp_async8(st + CKK + o, pb + o); }
+            }
             if (srcA == EPX_DFS_TIP) sa = tips[(size_t)d.x * Lp + p];
             if (srcB == EPX_DFS_TIP) sb = tips[(size_t)d.y * Lp + p];
             if (srcA == EPX_DFS_HBM) {
@@ -1006,9 +1027,7 @@ __global__ void __launch_bounds__(32) pruneK_dfs_kernel(const DfsOp* __restrict_
                 if (c >= C) break;
                 const double* row = Pm + c * KK;
                 const double* vc = v + c * K;
-                double acc = 0.0;                      // one chain, j ascending: the level kernels' order, so that an
-                for (int j = 0; j < K; j++) acc = fma(row[j], vc[j], acc);      // incremental re-evaluation is bit-identical
-                f[c] *= acc;
+                f[c] *= dot4(row, vc, K);              // the level kernel's summation order: incremental re-evaluation is bit-identical
             }
         }
         double m = 0.0;
