@@ -79,6 +79,9 @@ int epx_set_category_rates(epx_ctx* ctx, const double* rates, const double* weig
 int epx_set_tree(epx_ctx* ctx, const int32_t* parent, const double* height);
 /* states: [N][L] row-major; 0..K-1 = observed state, anything else = missing (all-ones tip vector, A10). */
 int epx_set_tip_states(epx_ctx* ctx, const int32_t* states);
+/* The same from bytes ([N][L] row-major; 0..K-1 = observed state, anything else, e.g. 255, = missing): a quarter of the
+ * host memory traffic of the int32 form -- sequence data are bytes to begin with. */
+int epx_set_tip_states_u8(epx_ctx* ctx, const uint8_t* states);
 /* wt: L pattern weights (a weight w == the pattern repeated w times), or NULL = all 1. */
 int epx_set_pattern_weights(epx_ctx* ctx, const double* wt);
 /* freqs: K root distribution, or NULL = the freqs of the epoch that contains the root height (A9). */

@@ -55,6 +55,7 @@ def lib():
     _sig(L, "epx_set_category_rates", i, vp, dp, dp)
     _sig(L, "epx_set_tree", i, vp, ip, dp)
     _sig(L, "epx_set_tip_states", i, vp, ip)
+    _sig(L, "epx_set_tip_states_u8", i, vp, ip)
     _sig(L, "epx_set_pattern_weights", i, vp, dp)
     _sig(L, "epx_set_root_frequencies", i, vp, dp)
     _sig(L, "epx_set_branches", i, vp, i, dp, dp)
@@ -181,6 +182,11 @@ class Epx:
         assert states.shape == (self.N, self.L)
         self._check(self._L.epx_set_tip_states(self._ctx, _ptr(states)))
 
+    def set_tip_states_u8(self, states) -> None:
+        states = np.ascontiguousarray(states, dtype=np.uint8)
+        assert states.shape == (self.N, self.L)
+        self._check(self._L.epx_set_tip_states_u8(self._ctx, _ptr(states)))
+
     def set_pattern_weights(self, wt) -> None:
         wt = None if wt is None else _f64(wt)
         self._check(self._L.epx_set_pattern_weights(self._ctx, _ptr(wt)))
@@ -305,16 +311,20 @@ class Epx:
         return n.value
 
 
-def set_problem(ctx: Epx, prob) -> None:
+def set_problem(ctx: Epx, prob, tip_states_u8=None) -> None:
     """Call every setter of `ctx` from a problem object (attributes as in workloads.EpochProblem; read by
-    attribute, nothing is imported)."""
+    attribute, nothing is imported).  `tip_states_u8`: the tip states as a host uint8 array, passed through
+    epx_set_tip_states_u8 instead of the int32 form."""
     ctx.set_epoch_boundaries(prob.tau)
     for e in range(prob.M):
         ctx.set_epoch_model(e, prob.Q[e], prob.freqs[e], prob.reversible)
     ctx.set_category_rates(prob.rates, prob.weights)
     if prob.N > 0:
         ctx.set_tree(prob.parent, prob.height)
-        ctx.set_tip_states(prob.tip_states)
+        if tip_states_u8 is not None:
+            ctx.set_tip_states_u8(tip_states_u8)
+        else:
+            ctx.set_tip_states(prob.tip_states)
         ctx.set_pattern_weights(prob.pattern_weights)
         ctx.set_root_frequencies(prob.root_freqs)
     else:

@@ -542,7 +542,11 @@ int epx_set_branch_rates(epx_ctx* c, const double* rates)
     return EPX_OK;
 }
 
-int epx_set_tip_states(epx_ctx* c, const int32_t* states)
+// Repack tip states (int32 or bytes) into the padded byte rows of the page-locked staging buffer.  Integer repacking,
+// split over host threads; no arithmetic of the method.
+extern "C++" {
+template <typename T>
+static int set_tips_impl(epx_ctx* c, const T* states)
 {
     if (!c || !states) return EPX_E_ARG;
     if (!c->tree_mode) return fail(c, EPX_E_STATE, "ctx is in branch-list mode");
@@ -561,20 +565,25 @@ int epx_set_tip_states(epx_ctx* c, const int32_t* states)
         // an earlier upload may still be reading the staging buffer
         CUDA_TRY(c, cudaStreamSynchronize(c->stream));
     }
-    const int K = c->K;
+    const unsigned K = (unsigned)c->K;
     uint8_t* const base = c->tips;
     auto convert_rows = [=](size_t t0, size_t t1) {
         for (size_t t = t0; t < t1; t++) {
-            const int32_t* src = states + t * L;
-            uint8_t* dst = base + t * Lp;
-            for (size_t p = 0; p < L; p++) {
-                const uint32_t s = (uint32_t)src[p];
-                dst[p] = s < (uint32_t)K ? (uint8_t)s : (uint8_t)255;
+            const T* __restrict__ src = states + t * L;
+            uint8_t* __restrict__ dst = base + t * Lp;
+            if (sizeof(T) == 1) {
+                const uint8_t k8 = (uint8_t)K;                // K <= 64
+                const uint8_t* __restrict__ s8 = reinterpret_cast<const uint8_t*>(src);
+                for (size_t p = 0; p < L; p++) dst[p] = (uint8_t)(s8[p] | (uint8_t)(0 - (uint8_t)(s8[p] >= k8)));   // byte-wide, vectorises
+            } else {
+                for (size_t p = 0; p < L; p++) {
+                    const unsigned s = (unsigned)src[p];      // negative int32 -> huge -> missing
+                    dst[p] = s < K ? (uint8_t)s : (uint8_t)255;
+                }
             }
             for (size_t p = L; p < Lp; p++) dst[p] = 255;
         }
     };
-    // integer repacking of the caller's int32 states into bytes, split over host threads (no arithmetic of the method)
     size_t nthreads = std::min<size_t>(std::min<size_t>(16, std::max(1u, std::thread::hardware_concurrency())), (N * L) >> 20);
     if (nthreads <= 1) {
         convert_rows(0, N);
@@ -586,6 +595,10 @@ int epx_set_tip_states(epx_ctx* c, const int32_t* states)
     c->has_tips = true; c->tips_dirty = true;
     return EPX_OK;
 }
+}  // extern "C++"
+
+int epx_set_tip_states(epx_ctx* c, const int32_t* states) { return set_tips_impl(c, states); }
+int epx_set_tip_states_u8(epx_ctx* c, const uint8_t* states) { return set_tips_impl(c, states); }
 
 int epx_set_pattern_weights(epx_ctx* c, const double* wt)
 {

@@ -274,3 +274,22 @@ def test_incremental_reevaluation(epx, orc_ld, cid, kw, opts):
     ctx.set_pattern_weights(np.full(prob.L, 2.0))
     assert abs(ctx.log_likelihood_incremental() - 2.0 * float(orc_ld.evaluate(dataclasses.replace(prob, pattern_weights=np.ones(prob.L)))["lnl"])) <= 1e-9 * abs(2 * lnl)
     ctx.close()
+
+
+def test_tip_states_from_bytes_and_two_contexts_on_two_streams(epx, orc_ld):
+    """epx_set_tip_states_u8 == epx_set_tip_states; two contexts on their own streams, interleaved call by call, do not
+    disturb each other (independent instances are independent contexts)."""
+    pa, pb = W.make_config(2, N=50, L=200), W.make_config(1, N=12, L=90)
+    ta = pa.tip_states.copy(); ta[::4, ::3] = -1
+    pa = dataclasses.replace(pa, tip_states=ta)
+    a, b = epx.from_problem(pa), epx.from_problem(pb)
+    la0 = a.log_likelihood()
+    a.set_tip_states_u8(np.where(ta >= 0, ta, 255).astype(np.uint8))
+    a.enqueue_log_likelihood(); b.enqueue_log_likelihood()
+    a.enqueue_log_likelihood(); b.enqueue_log_likelihood()
+    la, lb = a.fetch_log_likelihood(), b.fetch_log_likelihood()
+    assert la == la0
+    ra, rb = orc_ld.evaluate(pa), orc_ld.evaluate(pb)
+    assert abs(np.longdouble(la) - ra["lnl"]) <= LNL_RTOL * abs(ra["lnl"])
+    assert abs(np.longdouble(lb) - rb["lnl"]) <= LNL_RTOL * abs(rb["lnl"])
+    a.close(); b.close()
