@@ -23,7 +23,9 @@
  *     memory.  `dev_workspace` must stay alive and untouched while the ctx is bound to it.
  *   - A ctx is not thread-safe; distinct ctxs are independent.
  *   - Nothing is cached between compute calls: every epx_update_matrices / epx_*log_likelihood call re-runs
- *     all of its steps on the device.  Setters only re-upload the array they set.
+ *     all of its steps on the device.  Setters only re-upload the array they set.  The one exception is asked for by
+ *     name: epx_log_likelihood_incremental reuses the matrices and partials of the previous evaluation that a node move
+ *     cannot have changed.
  */
 #ifndef EPX_H
 #define EPX_H
