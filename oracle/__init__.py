@@ -109,7 +109,9 @@ class Oracle:
 
     # ---- O5 + O6
     def log_likelihood(self, parent, P, tip_states, root_freqs, cat_weights, pattern_weights=None,
-                       want_partials: bool = False):
+                       want_partials: bool = False, tip_partials=None):
+        """`tip_partials`: {tip index: array [L][K]} -- tip vectors of partially observed tips, used
+        instead of the indicator of the tip's state."""
         parent = np.ascontiguousarray(parent, dtype=np.int32)
         P = np.ascontiguousarray(P, dtype=self.real)
         tips = np.ascontiguousarray(tip_states, dtype=np.int32)
@@ -122,9 +124,17 @@ class Oracle:
         site = np.zeros(L, dtype=self.real)
         lnl = np.zeros(1, dtype=self.real)
         partials = np.zeros((n_nodes, C, L, K), dtype=self.real) if want_partials else None
-        rc = self.lib.orc_log_likelihood(K, C, N, L, _p(parent), _p(P), _p(tips), _p(root_freqs), _p(cat_weights),
-                                         None if wt is None else _p(wt), _p(site), _p(lnl),
-                                         None if partials is None else _p(partials))
+        tp = has = None
+        if tip_partials:
+            tp = np.zeros((N, L, K), dtype=np.float64)
+            has = np.zeros(N, dtype=np.uint8)
+            for t, v in tip_partials.items():
+                tp[t] = np.asarray(v, dtype=np.float64).reshape(L, K)
+                has[t] = 1
+        rc = self.lib.orc_log_likelihood_tp(K, C, N, L, _p(parent), _p(P), _p(tips), _p(root_freqs), _p(cat_weights),
+                                            None if wt is None else _p(wt), _p(site), _p(lnl),
+                                            None if partials is None else _p(partials),
+                                            None if tp is None else _p(tp), None if has is None else _p(has))
         if rc != 0:
             raise RuntimeError(f"orc_log_likelihood rc={rc}")
         return {"lnl": lnl[0], "site_lnl": site, "partials": partials}
@@ -141,7 +151,7 @@ class Oracle:
         return int(self.lib.orc_validate_tree((parent.shape[0] + 1) // 2, _p(parent), _p(height)))
 
     # ---- whole path on a problem object (duck-typed: tau, Q, rates, parent, height, ...)
-    def evaluate(self, prob, want_partials: bool = False, branches=None):
+    def evaluate(self, prob, want_partials: bool = False, branches=None, tip_partials=None):
         """Run O2..O6 on a problem. `branches` (index array) restricts O3/O4 to a sample of matrix slots
         (branch-list problems / sampled parity); the likelihood is then skipped."""
         if prob.N > 0:
@@ -163,6 +173,6 @@ class Oracle:
             else:
                 rf = prob.freqs[self.epoch_of_parent_end(np.max(prob.height), prob.tau)]
             out.update(self.log_likelihood(prob.parent, P, prob.tip_states, rf, prob.weights,
-                                           prob.pattern_weights, want_partials))
+                                           prob.pattern_weights, want_partials, tip_partials))
             out["root_freqs"] = np.asarray(rf, dtype=np.float64)
         return out

@@ -213,13 +213,17 @@ typedef struct {
     const int *left, *right;     /* children, -1 for tips */
     const REAL *P;               /* [node][C][K][K], row = parent-end state */
     const int *tips;             /* [N][L] */
+    const double *tip_partials;  /* optional [N][L][K]: tip vectors of partially observed tips */
+    const unsigned char *tip_has;/* optional [N]: 1 = use tip_partials for this tip */
     REAL *partials;              /* optional [node][C][L][K] */
 } prune_ctx;
 
 static void partial(const prune_ctx *x, int node, int p, int c, REAL *out)
 {
     int K = x->K;
-    if (x->left[node] < 0) {                                             /* tip: 0/1 indicator, all-ones if missing (L72) */
+    if (x->left[node] < 0 && x->tip_has && x->tip_has[node]) {           /* partially observed tip: its given vector (L72) */
+        for (int i = 0; i < K; i++) out[i] = (REAL)x->tip_partials[((size_t)node * x->L + p) * K + i];
+    } else if (x->left[node] < 0) {                                      /* tip: 0/1 indicator, all-ones if missing (L72) */
         int s = x->tips[(size_t)node * x->L + p];
         for (int i = 0; i < K; i++) out[i] = (s >= 0 && s < K) ? (i == s ? 1 : 0) : 1;
     } else {
@@ -244,9 +248,25 @@ static void partial(const prune_ctx *x, int node, int p, int c, REAL *out)
 /* ---------------------------------------------------------------- O6: root, sites, categories (L72) */
 /* site_lnl[p] = ln sum_c w_c sum_i pi_i L_root,c,p(i);  *lnl = sum_p wt_p site_lnl[p]  (Kahan-summed).
  * Returns 0, -2 for a malformed tree, -3 if some site likelihood is not a positive normal number. */
+int orc_log_likelihood_tp(int K, int C, int N, int L, const int *parent, const REAL *P, const int *tips,
+                          const double *root_freqs, const double *cat_weights, const double *pattern_wt,
+                          REAL *site_lnl, REAL *lnl, REAL *partials, const double *tip_partials,
+                          const unsigned char *tip_has);
+
 int orc_log_likelihood(int K, int C, int N, int L, const int *parent, const REAL *P, const int *tips,
                        const double *root_freqs, const double *cat_weights, const double *pattern_wt,
                        REAL *site_lnl, REAL *lnl, REAL *partials)
+{
+    return orc_log_likelihood_tp(K, C, N, L, parent, P, tips, root_freqs, cat_weights, pattern_wt, site_lnl, lnl, partials,
+                                 NULL, NULL);
+}
+
+/* The same with tip vectors for some tips: tip_has[t] = 1 => tip t's partial likelihoods are tip_partials[t][p][0..K-1]
+ * ("0 or 1 depending on whether trait i is (partially) observed") instead of the indicator of its state. */
+int orc_log_likelihood_tp(int K, int C, int N, int L, const int *parent, const REAL *P, const int *tips,
+                          const double *root_freqs, const double *cat_weights, const double *pattern_wt,
+                          REAL *site_lnl, REAL *lnl, REAL *partials, const double *tip_partials,
+                          const unsigned char *tip_has)
 {
     int n_nodes = 2 * N - 1, root = -1;
     int *left = malloc(sizeof(int) * n_nodes), *right = malloc(sizeof(int) * n_nodes);
@@ -261,7 +281,7 @@ int orc_log_likelihood(int K, int C, int N, int L, const int *parent, const REAL
     for (int i = N; i < n_nodes && ok; i++) if (left[i] < 0 || right[i] < 0) ok = 0;
     if (!ok || root < 0) { free(left); free(right); return -2; }
 
-    prune_ctx x = { K, C, N, L, left, right, P, tips, partials };
+    prune_ctx x = { K, C, N, L, left, right, P, tips, tip_partials, tip_has, partials };
     int bad = 0;
 #pragma omp parallel for schedule(dynamic, 8)
     for (int p = 0; p < L; p++) {
