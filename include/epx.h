@@ -84,6 +84,14 @@ int epx_set_tip_states(epx_ctx* ctx, const int32_t* states);
 /* The same from bytes ([N][L] row-major; 0..K-1 = observed state, anything else, e.g. 255, = missing): a quarter of the
  * host memory traffic of the int32 form -- sequence data are bytes to begin with. */
 int epx_set_tip_states_u8(epx_ctx* ctx, const uint8_t* states);
+/* Partially observed tips (tip vectors are "0 or 1 depending on whether trait i is (partially) observed").
+ * epx_reserve_tip_partials: how many tips may carry a vector at the same time (each costs one block of partials,
+ * C*L*K doubles, in the workspace); call before epx_workspace_bytes / epx_bind.  Default 0.
+ * epx_set_tip_partials: tip `tip` is described by partials[L][K] (>= 0, finite: 0/1 for an ambiguity set, any weights in
+ * general) instead of its state; NULL returns it to its state from epx_set_tip_states.  The same vector serves every
+ * rate category. */
+int epx_reserve_tip_partials(epx_ctx* ctx, int max_tips);
+int epx_set_tip_partials(epx_ctx* ctx, int tip, const double* partials);
 /* wt: L pattern weights (a weight w == the pattern repeated w times), or NULL = all 1. */
 int epx_set_pattern_weights(epx_ctx* ctx, const double* wt);
 /* freqs: K root distribution, or NULL = the freqs of the epoch that contains the root height (A9). */

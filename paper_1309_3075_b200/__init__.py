@@ -57,6 +57,8 @@ def lib():
     _sig(L, "epx_set_tip_states", i, vp, ip)
     _sig(L, "epx_set_tip_states_u8", i, vp, ip)
     _sig(L, "epx_set_pattern_weights", i, vp, dp)
+    _sig(L, "epx_reserve_tip_partials", i, vp, i)
+    _sig(L, "epx_set_tip_partials", i, vp, i, dp)
     _sig(L, "epx_set_root_frequencies", i, vp, dp)
     _sig(L, "epx_set_branches", i, vp, i, dp, dp)
     _sig(L, "epx_set_branch_rates", i, vp, dp)
@@ -186,6 +188,14 @@ class Epx:
         states = np.ascontiguousarray(states, dtype=np.uint8)
         assert states.shape == (self.N, self.L)
         self._check(self._L.epx_set_tip_states_u8(self._ctx, _ptr(states)))
+
+    def reserve_tip_partials(self, max_tips: int) -> None:
+        self._check(self._L.epx_reserve_tip_partials(self._ctx, int(max_tips)))
+
+    def set_tip_partials(self, tip: int, partials) -> None:
+        partials = None if partials is None else _f64(partials)
+        assert partials is None or partials.shape == (self.L, self.K)
+        self._check(self._L.epx_set_tip_partials(self._ctx, int(tip), _ptr(partials)))
 
     def set_pattern_weights(self, wt) -> None:
         wt = None if wt is None else _f64(wt)
@@ -331,9 +341,11 @@ def set_problem(ctx: Epx, prob, tip_states_u8=None) -> None:
         ctx.set_branches(prob.child_height, prob.parent_height)
 
 
-def from_problem(prob, device: int = 0, stream=None) -> Epx:
-    """Create, fill and bind a context for `prob`."""
+def from_problem(prob, device: int = 0, stream=None, tip_partials: int = 0) -> Epx:
+    """Create, fill and bind a context for `prob` (`tip_partials`: blocks to reserve for partially observed tips)."""
     ctx = Epx(prob.K, prob.M, prob.C, prob.N, prob.L if prob.N else 1, device)
+    if tip_partials:
+        ctx.reserve_tip_partials(tip_partials)
     if prob.N == 0:
         ctx.set_branches(prob.child_height, prob.parent_height)
     ctx.bind(stream)

@@ -83,8 +83,8 @@ size_t plan_workspace(const epx_ctx* c, char* base, DevBuffers* d)
     t.Efull = (double*)take(8 * M * C * K * K);
     t.P = (double*)take(8 * S * C * K * K);
     if (c->tree_mode) {
-        t.partials = (double*)take(8 * (N - 1) * C * L * K);
-        t.scale_exp = (int32_t*)take(4 * (N - 1) * L);
+        t.partials = (double*)take(8 * (N - 1 + (size_t)c->tip_cap) * C * L * K);
+        t.scale_exp = (int32_t*)take(4 * (N - 1 + (size_t)c->tip_cap) * L);
         t.site_lnl = (double*)take(8 * L);
         t.block_sums = (double*)take(8 * ((L + 255) / 256));
     }
@@ -103,6 +103,7 @@ size_t plan_workspace(const epx_ctx* c, char* base, DevBuffers* d)
 void drop_graphs(epx_ctx* c)
 {
     c->inc_valid = false;      // whatever invalidates the graphs also invalidates an incremental continuation
+    c->tipp_dirty = true;      // ... and may change the partials layout the tip blocks were written in
     if (c->graph_mat) { cudaGraphExecDestroy(c->graph_mat); c->graph_mat = nullptr; }
     if (c->graph_lik) { cudaGraphExecDestroy(c->graph_lik); c->graph_lik = nullptr; }
 }
@@ -147,6 +148,9 @@ int build_plan(epx_ctx* c)
     std::stable_sort(internal.begin(), internal.end(), [&](int a, int b) { return level[a] < level[b]; });
     c->node_pidx.assign(n, -1);
     for (size_t k = 0; k < internal.size(); k++) c->node_pidx[internal[k]] = (int)k;
+    if (c->tip_slot.empty()) c->tip_slot.assign(N, -1);
+    for (int t = 0; t < N; t++)
+        if (c->tip_slot[t] >= 0) c->node_pidx[t] = (N - 1) + c->tip_slot[t];      // its block of 0/1 (or weighted) partials
     c->ops.resize(internal.size());
     c->level_off.assign(max_level + 1, 0);
     for (size_t k = 0; k < internal.size(); k++) {
@@ -157,7 +161,7 @@ int build_plan(epx_ctx* c)
         op.child[0] = left[u];
         op.child[1] = right[u];
         for (int h = 0; h < 2; h++) {
-            op.child_is_tip[h] = op.child[h] < N;
+            op.child_is_tip[h] = op.child[h] < N && c->tip_slot[op.child[h]] < 0;
             op.cpidx[h] = c->node_pidx[op.child[h]];
         }
         c->level_off[level[u]]++;      // count per level (levels 1..max_level)
@@ -209,7 +213,8 @@ int build_plan(epx_ctx* c)
     }
     const bool has_top = !(cuts.size() == 1 && cuts[0] == root);
     // kind of a child as seen from the piece being walked: 0 tip, 1 internal (walk into it), 2 root of a bottom piece
-    auto kind = [&](int v, bool top) { return left[v] < 0 ? 0 : (top && is_cut[v]) ? 2 : 1; };
+    // (a tip with a partial vector is read from HBM like the root of another piece)
+    auto kind = [&](int v, bool top) { return left[v] < 0 ? (c->tip_slot[v] >= 0 ? 2 : 0) : (top && is_cut[v]) ? 2 : 1; };
     for (int pass = 0; pass < 2; pass++) {     // need[] below the cuts, then above them
         for (int k = n - 1; k >= 0; k--) {
             int u = order[k];
@@ -599,6 +604,51 @@ static int set_tips_impl(epx_ctx* c, const T* states)
 
 int epx_set_tip_states(epx_ctx* c, const int32_t* states) { return set_tips_impl(c, states); }
 int epx_set_tip_states_u8(epx_ctx* c, const uint8_t* states) { return set_tips_impl(c, states); }
+
+int epx_reserve_tip_partials(epx_ctx* c, int max_tips)
+{
+    if (!c || max_tips < 0) return EPX_E_ARG;
+    if (!c->tree_mode) return fail(c, EPX_E_STATE, "ctx is in branch-list mode");
+    if (c->bound) return fail(c, EPX_E_STATE, "epx_reserve_tip_partials must precede epx_bind");
+    if (max_tips > c->N) max_tips = c->N;
+    c->tip_cap = max_tips;
+    c->tip_slot.assign(c->N, -1);
+    c->tip_part.assign((size_t)max_tips * c->L * c->K, 0.0);
+    c->slot_free.clear();
+    for (int s = max_tips - 1; s >= 0; s--) c->slot_free.push_back(s);
+    return EPX_OK;
+}
+
+int epx_set_tip_partials(epx_ctx* c, int tip, const double* partials)
+{
+    if (!c) return EPX_E_ARG;
+    if (!c->tree_mode) return fail(c, EPX_E_STATE, "ctx is in branch-list mode");
+    if (tip < 0 || tip >= c->N) return fail(c, EPX_E_ARG, "tip %d out of range", tip);
+    if (c->tip_slot.empty()) c->tip_slot.assign(c->N, -1);
+    const size_t LK = (size_t)c->L * c->K;
+    int slot = c->tip_slot[tip];
+    if (!partials) {                                    // back to the tip's state
+        if (slot < 0) return EPX_OK;
+        c->slot_free.push_back(slot);
+        c->tip_slot[tip] = -1;
+    } else {
+        for (size_t i = 0; i < LK; i++)
+            if (!(partials[i] >= 0) || !std::isfinite(partials[i])) return fail(c, EPX_E_ARG, "tip partial %zu must be finite and >= 0", i);
+        if (slot < 0) {
+            if (c->slot_free.empty()) return fail(c, EPX_E_STATE, "no tip-partial block left: epx_reserve_tip_partials(%d)", c->tip_cap);
+            slot = c->slot_free.back(); c->slot_free.pop_back();
+            c->tip_slot[tip] = slot;
+        } else {
+            std::copy(partials, partials + LK, c->tip_part.begin() + (size_t)slot * LK);
+            c->tipp_dirty = true; c->inc_valid = false;
+            return EPX_OK;                              // same plan, new values
+        }
+        std::copy(partials, partials + LK, c->tip_part.begin() + (size_t)slot * LK);
+    }
+    drop_graphs(c);                                     // the plans change: this tip is now read as a vector / as a state
+    if (c->has_tree) { int rc = build_plan(c); if (rc) return rc; c->tree_dirty = true; }
+    return EPX_OK;
+}
 
 int epx_set_pattern_weights(epx_ctx* c, const double* wt)
 {

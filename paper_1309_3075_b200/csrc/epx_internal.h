@@ -136,6 +136,13 @@ struct epx_ctx {
     std::vector<int> dirty_nodes;
     bool inc_valid = false, heights_dirty = false;
     bool last_status_ok = false;        // device status word of the last fetched evaluation was 0
+    // f3: tips with a partial-likelihood vector instead of a state (partially observed).  Such a tip gets a
+    // block in the partials array (index N-1 + slot, exponents 0) and enters the pruning plans like an internal child.
+    int tip_cap = 0;                    // blocks reserved by epx_reserve_tip_partials (before epx_bind)
+    std::vector<int> tip_slot;          // [N] slot of a tip, -1 = plain state
+    std::vector<double> tip_part;       // [tip_cap][L][K] host copies
+    std::vector<int> slot_free;         // free slots
+    bool tipp_dirty = false;
     const int32_t* sub_list = nullptr;  // when set, the chain launchers recompute only these slots ...
     int sub_count = 0;                  // ... this many
     std::vector<DfsOp> dfs_ops;        // depth-first post-order walk with its stack-slot allocation

@@ -293,3 +293,55 @@ def test_tip_states_from_bytes_and_two_contexts_on_two_streams(epx, orc_ld):
     assert abs(np.longdouble(la) - ra["lnl"]) <= LNL_RTOL * abs(ra["lnl"])
     assert abs(np.longdouble(lb) - rb["lnl"]) <= LNL_RTOL * abs(rb["lnl"])
     a.close(); b.close()
+
+
+@pytest.mark.parametrize("cid,kw,opts", [(2, {"N": 60, "L": 203}, ()), (2, {"N": 60, "L": 203}, ((3, 2),)), (2, {"N": 60, "L": 203}, ((3, 3),)),
+                                         (2, {"N": 60, "L": 203}, ((3, 1), (1, 1))), (3, {"N": 9, "L": 40}, ()), (4, {"N": 40, "L": 3}, ())])
+def test_partially_observed_tips(epx, orc_ld, cid, kw, opts):
+    """f3: tips given as vectors -- ambiguity sets (0/1) and general weights -- on every pruning kernel."""
+    rng = np.random.default_rng(90 + cid)
+    prob = W.make_config(cid, **kw)
+    K, L = prob.K, prob.L
+    ctx = epx.from_problem(prob, tip_partials=4)
+    for o, v in opts:
+        ctx.set_option(o, v)
+    tp = {}
+    for t in (0, 3, 7):                                 # ambiguity sets of 2..K states, different per pattern
+        v = (rng.random((L, K)) < 0.5).astype(np.float64)
+        v[np.arange(L), rng.integers(0, K, L)] = 1.0    # never empty
+        tp[t] = v
+    tp[5] = rng.uniform(0.0, 1.0, (L, K))               # general weights
+    for t, v in tp.items():
+        ctx.set_tip_partials(t, v)
+    with pytest.raises(epx.EpxError):
+        ctx.set_tip_partials(6, np.ones((L, K)))         # only 4 blocks were reserved
+    lnl = ctx.log_likelihood()
+    ref = orc_ld.evaluate(prob, tip_partials=tp, want_partials=True)
+    assert abs(np.longdouble(lnl) - ref["lnl"]) <= LNL_RTOL * abs(ref["lnl"])
+    site = ctx.get_site_log_likelihoods()
+    assert np.max(np.abs(site.astype(np.longdouble) - ref["site_lnl"]) / np.abs(ref["site_lnl"])) <= LNL_RTOL
+    out, ex = ctx.get_partials(prob.n_nodes - 1)
+    got = np.ldexp(out.astype(np.longdouble), ex[None, :, None])
+    want = ref["partials"][prob.n_nodes - 1]
+    assert np.max(np.abs(got - want) / np.max(want, axis=(0, 2), keepdims=True)) <= 1e-10
+    o5, e5 = ctx.get_partials(5)
+    assert np.array_equal(o5[0], tp[5]) and not e5.any()
+    assert ctx.status() == 0
+    # clear one, change another: a different plan, new values
+    ctx.set_tip_partials(3, None)
+    tp.pop(3)
+    tp[0] = np.ones((L, K))                             # all ones == missing
+    ctx.set_tip_partials(0, tp[0])
+    lnl2 = ctx.log_likelihood()
+    ref2 = orc_ld.evaluate(prob, tip_partials=tp)
+    assert abs(np.longdouble(lnl2) - ref2["lnl"]) <= LNL_RTOL * abs(ref2["lnl"])
+    t = prob.tip_states.copy(); t[0, :] = -1
+    ref3 = orc_ld.evaluate(dataclasses.replace(prob, tip_states=t), tip_partials={k: v for k, v in tp.items() if k != 0})
+    assert abs(ref2["lnl"] - ref3["lnl"]) <= 1e-15 * abs(ref3["lnl"])
+    # an incremental move on top of it
+    nodes, new_h, h = _move_nodes(np.random.default_rng(5), prob, 2)
+    ctx.set_node_heights(nodes, new_h)
+    lnl3 = ctx.log_likelihood_incremental()
+    ref4 = orc_ld.evaluate(dataclasses.replace(prob, height=h), tip_partials=tp)
+    assert abs(np.longdouble(lnl3) - ref4["lnl"]) <= LNL_RTOL * abs(ref4["lnl"])
+    ctx.close()
