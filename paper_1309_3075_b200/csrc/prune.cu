@@ -828,16 +828,31 @@ __global__ void __launch_bounds__(MT) prune64_cluster_kernel(const PruneOp* __re
         if (ch) __syncthreads();                       // everyone is done with the first child's operands
         if (op.child_is_tip[ch])
             for (int p = tid; p < M_TP; p += MT) st[p] = p < np ? tips[(size_t)op.child[ch] * Lp + p0 + p] : 255;
+        // all global loads of the staging are issued before the first shared-memory store (one L2 round trip, not sixteen)
         const double* src = P + ((size_t)op.child[ch] * C + c) * KK;
-        for (int idx = tid; idx < 64 * 64; idx += MT) {
-            const int i = idx >> 6, j = idx & 63;
-            Pm[i * M_LD + j] = (i < K && j < K) ? src[i * K + j] : 0.0;
+        const double* cs = partials + (((size_t)op.cpidx[ch] * C + c) * L + p0) * K;
+        const bool internal = !op.child_is_tip[ch];
+        double tp[64 * 64 / MT], tv[M_TP * 64 / MT];
+#pragma unroll
+        for (int t = 0; t < 64 * 64 / MT; t++) {
+            const int idx = tid + t * MT, i = idx >> 6, j = idx & 63;
+            tp[t] = (i < K && j < K) ? src[i * K + j] : 0.0;
         }
-        if (!op.child_is_tip[ch]) {
-            const double* cs = partials + (((size_t)op.cpidx[ch] * C + c) * L + p0) * K;
-            for (int idx = tid; idx < M_TP * 64; idx += MT) {
-                const int p = idx >> 6, j = idx & 63;
-                V[p * M_LD + j] = (p < np && j < K) ? cs[p * K + j] : 0.0;
+#pragma unroll
+        for (int t = 0; t < M_TP * 64 / MT; t++) {
+            const int idx = tid + t * MT, p = idx >> 6, j = idx & 63;
+            tv[t] = (internal && p < np && j < K) ? cs[p * K + j] : 0.0;
+        }
+#pragma unroll
+        for (int t = 0; t < 64 * 64 / MT; t++) {
+            const int idx = tid + t * MT;
+            Pm[(idx >> 6) * M_LD + (idx & 63)] = tp[t];
+        }
+        if (internal) {
+#pragma unroll
+            for (int t = 0; t < M_TP * 64 / MT; t++) {
+                const int idx = tid + t * MT;
+                V[(idx >> 6) * M_LD + (idx & 63)] = tv[t];
             }
         }
         __syncthreads();
