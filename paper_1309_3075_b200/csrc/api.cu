@@ -86,7 +86,7 @@ size_t plan_workspace(const epx_ctx* c, char* base, DevBuffers* d)
         t.partials = (double*)take(8 * (N - 1 + (size_t)c->tip_cap) * C * L * K);
         t.scale_exp = (int32_t*)take(4 * (N - 1 + (size_t)c->tip_cap) * L);
         t.site_lnl = (double*)take(8 * L);
-        t.block_sums = (double*)take(8 * ((L + 255) / 256));
+        t.block_sums = (double*)take(8 * ((L + 7) / 8));
     }
     t.inc_slots = (int32_t*)take(4 * S);
     if (c->tree_mode) {
@@ -314,7 +314,7 @@ int epx_create(epx_ctx** out, int K, int M, int C, int N_tips, int L, int device
         c->Lp = (L + 31) & ~31;
         c->pattern_wt.assign(L, 1.0);
         c->wt_dirty = true;
-        c->reduce_blocks = (L + 255) / 256;
+        c->reduce_blocks = K > 8 ? (L + 7) / 8 : (L + 255) / 256;       // K > 8: one warp per pattern (root_site_warp_kernel)
     }
     if (M == 1) { c->has_tau = true; }
     *out = c;

@@ -1108,6 +1108,43 @@ __global__ void __launch_bounds__(256) root_site_kernel(int K, int C, int L, siz
     }
 }
 
+// K > 8: one warp per pattern, lanes over the states (coalesced reads of the root vectors), eight patterns per CTA.
+__global__ void __launch_bounds__(256) root_site_warp_kernel(int K, int C, int L, size_t sc, size_t sp, int root_pidx, int root_node,
+    const double* __restrict__ partials, const int32_t* __restrict__ scale_exp, const double* __restrict__ freqs,
+    const int32_t* __restrict__ e_hi, const double* __restrict__ root_freqs, const double* __restrict__ weights,
+    const double* __restrict__ pattern_wt, double* __restrict__ site_lnl, double* __restrict__ block_sums,
+    int32_t* __restrict__ status)
+{
+    __shared__ double red[8];
+    const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
+    const int p = blockIdx.x * 8 + w;
+    const double* rf = root_freqs ? root_freqs : freqs + (size_t)e_hi[root_node] * K;   // reading A9
+    double contrib = 0.0;
+    if (p < L) {
+        double site = 0.0;
+        for (int c = 0; c < C; c++) {               // per category: states in lane order, then a fixed butterfly
+            const double* v = partials + (size_t)root_pidx * C * L * K + c * sc + p * sp;
+            double s = 0.0;
+            for (int i = lane; i < K; i += 32) s = fma(rf[i], v[i], s);
+            for (int o = 16; o > 0; o >>= 1) s += __shfl_xor_sync(0xffffffffu, s, o);
+            site = fma(weights[c], s, site);
+        }
+        if (lane == 0) {
+            if (!(site > 0.0) || !(site < 1.7e308)) atomicOr(status, EPX_ST_BAD_SITE);
+            const double ln = log(site) + (double)scale_exp[(size_t)root_pidx * L + p] * 0.6931471805599453094;
+            site_lnl[p] = ln;
+            contrib = pattern_wt[p] * ln;
+        }
+    }
+    if (lane == 0) red[w] = contrib;
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        double t = 0.0;
+        for (int k = 0; k < 8; k++) t += red[k];
+        block_sums[blockIdx.x] = t;
+    }
+}
+
 __global__ void __launch_bounds__(256) final_sum_kernel(int n, const double* __restrict__ block_sums,
                                                         double* __restrict__ lnl)
 {
@@ -1354,6 +1391,11 @@ int launch_root_reduction(const epx_ctx* c, cudaStream_t s)
     const int root_pidx = c->node_pidx[c->root];
     size_t sc, sp;
     partial_strides(c, sc, sp);
+    if (c->K > 8)
+        root_site_warp_kernel<<<blocks, 256, 0, s>>>(c->K, c->C, c->L, sc, sp, root_pidx, c->root, d.partials, d.scale_exp, d.freqs,
+                                                     d.e_hi, c->has_root_freqs ? d.root_freqs : nullptr, d.weights,
+                                                     d.pattern_wt, d.site_lnl, d.block_sums, d.status);
+    else
     root_site_kernel<<<blocks, 256, 0, s>>>(c->K, c->C, c->L, sc, sp, root_pidx, c->root, d.partials, d.scale_exp, d.freqs,
                                             d.e_hi, c->has_root_freqs ? d.root_freqs : nullptr, d.weights,
                                             d.pattern_wt, d.site_lnl, d.block_sums, d.status);
