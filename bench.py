@@ -36,8 +36,9 @@ if ROOT not in sys.path:
 import workloads as W  # noqa: E402  (input generators only; shared with the oracle, holds no arithmetic of the method)
 
 # dram__bytes_read.sum + dram__bytes_write.sum of the pruning launches of one config-2 step, from the committed
-# `ncu --set full` capture (profiles/r1_prune4_dfs_ncu.md): 2550.7 + 22.8 MB (bottom pieces) + 3.8 + 31.8 MB (top piece)
-NCU_TRAFFIC_BYTES_PER_STEP = 2.6091e9
+# `ncu --set full` capture named here (re-captured whenever the pruning kernel changes; `--traffic` overrides it)
+NCU_TRAFFIC = {"bytes_per_step": 2.6091e9, "profile": "profiles/r1_prune4_dfs_ncu.md", "commit": "6984e86",
+               "kernel": "prune4_dfs_kernel<4, 2> + <4, 1>"}
 
 METRIC = "pruning partials GB/s (fp64) over the whole a1..a6 log-likelihood step; epoch branch matrices/s in `matrices`"
 UNIT = "GB/s"
@@ -62,6 +63,58 @@ def pruning_bytes(prob) -> dict:
     a6 = part + 4 * L + 8 * L + 8 * L
     flops = n_int * C * L * (4 * K * K + K)
     return {"a5": a5, "a6": a6, "flops": flops}
+
+
+def compulsory_bytes(prob) -> dict:
+    """HBM bytes the depth-first pruning has to move: every internal node's partials [C][L][K] f64 and
+    scale exponents [L] i32 are WRITTEN once (they are outputs: epx_get_partials, the incremental path) and never read back
+    -- a child's vector is handed to its parent in registers / shared memory --; every tip state is read once (1 B per tip
+    and pattern); the two children's C K x K matrices once per node.  a6 as in pruning_bytes()."""
+    K, C, L, N = prob.K, prob.C, prob.L, prob.N
+    part = C * L * K * 8
+    n_int = N - 1
+    a5 = n_int * (part + 4 * L + 2 * C * K * K * 8) + N * L
+    a6 = part + 4 * L + 8 * L + 8 * L
+    return {"a5": a5, "a6": a6}
+
+
+def tree_levels(parent, N: int) -> int:
+    """Post-order levels of the tree (host integer work on the input; a workload property for `config`)."""
+    par = np.asarray(parent)
+    n = par.shape[0]
+    kids = [[] for _ in range(n)]
+    root = -1
+    for v in range(n):
+        if par[v] >= 0:
+            kids[par[v]].append(v)
+        else:
+            root = v
+    level = np.zeros(n, dtype=np.int64)
+    order, stack = [], [root]
+    while stack:
+        u = stack.pop()
+        order.append(u)
+        stack.extend(kids[u])
+    for u in reversed(order):
+        if kids[u]:
+            level[u] = 1 + max(level[k] for k in kids[u])
+    return int(level.max())
+
+
+def workload_config(prob, cid: int, world: int) -> dict:
+    """`config` of the JSON line: the workload and how the timing treats L2 -- identical for both arms."""
+    cfg = {"workload": W.CONFIG_NAMES[cid], "K": prob.K, "M": prob.M, "C": prob.C, "seed": W.config_seed(cid),
+           "parallelism": f"replicas x{world} (no collective)"}
+    if prob.N:
+        part_gb = (prob.N - 1) * prob.C * prob.L * prob.K * 8 / 1e9
+        cfg.update({"N_tips": prob.N, "L": prob.L, "tree_levels": tree_levels(prob.parent, prob.N),
+                    "l2": f"inputs larger than L2: {part_gb:.2f} GB of partials rewritten every step vs 126 MB L2"
+                          if part_gb > 0.126 else f"working set {part_gb * 1e3:.1f} MB of partials fits the 126 MB L2 (latency-bound "
+                                                "configuration; no flush, steps run back to back)"})
+    else:
+        p_gb = prob.n_br * prob.C * prob.K * prob.K * 8 / 1e9
+        cfg.update({"n_br": prob.n_br, "l2": f"inputs larger than L2: {p_gb:.2f} GB of P written per step vs 126 MB L2"})
+    return cfg
 
 
 def chain_flops(K: int, C: int, n_seg: np.ndarray) -> dict:
@@ -162,7 +215,7 @@ def time_oracle(prob, target_s: float, steps: int = 1, warmup: int = 0):
         t0 = time.perf_counter()
         out = orc.evaluate(sample)
         times.append(time.perf_counter() - t0)
-    nbytes = pruning_bytes(sample)
+    nbytes = compulsory_bytes(sample)
     sec = float(np.mean(times))
     return {"value": (nbytes["a5"] + nbytes["a6"]) / sec / 1e9, "unit": UNIT, "cores": cores, "kind": "oracle",
             "sample": f"first {L_s} of {prob.L} site patterns of config 2, full 2000-tip tree, all {prob.n_br} x {prob.C} "
@@ -174,14 +227,15 @@ def run_reference(args) -> None:
     if int(os.environ.get("RANK", "0")) != 0:
         return
     prob = W.make_config(2)
+    world = int(os.environ.get("WORLD_SIZE", "1"))
     # bounded: (steps + warmup) passes of ~target seconds each, the whole run within a few minutes
     target = min(10.0, 150.0 / max(1, args.steps + args.warmup))
     r = time_oracle(prob, target, steps=args.steps, warmup=args.warmup)
     line = {"impl": "reference", "metric": METRIC, "value": r["value"], "unit": UNIT, "n_gpus": args.gpus,
             "steps": args.steps, "warmup": args.warmup, "ms_per_step": r["seconds_per_step"] * 1e3,
             "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
-            "config": {"workload": W.CONFIG_NAMES[2], "K": prob.K, "M": prob.M, "C": prob.C, "N_tips": prob.N,
-                       "L": prob.L, "note": "CPU oracle on a bounded pattern sample; rank 0 only"},
+            "config": workload_config(prob, 2, world),
+            "note": "CPU oracle (long-double build, OpenMP) on a bounded pattern sample of the config; rank 0 only",
             "cpu_baseline": {k: r[k] for k in ("value", "unit", "cores", "kind", "sample")},
             "e2e": {"value": r["value"], "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
             "gpu_launches": 0}
@@ -225,6 +279,39 @@ def whole_job_value(unit_bytes: float, ms_step: float, world: int) -> float:
     return world * unit_bytes / (ms_step * 1e-3) / 1e9
 
 
+def taylor_chain_flops(prob) -> dict:
+    """Useful flops (K not padded, 2 K^3 per dense product) the componentwise-Taylor chain kernel executes for a tree-mode
+    codon problem (A21): per dense exponential 6 products (powers M^2..M^4, three Horner steps) + s squarings with
+    2^s >= r d max|q_ii|; a (slot, category) exponentiates its first and last segment, takes interior epochs from the
+    full-epoch table, and multiplies its n_seg factors together.  Host integer / scalar bookkeeping for the flop count."""
+    K, C, M = prob.K, prob.C, prob.M
+    ch, ph = prob.branch_heights()
+    tau = np.asarray(prob.tau)
+    e_lo = np.searchsorted(tau, ch, side="right")
+    e_hi = np.searchsorted(tau, ph, side="left")
+    nseg = np.where(ph > ch, e_hi - e_lo + 1, 0)
+    qmax = np.max(-np.diagonal(prob.Q, axis1=1, axis2=2), axis=1)          # max_i |q_ii| per epoch
+
+    def products(e, d):       # dense exponential of epoch e over duration d, per category
+        n = 0
+        for r in prob.rates:
+            mu = r * d * qmax[e]
+            n += 6 + (int(np.ceil(np.log2(mu))) if mu > 1.0 else 0)
+        return n
+
+    total = 0
+    for b in range(len(ch)):
+        n = int(nseg[b])
+        if n == 0:
+            continue
+        if n == 1:
+            total += products(e_hi[b], ph[b] - ch[b])
+        else:
+            total += products(e_hi[b], ph[b] - tau[e_hi[b] - 1]) + products(e_lo[b], tau[e_lo[b]] - ch[b]) + (n - 1) * C
+    table = sum(products(e, tau[e] - tau[e - 1]) for e in range(1, M - 1)) if M >= 3 else 0
+    return {"chain_products": int(total), "table_products": int(table), "flops": int(total + table) * 2 * K ** 3}
+
+
 def run_cuda(args) -> None:
     import torch
     import torch.distributed as dist
@@ -241,6 +328,7 @@ def run_cuda(args) -> None:
     if world > 1:
         dist.barrier()
     import paper_1309_3075_b200 as epx
+    legs = set(args.legs.split(","))
 
     def barrier():
         if world > 1:
@@ -249,9 +337,11 @@ def run_cuda(args) -> None:
 
     K, Wm = args.steps, max(3, args.warmup)
     prob = W.make_config(2)
-    nb = pruning_bytes(prob)
-    unit_bytes = nb["a5"] + nb["a6"]
+    comp, lvl = compulsory_bytes(prob), pruning_bytes(prob)
+    unit_bytes = comp["a5"] + comp["a6"]
     ctx = epx.from_problem(prob, device=local)
+    for opt, val in args.opt:
+        ctx.set_option(opt, val)
     ctx.set_option(epx.EPX_OPT_STAGE_EVENTS, 1)
     stream = ctx.stream
     lnl = None
@@ -281,69 +371,110 @@ def run_cuda(args) -> None:
 
     # (3) end to end through the C ABI with HOST buffers: every setter (host -> device copies) + log_likelihood
     #     (device -> host read of logL and the status word) inside the timed region
-    def e2e_step():
-        epx.set_problem(ctx, prob)
-        return ctx.log_likelihood()
-    Ke = max(3, min(K, 20))
-    for _ in range(2):
-        e2e_step()
-    barrier()
-    ms_e2e = bracket(torch, stream, e2e_step, Ke) / Ke
-    barrier()
-    ms_e2e = max_over_ranks(ms_e2e, world)
-    n_nodes = prob.n_nodes
-    # tip states as bytes (rows padded to 32), pattern weights, parent + height, the two pruning plans (32 B per node each),
-    # models, boundaries, category rates + weights, root frequencies
-    h2d = (prob.N * ((prob.L + 31) // 32 * 32) + 8 * prob.L + 4 * n_nodes + 8 * n_nodes + 64 * (prob.N - 1) + 8 * prob.M * prob.K * prob.K +
-           8 * prob.M * prob.K + 8 * (prob.M - 1) + 16 * prob.C + 8 * prob.K)
+    e2e = None
+    if "e2e" in legs:
+        def e2e_step():
+            epx.set_problem(ctx, prob)
+            return ctx.log_likelihood()
+        Ke = max(3, min(K, 20))
+        for _ in range(2):
+            e2e_step()
+        barrier()
+        ms_e2e = bracket(torch, stream, e2e_step, Ke) / Ke
+        barrier()
+        ms_e2e = max_over_ranks(ms_e2e, world)
+        n_nodes = prob.n_nodes
+        # tip states as bytes (rows padded to 32), pattern weights, parent + height, the two pruning plans (32 B per node
+        # each), models, boundaries, category rates + weights, root frequencies
+        h2d = (prob.N * ((prob.L + 31) // 32 * 32) + 8 * prob.L + 4 * n_nodes + 8 * n_nodes + 64 * (prob.N - 1) +
+               8 * prob.M * prob.K * prob.K + 8 * prob.M * prob.K + 8 * (prob.M - 1) + 16 * prob.C + 8 * prob.K)
+        e2e = {"value": whole_job_value(unit_bytes, ms_e2e, world), "unit": UNIT, "h2d_bytes_per_step": h2d,
+               "d2h_bytes_per_step": 12, "ms_per_step": ms_e2e, "steps": Ke,
+               "what": "all epx_set_* calls from host arrays + epx_log_likelihood (syncs, reads logL + status)"}
     # (4) SURVEY.md 8(f) f1, reported beside the headline: one MCMC-style move (one random internal node slides between its
     #     children and its parent) followed by an incremental re-evaluation, host call to host result
-    inc = bench_incremental(torch, epx, ctx, prob, stream)
+    inc = bench_incremental(torch, epx, ctx, prob, stream) if "incremental" in legs else None
     clk = clocks.stop()
-    levels = ctx.tree_levels()
+    plan = ctx.plan_info()
     ws_bytes = ctx.workspace_bytes()
     ctx.close()
 
     hbm_peak, peak_src = load_peaks()
     prune_ms = float(stage_ms[3])
     prune_launches = int(stage_launches[3])
-    roofline = {"bound": "hbm", "kernel": "prune4_dfs_kernel<4, 2> (a5; depth-first walk, bottom pieces + top piece)",
-                "achieved": nb["a5"] / (prune_ms * 1e-3) / 1e9, "peak": hbm_peak, "unit": "GB/s",
-                "frac": nb["a5"] / (prune_ms * 1e-3) / 1e9 / hbm_peak,
-                "traffic": args.traffic if args.traffic is not None else NCU_TRAFFIC_BYTES_PER_STEP / prune_launches,
-                "traffic_note": "dram__bytes_read+write per launch (sum over the step's launches / launches), "
-                                "profiles/r1_prune4_dfs_ncu.md; below the algorithmic bytes because child partials "
-                                "stay in registers / shared memory and are never re-read from HBM",
+    traffic_step = args.traffic * prune_launches if args.traffic is not None else NCU_TRAFFIC["bytes_per_step"]
+    gbs = lambda nbytes: nbytes / (prune_ms * 1e-3) / 1e9      # noqa: E731
+    roofline = {"bound": "hbm", "kernel": PRUNE_KERNEL_NAME + " (a5; depth-first walk, bottom pieces + top piece)",
+                # algorithmic bytes of the depth-first pruning = its compulsory HBM traffic: partials +
+                # exponents written once, tips and matrices read once; a physical rate, comparable with the copy peak
+                "achieved": gbs(comp["a5"]), "peak": hbm_peak, "unit": "GB/s", "frac": gbs(comp["a5"]) / hbm_peak,
+                "compulsory_bytes": comp["a5"],
+                "traffic": traffic_step / prune_launches,
+                "dram_gbs": gbs(traffic_step), "dram_frac": gbs(traffic_step) / hbm_peak,
+                "traffic_source": ("--traffic" if args.traffic is not None else
+                                   f"dram__bytes_read.sum + dram__bytes_write.sum per launch (step total / launches), "
+                                   f"{NCU_TRAFFIC['profile']} ({NCU_TRAFFIC['kernel']}, captured at commit {NCU_TRAFFIC['commit']})"),
+                # SURVEY.md 8(d)'s level-by-level byte model (every child block read back once by its parent): NOT a physical
+                # rate -- the walk never performs those reads -- kept for comparison with round 1 and with level kernels
+                "level_model_bytes": lvl["a5"], "level_model_gbs": gbs(lvl["a5"]), "level_model_frac": gbs(lvl["a5"]) / hbm_peak,
                 "peak_source": peak_src, "launches_per_step": prune_launches,
-                "algorithmic_bytes_per_launch": nb["a5"] / prune_launches,
+                "algorithmic_bytes_per_launch": comp["a5"] / prune_launches,
                 "avg_launch_ms": prune_ms / prune_launches, "share_of_step": prune_ms / float(stage_ms.sum()),
                 "stage_ms": {n: float(v) for n, v in zip(epx.STAGE_NAMES, stage_ms)}}
 
+    cfg = workload_config(prob, 2, world)
+    assert cfg["tree_levels"] == plan["levels"]
     line = {"metric": METRIC, "value": whole_job_value(unit_bytes, ms_step, world), "unit": UNIT, "n_gpus": world,
             "steps": K, "warmup": Wm, "ms_per_step": ms_step, "higher_is_better": True, "scaling": "weak",
-            "vs_baseline": None, "dtype": "f64", "data": "synthetic",
-            "config": {"workload": W.CONFIG_NAMES[2], "K": prob.K, "M": prob.M, "C": prob.C, "N_tips": prob.N,
-                       "L": prob.L, "tree_levels": levels, "parallelism": f"replicas x{world} (no collective)",
-                       "l2": f"inputs larger than L2: {ws_bytes / 1e9:.2f} GB workspace, 2.56 GB of partials rewritten "
-                             "every step vs 126 MB L2", "seed": W.config_seed(2)},
-            "roofline": roofline,
-            "e2e": {"value": whole_job_value(unit_bytes, ms_e2e, world), "unit": UNIT, "h2d_bytes_per_step": h2d,
-                    "d2h_bytes_per_step": 12, "ms_per_step": ms_e2e, "steps": Ke,
-                    "what": "all epx_set_* calls from host arrays + epx_log_likelihood (syncs, reads logL + status)"},
-            "gpu_launches": int(gpu_launches), "clocks": clk, "log_likelihood": lnl,
+            "vs_baseline": None, "dtype": "f64", "data": "synthetic", "config": cfg,
+            "value_definition": "compulsory HBM bytes of a5 + a6 (partials + exponents written once, tips / matrices read "
+                                "once; DESIGN.md section 5) x replicas / time of the WHOLE a1..a6 step",
+            "value_level_model": whole_job_value(lvl["a5"] + lvl["a6"], ms_step, world),
+            "workspace_bytes": ws_bytes, "plan": plan,
+            "roofline": roofline, "gpu_launches": int(gpu_launches), "clocks": clk, "log_likelihood": lnl,
             "matrices_per_s_cfg2": world * prob.n_br * prob.C / (float(stage_ms[:3].sum()) * 1e-3)}
-
-    line["incremental"] = inc
-    if rank == 0 and not args.no_matrices:
-        line["matrices"] = bench_matrices(torch, epx, local, K)
-    if rank == 0 and not args.no_cpu_baseline and world == 1:
+    if e2e is not None:
+        line["e2e"] = e2e
+    if inc is not None:
+        line["incremental"] = inc
+    peaks = None
+    if rank == 0 and ("matrices" in legs or "other" in legs):
+        peaks = {"dfma": epx.measure_fp64_peak(0, 200.0, local), "dmma": epx.measure_fp64_peak(1, 200.0, local)}
+    if rank == 0 and "matrices" in legs:
+        line["matrices"] = bench_matrices(torch, epx, local, K, peaks)
+    if rank == 0 and "other" in legs:
+        line["other_configs"] = bench_other_configs(torch, epx, local, K, peaks)
+    if rank == 0 and "cpu" in legs and world == 1:
         r = time_oracle(prob, 15.0)
         line["cpu_baseline"] = {k: r[k] for k in ("value", "unit", "cores", "kind", "sample")}
+        line["cpu_baseline"]["cfg1_single_thread_s"] = time_oracle_single_thread_cfg1()
     if world > 1:
         dist.barrier()
         dist.destroy_process_group()
     if rank == 0:
         print(json.dumps(line), flush=True)
+
+
+PRUNE_KERNEL_NAME = "prune4_dfs_kernel<4, 2>"
+
+
+def time_oracle_single_thread_cfg1() -> float:
+    """Seconds of one oracle evaluation of config 1 (16 tips, 500 patterns) on ONE host thread."""
+    import ctypes
+    import oracle
+    orc = oracle.Oracle("ld")
+    gomp = ctypes.CDLL("libgomp.so.1")
+    gomp.omp_get_max_threads.restype = ctypes.c_int
+    before = gomp.omp_get_max_threads()
+    gomp.omp_set_num_threads(1)
+    try:
+        prob = W.make_config(1)
+        orc.evaluate(prob)
+        t0 = time.perf_counter()
+        orc.evaluate(prob)
+        return time.perf_counter() - t0
+    finally:
+        gomp.omp_set_num_threads(before)
 
 
 def bench_incremental(torch, epx, ctx, prob, stream, moves: int = 64) -> dict:
@@ -383,17 +514,21 @@ def bench_incremental(torch, epx, ctx, prob, stream, moves: int = 64) -> dict:
             "kernel_launches_per_move": launches, "moves": moves}
 
 
-def bench_matrices(torch, epx, device: int, K: int) -> dict:
+def bench_matrices(torch, epx, device: int, K: int, peaks: dict, options=(), label: str = "") -> dict:
     """Second half of the metric: config 5 (61-state matrix-convolution microbenchmark, a1..a4 only)."""
     prob = W.make_config(5)
     nseg = n_segments(prob)
     fl = chain_flops(prob.K, prob.C, nseg)
     ctx = epx.from_problem(prob, device=device)
+    for opt, val in options:
+        ctx.set_option(opt, val)
     ctx.set_option(epx.EPX_OPT_STAGE_EVENTS, 1)
     steps = max(3, min(K, 10))
     for _ in range(3):
         ctx.update_matrices()
     assert ctx.status() == 0
+    clocks = ClockSampler(device)
+    clocks.start()
     n0 = ctx.launch_count()
     ms = bracket(torch, ctx.stream, ctx.update_matrices, steps) / steps
     launches = ctx.launch_count() - n0
@@ -403,16 +538,16 @@ def bench_matrices(torch, epx, device: int, K: int) -> dict:
         m, _ = ctx.get_stage_ms()
         stage += m
     stage /= steps
+    clk = clocks.stop()
     ctx.close()
-    dfma = epx.measure_fp64_peak(0, 200.0, device)
-    dmma = epx.measure_fp64_peak(1, 200.0, device)
+    dfma, dmma = peaks["dfma"], peaks["dmma"]
     chain_ms = float(stage[2])
     achieved = fl["executed"] / (chain_ms * 1e-3) / 1e12
     n_mat = prob.n_br * prob.C
     return {"metric": "epoch branch matrices/s (fp64)", "value": n_mat / (ms * 1e-3), "unit": "matrices/s",
-            "ms_per_step": ms, "steps": steps, "gpu_launches": int(launches),
-            "config": {"workload": W.CONFIG_NAMES[5], "K": prob.K, "M": prob.M, "C": prob.C, "n_br": prob.n_br,
-                       "segments": int(nseg.sum()), "l2": "2.38 GB of P written per step vs 126 MB L2"},
+            "ms_per_step": ms, "steps": steps, "gpu_launches": int(launches), "clocks": clk,
+            "config": dict(workload_config(prob, 5, 1), segments=int(nseg.sum())),
+            "whole_step_useful_tflops": fl["executed"] / (ms * 1e-3) / 1e12,
             "roofline": {"bound": "alu", "kernel": "chain_dmma64_kernel (a3+a4 fused, mma.sync m8n8k4 f64)",
                          "tensor_pipe_active_ncu": 0.795,   # sm__pipe_tensor_subpipe_dmma_cycles_active, profiles/r1_chain_dmma64_ncu.md
                          "achieved": achieved, "peak": dmma, "unit": "TFLOP/s", "frac": achieved / dmma,
@@ -424,17 +559,97 @@ def bench_matrices(torch, epx, device: int, K: int) -> dict:
                          "stage_ms": {n: float(v) for n, v in zip(epx.STAGE_NAMES, stage)}}}
 
 
+def bench_other_configs(torch, epx, device: int, K: int, peaks: dict) -> dict:
+    """Configs 1, 3 and 4 (BASELINE.json; PAPER.md:L224 names the shapes of 3 and 4): whole a1..a6 step on the device, per-stage
+    CUDA-event times, launches.  Config 3's pruning and chain kernels get an `alu` roofline against the fp64 peak measured
+    in this run; configs 1 and 4 are latency-bound: time, tree levels and the dependent-operation chain."""
+    out = {}
+    clocks = ClockSampler(device)
+    clocks.start()
+    for cid in (1, 3, 4):
+        prob = W.make_config(cid)
+        ctx = epx.from_problem(prob, device=device)
+        ctx.set_option(epx.EPX_OPT_STAGE_EVENTS, 1)
+        lnl = None
+        for _ in range(3):
+            lnl = ctx.log_likelihood()
+        assert ctx.status() == 0 and np.isfinite(lnl)
+        steps = max(5, min(K, 50))
+        n0 = ctx.launch_count()
+        ms = bracket(torch, ctx.stream, ctx.enqueue_log_likelihood, steps) / steps
+        launches = (ctx.launch_count() - n0) // steps
+        stage = np.zeros(5)
+        sl = None
+        for _ in range(steps):
+            ctx.enqueue_log_likelihood()
+            m, sl = ctx.get_stage_ms()
+            stage += m
+        stage /= steps
+        plan = ctx.plan_info()
+        ctx.close()
+        o = {"config": workload_config(prob, cid, 1), "ms_per_step": ms, "steps": steps, "gpu_launches_per_step": int(launches),
+             "log_likelihood": lnl, "stage_ms": {n: float(v) for n, v in zip(epx.STAGE_NAMES, stage)},
+             "stage_launches": {n: int(v) for n, v in zip(epx.STAGE_NAMES, sl)}, "plan": plan}
+        if cid == 3:
+            Kc, C, L, n_int = prob.K, prob.C, prob.L, prob.N - 1
+            pf = n_int * C * L * (4 * Kc * Kc + Kc)              # SURVEY.md 8(d): O(K^2 N C L) with both children counted
+            prune_ms, chain_ms = float(stage[3]), float(stage[2])
+            tf = taylor_chain_flops(prob)
+            o["roofline_prune"] = {"bound": "alu", "kernel": PRUNE64_KERNEL_NAME + " (a5, 61 states on the FP64 tensor pipe)",
+                                   "achieved": pf / (prune_ms * 1e-3) / 1e12, "peak": peaks["dmma"], "unit": "TFLOP/s",
+                                   "frac": pf / (prune_ms * 1e-3) / 1e12 / peaks["dmma"], "traffic": None, "flops": pf,
+                                   "flops_definition": "n_int C L (4 K^2 + K), K = 61 (tip children counted like internal ones)",
+                                   "peak_source": "DMMA m8n8k4 register-only loop measured in this run",
+                                   "launches": int(sl[3]), "avg_launch_ms": prune_ms / max(1, int(sl[3]))}
+            o["roofline_chain"] = {"bound": "alu", "kernel": "pade_chain_kernel<1> + pade_full_epoch_kernel<1> (a3+a4, "
+                                                             "componentwise Taylor exponentials, reading A21)",
+                                   "achieved": tf["flops"] / (chain_ms * 1e-3) / 1e12, "peak": peaks["dmma"], "unit": "TFLOP/s",
+                                   "frac": tf["flops"] / (chain_ms * 1e-3) / 1e12 / peaks["dmma"], "traffic": None,
+                                   "flops": tf["flops"], "dense_products": tf["chain_products"] + tf["table_products"],
+                                   "launches": int(sl[2])}
+        else:
+            o["bound"] = ("latency: %d dependent operations (largest subtree piece + top piece) of %d, %d tree levels"
+                          % (plan["largest_piece_ops"] + plan["top_piece_ops"], plan["operations"], plan["levels"])
+                          if plan["depth_first"] else "latency: %d tree levels, one launch each" % plan["levels"])
+            o["us_per_step"] = ms * 1e3
+        out[W.CONFIG_NAMES[cid]] = o
+    out["clocks"] = clocks.stop()
+    return out
+
+
+PRUNE64_KERNEL_NAME = "prune64_cluster_kernel"
+
+
+def parse_opts(text: str):
+    """--opt 3=1,6=2 -> [(3, 1), (6, 2)]: EPX_OPT_* overrides for the config-2 context (kernel comparisons, ncu captures)."""
+    out = []
+    for item in filter(None, text.split(",")):
+        k, v = item.split("=")
+        out.append((int(k), int(v)))
+    return out
+
+
 def main() -> None:
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
     ap.add_argument("--steps", type=int, default=100)
     ap.add_argument("--warmup", type=int, default=5)
     ap.add_argument("--impl", choices=["cuda", "reference"], default="cuda")
+    ap.add_argument("--legs", default="e2e,incremental,matrices,other,cpu",
+                    help="optional legs beside the config-2 headline + roofline: e2e, incremental, matrices (config 5), "
+                         "other (configs 1, 3, 4), cpu (oracle on the host cores)")
     ap.add_argument("--no-matrices", action="store_true", help="skip the config-5 matrices/s leg")
     ap.add_argument("--no-cpu-baseline", action="store_true", help="skip timing the oracle on the host cores")
+    ap.add_argument("--opt", type=parse_opts, default=[], help="EPX_OPT overrides for the config-2 context, e.g. 3=2,6=1")
     ap.add_argument("--traffic", type=float, default=None,
                     help="dram bytes per launch of the dominant kernel from the committed ncu capture (profiles/)")
     args = ap.parse_args()
+    legs = [x for x in args.legs.split(",") if x]
+    if args.no_matrices and "matrices" in legs:
+        legs.remove("matrices")
+    if args.no_cpu_baseline and "cpu" in legs:
+        legs.remove("cpu")
+    args.legs = ",".join(legs)
     if args.impl == "reference":
         if args.steps == 100 and args.warmup == 5:
             args.steps, args.warmup = 5, 1

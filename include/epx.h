@@ -94,7 +94,11 @@ int epx_reserve_tip_partials(epx_ctx* ctx, int max_tips);
 int epx_set_tip_partials(epx_ctx* ctx, int tip, const double* partials);
 /* wt: L pattern weights (a weight w == the pattern repeated w times), or NULL = all 1. */
 int epx_set_pattern_weights(epx_ctx* ctx, const double* wt);
-/* freqs: K root distribution, or NULL = the freqs of the epoch that contains the root height (A9). */
+/* freqs: K root distribution, or NULL (default) = the freqs of the root's epoch (A9).  The root's epoch follows the
+ * parent-end rule of a branch (A3): e = #{k : tau[k] < height[root]}.  A root exactly ON a boundary tau[k] therefore takes
+ * the YOUNGER epoch k (the process everything below it evolved under), although as a child end that height would open
+ * epoch k+1: the half-open intervals [tau[e-1], tau[e]) above describe child ends; parent ends (and the root) use
+ * (tau[e-1], tau[e]]. */
 int epx_set_root_frequencies(epx_ctx* ctx, const double* freqs);
 
 /* ---- branch-list mode ---- */
@@ -161,7 +165,8 @@ enum {
     EPX_STAGE_ROOT = 4,    /* a6 */
     EPX_N_STAGES = 5
 };
-/* With EPX_OPT_STAGE_EVENTS = 1 every compute call records a CUDA event on the stream before the first stage and
+/* With EPX_OPT_STAGE_EVENTS = 1 every compute call -- epx_log_likelihood_incremental included (its a2 stage is empty: the
+ * eigensystems are reused) -- records a CUDA event on the stream before the first stage and
  * after each stage (inside the CUDA graph when one is used).  This call synchronises the stream and writes the device
  * time of each stage of the LAST compute call to ms[EPX_N_STAGES] and the number of kernels each stage launched to
  * launches[EPX_N_STAGES] (either may be NULL).  Stages the call did not run report 0 ms / 0 launches.
@@ -198,8 +203,15 @@ int epx_set_option(epx_ctx* ctx, int option, int value);
 int epx_status(epx_ctx* ctx, int* status);
 /* Whole CSR segment list of the last compute call: seg_off[n_slots+1], epoch/dur with capacity `cap` entries. */
 int epx_get_all_segments(epx_ctx* ctx, int32_t* seg_off, int32_t* epoch, double* dur, int cap);
-/* Number of post-order levels of the tree (= pruning launches per likelihood call). */
+/* Number of post-order levels of the tree (= pruning launches per likelihood call of the level kernels). */
 int epx_tree_levels(const epx_ctx* ctx, int* n_levels);
+/* Shape of the pruning plan of the current tree (host integers; tree mode, after epx_set_tree; EPX_E_STATE otherwise):
+ * info[0] post-order levels; [1] pruning operations (internal nodes); [2] 1 if this ctx prunes with a depth-first walk
+ * (pieces of the tree walked by independent warps), 0 if level by level; [3] bottom pieces (independent subtrees, one
+ * launch); [4] operations of the largest bottom piece; [5] operations of the top piece (second launch; 0 = none);
+ * [6] stack slots a walk needs; [7] pruning kernel launches per full evaluation.  [4] + [5] is the dependent-operation
+ * chain that bounds the walk when there are few site patterns (PAPER.md L224 workload A, config 4). */
+int epx_plan_info(const epx_ctx* ctx, int32_t info[8]);
 
 #ifdef __cplusplus
 }

@@ -19,7 +19,10 @@
  * Pins (tests/test_oracle_pins.py): JC69 closed form, K-state equal-input multi-epoch closed form (fixes the
  * product ORDER), row sums, homogeneous collapse, redundant boundaries, scipy.linalg.expm, Taylor vs
  * uniformisation, detailed balance / stationarity, brute-force enumeration of ancestral states, two-tip
- * closed form, all-missing tips, pattern-weight and category invariances.  Nothing is "parity unpinned".
+ * closed form, all-missing tips, pattern-weight and category invariances; the root-epoch rule of reading A9
+ * (orc_epoch_of_parent_end) by hand-stated epochs -- inside an epoch, above the last boundary, exactly on a
+ * boundary -- and by two-tip likelihoods evaluated with the frequencies of the epoch named by hand.  Nothing is
+ * "parity unpinned".
  *
  * Height convention: time runs backwards from the most recent tip; epoch e (0 = most recent) covers heights
  * [tau[e-1], tau[e]) with tau[-1] = -inf and tau[M-1] = +inf; `tau` holds the M-1 finite boundaries.
@@ -87,7 +90,9 @@ int orc_segments(int n_br, const double *child_h, const double *parent_h, int M,
     return total;
 }
 
-/* epoch containing the root: #{k : tau_k < h_root}  (reading A9) */
+/* epoch containing the root: #{k : tau_k < h_root}  (reading A9: the parent-end rule of A3, so a root exactly on a
+ * boundary takes the YOUNGER epoch -- everything below it evolved under that process).  Pinned by
+ * tests/test_oracle_pins.py::test_root_epoch_selection_hand_stated and ::test_two_tip_likelihood_uses_the_root_epochs_frequencies. */
 int orc_epoch_of_parent_end(double h, int M, const double *tau)
 {
     int e = 0;

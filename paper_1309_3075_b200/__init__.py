@@ -76,6 +76,7 @@ def lib():
     _sig(L, "epx_get_site_log_likelihoods", i, vp, dp)
     _sig(L, "epx_launch_count", i, vp, ct.POINTER(ct.c_longlong))
     _sig(L, "epx_tree_levels", i, vp, ct.POINTER(i))
+    _sig(L, "epx_plan_info", i, vp, ip)
     _sig(L, "epx_get_stage_ms", i, vp, ct.c_void_p, ct.c_void_p)
     _sig(L, "epx_status", i, vp, ct.POINTER(i))
     _sig(L, "epx_set_option", i, vp, i, i)
@@ -314,6 +315,13 @@ class Epx:
         n = ct.c_int()
         self._check(self._L.epx_tree_levels(self._ctx, ct.byref(n)))
         return n.value
+
+    def plan_info(self) -> dict:
+        info = np.zeros(8, dtype=np.int32)
+        self._check(self._L.epx_plan_info(self._ctx, _ptr(info)))
+        keys = ("levels", "operations", "depth_first", "bottom_pieces", "largest_piece_ops", "top_piece_ops", "stack_slots",
+                "prune_launches")
+        return {k: int(v) for k, v in zip(keys, info)}
 
     def status(self) -> int:
         n = ct.c_int()

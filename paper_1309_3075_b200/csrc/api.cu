@@ -610,6 +610,8 @@ int epx_reserve_tip_partials(epx_ctx* c, int max_tips)
     if (!c || max_tips < 0) return EPX_E_ARG;
     if (!c->tree_mode) return fail(c, EPX_E_STATE, "ctx is in branch-list mode");
     if (c->bound) return fail(c, EPX_E_STATE, "epx_reserve_tip_partials must precede epx_bind");
+    for (int slot : c->tip_slot)
+        if (slot >= 0) return fail(c, EPX_E_STATE, "a tip still carries a vector: epx_set_tip_partials(tip, NULL) first");
     if (max_tips > c->N) max_tips = c->N;
     c->tip_cap = max_tips;
     c->tip_slot.assign(c->N, -1);

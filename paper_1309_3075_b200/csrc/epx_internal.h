@@ -135,7 +135,8 @@ struct epx_ctx {
     // holds a complete evaluation of the current inputs that an incremental call can build on
     std::vector<int> dirty_nodes;
     bool inc_valid = false, heights_dirty = false;
-    bool last_status_ok = false;        // device status word of the last fetched evaluation was 0
+    bool last_status_ok = false;        // device status word of the last evaluation was read and was 0
+    bool status_known = false;          // ... was read at all (an enqueue without a fetch leaves it unknown)
     // f3: tips with a partial-likelihood vector instead of a state (partially observed).  Such a tip gets a
     // block in the partials array (index N-1 + slot, exponents 0) and enters the pruning plans like an internal child.
     int tip_cap = 0;                    // blocks reserved by epx_reserve_tip_partials (before epx_bind)
@@ -207,6 +208,7 @@ int eigen_init_attributes();
 int prune_init_attributes();
 int prune_tile(int K, int C);   // patterns per CTA of the generic pruning kernel
 int dfs_tiles(const epx_ctx* c);         // warps per piece of the depth-first walk
+bool prune_uses_kdfs(const epx_ctx* c);  // K != 4 depth-first walk for few patterns (generic partials layout)
 bool prune_uses_dfs(const epx_ctx* c);   // K == 4 depth-first walk: partials are laid out [node][L][C][4]
 // element (category c, pattern p, state i) of a node's partials sits at c * sc + p * sp + i
 inline void partial_strides(const epx_ctx* c, size_t& sc, size_t& sp)

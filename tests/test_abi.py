@@ -133,3 +133,27 @@ def test_workspace_scales_with_problem(L):
     partials = 1999 * 4 * 10000 * 4 * 8
     assert partials < need < partials * 1.2          # the partials buffer dominates (cfg 2: 2.56 GB)
     a.close()
+
+
+def test_plan_info_and_tip_partial_reservation_state(L):
+    import paper_1309_3075_b200 as epx
+    import workloads as W
+    prob = W.make_config(2, N=33, L=40)
+    c = epx.Epx(prob.K, prob.M, prob.C, prob.N, prob.L)
+    with pytest.raises(epx.EpxError) as e:
+        c.plan_info()                                   # no tree yet
+    assert e.value.code == epx.EPX_E_STATE
+    c.set_tree(prob.parent, prob.height)
+    info = c.plan_info()
+    assert info["operations"] == prob.N - 1 and info["levels"] >= 6 and info["depth_first"] == 1
+    assert info["bottom_pieces"] >= 1 and info["stack_slots"] >= 1
+    assert info["largest_piece_ops"] + info["top_piece_ops"] <= prob.N - 1
+    # a second reservation while a tip still carries a vector would orphan its block: refused
+    c.reserve_tip_partials(2)
+    c.set_tip_partials(3, np.ones((prob.L, prob.K)))
+    with pytest.raises(epx.EpxError) as e:
+        c.reserve_tip_partials(4)
+    assert e.value.code == epx.EPX_E_STATE
+    c.set_tip_partials(3, None)
+    c.reserve_tip_partials(4)
+    c.close()

@@ -34,6 +34,44 @@ def test_config2_algorithmic_bytes_is_the_surveyed_5_2_GB():
     assert 5.1e9 < nb["a5"] + nb["a6"] < 5.4e9          # ~5.20 GB
 
 
+def test_compulsory_bytes_is_what_the_walk_has_to_move():
+    # every node's partials + exponents written once, every tip byte and every matrix read once;
+    # for config 2 that is the 2.56 GB of partials + 80 MB of exponents + 20 MB of tips + 2 MB of matrices
+    import bench
+    prob = W.make_config(2)
+    cb = bench.compulsory_bytes(prob)
+    assert cb["a5"] == 1999 * (4 * 10000 * 4 * 8 + 4 * 10000 + 2 * 4 * 16 * 8) + 2000 * 10000
+    assert 2.6e9 < cb["a5"] < 2.7e9
+    assert cb["a5"] < bench.pruning_bytes(prob)["a5"]            # the level model counts each child block a second time
+
+
+def test_workload_config_is_shared_by_both_arms():
+    import bench
+    prob = W.make_config(2, N=50, L=64)
+    cfg = bench.workload_config(prob, 2, 1)
+    assert cfg["workload"] == W.CONFIG_NAMES[2] and cfg["N_tips"] == 50 and cfg["L"] == 64 and "l2" in cfg
+    # post-order levels restated with the heights-free definition: longest tip-to-root path in edges
+    depth = 0
+    for t in range(prob.N):
+        d, v = 0, t
+        while prob.parent[v] >= 0:
+            v = prob.parent[v]; d += 1
+        depth = max(depth, d)
+    assert cfg["tree_levels"] == depth
+    assert bench.workload_config(W.make_config(5, n_br=10), 5, 2)["parallelism"].startswith("replicas x2")
+
+
+def test_taylor_chain_flop_count_small_case():
+    import bench
+    prob = W.make_config(3, N=4, L=2)
+    tf = bench.taylor_chain_flops(prob)
+    nseg = bench.n_segments(prob)
+    # at least 6 dense products per exponential, one or two exponentials per (slot, category), n_seg - 1 chain products
+    lo = sum((6 * min(int(n), 2) + int(n) - 1) * prob.C for n in nseg if n > 0)
+    assert tf["chain_products"] >= lo and tf["table_products"] >= 6 * prob.C * (prob.M - 2)
+    assert tf["flops"] == (tf["chain_products"] + tf["table_products"]) * 2 * 61 ** 3
+
+
 def test_segment_counts_and_chain_flops(orc_ld):
     import bench
     prob = W.make_config(5, n_br=500)
@@ -96,6 +134,8 @@ def test_reference_arm_prints_the_contract_line():
         assert key in d, key
     assert d["impl"] == "reference" and d["dtype"] == "f64" and d["vs_baseline"] is None and d["unit"] == "GB/s"
     assert d["config"]["workload"] == W.CONFIG_NAMES[2]
+    import bench
+    assert d["config"] == bench.workload_config(W.make_config(2), 2, 1)      # the CUDA arm prints the same dict
     assert d["cpu_baseline"]["kind"] == "oracle" and d["cpu_baseline"]["value"] == d["value"] and d["cpu_baseline"]["cores"] >= 1
     assert d["e2e"] == {"value": d["value"], "unit": d["unit"], "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0}
     assert d["value"] > 0

@@ -94,13 +94,17 @@ def test_config2_reduced(epx, orc_ld):
     # several pattern tiles plus a ragged tail (L = 777 = 3*256 + 9 = 97*8 + 1), 10 epochs, dated tips
     prob = W.make_config(2, N=150, L=777)
     run_tree(epx, orc_ld, prob)                                                  # depth-first walk (default)
+    # the instantiations bench.py times at full size (C = 4; 2 patterns per lane is chosen there because L >= 4096): every
+    # node's partials against the oracle
+    for ppl in (1, 2, 4):
+        run_tree(epx, orc_ld, prob, options=[(epx.EPX_OPT_DFS_PPL, ppl)])
     run_tree(epx, orc_ld, prob, options=[(epx.EPX_OPT_PRUNE_KERNEL, 3)])         # depth-first walk, 4x4 products on the FP64 tensor pipe
     run_tree(epx, orc_ld, prob, options=[(epx.EPX_OPT_PRUNE_KERNEL, 3), (epx.EPX_OPT_DFS_PPL, 2)])
     run_tree(epx, orc_ld, prob, options=[(epx.EPX_OPT_PRUNE_KERNEL, 2)])         # level-by-level register kernel
     run_tree(epx, orc_ld, prob, options=[(epx.EPX_OPT_PRUNE_KERNEL, 1)])         # generic shared-memory kernel
 
 
-@pytest.mark.parametrize("C", [1, 2, 3, 5, 8])
+@pytest.mark.parametrize("C", [1, 2, 3, 4, 5, 6, 7, 8])
 def test_k4_every_category_count(epx, orc_ld, C):
     # lanes per pattern G = 1, 2, 4, 8, 8 with C < G idle lanes; missing tip states; ragged L
     import dataclasses
@@ -157,8 +161,29 @@ def test_k4_extreme_tree_shapes(epx, orc_ld, shape, N):
 
 def test_config2_full_size(epx, orc_ld):
     # the configuration bench.py times; the oracle's naive recursion takes ~1 min here
+    import dataclasses
     prob = W.make_config(2)
-    run_tree(epx, orc_ld, prob, partial_nodes=())   # oracle partials of every node would be 10 GB; reduced test covers them
+    run_tree(epx, orc_ld, prob, partial_nodes=())   # all 10 000 site log-likelihoods, every P entry, every segment
+    # Every node's partials in the launch configuration bench.py times, on sampled patterns the oracle computes one by one
+    # (its partials of all 10 000 patterns would be 10 GB): the first and last pattern tiles and a seeded spread.
+    rng = np.random.default_rng(22)
+    sample = np.unique(np.concatenate([np.arange(16), np.arange(prob.L - 17, prob.L), rng.choice(prob.L, 40, replace=False)]))
+    sub = dataclasses.replace(prob, L=int(sample.size), tip_states=np.ascontiguousarray(prob.tip_states[:, sample]),
+                              pattern_weights=np.ascontiguousarray(prob.pattern_weights[sample]))
+    ref = orc_ld.evaluate(sub, want_partials=True)
+    ctx = epx.from_problem(prob)
+    ctx.log_likelihood()
+    site = ctx.get_site_log_likelihoods()[sample]
+    assert np.max(np.abs(site.astype(np.longdouble) - ref["site_lnl"]) / np.abs(ref["site_lnl"])) <= LNL_RTOL
+    worst = 0.0
+    for node in range(prob.N, prob.n_nodes):
+        out, ex = ctx.get_partials(node)
+        got = np.ldexp(out[:, sample, :].astype(np.longdouble), ex[None, sample, None])
+        want = ref["partials"][node]
+        scale = np.max(want, axis=(0, 2), keepdims=True)
+        worst = max(worst, float(np.max(np.abs(got - want) / scale)))
+    assert worst <= PARTIAL_RTOL, worst
+    ctx.close()
 
 
 def test_config3_reduced(epx, orc_ld):
@@ -176,7 +201,13 @@ def test_config3_reduced(epx, orc_ld):
 def test_config3_full_size(epx, orc_ld):
     prob = W.make_config(3)
     run_tree(epx, orc_ld, prob, partial_nodes=[prob.N, prob.n_nodes - 1])
-    run_tree(epx, orc_ld, prob, options=[(epx.EPX_OPT_EXP_METHOD, 1)], partial_nodes=(), likelihood=False)
+    # Reading A21 as evidence: the spectral path (Jacobi eigensystem, eigenbasis chain) meets the 1e-12 ABSOLUTE bound on
+    # every P entry (checked by run_tree) and still misses the 1e-9 RELATIVE bound on the log-likelihood of this codon
+    # workload -- which is why tree-mode codon contexts default to the componentwise exponential.  If this assertion ever
+    # fails because the spectral logL became accurate, A21 and EPX_OPT_EXP_METHOD's default need revisiting.
+    lnl_spectral, ref = run_tree(epx, orc_ld, prob, options=[(epx.EPX_OPT_EXP_METHOD, 1)], partial_nodes=(), likelihood=False)
+    rel = float(abs(np.longdouble(lnl_spectral) - ref["lnl"]) / abs(ref["lnl"]))
+    assert LNL_RTOL < rel < 1e-4, rel
 
 
 def test_config4_reduced(epx, orc_ld):
@@ -210,7 +241,10 @@ def test_config5_full_size_sampled(epx, orc_ld):
     off = check_segments(ctx, {"seg_off": off_ref, "seg_epoch": ep_ref, "seg_dur": du_ref})
     nseg = np.diff(off)
     rng = np.random.default_rng(5)
-    sample = np.unique(np.concatenate([np.argsort(nseg)[-8:], np.argsort(nseg)[:4], rng.choice(prob.n_br, 48, replace=False)]))
+    # every 20th branch, the 8 longest and the 4 shortest chains, 48 random ones: > 1 000 of the 20 000 (Eq. 7 element-wise)
+    sample = np.unique(np.concatenate([np.arange(0, prob.n_br, 20), np.argsort(nseg)[-8:], np.argsort(nseg)[:4],
+                                       rng.choice(prob.n_br, 48, replace=False)]))
+    assert sample.size >= 1000
     ref = orc_ld.evaluate(prob, branches=sample)
     P = ctx.get_all_matrices()
     err = np.max(np.abs(P[sample].astype(np.longdouble) - ref["P"]))

@@ -185,6 +185,51 @@ def test_homogeneous_collapse_and_redundant_boundaries(orc_ld):
     assert np.max(np.abs(Pa.sum(-1) - 1)) < 1e-15 and Pa.min() >= 0     # Q's rows sum to 0 only to double rounding
 
 
+# ------------------------------------------------------------------ A9: which epoch's frequencies sit at the root
+
+def test_root_epoch_selection_hand_stated(orc_ld):
+    """Reading A9 (PAPER.md:L72 writes one pi in sum_i L_root(i) pi_i): the root takes the frequencies of the
+    epoch that holds its height by the parent-end rule of A3, e = #{k : tau_k < h_root} -- a root exactly ON a boundary
+    belongs to the YOUNGER epoch (everything below it evolved under that process; no branch enters the older one).
+    The expected epochs are written out by hand, not taken from the oracle."""
+    tau = np.array([0.3, 0.6, 0.9])                      # M = 4: epoch 0 = [.., 0.3), 1 = [0.3, 0.6), 2 = [0.6, 0.9), 3 = [0.9, ..)
+    hand = [(0.2, 0), (0.29999, 0), (0.45, 1), (0.75, 2), (1.5, 3), (0.95, 3),     # strictly inside an epoch
+            (0.3, 0), (0.6, 1), (0.9, 2),                                           # exactly on a boundary: the younger side
+            (np.nextafter(0.3, 1.0), 1), (np.nextafter(0.9, 2.0), 3), (-1.0, 0)]    # one ulp above a boundary; below every tip
+    for h, e in hand:
+        assert orc_ld.epoch_of_parent_end(h, tau) == e, (h, e)
+    assert orc_ld.epoch_of_parent_end(5.0, np.zeros(0)) == 0                       # M = 1: the only epoch
+
+
+@pytest.mark.parametrize("h_root,epoch", [(0.2, 0), (0.45, 1), (1.5, 3), (0.6, 1), (0.9, 2), (0.3, 0)])
+def test_two_tip_likelihood_uses_the_root_epochs_frequencies(orc_ld, h_root, epoch):
+    """Two tips under a root at a stated height, four epochs whose pi differ visibly:
+    l = sum_i pi^(e)_i P_v[i,x] P_w[i,y]  (Eq. 4 + L72) with the epoch e NAMED BY HAND.  The other epochs' frequencies give
+    a visibly different value, so a wrong comparison (<= for <) or counting from the wrong end fails here."""
+    K, M = 4, 4
+    tau = np.array([0.3, 0.6, 0.9])
+    F = np.array([[0.70, 0.10, 0.10, 0.10], [0.10, 0.70, 0.10, 0.10], [0.10, 0.10, 0.70, 0.10], [0.10, 0.10, 0.10, 0.70]])
+    Q = np.stack([models.hky(2.0 + e, F[e]) for e in range(M)])
+    parent = np.array([2, 2, -1], dtype=np.int32)
+    height = np.array([0.0, 0.05, h_root])
+    tips = np.array([[0, 1, 2, 3, 0, 2], [0, 1, 2, 3, 3, 1]], dtype=np.int32)
+    L = tips.shape[1]
+    prob = W.EpochProblem("root_epoch", K, M, 1, 2, L, tau, Q, F, True, np.ones(1), np.ones(1), parent=parent,
+                          height=height, tip_states=tips, pattern_weights=np.ones(L))
+    out = orc_ld.evaluate(prob)
+    Pv, Pw = out["P"][0, 0], out["P"][1, 0]              # the matrices themselves are pinned by the closed forms above
+
+    def site_lnl(pi):
+        return np.array([np.log(np.sum(pi.astype(LD) * Pv[:, tips[0, p]] * Pw[:, tips[1, p]])) for p in range(L)], dtype=LD)
+
+    want = site_lnl(F[epoch])
+    assert np.max(np.abs(out["site_lnl"] - want)) < 1e-17
+    assert abs(out["lnl"] - want.sum()) < 1e-16
+    for other in range(M):
+        if other != epoch:
+            assert np.max(np.abs(site_lnl(F[other]) - want)) > 1e-2      # the pin can tell the epochs apart
+
+
 # ------------------------------------------------------------------ O5+O6: pruning and aggregation
 
 def _brute_force_site_likelihood(parent, P, tips_col, root_freqs, K):
@@ -305,14 +350,6 @@ def test_pulley_principle_only_when_homogeneous(orc_ld):
     root = int(np.argmax(prob.height))
     kids = np.where(prob.parent == root)[0]
     lo = prob.height[kids].max()
-
-    def with_root_moved(p, Qs):
-        # re-hang: keep the path length between the two root children constant, move the root's position on it
-        h = p.height.copy()
-        total = (h[root] - h[kids[0]]) + (h[root] - h[kids[1]])
-        new_root_h = lo + 0.25 * (total - (lo - h[kids[0]]) - (lo - h[kids[1]])) / 2
-        # path lengths must be preserved => only possible by changing heights of one side; use branch-length view:
-        return new_root_h
 
     # branch-length formulation: evaluate with explicit matrices instead of heights
     Q = prob.Q[0]
