@@ -404,7 +404,7 @@ def run_cuda(args) -> None:
     prune_launches = int(stage_launches[3])
     traffic_step = args.traffic * prune_launches if args.traffic is not None else NCU_TRAFFIC["bytes_per_step"]
     gbs = lambda nbytes: nbytes / (prune_ms * 1e-3) / 1e9      # noqa: E731
-    roofline = {"bound": "hbm", "kernel": PRUNE_KERNEL_NAME + " (a5; depth-first walk, bottom pieces + top piece)",
+    roofline = {"bound": "hbm", "kernel": prune_kernel_name(args.opt, prob.L) + " (a5; depth-first walk, bottom pieces + top piece)",
                 # algorithmic bytes of the depth-first pruning = its compulsory HBM traffic: partials +
                 # exponents written once, tips and matrices read once; a physical rate, comparable with the copy peak
                 "achieved": gbs(comp["a5"]), "peak": hbm_peak, "unit": "GB/s", "frac": gbs(comp["a5"]) / hbm_peak,
@@ -455,7 +455,19 @@ def run_cuda(args) -> None:
         print(json.dumps(line), flush=True)
 
 
-PRUNE_KERNEL_NAME = "prune4_dfs_kernel<4, 2>"
+def prune_kernel_name(opts, L: int) -> str:
+    """Name of the K = 4 pruning kernel the config-2 context launches under the EPX_OPT overrides of --opt."""
+    o = dict(opts)
+    kernel, ppl = o.get(3, 0), o.get(6, 0)
+    if kernel == 5:
+        return "prune4_dfs_kernel<4, %d>" % (ppl or (2 if L >= 4096 else 1))
+    if kernel == 3:
+        return "prune4_mma_kernel<4>"
+    if kernel == 2:
+        return "prune4_kernel<4> (level by level)"
+    if kernel == 1:
+        return "prune_generic_kernel (level by level)"
+    return "prune4_lane_kernel<4, %d, false> + <4, 1, true>" % (ppl or 1)
 
 
 def time_oracle_single_thread_cfg1() -> float:

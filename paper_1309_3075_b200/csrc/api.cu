@@ -192,10 +192,15 @@ int build_plan(epx_ctx* c)
         const long tiles = dfs_tiles(c);
         // pieces wanted (< 8 = no cut): 4 x the number needed for 24 warps per SM; measured on config 2 (625 tiles):
         // 12 -> 0.69 ms, 24 -> 0.68 ms, 48 -> 0.70 ms, 64 -> 0.73 ms
-        const long want = std::min<long>(64, 4 * ((148L * 24 + tiles - 1) / tiles));
+        // lane-per-pattern walk (K == 4 default; ~10 one-warp CTAs per SM): ~5 000 warps in flight keep the store stream
+        // saturated; measured on config 2 (313 tiles): 8 -> 0.520 ms, 12 -> 0.486, 16 -> 0.483, 24 -> 0.485, 48 -> 0.501
+        const long auto_want = prune_uses_lane(c) ? std::min<long>(64, (5000 + tiles - 1) / tiles)
+                                                  : std::min<long>(64, 4 * ((148L * 24 + tiles - 1) / tiles));
+        const long want = c->dfs_want > 0 ? c->dfs_want : auto_want;
         std::vector<int> heap{root};          // max-heap on subtree size
         auto cmp = [&](int x, int y) { return size[x] < size[y]; };
-        while (want >= 8 && (long)heap.size() + (long)cuts.size() < want) {
+        const long min_cut = c->dfs_want > 0 ? 2 : 8;
+        while (want >= min_cut && (long)heap.size() + (long)cuts.size() < want) {
             std::pop_heap(heap.begin(), heap.end(), cmp);
             int u = heap.back(); heap.pop_back();
             if (size[u] <= 8) { heap.push_back(u); std::push_heap(heap.begin(), heap.end(), cmp); break; }
@@ -381,6 +386,11 @@ int epx_set_option(epx_ctx* c, int option, int value)
         case 6:
             if (value != 0 && value != 1 && value != 2 && value != 4) return fail(c, EPX_E_ARG, "patterns per lane %d", value);
             c->dfs_ppl = value;
+            if (c->has_tree) { int rc = build_plan(c); if (rc) return rc; c->tree_dirty = true; }
+            break;
+        case 7:
+            if (value < 0 || value > 4096) return fail(c, EPX_E_ARG, "pieces %d", value);
+            c->dfs_want = value;
             if (c->has_tree) { int rc = build_plan(c); if (rc) return rc; c->tree_dirty = true; }
             break;
         default: return fail(c, EPX_E_ARG, "unknown option %d", option);

@@ -2,6 +2,7 @@
 #pragma once
 #include <cuda_runtime.h>
 #include <stdint.h>
+#include <algorithm>
 #include <string>
 #include <vector>
 
@@ -40,6 +41,10 @@ struct __align__(16) DfsOp {
     int32_t pa, pb;      // partials index of an HBM-sourced child
     int32_t pad0, pad1;
 };
+// bits 24 / 25 of code: the HBM operand a / b is written earlier in the SAME launch (incremental pieces): load it when the
+// operation runs, never ahead of time
+#define EPX_DFS_LATE_A (1 << 24)
+#define EPX_DFS_LATE_B (1 << 25)
 #define EPX_DFS_HBM (-3)
 #define EPX_DFS_TIP (-2)
 #define EPX_DFS_PREV (-1)
@@ -110,6 +115,7 @@ struct epx_ctx {
     int use_graph = 1;     // EPX_OPT_USE_GRAPH
     int prune_kernel = 0;  // EPX_OPT_PRUNE_KERNEL: 0 auto, 1 force the generic shared-memory kernel
     int dfs_ppl = 0;       // EPX_OPT_DFS_PPL: patterns per lane of the depth-first pruning walk (0 auto, 1, 2, 4)
+    int dfs_want = 0;      // EPX_OPT_DFS_PIECES: pieces the tree is cut into for the depth-first walks (0 auto)
     int exp_method = 0;    // EPX_OPT_EXP_METHOD: 0 auto, 1 spectral (Jacobi / Pade), 2 componentwise (shifted Taylor)
     std::vector<char> model_sparse;   // per epoch: Q has a structural zero off the diagonal
 
@@ -209,7 +215,14 @@ int prune_init_attributes();
 int prune_tile(int K, int C);   // patterns per CTA of the generic pruning kernel
 int dfs_tiles(const epx_ctx* c);         // warps per piece of the depth-first walk
 bool prune_uses_kdfs(const epx_ctx* c);  // K != 4 depth-first walk for few patterns (generic partials layout)
-bool prune_uses_dfs(const epx_ctx* c);   // K == 4 depth-first walk: partials are laid out [node][L][C][4]
+bool prune_uses_lane(const epx_ctx* c);  // K == 4 depth-first walk, one lane per pattern (default; generic partials layout)
+bool prune_uses_dfs(const epx_ctx* c);   // K == 4 depth-first walk, lane = (pattern, category): partials are laid out [node][L][C][4]
+inline bool prune_walk4(const epx_ctx* c) { return prune_uses_lane(c) || prune_uses_dfs(c); }   // any K == 4 walk (DfsOp plans)
+// prune_lane.cu
+int lane_patterns_per_lane(const epx_ctx* c);
+size_t lane_smem_bytes(const epx_ctx* c, int depth);
+int prune_lane_init_attributes();
+void launch_prune4_lane(const epx_ctx* c, const DfsOp* ops, const DfsPiece* pieces, int n_pieces, cudaStream_t s, bool hbm_operands);
 // element (category c, pattern p, state i) of a node's partials sits at c * sc + p * sp + i
 inline void partial_strides(const epx_ctx* c, size_t& sc, size_t& sp)
 {

@@ -1198,6 +1198,7 @@ int prune_init_attributes()
 {
     if (dfs_set_attr<1>() || dfs_set_attr<2>() || dfs_set_attr<3>() || dfs_set_attr<4>() || dfs_set_attr<5>() ||
         dfs_set_attr<6>() || dfs_set_attr<7>() || dfs_set_attr<8>()) return -1;
+    if (prune_lane_init_attributes()) return -1;
     if (cudaFuncSetAttribute(prune64_mma_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024) != cudaSuccess) return -1;
     if (cudaFuncSetAttribute(pruneK_dfs_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, 100 * 1024) != cudaSuccess) return -1;
     if (cudaFuncSetAttribute(prune64_cluster_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024) != cudaSuccess) return -1;
@@ -1224,17 +1225,25 @@ bool prune_uses_kdfs(const epx_ctx* c)
 int dfs_tiles(const epx_ctx* c)
 {
     if (c->K != 4) return c->L;                                // pruneK_dfs_kernel: one warp per pattern
+    if (c->prune_kernel == 0) { const int pw = 32 * lane_patterns_per_lane(c); return (c->L + pw - 1) / pw; }
     if (c->prune_kernel == 3) return (c->L + 7) / 8;          // tensor-core walk: 8 patterns per warp
     const int pw = dfs_patterns_per_lane(c) * (32 / dfs_lanes_of(c->C));
     return (c->L + pw - 1) / pw;
 }
 
+bool prune_uses_lane(const epx_ctx* c)
+{
+    if (!(c->tree_mode && c->K == 4 && c->prune_kernel == 0)) return false;
+    if ((double)(c->N - 1 + c->tip_cap) * c->L * c->C >= 4294967296.0) return false;       // 32-bit state-vector indices
+    return lane_smem_bytes(c, c->dfs_depth > 0 ? c->dfs_depth : 1) <= 227 * 1024;
+}
+
 bool prune_uses_dfs(const epx_ctx* c)
 {
-    if (!(c->tree_mode && c->K == 4 && (c->prune_kernel == 0 || c->prune_kernel == 3))) return false;
+    if (!(c->tree_mode && c->K == 4 && (c->prune_kernel == 5 || c->prune_kernel == 3))) return false;
     const int depth = c->dfs_depth > 0 ? c->dfs_depth : 1;
     if (c->prune_kernel == 3) return (double)c->L * c->C * 4 < 4294967296.0 && mma_smem(c->C, depth) <= 227 * 1024;
-    if ((double)(c->N - 1) * c->L * c->C >= 4294967296.0) return false;
+    if ((double)(c->N - 1 + c->tip_cap) * c->L * c->C >= 4294967296.0) return false;
     return dfs_smem(dfs_lanes_of(c->C), depth, dfs_patterns_per_lane(c)) <= 227 * 1024;
 }
 
@@ -1253,7 +1262,7 @@ static void launch_dfs(const epx_ctx* c, const DfsOp* ops, const DfsPiece* piece
 {
     // the top piece is a few dozen operations whose operands come from HBM: one pattern per lane doubles the warps that
     // hide that latency (measured 41 -> 20 us on config 2)
-    if (top && c->prune_kernel == 0 && c->dfs_ppl == 0) { launch_dfs2<C, 1>(c, ops, pieces, n_pieces, s); return; }
+    if (top && c->prune_kernel == 5 && c->dfs_ppl == 0) { launch_dfs2<C, 1>(c, ops, pieces, n_pieces, s); return; }
     if (c->prune_kernel == 3) {
         const DevBuffers& d = c->d;
         const int tiles = dfs_tiles(c);
@@ -1290,7 +1299,8 @@ static int launch_pruning_dfs(const epx_ctx* c, cudaStream_t s)
     for (int pass = 0; pass < 2; pass++) {
         const int first = pass == 0 ? 0 : c->dfs_bottom, count = pass == 0 ? c->dfs_bottom : total - c->dfs_bottom;
         if (count <= 0) continue;
-        launch_dfs_any(c, c->d.dfs_ops, c->d.dfs_pieces + first, count, s, pass == 1);
+        if (prune_uses_lane(c)) launch_prune4_lane(c, c->d.dfs_ops, c->d.dfs_pieces + first, count, s, pass == 1);
+        else launch_dfs_any(c, c->d.dfs_ops, c->d.dfs_pieces + first, count, s, pass == 1);
         launched++;
     }
     return cudaGetLastError() == cudaSuccess ? launched : -1;
@@ -1341,7 +1351,7 @@ static void launch_level(const epx_ctx* c, const PruneOp* ops, int nops, cudaStr
 
 int launch_pruning(const epx_ctx* c, cudaStream_t s)
 {
-    if (prune_uses_dfs(c)) return launch_pruning_dfs(c, s);
+    if (prune_walk4(c)) return launch_pruning_dfs(c, s);
     if (prune_uses_kdfs(c)) {
         const DevBuffers& d = c->d;
         const int total = (int)c->dfs_pieces.size();
@@ -1372,7 +1382,10 @@ int launch_pruning(const epx_ctx* c, cudaStream_t s)
 int launch_pruning_incremental(const epx_ctx* c, const std::vector<int>& group_off, cudaStream_t s)
 {
     int launched = 0;
-    if (prune_uses_dfs(c)) {
+    if (prune_uses_lane(c)) {
+        launch_prune4_lane(c, c->d.inc_ops, c->d.inc_piece, 1, s, true);
+        launched = 1;
+    } else if (prune_uses_dfs(c)) {
         launch_dfs_any(c, c->d.inc_ops, c->d.inc_piece, 1, s, true);
         launched = 1;
     } else {

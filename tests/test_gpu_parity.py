@@ -93,11 +93,16 @@ def test_config1_generic_kernels_and_no_graph(epx, orc_ld):
 def test_config2_reduced(epx, orc_ld):
     # several pattern tiles plus a ragged tail (L = 777 = 3*256 + 9 = 97*8 + 1), 10 epochs, dated tips
     prob = W.make_config(2, N=150, L=777)
-    run_tree(epx, orc_ld, prob)                                                  # depth-first walk (default)
-    # the instantiations bench.py times at full size (C = 4; 2 patterns per lane is chosen there because L >= 4096): every
-    # node's partials against the oracle
-    for ppl in (1, 2, 4):
+    run_tree(epx, orc_ld, prob)                                                  # depth-first walk, one lane per pattern (default)
+    # every instantiation bench.py can time at full size (C = 4), every node's partials against the oracle:
+    # the lane-per-pattern walk with 1 and 2 patterns per lane, cut into few / many pieces ...
+    for ppl in (1, 2):
         run_tree(epx, orc_ld, prob, options=[(epx.EPX_OPT_DFS_PPL, ppl)])
+    for pieces in (2, 5, 64):
+        run_tree(epx, orc_ld, prob, options=[(epx.EPX_OPT_DFS_PIECES, pieces)])
+    # ... and round 1's walk (lane = (pattern, category)) with 1, 2, 4 patterns per lane
+    for ppl in (1, 2, 4):
+        run_tree(epx, orc_ld, prob, options=[(epx.EPX_OPT_PRUNE_KERNEL, 5), (epx.EPX_OPT_DFS_PPL, ppl)])
     run_tree(epx, orc_ld, prob, options=[(epx.EPX_OPT_PRUNE_KERNEL, 3)])         # depth-first walk, 4x4 products on the FP64 tensor pipe
     run_tree(epx, orc_ld, prob, options=[(epx.EPX_OPT_PRUNE_KERNEL, 3), (epx.EPX_OPT_DFS_PPL, 2)])
     run_tree(epx, orc_ld, prob, options=[(epx.EPX_OPT_PRUNE_KERNEL, 2)])         # level-by-level register kernel
@@ -114,9 +119,12 @@ def test_k4_every_category_count(epx, orc_ld, C):
     tips[::3, ::7] = -1
     tips[5, :] = 99
     prob = dataclasses.replace(prob, C=C, rates=rates, weights=weights, tip_states=tips)
-    run_tree(epx, orc_ld, prob)
-    for ppl in (2, 4):                                  # 2 / 4 patterns per lane: tiles of 16..128 patterns, ragged tail
-        run_tree(epx, orc_ld, prob, options=[(epx.EPX_OPT_DFS_PPL, ppl)], partial_nodes=[prob.n_nodes - 1, prob.N])
+    run_tree(epx, orc_ld, prob)                         # lane per pattern: tiles of 32 patterns, ragged tail (203 = 6*32 + 11)
+    run_tree(epx, orc_ld, prob, options=[(epx.EPX_OPT_DFS_PPL, 2)])
+    run_tree(epx, orc_ld, prob, options=[(epx.EPX_OPT_PRUNE_KERNEL, 5)])
+    for ppl in (2, 4):                                  # lane per (pattern, category), 2 / 4 patterns per lane: tiles of 16..128
+        run_tree(epx, orc_ld, prob, options=[(epx.EPX_OPT_PRUNE_KERNEL, 5), (epx.EPX_OPT_DFS_PPL, ppl)],
+                 partial_nodes=[prob.n_nodes - 1, prob.N])
     run_tree(epx, orc_ld, prob, options=[(epx.EPX_OPT_PRUNE_KERNEL, 3)])
     run_tree(epx, orc_ld, prob, options=[(epx.EPX_OPT_PRUNE_KERNEL, 2)], partial_nodes=[prob.n_nodes - 1])
 
@@ -156,6 +164,8 @@ def test_k4_extreme_tree_shapes(epx, orc_ld, shape, N):
     parent, height = _shaped_tree(shape, N)
     prob = dataclasses.replace(prob, parent=parent, height=height)
     run_tree(epx, orc_ld, prob)
+    run_tree(epx, orc_ld, prob, options=[(epx.EPX_OPT_DFS_PPL, 2)])
+    run_tree(epx, orc_ld, prob, options=[(epx.EPX_OPT_PRUNE_KERNEL, 5)])
     run_tree(epx, orc_ld, prob, options=[(epx.EPX_OPT_PRUNE_KERNEL, 3)])
 
 
