@@ -629,7 +629,7 @@ def bench_other_configs(torch, epx, device: int, K: int, peaks: dict) -> dict:
     return out
 
 
-PRUNE64_KERNEL_NAME = "prune64_cluster_kernel"
+PRUNE64_KERNEL_NAME = "prune_mma_kernel<64> (+ pb_swizzle_kernel<64>)"
 
 
 def parse_opts(text: str):

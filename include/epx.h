@@ -179,16 +179,18 @@ int epx_get_stage_ms(epx_ctx* ctx, float* ms, int* launches);
  * compiler from deleting the arithmetic).  Synchronises the stream. */
 int epx_measure_fp64_peak(int device, int kind, double ms_target, void* dev_scratch, void* cuda_stream, double* tflops);
 
-/* ---- tuning / test hooks (options 1-3, 6, 7 have no effect on results) ---- */
+/* ---- tuning / test hooks (options 1-3, 6-8 have no effect on results) ---- */
 enum {
     EPX_OPT_CHAIN_KERNEL = 1, /* 0 auto (default); 1 force the generic shared-memory chain kernel */
     EPX_OPT_USE_GRAPH = 2,    /* 1 (default) replay the kernel sequence from a CUDA graph on non-default streams; 0 launch directly */
-    EPX_OPT_PRUNE_KERNEL = 3, /* 0 auto (default: K == 4 walks the tree depth first, one lane per site pattern, partials never
-                                 re-read from HBM); 1 force the generic shared-memory level kernel; 2 (K == 4) the level-by-level
-                                 register kernel; 3 (K == 4) the depth-first walk with the 4x4 products on the FP64 tensor pipe
-                                 (mma.sync m8n8k4; kept for comparison); 4 (32 < K <= 64) one CTA per (node, tile) looping over
-                                 the categories instead of a cluster of one CTA per category; 5 (K == 4) round 1's depth-first
-                                 walk with one lane per (pattern, category) (kept for comparison) */
+    EPX_OPT_PRUNE_KERNEL = 3, /* 0 auto (default).  K == 4: depth-first walk, one lane per site pattern, partials never
+                                 re-read from HBM.  8 < K <= 64: level kernel on the FP64 tensor pipe, matrices staged by TMA in
+                                 fragment order (few patterns and K <= 32: a depth-first walk instead).  Other K: generic.
+                                 1 force the generic shared-memory level kernel; 2 (K == 4) the level-by-level register kernel;
+                                 3 (K == 4) the depth-first walk with the 4x4 products on the FP64 tensor pipe; 5 (K == 4) round
+                                 1's walk with one lane per (pattern, category); 4 / 6 (32 < K <= 64) round 1's tensor-pipe level
+                                 kernels (one CTA per (node, tile) looping over the categories / a cluster of one CTA per
+                                 category).  2-6 are kept for comparison */
     EPX_OPT_EXP_METHOD = 4,   /* a3 method.  1 spectral: Jacobi eigensystem (reversible) / Pade 13 (asymmetric), absolute
                                  error ~1e-14 per entry.  2 componentwise: shifted non-negative Taylor scaling-and-squaring,
                                  every entry to a few hundred ulp RELATIVE, ~8 dense products per segment.  0 auto (default):
@@ -197,8 +199,9 @@ enum {
                                  else 1.  This one DOES change results, within the tolerances above (A21). */
     EPX_OPT_STAGE_EVENTS = 5, /* 1 record per-stage CUDA events for epx_get_stage_ms; 0 (default) none */
     EPX_OPT_DFS_PPL = 6,      /* K == 4 depth-first pruning: site patterns per lane, 1, 2 or 4 (4: kernel 5 only); 0 (default) auto */
-    EPX_OPT_DFS_PIECES = 7    /* depth-first pruning: number of pieces the tree is cut into (independent subtrees walked by
+    EPX_OPT_DFS_PIECES = 7,   /* depth-first pruning: number of pieces the tree is cut into (independent subtrees walked by
                                  different warps + the part above them); 0 (default) auto */
+    EPX_OPT_MMA_CHUNK = 8     /* 8 < K <= 64 tensor-pipe level kernel: site patterns per CTA (rounded up to 8); 0 (default) auto */
 };
 int epx_set_option(epx_ctx* ctx, int option, int value);
 /* Device status word of the last compute call (0 = all numeric checks passed); synchronises. */

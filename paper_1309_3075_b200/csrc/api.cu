@@ -59,6 +59,7 @@ size_t plan_workspace(const epx_ctx* c, char* base, DevBuffers* d)
         t.height = (double*)take(8 * S);
         t.tips = (uint8_t*)take(N * (size_t)c->Lp);
         t.pattern_wt = (double*)take(8 * L);
+        t.tip_vec = (uint8_t*)take(N);
         t.ops = (PruneOp*)take(sizeof(PruneOp) * (N - 1));
         t.dfs_ops = (DfsOp*)take(sizeof(DfsOp) * (N - 1));
         t.dfs_pieces = (DfsPiece*)take(sizeof(DfsPiece) * (N - 1));
@@ -83,8 +84,11 @@ size_t plan_workspace(const epx_ctx* c, char* base, DevBuffers* d)
     t.Efull = (double*)take(8 * M * C * K * K);
     t.P = (double*)take(8 * S * C * K * K);
     if (c->tree_mode) {
-        t.partials = (double*)take(8 * (N - 1 + (size_t)c->tip_cap) * C * L * K);
-        t.scale_exp = (int32_t*)take(4 * (N - 1 + (size_t)c->tip_cap) * L);
+        // sized for every layout an option can select later: states padded to 8 and one exponent per category when K > 8
+        const size_t Kalloc = K > 8 ? (size_t)prune_kp(c) : K;
+        t.PB = (double*)take(K > 8 ? 8 * S * C * Kalloc * Kalloc : 0);
+        t.partials = (double*)take(8 * (N - 1 + (size_t)c->tip_cap) * C * L * Kalloc);
+        t.scale_exp = (int32_t*)take(4 * (N - 1 + (size_t)c->tip_cap) * L * (K > 8 ? C : 1));
         t.site_lnl = (double*)take(8 * L);
         t.block_sums = (double*)take(8 * ((L + 7) / 8));
     }
@@ -360,7 +364,8 @@ int epx_bind(epx_ctx* c, void* ws, size_t bytes, void* stream)
     CUDA_TRY(c, cudaPointerGetAttributes(&attr, ws));
     if (attr.type != cudaMemoryTypeDevice && attr.type != cudaMemoryTypeManaged)
         return fail(c, EPX_E_WORKSPACE, "workspace is not device memory");
-    if (chain_init_attributes() || pade_init_attributes() || eigen_init_attributes() || prune_init_attributes())
+    if (chain_init_attributes() || pade_init_attributes() || eigen_init_attributes() || prune_init_attributes() ||
+        prune_mma_init_attributes())
         return fail(c, EPX_E_CUDA, "cudaFuncSetAttribute: %s", cudaGetErrorString(cudaGetLastError()));
     drop_graphs(c);
     plan_workspace(c, (char*)ws, &c->d);
@@ -387,6 +392,10 @@ int epx_set_option(epx_ctx* c, int option, int value)
             if (value != 0 && value != 1 && value != 2 && value != 4) return fail(c, EPX_E_ARG, "patterns per lane %d", value);
             c->dfs_ppl = value;
             if (c->has_tree) { int rc = build_plan(c); if (rc) return rc; c->tree_dirty = true; }
+            break;
+        case 8:
+            if (value < 0 || value > (1 << 20)) return fail(c, EPX_E_ARG, "chunk %d", value);
+            c->mma_chunk = value;
             break;
         case 7:
             if (value < 0 || value > 4096) return fail(c, EPX_E_ARG, "pieces %d", value);

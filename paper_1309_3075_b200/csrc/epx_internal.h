@@ -67,6 +67,7 @@ struct DevBuffers {
     double* brate;        // [n_slots] branch rate scalars (valid iff has_brates)
     uint8_t* tips;        // [N][Lp] 0..K-1, 255 = missing; rows padded to Lp = L rounded up to 32
     double* pattern_wt;   // [L]
+    uint8_t* tip_vec;     // [N] 1 = the tip carries a partial vector (f3) and is read like an internal child
     PruneOp* ops;         // [N-1] sorted by level
     DfsOp* dfs_ops;       // [N-1] depth-first post-order (K == 4 pruning walk), piece after piece
     DfsPiece* dfs_pieces; // [<= N-1] op ranges of the pieces: bottom pieces (largest first), then the top piece
@@ -89,6 +90,7 @@ struct DevBuffers {
     double* Efull;        // [M][C][K][K] exp(Q_e r_c (tau_e - tau_{e-1})) for interior epochs 1..M-2
     // a3/a4 output
     double* P;            // [n_slots][C][K][K]
+    double* PB;           // [n_slots][C][KP*KP] the same matrices in mma.m8n8k4 B-fragment order (tree mode, K > 8; prune_mma.cu)
     // a5
     double* partials;     // [N-1][C][L][K] internal nodes only, in op order
     int32_t* scale_exp;   // [N-1][L]
@@ -116,6 +118,7 @@ struct epx_ctx {
     int prune_kernel = 0;  // EPX_OPT_PRUNE_KERNEL: 0 auto, 1 force the generic shared-memory kernel
     int dfs_ppl = 0;       // EPX_OPT_DFS_PPL: patterns per lane of the depth-first pruning walk (0 auto, 1, 2, 4)
     int dfs_want = 0;      // EPX_OPT_DFS_PIECES: pieces the tree is cut into for the depth-first walks (0 auto)
+    int mma_chunk = 0;     // EPX_OPT_MMA_CHUNK: site patterns per CTA of the tensor-pipe level kernel (0 auto)
     int exp_method = 0;    // EPX_OPT_EXP_METHOD: 0 auto, 1 spectral (Jacobi / Pade), 2 componentwise (shifted Taylor)
     std::vector<char> model_sparse;   // per epoch: Q has a structural zero off the diagonal
 
@@ -223,9 +226,23 @@ int lane_patterns_per_lane(const epx_ctx* c);
 size_t lane_smem_bytes(const epx_ctx* c, int depth);
 int prune_lane_init_attributes();
 void launch_prune4_lane(const epx_ctx* c, const DfsOp* ops, const DfsPiece* pieces, int n_pieces, cudaStream_t s, bool hbm_operands);
-// element (category c, pattern p, state i) of a node's partials sits at c * sc + p * sp + i
-inline void partial_strides(const epx_ctx* c, size_t& sc, size_t& sp)
+// prune_mma.cu: level kernel on the FP64 tensor pipe for 8 < K <= 64
+inline int prune_kp(const epx_ctx* c) { return (c->K + 7) & ~7; }
+bool prune_uses_mma(const epx_ctx* c);
+int prune_mma_chunk(const epx_ctx* c, int nops);
+int prune_mma_init_attributes();
+void launch_prune_mma_level(const epx_ctx* c, const PruneOp* ops, int nops, cudaStream_t s);
+void launch_pb_swizzle(const epx_ctx* c, cudaStream_t s);
+
+// Where the pruning kernels of this ctx keep partials and scale exponents.  Element (node block n, category c, pattern p,
+// state i) sits at n * node + c * sc + p * sp + i; its exponent at (n * C + c) * L + p if exp_per_cat, else at n * L + p.
+struct PartialLayout { size_t node, sc, sp; int ks; bool exp_per_cat; };
+inline PartialLayout partial_layout(const epx_ctx* c)
 {
-    if (prune_uses_dfs(c)) { sc = (size_t)c->K; sp = (size_t)c->C * c->K; }
-    else { sc = (size_t)c->L * c->K; sp = (size_t)c->K; }
+    PartialLayout l;
+    const size_t K = c->K, C = c->C, L = c->L;
+    if (prune_uses_mma(c)) { const size_t KP = prune_kp(c); l = {C * L * KP, L * KP, KP, (int)KP, true}; }
+    else if (prune_uses_dfs(c)) l = {C * L * K, K, C * K, (int)K, false};
+    else l = {C * L * K, L * K, K, (int)K, false};
+    return l;
 }

@@ -1109,7 +1109,10 @@ __global__ void __launch_bounds__(256) root_site_kernel(int K, int C, int L, siz
 }
 
 // K > 8: one warp per pattern, lanes over the states (coalesced reads of the root vectors), eight patterns per CTA.
-__global__ void __launch_bounds__(256) root_site_warp_kernel(int K, int C, int L, size_t sc, size_t sp, int root_pidx, int root_node,
+// exp_per_cat: the pruning kernel kept one scale exponent per (category, pattern) (prune_mma.cu): the categories are summed
+// relative to the pattern's largest exponent (exact power-of-two factors).
+__global__ void __launch_bounds__(256) root_site_warp_kernel(int K, int C, int L, size_t node_off, size_t sc, size_t sp, int exp_per_cat,
+    int root_pidx, int root_node,
     const double* __restrict__ partials, const int32_t* __restrict__ scale_exp, const double* __restrict__ freqs,
     const int32_t* __restrict__ e_hi, const double* __restrict__ root_freqs, const double* __restrict__ weights,
     const double* __restrict__ pattern_wt, double* __restrict__ site_lnl, double* __restrict__ block_sums,
@@ -1121,17 +1124,25 @@ __global__ void __launch_bounds__(256) root_site_warp_kernel(int K, int C, int L
     const double* rf = root_freqs ? root_freqs : freqs + (size_t)e_hi[root_node] * K;   // reading A9
     double contrib = 0.0;
     if (p < L) {
+        int emax = 0;
+        if (exp_per_cat) {
+            emax = scale_exp[((size_t)root_pidx * C) * L + p];
+            for (int c = 1; c < C; c++) emax = max(emax, scale_exp[((size_t)root_pidx * C + c) * L + p]);
+        } else {
+            emax = scale_exp[(size_t)root_pidx * L + p];
+        }
         double site = 0.0;
         for (int c = 0; c < C; c++) {               // per category: states in lane order, then a fixed butterfly
-            const double* v = partials + (size_t)root_pidx * C * L * K + c * sc + p * sp;
+            const double* v = partials + node_off + c * sc + p * sp;
             double s = 0.0;
             for (int i = lane; i < K; i += 32) s = fma(rf[i], v[i], s);
             for (int o = 16; o > 0; o >>= 1) s += __shfl_xor_sync(0xffffffffu, s, o);
+            if (exp_per_cat) s = scalbn(s, scale_exp[((size_t)root_pidx * C + c) * L + p] - emax);
             site = fma(weights[c], s, site);
         }
         if (lane == 0) {
             if (!(site > 0.0) || !(site < 1.7e308)) atomicOr(status, EPX_ST_BAD_SITE);
-            const double ln = log(site) + (double)scale_exp[(size_t)root_pidx * L + p] * 0.6931471805599453094;
+            const double ln = log(site) + (double)emax * 0.6931471805599453094;
             site_lnl[p] = ln;
             contrib = pattern_wt[p] * ln;
         }
@@ -1220,6 +1231,12 @@ bool prune_uses_kdfs(const epx_ctx* c)
 {
     return c->tree_mode && c->K != 4 && c->K <= 32 && c->C <= KD_MAXC && c->prune_kernel == 0 && (long)c->L * c->C <= 64 &&
            c->N >= 8 && kdfs_smem(c->K, c->C, c->dfs_depth > 0 ? c->dfs_depth : 1) <= 100 * 1024;
+}
+
+// 8 < K <= 64 with enough patterns for 8-pattern tensor tiles: level kernel of prune_mma.cu
+bool prune_uses_mma(const epx_ctx* c)
+{
+    return c->tree_mode && c->K > 8 && c->prune_kernel == 0 && !prune_uses_kdfs(c);
 }
 
 int dfs_tiles(const epx_ctx* c)
@@ -1322,9 +1339,11 @@ static void launch_level(const epx_ctx* c, const PruneOp* ops, int nops, cudaStr
             case 7: launch_prune4<7>(ops, nops, L, d, s); break;
             default: launch_prune4<8>(ops, nops, L, d, s); break;
         }
-    } else if (K > 32 && c->prune_kernel != 1 && mma64_smem(K, C) <= 227 * 1024) {
+    } else if (prune_uses_mma(c)) {
+        launch_prune_mma_level(c, ops, nops, s);
+    } else if (K > 32 && (c->prune_kernel == 4 || c->prune_kernel == 6) && mma64_smem(K, C) <= 227 * 1024) {
         const int tiles = (L + M_TP - 1) / M_TP;
-        if (c->prune_kernel == 0) {              // one CTA per category, clusters of C
+        if (c->prune_kernel == 6) {              // round 1: one CTA per category, clusters of C
             cudaLaunchConfig_t cfg{};
             cfg.gridDim = dim3((unsigned)(nops * tiles * C));
             cfg.blockDim = dim3(MT);
@@ -1367,6 +1386,7 @@ int launch_pruning(const epx_ctx* c, cudaStream_t s)
         return cudaGetLastError() == cudaSuccess ? n : -1;
     }
     int launched = 0;
+    if (prune_uses_mma(c)) { launch_pb_swizzle(c, s); launched++; }      // matrices in B-fragment order for the TMA staging
     const int n_levels = (int)c->level_off.size() - 1;
     for (int l = 0; l < n_levels; l++) {
         const int first = c->level_off[l], nops = c->level_off[l + 1] - first;
@@ -1389,6 +1409,7 @@ int launch_pruning_incremental(const epx_ctx* c, const std::vector<int>& group_o
         launch_dfs_any(c, c->d.inc_ops, c->d.inc_piece, 1, s, true);
         launched = 1;
     } else {
+        if (prune_uses_mma(c)) { launch_pb_swizzle(c, s); launched++; }  // (the slots of c->sub_list)
         for (size_t g = 0; g + 1 < group_off.size(); g++) {
             launch_level(c, c->d.inc_pops + group_off[g], group_off[g + 1] - group_off[g], s);
             launched++;
@@ -1402,14 +1423,14 @@ int launch_root_reduction(const epx_ctx* c, cudaStream_t s)
     const DevBuffers& d = c->d;
     const int blocks = c->reduce_blocks;
     const int root_pidx = c->node_pidx[c->root];
-    size_t sc, sp;
-    partial_strides(c, sc, sp);
+    const PartialLayout lay = partial_layout(c);
     if (c->K > 8)
-        root_site_warp_kernel<<<blocks, 256, 0, s>>>(c->K, c->C, c->L, sc, sp, root_pidx, c->root, d.partials, d.scale_exp, d.freqs,
+        root_site_warp_kernel<<<blocks, 256, 0, s>>>(c->K, c->C, c->L, (size_t)root_pidx * lay.node, lay.sc, lay.sp, lay.exp_per_cat ? 1 : 0,
+                                                     root_pidx, c->root, d.partials, d.scale_exp, d.freqs,
                                                      d.e_hi, c->has_root_freqs ? d.root_freqs : nullptr, d.weights,
                                                      d.pattern_wt, d.site_lnl, d.block_sums, d.status);
     else
-    root_site_kernel<<<blocks, 256, 0, s>>>(c->K, c->C, c->L, sc, sp, root_pidx, c->root, d.partials, d.scale_exp, d.freqs,
+    root_site_kernel<<<blocks, 256, 0, s>>>(c->K, c->C, c->L, lay.sc, lay.sp, root_pidx, c->root, d.partials, d.scale_exp, d.freqs,
                                             d.e_hi, c->has_root_freqs ? d.root_freqs : nullptr, d.weights,
                                             d.pattern_wt, d.site_lnl, d.block_sums, d.status);
     final_sum_kernel<<<1, 256, 0, s>>>(blocks, d.block_sums, d.lnl);

@@ -7,10 +7,13 @@
 //     pb_swizzle_kernel keeps in mma.m8n8k4 B-fragment order (PB), so the inner loop reads it with conflict-free 64-bit
 //     shared-memory loads -- round 1's kernel staged 61 x 61 doubles with strided 8-byte loads per 32 patterns and spent its
 //     time there (profiles/r1_other_configs_ncu.md: DMMA pipe 21-27 % busy);
-//   * a warp owns 8 patterns; lane (g, q) = pattern g, states q S .. q S + S - 1 (S = KP / 4).  The contraction index of
-//     k-step kt at position q is state q S + kt and column 2 q + h of n-tile nt is state q S + 2 nt + h, so a lane's A operand
-//     (child vector) AND its D fragment (result) are the same S CONTIGUOUS states: vectors go from global memory to the
-//     tensor pipe and back with 128-bit accesses and no shared-memory round trip;
+//   * a warp owns 8 patterns; lane (g, q) = pattern g and S = KP / 4 of its states, VW (4, or 2 if S is odd-ish) at a time:
+//     element e of lane q is state st(q, e) = (e / VW) 4 VW + q VW + e % VW, so the 4 lanes of a pattern read / write 4 VW
+//     CONTIGUOUS doubles per instruction (a full 128-byte line with 256-bit accesses).  The contraction index of k-step kt
+//     at position q is state st(q, kt) and column 2 q + h of n-tile nt is state st(q, 2 nt + h): a lane's A operand (child
+//     vector) AND its D fragment (result) are the same S elements, so vectors go from global memory to the tensor pipe and
+//     back with no shared-memory round trip.  (A first version gave a lane S contiguous states: every 128-bit load of a
+//     warp then touched 32 different lines and the kernel was bound by L1 tag lookups, l1tex 85 % busy.)
 //   * tip children are gathers P[i][state] from the row-major matrix (no product, no staging).
 // Rescaling (reading A12) is per (node, CATEGORY, pattern) here -- a category is a CTA of its own, and a power-of-two factor
 // per category is as exact as one per pattern; the root reduction and epx_get_partials fold the C exponents together.
@@ -23,29 +26,59 @@ namespace {
 
 constexpr int MMA_T = 256;        // 8 warps x 8 patterns = 64 patterns per pass over the chunk
 
-// PB[slot][c][(kt * NT + nt) * 32 + 4 g + q] = P[i][j],  j = q S + kt (contraction),  i = (g >> 1) S + 2 nt + (g & 1)
 template <int KP>
-__global__ void __launch_bounds__(256) pb_swizzle_kernel(int K, int C, const int32_t* __restrict__ list, const double* __restrict__ P,
+struct Frag {
+    static constexpr int S = KP / 4, NT = KP / 8, KT = KP / 4, MAT = KP * KP;
+    static constexpr int VW = (S % 4 == 0) ? 4 : 2;          // doubles per vector access
+    static constexpr int NC = S / VW;                        // vector accesses per lane and state vector
+    __host__ __device__ static constexpr int st(int q, int e) { return (e / VW) * 4 * VW + q * VW + e % VW; }
+};
+
+// Internal nodes' slots: PB[slot][c][(kt * NT + nt) * 32 + 4 g + q] = P[i][j],  j = st(q, kt) (contraction),
+//                                                                    i = st(g >> 1, 2 nt + (g & 1))   (B-fragment order)
+template <int KP>
+__global__ void __launch_bounds__(256) pb_swizzle_kernel(int K, int C, int n_tips, const uint8_t* __restrict__ tip_vec,
+                                                         const int32_t* __restrict__ list, const double* __restrict__ P,
                                                          double* __restrict__ PB)
 {
-    constexpr int S = KP / 4, NT = KP / 8;
+    using F = Frag<KP>;
+    constexpr int NT = F::NT;
     const int slot = list ? list[blockIdx.x / C] : blockIdx.x / C, c = blockIdx.x % C;
     const double* src = P + ((size_t)slot * C + c) * K * K;
     double* dst = PB + ((size_t)slot * C + c) * KP * KP;
+    if (slot < n_tips && !tip_vec[slot]) {           // (a tip with a partial vector is multiplied like an internal child)
+        __shared__ double tile[32][33];
+        for (int s0 = 0; s0 < KP; s0 += 32)
+            for (int i0 = 0; i0 < KP; i0 += 32) {
+                const int tx = threadIdx.x & 31, ty = threadIdx.x >> 5;
+                for (int r = ty; r < 32; r += 8) {      // read P[i0 + r][s0 + tx] (coalesced along s)
+                    const int i = i0 + r, sidx = s0 + tx;
+                    tile[r][tx] = (i < K && sidx < K) ? src[i * K + sidx] : 0.0;
+                }
+                __syncthreads();
+                for (int r = ty; r < 32; r += 8) {      // write PT[s0 + r][i0 + tx] (coalesced along i)
+                    const int sidx = s0 + r, i = i0 + tx;
+                    if (sidx < KP && i < KP) dst[sidx * KP + i] = tile[tx][r];
+                }
+                __syncthreads();
+            }
+        return;
+    }
     for (int idx = threadIdx.x; idx < KP * KP; idx += 256) {
         const int lane = idx & 31, t = idx >> 5, nt = t % NT, kt = t / NT;
         const int g = lane >> 2, q = lane & 3;
-        const int j = q * S + kt, i = (g >> 1) * S + 2 * nt + (g & 1);
+        const int j = F::st(q, kt), i = F::st(g >> 1, 2 * nt + (g & 1));
         dst[idx] = (i < K && j < K) ? src[i * K + j] : 0.0;
     }
 }
 
 template <int KP>
-__global__ void __launch_bounds__(MMA_T) prune_mma_kernel(const PruneOp* __restrict__ ops, int chunks, int chunk_p, int K, int C,
-    int L, int Lp, const double* __restrict__ P, const double* __restrict__ PB, const uint8_t* __restrict__ tips,
+__global__ void __launch_bounds__(MMA_T, KP > 48 ? 2 : 3) prune_mma_kernel(const PruneOp* __restrict__ ops, int chunks, int chunk_p, int K, int C,
+    int L, int Lp, const double* __restrict__ PB, const uint8_t* __restrict__ tips,
     double* __restrict__ partials, int32_t* __restrict__ scale_exp)
 {
-    constexpr int S = KP / 4, NT = KP / 8, KT = KP / 4, MAT = KP * KP;
+    using F = Frag<KP>;
+    constexpr int S = F::S, NT = F::NT, KT = F::KT, MAT = F::MAT, VW = F::VW, NC = F::NC;
     extern __shared__ __align__(128) unsigned char smraw[];
     double* Bs = reinterpret_cast<double*>(smraw);                      // [2][KP * KP] fragment-ordered child matrices
     uint64_t* bar = reinterpret_cast<uint64_t*>(Bs + 2 * MAT);          // [2]
@@ -72,29 +105,42 @@ __global__ void __launch_bounds__(MMA_T) prune_mma_kernel(const PruneOp* __restr
     for (int p8 = p_begin + 8 * w; p8 < p_end; p8 += 8 * (MMA_T / 32)) {
         const int p = p8 + g;
         const bool live = p < p_end;
-        double f[S];
-        int ex = 0;
+        // both children's operands are requested before the first product starts: an internal child's vector (S contiguous
+        // states of pattern g), or for a tip child the column its state selects = a row of the transposed copy
+        double a[2][S];
+        int ex = 0, tip_s[2] = {0, 0};
 #pragma unroll
         for (int ch = 0; ch < 2; ch++) {
-            double t[S];
+            const double* v;
             if (op.child_is_tip[ch]) {
                 const int s = live ? tips[(size_t)op.child[ch] * Lp + p] : 255;
-                const double* Pm = P + ((size_t)op.child[ch] * C + c) * K * K;
+                tip_s[ch] = s;
+                v = PB + ((size_t)op.child[ch] * C + c) * MAT + (size_t)min(s, K - 1) * KP + q * VW;
+            } else {
+                v = partials + ((size_t)op.cpidx[ch] * C + c) * LK + (size_t)(live ? p : p_begin) * KP + q * VW;
+                if (live) ex += scale_exp[((size_t)op.cpidx[ch] * C + c) * L + p];
+            }
+#pragma unroll
+            for (int m = 0; m < NC; m++) {
+                if (VW == 4) {
+                    const double4a r = ld256(v + m * 16);
+                    a[ch][4 * m] = r.x; a[ch][4 * m + 1] = r.y; a[ch][4 * m + 2] = r.z; a[ch][4 * m + 3] = r.w;
+                } else {
+                    const double2 r = *reinterpret_cast<const double2*>(v + m * 8);
+                    a[ch][2 * m] = r.x; a[ch][2 * m + 1] = r.y;
+                }
+            }
+        }
+        double f[S];
+#pragma unroll
+        for (int ch = 0; ch < 2; ch++) {
+            if (op.child_is_tip[ch]) {
 #pragma unroll
                 for (int k = 0; k < S; k++) {
-                    const int i = q * S + k;
-                    t[k] = i < K ? (s < K ? __ldg(Pm + i * K + s) : 1.0) : 0.0;
+                    const double t = tip_s[ch] < K ? a[ch][k] : (F::st(q, k) < K ? 1.0 : 0.0);     // missing state: all ones
+                    f[k] = ch ? f[k] * t : t;
                 }
             } else {
-                double a[S];
-                const double* v = partials + ((size_t)op.cpidx[ch] * C + c) * LK + (size_t)p * KP + q * S;
-#pragma unroll
-                for (int k = 0; k < S; k += 2) {
-                    double2 r = make_double2(0.0, 0.0);
-                    if (live) r = *reinterpret_cast<const double2*>(v + k);
-                    a[k] = r.x; a[k + 1] = r.y;
-                }
-                if (live) ex += scale_exp[((size_t)op.cpidx[ch] * C + c) * L + p];
                 double acc[NT][2];
 #pragma unroll
                 for (int nt = 0; nt < NT; nt++) acc[nt][0] = acc[nt][1] = 0.0;
@@ -103,12 +149,13 @@ __global__ void __launch_bounds__(MMA_T) prune_mma_kernel(const PruneOp* __restr
 #pragma unroll
                 for (int kt = 0; kt < KT; kt++)
 #pragma unroll
-                    for (int nt = 0; nt < NT; nt++) dmma884(acc[nt][0], acc[nt][1], a[kt], Bc[(kt * NT + nt) * 32]);
+                    for (int nt = 0; nt < NT; nt++) dmma884(acc[nt][0], acc[nt][1], a[ch][kt], Bc[(kt * NT + nt) * 32]);
 #pragma unroll
-                for (int nt = 0; nt < NT; nt++) { t[2 * nt] = acc[nt][0]; t[2 * nt + 1] = acc[nt][1]; }
+                for (int nt = 0; nt < NT; nt++) {
+                    f[2 * nt] = ch ? f[2 * nt] * acc[nt][0] : acc[nt][0];
+                    f[2 * nt + 1] = ch ? f[2 * nt + 1] * acc[nt][1] : acc[nt][1];
+                }
             }
-#pragma unroll
-            for (int k = 0; k < S; k++) f[k] = ch ? f[k] * t[k] : t[k];
         }
         // all values are >= 0: the largest has the largest high word; 4 lanes hold a pattern's K states
         int hmax = 0;
@@ -122,9 +169,12 @@ __global__ void __launch_bounds__(MMA_T) prune_mma_kernel(const PruneOp* __restr
             if (e > -1000 && hmax < 0x7fe00000) { sc = pow2_neg(e); ex += e; }
         }
         if (live) {
-            double* dst = partials + ((size_t)op.pidx * C + c) * LK + (size_t)p * KP + q * S;
+            double* dst = partials + ((size_t)op.pidx * C + c) * LK + (size_t)p * KP + q * VW;
 #pragma unroll
-            for (int k = 0; k < S; k += 2) *reinterpret_cast<double2*>(dst + k) = make_double2(f[k] * sc, f[k + 1] * sc);
+            for (int m = 0; m < NC; m++) {
+                if (VW == 4) st256(dst + m * 16, f[4 * m] * sc, f[4 * m + 1] * sc, f[4 * m + 2] * sc, f[4 * m + 3] * sc);
+                else *reinterpret_cast<double2*>(dst + m * 8) = make_double2(f[2 * m] * sc, f[2 * m + 1] * sc);
+            }
             if (q == 0) scale_exp[((size_t)op.pidx * C + c) * L + p] = ex;
         }
     }
@@ -143,8 +193,8 @@ template <int KP>
 void mma_launch(const epx_ctx* c, const PruneOp* ops, int nops, cudaStream_t s)
 {
     const DevBuffers& d = c->d;
-    const int chunk_p = prune_mma_chunk(c), chunks = (c->L + chunk_p - 1) / chunk_p;
-    prune_mma_kernel<KP><<<nops * c->C * chunks, MMA_T, mma_smem<KP>(), s>>>(ops, chunks, chunk_p, c->K, c->C, c->L, c->Lp, d.P, d.PB,
+    const int chunk_p = prune_mma_chunk(c, nops), chunks = (c->L + chunk_p - 1) / chunk_p;
+    prune_mma_kernel<KP><<<nops * c->C * chunks, MMA_T, mma_smem<KP>(), s>>>(ops, chunks, chunk_p, c->K, c->C, c->L, c->Lp, d.PB,
                                                                              d.tips, d.partials, d.scale_exp);
 }
 
@@ -152,15 +202,18 @@ template <int KP>
 void swz_launch(const epx_ctx* c, cudaStream_t s)
 {
     const int n = c->sub_list ? c->sub_count : c->n_slots;
-    if (n > 0) pb_swizzle_kernel<KP><<<n * c->C, 256, 0, s>>>(c->K, c->C, c->sub_list, c->d.P, c->d.PB);
+    if (n > 0) pb_swizzle_kernel<KP><<<n * c->C, 256, 0, s>>>(c->K, c->C, c->N, c->d.tip_vec, c->sub_list, c->d.P, c->d.PB);
 }
 
 }  // namespace
 
-int prune_mma_chunk(const epx_ctx* c)
+// Site patterns per CTA for a level of `nops` operations: 64 (one 8-pattern tile per warp) unless the level then has more
+// than ~4 waves of CTAs, where a CTA loops over 128 or 256 patterns with its staged matrices.
+int prune_mma_chunk(const epx_ctx* c, int nops)
 {
     if (c->mma_chunk > 0) return (c->mma_chunk + 7) & ~7;
-    return 64;
+    const long ctas64 = (long)nops * c->C * ((c->L + 63) / 64);
+    return ctas64 > 8 * 296 ? 256 : ctas64 > 4 * 296 ? 128 : 64;
 }
 
 int prune_mma_init_attributes()

@@ -247,7 +247,7 @@ def test_incremental_reevaluation(epx, orc_ld, cid, kw, opts):
         ctx.set_node_heights(nodes, new_h)
         lnl = ctx.log_likelihood_incremental()
         used = ctx.launch_count() - n0
-        full_cost = 10 if (prob.K == 4 and not opts) else 3 + 2 + 2 + ctx.tree_levels()
+        full_cost = 10 if (prob.K == 4 and not opts) else 3 + 2 + 2 + ctx.tree_levels() + 1     # (+1: fragment-order copies)
         if prob.K == 4 and (not opts or opts[0][0] == 6 or opts[0] == (3, 5)):
             assert used == 3 + 1 + 1 + 2            # segmenter, chain, ONE pruning walk over the dirty path, root
         else:

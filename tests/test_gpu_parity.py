@@ -200,6 +200,10 @@ def test_config3_reduced(epx, orc_ld):
     prob = W.make_config(3, N=12, L=70)
     run_tree(epx, orc_ld, prob)     # auto: componentwise (shifted Taylor) exponentials, A21; DMMA pruning
     run_tree(epx, orc_ld, prob, options=[(epx.EPX_OPT_PRUNE_KERNEL, 1)])      # scalar shared-memory pruning kernel
+    run_tree(epx, orc_ld, prob, options=[(epx.EPX_OPT_MMA_CHUNK, 8)])         # one 8-pattern tile per CTA, 7 idle warps
+    run_tree(epx, orc_ld, prob, options=[(epx.EPX_OPT_MMA_CHUNK, 200)])       # a CTA loops over its chunk
+    for kernel in (4, 6):                                                     # round 1's tensor-pipe level kernels
+        run_tree(epx, orc_ld, prob, options=[(epx.EPX_OPT_PRUNE_KERNEL, kernel)])
     # The spectral path (Jacobi + eigenbasis chain; DMMA and generic kernels) meets the 1e-12 absolute bound on P, but
     # its ~1e-14 absolute error swamps the entries of order t^3 that decide codon likelihoods on short branches:
     # matrices only.
