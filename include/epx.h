@@ -179,7 +179,7 @@ int epx_get_stage_ms(epx_ctx* ctx, float* ms, int* launches);
  * compiler from deleting the arithmetic).  Synchronises the stream. */
 int epx_measure_fp64_peak(int device, int kind, double ms_target, void* dev_scratch, void* cuda_stream, double* tflops);
 
-/* ---- tuning / test hooks (options 1-3, 6-8 have no effect on results) ---- */
+/* ---- tuning / test hooks (options 1-3, 6-8 have no effect on results; 9 only within rounding) ---- */
 enum {
     EPX_OPT_CHAIN_KERNEL = 1, /* 0 auto (default); 1 force the generic shared-memory chain kernel */
     EPX_OPT_USE_GRAPH = 2,    /* 1 (default) replay the kernel sequence from a CUDA graph on non-default streams; 0 launch directly */
@@ -201,7 +201,8 @@ enum {
     EPX_OPT_DFS_PPL = 6,      /* K == 4 depth-first pruning: site patterns per lane, 1, 2 or 4 (4: kernel 5 only); 0 (default) auto */
     EPX_OPT_DFS_PIECES = 7,   /* depth-first pruning: number of pieces the tree is cut into (independent subtrees walked by
                                  different warps + the part above them); 0 (default) auto */
-    EPX_OPT_MMA_CHUNK = 8     /* 8 < K <= 64 tensor-pipe level kernel: site patterns per CTA (rounded up to 8); 0 (default) auto */
+    EPX_OPT_MMA_CHUNK = 8,    /* 8 < K <= 64 tensor-pipe level kernel: site patterns per CTA (rounded up to 8); 0 (default) auto */
+    EPX_OPT_JACOBI_KERNEL = 9 /* a2: 0 (default) the one-barrier-per-round Jacobi for K <= 62; 1 round 1's two-barrier kernel */
 };
 int epx_set_option(epx_ctx* ctx, int option, int value);
 /* Device status word of the last compute call (0 = all numeric checks passed); synchronises. */

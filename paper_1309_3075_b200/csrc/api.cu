@@ -393,6 +393,7 @@ int epx_set_option(epx_ctx* c, int option, int value)
             c->dfs_ppl = value;
             if (c->has_tree) { int rc = build_plan(c); if (rc) return rc; c->tree_dirty = true; }
             break;
+        case 9: c->jacobi_kernel = value ? 1 : 0; break;
         case 8:
             if (value < 0 || value > (1 << 20)) return fail(c, EPX_E_ARG, "chunk %d", value);
             c->mma_chunk = value;

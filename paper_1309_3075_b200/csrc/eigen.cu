@@ -158,6 +158,199 @@ __global__ void __launch_bounds__(JT_MAX) jacobi_kernel(int K, int Kp, const dou
     }
 }
 
+// ------------------------------------------------------------------------------------------------ K <= 62: one barrier per round
+// The same two-sided round-robin Jacobi, reorganised so that a round costs ONE barrier and no index arithmetic (the kernel
+// above spends 221 instructions per warp and round, half of them on indices, and its 16 CTAs were 15 % of config 5's step):
+//   * the players are kept physically in pairing order: pair a = rows / columns 2a, 2a+1.  After a round the tournament
+//     rotates by a FIXED permutation (player at position p moves to newpos(p)), so thread (a, b) always reads the 2x2 block
+//     at the same addresses of the current buffer and writes its rotated block to the same four addresses of the other
+//     buffer (ping-pong): every address is a per-thread constant.  V's columns travel with the players.
+//   * the rotation of a NEW pair j needs three entries of the updated matrix (two diagonal ones, the new pivot).  A spare
+//     warp computes them directly from the OLD matrix and the OLD rotations (closed forms of the 2x2 updates) while the
+//     other warps update S and V, so the next round's rotations are ready at the same barrier.
+//   * an odd K gets a dummy player whose row and column stay zero (its rotations are the identity).
+// After every sweep (n - 1 rounds) the players are back in their original order.
+__device__ __forceinline__ int jac_newpos(int pos, int m)
+{
+    if (pos == 0 || m == 1) return pos;
+    const int k = pos >> 1;
+    if ((pos & 1) == 0) return k <= m - 2 ? 2 * k + 2 : 2 * m - 1;       // top row moves right, its last player drops down
+    return k == 0 ? 2 : 2 * k - 1;                                       // bottom row moves left, its first player goes up
+}
+
+__device__ __forceinline__ double2 jac_rotation(double spp, double sqq, double apq)
+{
+    double c = 1.0, s = 0.0;
+    if (fabs(apq) > 1e-300) {
+        // t = tan of the rotation angle, the root of smaller magnitude of t^2 + 2 theta t - 1 = 0 with theta = d / h
+        const double d = sqq - spp, h = 2.0 * apq;
+        const double r2 = fma(d, d, h * h);
+        const double r = r2 * rsqrt(r2);
+        const double t = (d < 0 ? -h : h) / (fabs(d) + r);
+        c = rsqrt(fma(t, t, 1.0));
+        s = t * c;
+    }
+    return make_double2(c, s);
+}
+
+__global__ void __launch_bounds__(1024) jacobi1_kernel(int K, int Kp, const double* __restrict__ Qall,
+                                                       const double* __restrict__ freqs, double* __restrict__ lam,
+                                                       double* __restrict__ Uout, double* __restrict__ sp_out,
+                                                       double* __restrict__ isp_out, int32_t* __restrict__ status)
+{
+    extern __shared__ __align__(16) double sm[];
+    const int m = (K + 1) >> 1, n = 2 * m;              // pairs, players
+    const int NB = blockDim.x - 32;                     // block / V threads; the last warp prepares the rotations
+    const int nn = n * n, kn = K * n;
+    double* const S0 = sm;                              // [2][n][n] ping-pong
+    double* const V0 = S0 + 2 * nn;                     // [2][K][n] ping-pong
+    double2* const R0 = reinterpret_cast<double2*>(V0 + 2 * kn);                          // [2][m] (cos, sin)
+    double* const red = reinterpret_cast<double*>(R0 + 2 * m);                            // [33]
+    const int e = blockIdx.x, tid = threadIdx.x, T = blockDim.x;
+    const double* Q = Qall + (size_t)e * K * K;
+    const double* pi = freqs + (size_t)e * K;
+
+    for (int idx = tid; idx < n * n; idx += T) {
+        const int i = idx / n, j = idx - i * n;
+        double v = 0.0;
+        if (i < K && j < K) {
+            const double a = sqrt(pi[i]) * Q[i * K + j] / sqrt(pi[j]);
+            const double b = sqrt(pi[j]) * Q[j * K + i] / sqrt(pi[i]);
+            v = 0.5 * (a + b);
+        }
+        S0[idx] = v;
+    }
+    for (int idx = tid; idx < K * n; idx += T) { const int i = idx / n, j = idx - i * n; V0[idx] = (i == j) ? 1.0 : 0.0; }
+    __syncthreads();
+    auto block_sum = [&](double v) -> double {          // all threads call
+        for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
+        if ((tid & 31) == 0) red[tid >> 5] = v;
+        __syncthreads();
+        double t = 0;
+        for (int w = 0; w < T / 32; w++) t += red[w];
+        __syncthreads();
+        return t;
+    };
+    double tot2;
+    {
+        double t = 0;
+        for (int idx = tid; idx < n * n; idx += T) { const double x = S0[idx]; t += x * x; }
+        tot2 = block_sum(t);
+    }
+
+    // per-thread constants
+    const bool is_blk = tid < m * m;
+    const int a = is_blk ? tid / m : 0, b = is_blk ? tid - a * m : 0;
+    const int rd0 = (2 * a) * n + 2 * b, rd1 = rd0 + n;
+    const int na0 = jac_newpos(2 * a, m) * n, na1 = jac_newpos(2 * a + 1, m) * n;
+    const int nb0 = jac_newpos(2 * b, m), nb1 = jac_newpos(2 * b + 1, m);
+    int v_rd[2], v_w0[2], v_w1[2], v_k[2];
+#pragma unroll
+    for (int u = 0; u < 2; u++) {
+        const int t = tid + u * NB;
+        const bool on = tid < NB && t < K * m;
+        const int i = on ? t / m : 0, k = on ? t - i * m : 0;
+        v_k[u] = on ? k : -1;
+        v_rd[u] = i * n + 2 * k;
+        v_w0[u] = i * n + jac_newpos(2 * k, m);
+        v_w1[u] = i * n + jac_newpos(2 * k + 1, m);
+    }
+    // rotation warp, lane j < m: the players that form NEW pair j sit at old positions x (top) and y (bottom)
+    const int j = tid - NB;
+    const bool is_rot = j >= 0 && j < m;
+    int x = 0, y = 1;
+    if (is_rot)
+        for (int p = 0; p < n; p++) {
+            const int q = jac_newpos(p, m);
+            if (q == 2 * j) x = p;
+            if (q == 2 * j + 1) y = p;
+        }
+    const int ax = x >> 1, ay = y >> 1, px = x & 1, py = y & 1;
+
+    if (is_rot) R0[j] = jac_rotation(S0[(2 * j) * n + 2 * j], S0[(2 * j + 1) * n + 2 * j + 1], S0[(2 * j) * n + 2 * j + 1]);
+    __syncthreads();
+
+    int cur = 0;
+    bool converged = false;
+    double off2 = 0.0;
+    for (int sweep = 0; sweep < 40 && !converged; sweep++) {
+        double my_off = 0.0;
+        for (int r = 0; r < n - 1; r++) {
+            const double* S = S0 + cur * nn;
+            double* Sn = S0 + (cur ^ 1) * nn;
+            const double2* R = R0 + cur * m;
+            if (is_blk) {
+                const double2 ra = R[a], rb = R[b];
+                const double2 x0 = *reinterpret_cast<const double2*>(S + rd0), x1 = *reinterpret_cast<const double2*>(S + rd1);
+                // columns (pair b), then rows (pair a): S <- J^T S J on this 2x2 block
+                const double t00 = rb.x * x0.x - rb.y * x0.y, t01 = rb.y * x0.x + rb.x * x0.y;
+                const double t10 = rb.x * x1.x - rb.y * x1.y, t11 = rb.y * x1.x + rb.x * x1.y;
+                double y00 = ra.x * t00 - ra.y * t10, y01 = ra.x * t01 - ra.y * t11;
+                double y10 = ra.y * t00 + ra.x * t10, y11 = ra.y * t01 + ra.x * t11;
+                if (a == b) { y01 = 0.0; y10 = 0.0; }            // the pivot pair is annihilated exactly
+                Sn[na0 + nb0] = y00; Sn[na0 + nb1] = y01; Sn[na1 + nb0] = y10; Sn[na1 + nb1] = y11;
+                if (r == n - 2) my_off = a == b ? 0.0 : fma(y00, y00, fma(y01, y01, fma(y10, y10, y11 * y11)));
+            }
+            if (tid < NB) {
+                const double* V = V0 + cur * kn;
+                double* Vn = V0 + (cur ^ 1) * kn;
+#pragma unroll
+                for (int u = 0; u < 2; u++)
+                    if (v_k[u] >= 0) {
+                        const double2 rk = R[v_k[u]];
+                        const double2 v = *reinterpret_cast<const double2*>(V + v_rd[u]);
+                        Vn[v_w0[u]] = rk.x * v.x - rk.y * v.y;
+                        Vn[v_w1[u]] = rk.y * v.x + rk.x * v.y;
+                    }
+            } else if (is_rot) {
+                double2 nr = make_double2(1.0, 0.0);
+                if (ax != ay) {
+                    const double2 ra = R[ax], rb = R[ay];
+                    const double app = S[(2 * ax) * n + 2 * ax], apq = S[(2 * ax) * n + 2 * ax + 1], aqq = S[(2 * ax + 1) * n + 2 * ax + 1];
+                    const double bpp = S[(2 * ay) * n + 2 * ay], bpq = S[(2 * ay) * n + 2 * ay + 1], bqq = S[(2 * ay + 1) * n + 2 * ay + 1];
+                    const double2 x0 = *reinterpret_cast<const double2*>(S + (2 * ax) * n + 2 * ay);
+                    const double2 x1 = *reinterpret_cast<const double2*>(S + (2 * ax + 1) * n + 2 * ay);
+                    // the player's updated diagonal entry: (J^T S J)_pp = c^2 Spp - 2 c s Spq + s^2 Sqq, _qq = s^2 Spp + 2 c s Spq + c^2 Sqq
+                    const double ca2 = ra.x * ra.x, sa2 = ra.y * ra.y, csa = 2.0 * ra.x * ra.y;
+                    const double cb2 = rb.x * rb.x, sb2 = rb.y * rb.y, csb = 2.0 * rb.x * rb.y;
+                    const double dx = px ? fma(sa2, app, fma(csa, apq, ca2 * aqq)) : fma(ca2, app, fma(-csa, apq, sa2 * aqq));
+                    const double dy = py ? fma(sb2, bpp, fma(csb, bpq, cb2 * bqq)) : fma(cb2, bpp, fma(-csb, bpq, sb2 * bqq));
+                    // the new pivot = entry (px, py) of the updated block (ax, ay)
+                    const double t0 = py ? rb.y * x0.x + rb.x * x0.y : rb.x * x0.x - rb.y * x0.y;
+                    const double t1 = py ? rb.y * x1.x + rb.x * x1.y : rb.x * x1.x - rb.y * x1.y;
+                    const double piv = px ? ra.y * t0 + ra.x * t1 : ra.x * t0 - ra.y * t1;
+                    nr = jac_rotation(dx, dy, piv);
+                }
+                R0[(cur ^ 1) * m + j] = nr;
+            }
+            __syncthreads();
+            cur ^= 1;
+        }
+        off2 = block_sum(my_off);
+        converged = off2 <= 0.25 * 2.220446049250313e-16 * 2.220446049250313e-16 * tot2;
+    }
+    if (tid == 0 && !(off2 <= 1e-28 * tot2)) atomicOr(status, EPX_ST_JACOBI_NOCONV);
+
+    const double* S = S0 + cur * nn;
+    const double* V = V0 + cur * kn;
+    double* U = Uout + (size_t)e * Kp * Kp;
+    for (int idx = tid; idx < Kp * Kp; idx += T) {
+        const int i = idx / Kp, jj = idx % Kp;
+        U[idx] = (i < K && jj < K) ? V[i * n + jj] : 0.0;
+    }
+    for (int i = tid; i < Kp; i += T) {
+        lam[(size_t)e * Kp + i] = i < K ? S[i * n + i] : 0.0;
+        sp_out[(size_t)e * Kp + i] = i < K ? sqrt(pi[i]) : 0.0;
+        isp_out[(size_t)e * Kp + i] = i < K ? 1.0 / sqrt(pi[i]) : 0.0;
+    }
+}
+
+size_t jacobi1_smem(int K)
+{
+    const size_t m = (K + 1) / 2, n = 2 * m;
+    return sizeof(double) * (2 * n * n + 2 * (size_t)K * n + 4 * m + 34) + 16;
+}
+
 constexpr int JT = 256;   // threads per CTA of the prep kernels
 
 // W_e[a][b] = sum_k U_e[k][a] * sqrt(pi_e[k] / pi_{e-1}[k]) * U_{e-1}[k][b]   (e >= 1)
@@ -237,6 +430,7 @@ __global__ void __launch_bounds__(JT) prep64_kernel(const double* __restrict__ U
 
 int eigen_init_attributes()
 {
+    if (cudaFuncSetAttribute(jacobi1_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)jacobi1_smem(62)) != cudaSuccess) return -1;
     return cudaFuncSetAttribute(jacobi_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, 96 * 1024) == cudaSuccess ? 0 : -1;
 }
 
@@ -246,7 +440,12 @@ int launch_eigensystems(const epx_ctx* c, cudaStream_t s)
     const int K = c->K, Kp = c->Kp;
     const int ld = K | 1;
     size_t smem = sizeof(double) * (2 * (size_t)K * ld + 2 * (K / 2 + 1) + 32) + sizeof(int) * 2 * (K / 2 + 1);
-    jacobi_kernel<<<c->M, K > 32 ? JT_MAX : 256, smem, s>>>(K, Kp, d.Q, d.freqs, d.lam, d.U, d.sp, d.isp, d.status);
+    if (K <= 62 && c->jacobi_kernel == 0) {
+        const int m = (K + 1) / 2;
+        jacobi1_kernel<<<c->M, ((m * m + 31) & ~31) + 32, jacobi1_smem(K), s>>>(K, Kp, d.Q, d.freqs, d.lam, d.U, d.sp, d.isp, d.status);
+    } else {
+        jacobi_kernel<<<c->M, K > 32 ? JT_MAX : 256, smem, s>>>(K, Kp, d.Q, d.freqs, d.lam, d.U, d.sp, d.isp, d.status);
+    }
     if (Kp == 64) prep64_kernel<<<dim3(c->M, 8), JT, 0, s>>>(d.U, d.sp, d.isp, d.W, d.WB, d.UTB);
     else prep_kernel<<<c->M, JT, 0, s>>>(Kp, d.U, d.sp, d.isp, d.W, d.WB, d.UTB);
     return cudaGetLastError() == cudaSuccess ? 2 : -1;

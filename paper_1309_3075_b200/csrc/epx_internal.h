@@ -118,6 +118,7 @@ struct epx_ctx {
     int prune_kernel = 0;  // EPX_OPT_PRUNE_KERNEL: 0 auto, 1 force the generic shared-memory kernel
     int dfs_ppl = 0;       // EPX_OPT_DFS_PPL: patterns per lane of the depth-first pruning walk (0 auto, 1, 2, 4)
     int dfs_want = 0;      // EPX_OPT_DFS_PIECES: pieces the tree is cut into for the depth-first walks (0 auto)
+    int jacobi_kernel = 0; // EPX_OPT_JACOBI_KERNEL: 0 auto (K <= 62: one barrier per round), 1 round 1's two-barrier kernel
     int mma_chunk = 0;     // EPX_OPT_MMA_CHUNK: site patterns per CTA of the tensor-pipe level kernel (0 auto)
     int exp_method = 0;    // EPX_OPT_EXP_METHOD: 0 auto, 1 spectral (Jacobi / Pade), 2 componentwise (shifted Taylor)
     std::vector<char> model_sparse;   // per epoch: Q has a structural zero off the diagonal

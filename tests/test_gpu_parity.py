@@ -234,9 +234,10 @@ def test_config4_full_size(epx, orc_ld):
 
 def test_config5_reduced_every_branch(epx, orc_ld):
     prob = W.make_config(5, n_br=300)
-    for kernel in (0, 1):
+    for kernel, jacobi in ((0, 0), (1, 0), (0, 1)):        # DMMA / generic chain kernel; one-barrier / round-1 Jacobi
         ctx = epx.from_problem(prob)
         ctx.set_option(epx.EPX_OPT_CHAIN_KERNEL, kernel)
+        ctx.set_option(epx.EPX_OPT_JACOBI_KERNEL, jacobi)
         ctx.update_matrices()
         ref = orc_ld.evaluate(prob)
         check_segments(ctx, ref)
