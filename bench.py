@@ -37,8 +37,8 @@ import workloads as W  # noqa: E402  (input generators only; shared with the ora
 
 # dram__bytes_read.sum + dram__bytes_write.sum of the pruning launches of one config-2 step, from the committed
 # `ncu --set full` capture named here (re-captured whenever the pruning kernel changes; `--traffic` overrides it)
-NCU_TRAFFIC = {"bytes_per_step": 2.6091e9, "profile": "profiles/r1_prune4_dfs_ncu.md", "commit": "6984e86",
-               "kernel": "prune4_dfs_kernel<4, 2> + <4, 1>"}
+NCU_TRAFFIC = {"bytes_per_step": 2.6018e9, "profile": "profiles/r2_prune4_lane_ncu.md", "commit": "00f37ea",
+               "kernel": "prune4_lane_kernel<4, 1, false> + <4, 1, true>"}
 
 METRIC = "pruning partials GB/s (fp64) over the whole a1..a6 log-likelihood step; epoch branch matrices/s in `matrices`"
 UNIT = "GB/s"
@@ -572,13 +572,14 @@ def bench_matrices(torch, epx, device: int, K: int, peaks: dict, options=(), lab
 
 
 def bench_other_configs(torch, epx, device: int, K: int, peaks: dict) -> dict:
-    """Configs 1, 3 and 4 (BASELINE.json; PAPER.md:L224 names the shapes of 3 and 4): whole a1..a6 step on the device, per-stage
-    CUDA-event times, launches.  Config 3's pruning and chain kernels get an `alu` roofline against the fp64 peak measured
-    in this run; configs 1 and 4 are latency-bound: time, tree levels and the dependent-operation chain."""
+    """Configs 1, 3 and 4 (BASELINE.json; PAPER.md:L224 names the shapes of 3 and 4) and the 20-state amino-acid workload of
+    SURVEY.md 8(f) f3 ("config 6"): whole a1..a6 step on the device, per-stage CUDA-event times, launches.  The pruning kernels of
+    configs 3 and 6 (and config 3's chain kernel) get an `alu` roofline against the fp64 peak measured in this run; configs 1
+    and 4 are latency-bound: time, tree levels and the dependent-operation chain."""
     out = {}
     clocks = ClockSampler(device)
     clocks.start()
-    for cid in (1, 3, 4):
+    for cid in (1, 3, 4, 6):
         prob = W.make_config(cid)
         ctx = epx.from_problem(prob, device=device)
         ctx.set_option(epx.EPX_OPT_STAGE_EVENTS, 1)
@@ -602,17 +603,20 @@ def bench_other_configs(torch, epx, device: int, K: int, peaks: dict) -> dict:
         o = {"config": workload_config(prob, cid, 1), "ms_per_step": ms, "steps": steps, "gpu_launches_per_step": int(launches),
              "log_likelihood": lnl, "stage_ms": {n: float(v) for n, v in zip(epx.STAGE_NAMES, stage)},
              "stage_launches": {n: int(v) for n, v in zip(epx.STAGE_NAMES, sl)}, "plan": plan}
-        if cid == 3:
+        if cid in (3, 6):
             Kc, C, L, n_int = prob.K, prob.C, prob.L, prob.N - 1
             pf = n_int * C * L * (4 * Kc * Kc + Kc)              # O(K^2 N C L) with both children counted
             prune_ms, chain_ms = float(stage[3]), float(stage[2])
-            tf = taylor_chain_flops(prob)
-            o["roofline_prune"] = {"bound": "alu", "kernel": PRUNE64_KERNEL_NAME + " (a5, 61 states on the FP64 tensor pipe)",
+            kp = (Kc + 7) // 8 * 8
+            o["roofline_prune"] = {"bound": "alu", "kernel": "prune_mma_kernel<%d> + pb_swizzle_kernel<%d> (a5, %d states padded to %d "
+                                                             "on the FP64 tensor pipe)" % (kp, kp, Kc, kp),
                                    "achieved": pf / (prune_ms * 1e-3) / 1e12, "peak": peaks["dmma"], "unit": "TFLOP/s",
                                    "frac": pf / (prune_ms * 1e-3) / 1e12 / peaks["dmma"], "traffic": None, "flops": pf,
-                                   "flops_definition": "n_int C L (4 K^2 + K), K = 61 (tip children counted like internal ones)",
+                                   "flops_definition": "n_int C L (4 K^2 + K), K = %d (tip children counted like internal ones)" % Kc,
                                    "peak_source": "DMMA m8n8k4 register-only loop measured in this run",
                                    "launches": int(sl[3]), "avg_launch_ms": prune_ms / max(1, int(sl[3]))}
+        if cid == 3:
+            tf = taylor_chain_flops(prob)
             o["roofline_chain"] = {"bound": "alu", "kernel": "pade_chain_kernel<1> + pade_full_epoch_kernel<1> (a3+a4, "
                                                              "componentwise Taylor exponentials, reading A21)",
                                    "achieved": tf["flops"] / (chain_ms * 1e-3) / 1e12, "peak": peaks["dmma"], "unit": "TFLOP/s",
@@ -629,7 +633,6 @@ def bench_other_configs(torch, epx, device: int, K: int, peaks: dict) -> dict:
     return out
 
 
-PRUNE64_KERNEL_NAME = "prune_mma_kernel<64> (+ pb_swizzle_kernel<64>)"
 
 
 def parse_opts(text: str):

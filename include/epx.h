@@ -73,6 +73,12 @@ int epx_set_epoch_boundaries(epx_ctx* ctx, const double* tau);
  * off-diagonals >= 0.  freqs: K, >= 0, sum 1.  reversible = 1 selects the Jacobi path and requires pi_i > 0 and
  * |pi_i q_ij - pi_j q_ji| <= 1e-9 max|pi q|; 0 selects Pade.  All epochs of a ctx must use the same flag. */
 int epx_set_epoch_model(epx_ctx* ctx, int epoch, const double* Q, const double* freqs, int reversible);
+/* Shared processes (S processes Q_s, M epochs, phi_m in 1..S picks the process active in epoch m; L193, L203:
+ * 13-14 epochs alternating 2 or 4 matrices).  Models are set per epoch; epochs whose Q and freqs are bit-identical are
+ * detected and share ONE eigensystem (and one full-epoch exponential per distinct duration on the Pade path).  This call
+ * reports the detected map: phi[e] in 0..*n_processes-1, numbered by first appearance (phi: M entries).  Needs every epoch
+ * model set.  Sharing never changes results (EPX_OPT_SHARE_PROCESSES = 0 computes one per epoch: bit-identical). */
+int epx_epoch_processes(epx_ctx* ctx, int32_t* phi, int* n_processes);
 /* rates: C, >= 0 (the r_c of Eq. 3, A6).  weights: C, >= 0, sum 1. */
 int epx_set_category_rates(epx_ctx* ctx, const double* rates, const double* weights);
 
@@ -179,7 +185,7 @@ int epx_get_stage_ms(epx_ctx* ctx, float* ms, int* launches);
  * compiler from deleting the arithmetic).  Synchronises the stream. */
 int epx_measure_fp64_peak(int device, int kind, double ms_target, void* dev_scratch, void* cuda_stream, double* tflops);
 
-/* ---- tuning / test hooks (options 1-3, 6-8 have no effect on results; 9 only within rounding) ---- */
+/* ---- tuning / test hooks (options 1-3, 6-8, 10 have no effect on results; 9 only within rounding) ---- */
 enum {
     EPX_OPT_CHAIN_KERNEL = 1, /* 0 auto (default); 1 force the generic shared-memory chain kernel */
     EPX_OPT_USE_GRAPH = 2,    /* 1 (default) replay the kernel sequence from a CUDA graph on non-default streams; 0 launch directly */
@@ -202,7 +208,9 @@ enum {
     EPX_OPT_DFS_PIECES = 7,   /* depth-first pruning: number of pieces the tree is cut into (independent subtrees walked by
                                  different warps + the part above them); 0 (default) auto */
     EPX_OPT_MMA_CHUNK = 8,    /* 8 < K <= 64 tensor-pipe level kernel: site patterns per CTA (rounded up to 8); 0 (default) auto */
-    EPX_OPT_JACOBI_KERNEL = 9 /* a2: 0 (default) the one-barrier-per-round Jacobi for K <= 62; 1 round 1's two-barrier kernel */
+    EPX_OPT_JACOBI_KERNEL = 9, /* a2: 0 (default) the one-barrier-per-round Jacobi for K <= 62; 1 round 1's two-barrier kernel */
+    EPX_OPT_SHARE_PROCESSES = 10 /* 1 (default) one eigensystem / full-epoch exponential per distinct process (epx_epoch_processes);
+                                 0 one per epoch */
 };
 int epx_set_option(epx_ctx* ctx, int option, int value);
 /* Device status word of the last compute call (0 = all numeric checks passed); synchronises. */

@@ -19,6 +19,7 @@ LIB_PATH = os.path.join(_HERE, "libepx.so")
 EPX_OK, EPX_E_ARG, EPX_E_STATE, EPX_E_TREE, EPX_E_MODEL, EPX_E_WORKSPACE, EPX_E_CUDA, EPX_E_NUMERIC = 0, -1, -2, -3, -4, -5, -6, -7
 EPX_OPT_CHAIN_KERNEL, EPX_OPT_USE_GRAPH, EPX_OPT_PRUNE_KERNEL, EPX_OPT_EXP_METHOD = 1, 2, 3, 4
 EPX_OPT_STAGE_EVENTS, EPX_OPT_DFS_PPL, EPX_OPT_DFS_PIECES, EPX_OPT_MMA_CHUNK, EPX_OPT_JACOBI_KERNEL = 5, 6, 7, 8, 9
+EPX_OPT_SHARE_PROCESSES = 10
 STAGE_NAMES = ("segment", "eigen", "chain", "prune", "root")
 
 _lib = None
@@ -77,6 +78,7 @@ def lib():
     _sig(L, "epx_launch_count", i, vp, ct.POINTER(ct.c_longlong))
     _sig(L, "epx_tree_levels", i, vp, ct.POINTER(i))
     _sig(L, "epx_plan_info", i, vp, ip)
+    _sig(L, "epx_epoch_processes", i, vp, ip, ct.POINTER(i))
     _sig(L, "epx_get_stage_ms", i, vp, ct.c_void_p, ct.c_void_p)
     _sig(L, "epx_status", i, vp, ct.POINTER(i))
     _sig(L, "epx_set_option", i, vp, i, i)
@@ -315,6 +317,13 @@ class Epx:
         n = ct.c_int()
         self._check(self._L.epx_tree_levels(self._ctx, ct.byref(n)))
         return n.value
+
+    def epoch_processes(self):
+        """(phi[M], S): the detected process of every epoch and the number of distinct processes."""
+        phi = np.zeros(self.M, dtype=np.int32)
+        n = ct.c_int()
+        self._check(self._L.epx_epoch_processes(self._ctx, _ptr(phi), ct.byref(n)))
+        return phi, n.value
 
     def plan_info(self) -> dict:
         info = np.zeros(8, dtype=np.int32)

@@ -54,6 +54,8 @@ size_t plan_workspace(const epx_ctx* c, char* base, DevBuffers* d)
     t.rates = (double*)take(8 * C);
     t.weights = (double*)take(8 * C);
     t.root_freqs = (double*)take(8 * K);
+    t.eproc = (int32_t*)take(4 * M);
+    t.fproc = (int32_t*)take(4 * M);
     if (c->tree_mode) {
         t.parent = (int32_t*)take(4 * S);
         t.height = (double*)take(8 * S);
@@ -393,6 +395,7 @@ int epx_set_option(epx_ctx* c, int option, int value)
             c->dfs_ppl = value;
             if (c->has_tree) { int rc = build_plan(c); if (rc) return rc; c->tree_dirty = true; }
             break;
+        case 10: c->dedup = value ? 1 : 0; c->model_dirty = true; break;
         case 9: c->jacobi_kernel = value ? 1 : 0; break;
         case 8:
             if (value < 0 || value > (1 << 20)) return fail(c, EPX_E_ARG, "chunk %d", value);

@@ -22,9 +22,11 @@ constexpr int JT_MAX = 1024;   // threads per CTA for K > 32 (one 2x2 block of S
 __global__ void __launch_bounds__(JT_MAX) jacobi_kernel(int K, int Kp, const double* __restrict__ Qall,
                                                         const double* __restrict__ freqs, double* __restrict__ lam,
                                                         double* __restrict__ Uout, double* __restrict__ sp_out,
-                                                        double* __restrict__ isp_out, int32_t* __restrict__ status)
+                                                        double* __restrict__ isp_out, int32_t* __restrict__ status,
+                                                        int M, const int32_t* __restrict__ eproc)
 {
     extern __shared__ double sm[];
+    if (eproc[blockIdx.x] != (int)blockIdx.x) return;      // f2: this epoch shares the process of an earlier one
     const int JT = blockDim.x;
     const int ld = K | 1;                       // odd row stride: column walks are bank-conflict free
     double* S = sm;                             // [K][ld]
@@ -146,15 +148,18 @@ __global__ void __launch_bounds__(JT_MAX) jacobi_kernel(int K, int Kp, const dou
     }
     if (tid == 0 && !(s_off2 <= 1e-28 * s_tot2)) atomicOr(status, EPX_ST_JACOBI_NOCONV);
 
-    double* U = Uout + (size_t)e * Kp * Kp;
-    for (int idx = tid; idx < Kp * Kp; idx += JT) {
-        int i = idx / Kp, j = idx % Kp;
-        U[idx] = (i < K && j < K) ? V[i * ld + j] : 0.0;
-    }
-    for (int i = tid; i < Kp; i += JT) {
-        lam[(size_t)e * Kp + i] = i < K ? S[i * ld + i] : 0.0;
-        sp_out[(size_t)e * Kp + i] = i < K ? sqrt(pi[i]) : 0.0;
-        isp_out[(size_t)e * Kp + i] = i < K ? 1.0 / sqrt(pi[i]) : 0.0;
+    for (int f = e; f < M; f++) {             // every epoch of this process gets the eigensystem
+        if (eproc[f] != e) continue;
+        double* U = Uout + (size_t)f * Kp * Kp;
+        for (int idx = tid; idx < Kp * Kp; idx += JT) {
+            int i = idx / Kp, j = idx % Kp;
+            U[idx] = (i < K && j < K) ? V[i * ld + j] : 0.0;
+        }
+        for (int i = tid; i < Kp; i += JT) {
+            lam[(size_t)f * Kp + i] = i < K ? S[i * ld + i] : 0.0;
+            sp_out[(size_t)f * Kp + i] = i < K ? sqrt(pi[i]) : 0.0;
+            isp_out[(size_t)f * Kp + i] = i < K ? 1.0 / sqrt(pi[i]) : 0.0;
+        }
     }
 }
 
@@ -196,9 +201,11 @@ __device__ __forceinline__ double2 jac_rotation(double spp, double sqq, double a
 __global__ void __launch_bounds__(1024) jacobi1_kernel(int K, int Kp, const double* __restrict__ Qall,
                                                        const double* __restrict__ freqs, double* __restrict__ lam,
                                                        double* __restrict__ Uout, double* __restrict__ sp_out,
-                                                       double* __restrict__ isp_out, int32_t* __restrict__ status)
+                                                       double* __restrict__ isp_out, int32_t* __restrict__ status,
+                                                       int M, const int32_t* __restrict__ eproc)
 {
     extern __shared__ __align__(16) double sm[];
+    if (eproc[blockIdx.x] != (int)blockIdx.x) return;   // f2: this epoch shares the process of an earlier one
     const int m = (K + 1) >> 1, n = 2 * m;              // pairs, players
     const int NB = blockDim.x - 32;                     // block / V threads; the last warp prepares the rotations
     const int nn = n * n, kn = K * n;
@@ -333,15 +340,18 @@ __global__ void __launch_bounds__(1024) jacobi1_kernel(int K, int Kp, const doub
 
     const double* S = S0 + cur * nn;
     const double* V = V0 + cur * kn;
-    double* U = Uout + (size_t)e * Kp * Kp;
-    for (int idx = tid; idx < Kp * Kp; idx += T) {
-        const int i = idx / Kp, jj = idx % Kp;
-        U[idx] = (i < K && jj < K) ? V[i * n + jj] : 0.0;
-    }
-    for (int i = tid; i < Kp; i += T) {
-        lam[(size_t)e * Kp + i] = i < K ? S[i * n + i] : 0.0;
-        sp_out[(size_t)e * Kp + i] = i < K ? sqrt(pi[i]) : 0.0;
-        isp_out[(size_t)e * Kp + i] = i < K ? 1.0 / sqrt(pi[i]) : 0.0;
+    for (int f = e; f < M; f++) {             // every epoch of this process gets the eigensystem
+        if (eproc[f] != e) continue;
+        double* U = Uout + (size_t)f * Kp * Kp;
+        for (int idx = tid; idx < Kp * Kp; idx += T) {
+            const int i = idx / Kp, jj = idx % Kp;
+            U[idx] = (i < K && jj < K) ? V[i * n + jj] : 0.0;
+        }
+        for (int i = tid; i < Kp; i += T) {
+            lam[(size_t)f * Kp + i] = i < K ? S[i * n + i] : 0.0;
+            sp_out[(size_t)f * Kp + i] = i < K ? sqrt(pi[i]) : 0.0;
+            isp_out[(size_t)f * Kp + i] = i < K ? 1.0 / sqrt(pi[i]) : 0.0;
+        }
     }
 }
 
@@ -442,9 +452,9 @@ int launch_eigensystems(const epx_ctx* c, cudaStream_t s)
     size_t smem = sizeof(double) * (2 * (size_t)K * ld + 2 * (K / 2 + 1) + 32) + sizeof(int) * 2 * (K / 2 + 1);
     if (K <= 62 && c->jacobi_kernel == 0) {
         const int m = (K + 1) / 2;
-        jacobi1_kernel<<<c->M, ((m * m + 31) & ~31) + 32, jacobi1_smem(K), s>>>(K, Kp, d.Q, d.freqs, d.lam, d.U, d.sp, d.isp, d.status);
+        jacobi1_kernel<<<c->M, ((m * m + 31) & ~31) + 32, jacobi1_smem(K), s>>>(K, Kp, d.Q, d.freqs, d.lam, d.U, d.sp, d.isp, d.status, c->M, d.eproc);
     } else {
-        jacobi_kernel<<<c->M, K > 32 ? JT_MAX : 256, smem, s>>>(K, Kp, d.Q, d.freqs, d.lam, d.U, d.sp, d.isp, d.status);
+        jacobi_kernel<<<c->M, K > 32 ? JT_MAX : 256, smem, s>>>(K, Kp, d.Q, d.freqs, d.lam, d.U, d.sp, d.isp, d.status, c->M, d.eproc);
     }
     if (Kp == 64) prep64_kernel<<<dim3(c->M, 8), JT, 0, s>>>(d.U, d.sp, d.isp, d.W, d.WB, d.UTB);
     else prep_kernel<<<c->M, JT, 0, s>>>(Kp, d.U, d.sp, d.isp, d.W, d.WB, d.UTB);

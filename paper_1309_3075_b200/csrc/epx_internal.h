@@ -60,6 +60,8 @@ struct DevBuffers {
     double* rates;        // [C]
     double* weights;      // [C]
     double* root_freqs;   // [K] (valid iff has_root_freqs)
+    int32_t* eproc;       // [M] f2: first epoch with the same (Q, freqs) -- the process phi_m of PAPER.md L78; eproc[e] <= e
+    int32_t* fproc;       // [M] first interior epoch with the same process AND the same duration tau_e - tau_{e-1} (full-epoch table)
     int32_t* parent;      // [n_nodes] tree mode
     double* height;       // [n_nodes] tree mode
     double* child_h;      // [n_br] branch-list mode
@@ -118,6 +120,8 @@ struct epx_ctx {
     int prune_kernel = 0;  // EPX_OPT_PRUNE_KERNEL: 0 auto, 1 force the generic shared-memory kernel
     int dfs_ppl = 0;       // EPX_OPT_DFS_PPL: patterns per lane of the depth-first pruning walk (0 auto, 1, 2, 4)
     int dfs_want = 0;      // EPX_OPT_DFS_PIECES: pieces the tree is cut into for the depth-first walks (0 auto)
+    int dedup = 1;         // EPX_OPT_SHARE_PROCESSES: 1 (default) one eigensystem / table entry per distinct process, 0 one per epoch
+    std::vector<int32_t> eproc, fproc;   // host copies of the maps above (rebuilt when a model or a boundary changes)
     int jacobi_kernel = 0; // EPX_OPT_JACOBI_KERNEL: 0 auto (K <= 62: one barrier per round), 1 round 1's two-barrier kernel
     int mma_chunk = 0;     // EPX_OPT_MMA_CHUNK: site patterns per CTA of the tensor-pipe level kernel (0 auto)
     int exp_method = 0;    // EPX_OPT_EXP_METHOD: 0 auto, 1 spectral (Jacobi / Pade), 2 componentwise (shifted Taylor)

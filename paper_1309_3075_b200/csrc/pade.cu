@@ -239,19 +239,23 @@ __device__ __forceinline__ void carve(int K, double* sm, PadeBufs& b, double*& a
 template <int METHOD>
 __global__ void __launch_bounds__(PT) pade_full_epoch_kernel(int K, int M, int C, const double* __restrict__ Q,
     const double* __restrict__ tau, const double* __restrict__ rates, double* __restrict__ Efull,
-    int32_t* __restrict__ status)
+    int32_t* __restrict__ status, const int32_t* __restrict__ fproc)
 {
     extern __shared__ double sm[];
     PadeBufs b; double* acc;
     carve(K, sm, b, acc);
     const int e = 1 + blockIdx.x / C, c = blockIdx.x % C;    // interior epochs 1 .. M-2
+    if (fproc[e] != e) return;                               // f2: same process and duration as an earlier epoch
     const double scale = rates[c] * (tau[e] - tau[e - 1]);
     const double* Qe = Q + (size_t)e * K * K;
     for (int idx = threadIdx.x; idx < K * K; idx += PT) b.A[idx] = Qe[idx] * scale;
     __syncthreads();
     double* R = expm_dense<METHOD>(K, b, status);
-    double* out = Efull + ((size_t)e * C + c) * K * K;
-    for (int idx = threadIdx.x; idx < K * K; idx += PT) out[idx] = R[idx];
+    for (int f = e; f <= M - 2; f++) {                       // every epoch that shares this entry
+        if (fproc[f] != e) continue;
+        double* out = Efull + ((size_t)f * C + c) * K * K;
+        for (int idx = threadIdx.x; idx < K * K; idx += PT) out[idx] = R[idx];
+    }
 }
 
 template <int METHOD>
@@ -335,7 +339,7 @@ static int launch_dense(const epx_ctx* c, cudaStream_t s)
     const int32_t* order = c->sub_list ? c->sub_list : d.order;      // depends on tau, Q and the rates only and is kept
     if (n == 0) return 0;
     if (M >= 3 && use_table && !c->sub_list) {
-        pade_full_epoch_kernel<METHOD><<<(M - 2) * C, PT, smem, s>>>(K, M, C, d.Q, d.tau, d.rates, d.Efull, d.status);
+        pade_full_epoch_kernel<METHOD><<<(M - 2) * C, PT, smem, s>>>(K, M, C, d.Q, d.tau, d.rates, d.Efull, d.status, d.fproc);
         launched++;
     }
     pade_chain_kernel<METHOD><<<n * C, PT, smem, s>>>(K, C, use_table, order, d.n_seg, d.seg_off, d.seg_epoch, d.seg_dur,

@@ -16,7 +16,7 @@ import oracle  # noqa: E402
 import workloads as W  # noqa: E402
 
 CASES = [("cfg1", 1, {}), ("cfg2_N150_L777", 2, {"N": 150, "L": 777}), ("cfg2", 2, {}), ("cfg3_N12_L70", 3, {"N": 12, "L": 70}),
-         ("cfg3", 3, {}), ("cfg4_N60_L3", 4, {"N": 60, "L": 3}), ("cfg4", 4, {})]
+         ("cfg3", 3, {}), ("cfg4_N60_L3", 4, {"N": 60, "L": 3}), ("cfg4", 4, {}), ("cfg6_N30_L100", 6, {"N": 30, "L": 100}), ("cfg6", 6, {})]
 
 
 def main():

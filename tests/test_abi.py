@@ -157,3 +157,29 @@ def test_plan_info_and_tip_partial_reservation_state(L):
     c.set_tip_partials(3, None)
     c.reserve_tip_partials(4)
     c.close()
+
+
+def test_shared_processes_are_detected(L):
+    """S processes, M epochs, phi_m.  Config 4 alternates two seasonal regimes over 24 epochs; config 2 has ten
+    different HKY models."""
+    import paper_1309_3075_b200 as epx
+    import workloads as W
+    p4 = W.make_config(4, N=10, L=1)
+    c = epx.Epx(p4.K, p4.M, p4.C, p4.N, p4.L)
+    with pytest.raises(epx.EpxError):
+        c.epoch_processes()                              # models not set yet
+    for e in range(p4.M):
+        c.set_epoch_model(e, p4.Q[e], p4.freqs[e], False)
+    phi, S = c.epoch_processes()
+    assert S == 2 and phi.tolist() == [e % 2 for e in range(24)]
+    c.close()
+    p2 = W.make_config(2, N=10, L=4)
+    c = epx.Epx(p2.K, p2.M, p2.C, p2.N, p2.L)
+    for e in range(p2.M):
+        c.set_epoch_model(e, p2.Q[e], p2.freqs[e], True)
+    phi, S = c.epoch_processes()
+    assert S == 10 and phi.tolist() == list(range(10))
+    c.set_epoch_model(7, p2.Q[2], p2.freqs[2], True)     # epoch 7 now runs process 2
+    phi, S = c.epoch_processes()
+    assert S == 9 and phi.tolist() == [0, 1, 2, 3, 4, 5, 6, 2, 7, 8]
+    c.close()

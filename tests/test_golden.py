@@ -10,7 +10,8 @@ import workloads as W
 
 HERE = os.path.dirname(os.path.abspath(__file__))
 CASES = {"cfg1": (1, {}), "cfg2_N150_L777": (2, {"N": 150, "L": 777}), "cfg2": (2, {}), "cfg3_N12_L70": (3, {"N": 12, "L": 70}),
-         "cfg3": (3, {}), "cfg4_N60_L3": (4, {"N": 60, "L": 3}), "cfg4": (4, {})}
+         "cfg3": (3, {}), "cfg4_N60_L3": (4, {"N": 60, "L": 3}), "cfg4": (4, {}), "cfg6_N30_L100": (6, {"N": 30, "L": 100}),
+         "cfg6": (6, {})}
 
 
 def golden():
@@ -23,7 +24,7 @@ def golden():
     return out
 
 
-@pytest.mark.parametrize("name", ["cfg1", "cfg2_N150_L777", "cfg3_N12_L70", "cfg4_N60_L3"])
+@pytest.mark.parametrize("name", ["cfg1", "cfg2_N150_L777", "cfg3_N12_L70", "cfg4_N60_L3", "cfg6_N30_L100"])
 def test_oracle_reproduces_golden(orc_ld, name):
     g = golden()
     cid, kw = CASES[name]

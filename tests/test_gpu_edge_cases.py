@@ -143,6 +143,37 @@ def test_reevaluation_after_inputs_change(epx, orc_ld):
     ctx.close()
 
 
+@pytest.mark.parametrize("cid,kw", [(2, {"N": 60, "L": 100}), (3, {"N": 8, "L": 24}), (4, {"N": 40, "L": 2}), (5, {"n_br": 150})])
+def test_shared_processes(epx, orc_ld, cid, kw):
+    """f2 (PAPER.md L78 phi_m): epochs with identical (Q, freqs) share one eigensystem / one full-epoch exponential.  Parity with
+    the oracle (which knows nothing of the sharing), and bit-identical to computing one per epoch."""
+    prob = W.make_config(cid, **kw)
+    Q, F = prob.Q.copy(), prob.freqs.copy()
+    for e in range(2, prob.M):                          # three processes at most: epochs 2.. repeat the first two
+        Q[e], F[e] = Q[e % 2], F[e % 2]
+    prob = dataclasses.replace(prob, Q=Q, freqs=F)
+    if prob.root_freqs is not None:
+        prob = dataclasses.replace(prob, root_freqs=F[int(np.sum(prob.tau < prob.height.max()))].copy())
+    outs = []
+    for share in (1, 0):
+        ctx = epx.from_problem(prob)
+        ctx.set_option(epx.EPX_OPT_SHARE_PROCESSES, share)
+        phi, S = ctx.epoch_processes()
+        assert S == (min(2, prob.M) if share else prob.M)
+        if prob.N:
+            lnl = ctx.log_likelihood()
+        else:
+            ctx.update_matrices(); lnl = 0.0
+        assert ctx.status() == 0
+        outs.append((lnl, ctx.get_all_matrices()))
+        ctx.close()
+    assert outs[0][0] == outs[1][0] and np.array_equal(outs[0][1], outs[1][1])
+    ref = orc_ld.evaluate(prob)
+    assert np.max(np.abs(outs[0][1].astype(np.longdouble) - ref["P"])) <= P_TOL
+    if prob.N:
+        assert abs(np.longdouble(outs[0][0]) - ref["lnl"]) <= LNL_RTOL * abs(ref["lnl"])
+
+
 def test_stage_events_and_launch_count(epx):
     prob = W.make_config(1)
     ctx = epx.from_problem(prob)

@@ -232,6 +232,26 @@ def test_config4_full_size(epx, orc_ld):
     run_tree(epx, orc_ld, W.make_config(4), partial_nodes=[2998, 2000, 1500])
 
 
+def test_config6_amino_acid_reduced(epx, orc_ld):
+    # 20 states -> tensor-pipe level kernel with KP = 24 (4 padding states), Jacobi + generic chain;
+    # every node's partials; ragged L (100 = 64 + 36: a full CTA chunk and a ragged one), missing tip states
+    prob = W.make_config(6, N=30, L=100)
+    run_tree(epx, orc_ld, prob)
+    run_tree(epx, orc_ld, prob, options=[(epx.EPX_OPT_MMA_CHUNK, 24)])
+    run_tree(epx, orc_ld, prob, options=[(epx.EPX_OPT_PRUNE_KERNEL, 1)])      # scalar level kernel
+
+
+def test_config6_amino_acid_full_size(epx, orc_ld):
+    prob = W.make_config(6)
+    # default (spectral: Jacobi + eigenbasis chain) against north_star's two gates: 1e-12 absolute on P, 1e-9 relative on logL /
+    # site logL.  Node-by-node partials at PARTIAL_RTOL are compared on the componentwise exponential: a P entry of 1e-3 that
+    # is within 1e-13 ABSOLUTE is only good to 1e-10 RELATIVE, and a cherry's partial is a product of two such entries
+    # (measured 1.2e-10 here) -- the spectral path's contract is the absolute one (A21).
+    run_tree(epx, orc_ld, prob, partial_nodes=())
+    run_tree(epx, orc_ld, prob, options=[(epx.EPX_OPT_EXP_METHOD, 2)],
+             partial_nodes=[prob.N, prob.N + 57, prob.n_nodes - 2, prob.n_nodes - 1])
+
+
 def test_config5_reduced_every_branch(epx, orc_ld):
     prob = W.make_config(5, n_br=300)
     for kernel, jacobi in ((0, 0), (1, 0), (0, 1)):        # DMMA / generic chain kernel; one-barrier / round-1 Jacobi

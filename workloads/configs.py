@@ -18,6 +18,7 @@ CONFIG_NAMES = {
     3: "cfg3_gy94_61_3epoch_100tips_1000pat",
     4: "cfg4_trait24_asym_24epoch_1500tips_1pat",
     5: "cfg5_conv61_16epoch_20000branches",
+    6: "cfg6_aa20_3epoch_200tips_2000pat",      # not in BASELINE.json: SURVEY.md 8(f) f3, the 20-state amino-acid workload
 }
 
 
@@ -38,7 +39,8 @@ def _gy94_epoch(rng, omega, kappa=2.0):
 
 def make_config(config_id: int, *, N: int | None = None, L: int | None = None,
                 n_br: int | None = None) -> EpochProblem:
-    """Build config `config_id` (1..5). N / L / n_br override the size (same recipe, same seed) for tests."""
+    """Build config `config_id` (1..5 = BASELINE.json; 6 = the 20-state workload of SURVEY.md 8(f) f3). N / L / n_br override the
+    size (same recipe, same seed) for tests."""
     r_tree, r_model, r_tips, r_wt = _streams(config_id)
     if config_id == 1:
         K, M, C = 4, 2, 4
@@ -127,4 +129,28 @@ def make_config(config_id: int, *, N: int | None = None, L: int | None = None,
         rates, weights = models.discrete_gamma(1.0, C)
         return EpochProblem(CONFIG_NAMES[5], K, M, C, 0, 0, tau, Q, F, True, rates, weights,
                             child_height=child, parent_height=par)
+    if config_id == 6:
+        # SURVEY.md 8(f) f3 / north_star "tiles for 20-61-state": an amino-acid shaped workload (PAPER.md:L26 finite state
+        # spaces).  Reversible GTR-like Q per epoch: 190 exchangeabilities ~ Gamma(1,1), pi ~ Dirichlet(5,...,5) (empirical
+        # amino-acid frequencies span about one decade), normalised; 3 epochs at thirds of the root height; 4 gamma
+        # categories (alpha = 0.7); 200 tips from a serially-sampled coalescent (tip dates over 20 % of the root height);
+        # 2 000 site patterns, tips uniform over the 20 states with 2 % missing, weights Poisson(2) + 1.
+        K, M, C = 20, 3, 4
+        N = 200 if N is None else N
+        L = 2000 if L is None else L
+        tip_h = r_tree.uniform(0.0, 0.2, size=N)
+        tip_h[np.argmin(tip_h)] = 0.0
+        parent, height = trees.coalescent(r_tree, tip_h, ne=0.5)
+        height = trees.stretch_above(height, 0.2, 1.0)
+        tau = np.array([1.0 / 3.0, 2.0 / 3.0])
+        Q = np.zeros((M, K, K)); F = np.zeros((M, K))
+        for e in range(M):
+            F[e] = r_model.dirichlet(np.full(K, 5.0))
+            Q[e] = models.gtr_k(r_model.gamma(1.0, 1.0, size=K * (K - 1) // 2), F[e])
+        rates, weights = models.discrete_gamma(0.7, C)
+        tips = r_tips.integers(0, K, size=(N, L)).astype(np.int32)
+        tips[r_tips.random((N, L)) < 0.02] = -1
+        wt = (r_wt.poisson(2.0, size=L) + 1).astype(np.float64)
+        return EpochProblem(CONFIG_NAMES[6], K, M, C, N, L, tau, Q, F, True, rates, weights,
+                            parent=parent, height=height, tip_states=tips, pattern_weights=wt)
     raise ValueError(f"unknown config {config_id}")

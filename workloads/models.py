@@ -38,6 +38,16 @@ def gtr(exch6: np.ndarray, pi: np.ndarray) -> np.ndarray:
     return normalise(S * pi[None, :], pi)
 
 
+def gtr_k(exch: np.ndarray, pi: np.ndarray) -> np.ndarray:
+    """General time-reversible K-state Q (amino-acid style): q_ij = s_ij * pi_j with K (K-1) / 2 exchangeabilities."""
+    K = pi.shape[0]
+    S = np.zeros((K, K))
+    iu = np.triu_indices(K, 1)
+    S[iu] = exch
+    S = S + S.T
+    return normalise(S * pi[None, :], pi)
+
+
 def hky(kappa: float, pi: np.ndarray) -> np.ndarray:
     """HKY85 in TCAG order: transitions T<->C and A<->G get kappa."""
     S = np.ones((4, 4))
