@@ -444,6 +444,8 @@ def run_cuda(args) -> None:
         line["matrices"] = bench_matrices(torch, epx, local, K, peaks)
     if rank == 0 and "other" in legs:
         line["other_configs"] = bench_other_configs(torch, epx, local, K, peaks)
+    if rank == 0 and "batch" in legs:
+        line["batch"] = bench_batch(torch, epx, local)
     if rank == 0 and "cpu" in legs and world == 1:
         r = time_oracle(prob, 15.0)
         line["cpu_baseline"] = {k: r[k] for k in ("value", "unit", "cores", "kind", "sample")}
@@ -635,6 +637,42 @@ def bench_other_configs(torch, epx, device: int, K: int, peaks: dict) -> dict:
 
 
 
+def bench_batch(torch, epx, device: int) -> dict:
+    """many independent instances through epx_log_likelihood_batch (every context on its own stream, all
+    enqueued before the first fetch) against the same contexts evaluated one after the other.  Host wall clock around
+    synchronised calls: the API-level cost a caller sees."""
+    import dataclasses
+    out = {}
+    for label, cid, count in (("8 x config 3 (eight codon data sets, PAPER.md:L157-L161)", 3, 8), ("64 x config 1", 1, 64),
+                              ("16 x config 4", 4, 16)):
+        base = W.make_config(cid)
+        rng = np.random.default_rng(W.config_seed(cid) + 7)
+        ctxs = []
+        for k in range(count):                           # same shapes, different data per instance
+            tips = rng.integers(0, base.K, base.tip_states.shape).astype(np.int32)
+            ctxs.append(epx.from_problem(dataclasses.replace(base, tip_states=tips), device=device))
+        single = [c.log_likelihood() for c in ctxs]
+        for _ in range(3):
+            got = epx.log_likelihood_batch(ctxs)
+        assert np.array_equal(got, np.array(single))
+        reps = 20
+        torch.cuda.synchronize()
+        t0 = time.perf_counter()
+        for _ in range(reps):
+            for c in ctxs:
+                c.log_likelihood()
+        t_seq = (time.perf_counter() - t0) / reps
+        t0 = time.perf_counter()
+        for _ in range(reps):
+            epx.log_likelihood_batch(ctxs)
+        t_batch = (time.perf_counter() - t0) / reps
+        for c in ctxs:
+            c.close()
+        out[label] = {"instances": count, "ms_one_after_the_other": t_seq * 1e3, "ms_batch": t_batch * 1e3,
+                      "instances_per_s_batch": count / t_batch, "speedup": t_seq / t_batch}
+    return out
+
+
 def parse_opts(text: str):
     """--opt 3=1,6=2 -> [(3, 1), (6, 2)]: EPX_OPT_* overrides for the config-2 context (kernel comparisons, ncu captures)."""
     out = []
@@ -650,9 +688,9 @@ def main() -> None:
     ap.add_argument("--steps", type=int, default=100)
     ap.add_argument("--warmup", type=int, default=5)
     ap.add_argument("--impl", choices=["cuda", "reference"], default="cuda")
-    ap.add_argument("--legs", default="e2e,incremental,matrices,other,cpu",
+    ap.add_argument("--legs", default="e2e,incremental,matrices,other,batch,cpu",
                     help="optional legs beside the config-2 headline + roofline: e2e, incremental, matrices (config 5), "
-                         "other (configs 1, 3, 4), cpu (oracle on the host cores)")
+                         "other (configs 1, 3, 4, 6), batch (many instances, f4), cpu (oracle on the host cores)")
     ap.add_argument("--no-matrices", action="store_true", help="skip the config-5 matrices/s leg")
     ap.add_argument("--no-cpu-baseline", action="store_true", help="skip timing the oracle on the host cores")
     ap.add_argument("--opt", type=parse_opts, default=[], help="EPX_OPT overrides for the config-2 context, e.g. 3=2,6=1")

@@ -130,6 +130,13 @@ int epx_log_likelihood(epx_ctx* ctx, double* logL);
 /* Synchronise and fetch the result of the last enqueue (same checks as epx_log_likelihood). */
 int epx_fetch_log_likelihood(epx_ctx* ctx, double* logL);
 
+/* Many independent instances (eight patients, one codon model each): the same as
+ * epx_log_likelihood on each of the n contexts, but every context's work is enqueued (on the stream it was bound with) before
+ * the first result is fetched, so the kernel sequences of contexts bound to DIFFERENT streams overlap on the device; contexts
+ * that share a stream run one after the other.  logL: n host doubles.  rc: n per-context return codes, or NULL.  Returns
+ * EPX_OK or the first non-zero code; the other contexts are still evaluated.  Results are bit-identical to single calls. */
+int epx_log_likelihood_batch(epx_ctx* const* ctxs, int n, double* logL, int* rc);
+
 /* ---- incremental re-evaluation (an MCMC step re-dispatches only what its proposal
  * touches) ----
  * epx_set_node_heights: move `n` nodes (node ids, new heights) without changing the topology; every moved node must stay

@@ -69,6 +69,7 @@ def lib():
     _sig(L, "epx_enqueue_log_likelihood", i, vp)
     _sig(L, "epx_log_likelihood", i, vp, ct.POINTER(ct.c_double))
     _sig(L, "epx_fetch_log_likelihood", i, vp, ct.POINTER(ct.c_double))
+    _sig(L, "epx_log_likelihood_batch", i, vp, i, dp, ip)
     _sig(L, "epx_get_segments", i, vp, i, ct.POINTER(i), ip, dp)
     _sig(L, "epx_get_all_segments", i, vp, ip, ip, dp, i)
     _sig(L, "epx_get_matrix", i, vp, i, i, dp)
@@ -368,6 +369,19 @@ def from_problem(prob, device: int = 0, stream=None, tip_partials: int = 0) -> E
     ctx.bind(stream)
     set_problem(ctx, prob)
     return ctx
+
+
+def log_likelihood_batch(ctxs) -> np.ndarray:
+    """epx_log_likelihood_batch: every context's work is enqueued before the first result is fetched."""
+    n = len(ctxs)
+    arr = (ct.c_void_p * n)(*[c._ctx for c in ctxs])
+    out = np.zeros(n, dtype=np.float64)
+    rc = np.zeros(n, dtype=np.int32)
+    code = lib().epx_log_likelihood_batch(arr, n, _ptr(out), _ptr(rc))
+    if code != EPX_OK:
+        bad = int(np.nonzero(rc)[0][0])
+        raise EpxError(int(rc[bad]), f"context {bad}: {ctxs[bad].last_error()}")
+    return out
 
 
 def measure_fp64_peak(kind: int, ms_target: float = 50.0, device: int = 0) -> float:

@@ -327,6 +327,34 @@ def test_tip_states_from_bytes_and_two_contexts_on_two_streams(epx, orc_ld):
     a.close(); b.close()
 
 
+def test_batch_of_independent_instances(epx, orc_ld):
+    """f4 (eight patients, one codon model each): epx_log_likelihood_batch over contexts of different
+    shapes, each on its own stream; bit-identical to single calls, parity with the oracle, errors reported per context."""
+    rng = np.random.default_rng(44)
+    probs = []
+    for k in range(8):                                   # eight codon data sets with their own trees, tips and sizes
+        p = W.make_config(3, N=6 + k, L=24 + 5 * k)
+        probs.append(dataclasses.replace(p, tip_states=rng.integers(0, 61, p.tip_states.shape).astype(np.int32)))
+    probs += [W.make_config(1), W.make_config(2, N=40, L=90), W.make_config(4, N=30, L=2)]
+    ctxs = [epx.from_problem(p) for p in probs]
+    single = np.array([c.log_likelihood() for c in ctxs])
+    for _ in range(3):
+        got = epx.log_likelihood_batch(ctxs)
+        assert np.array_equal(got, single)
+    for k in (0, 7, 9):
+        ref = orc_ld.evaluate(probs[k])
+        assert abs(np.longdouble(got[k]) - ref["lnl"]) <= LNL_RTOL * abs(ref["lnl"])
+    assert epx.log_likelihood_batch([]).size == 0
+    # a context that cannot run is reported, the others are unaffected
+    broken = epx.Epx(4, 2, 2, 3, 5)
+    with pytest.raises(epx.EpxError) as e:
+        epx.log_likelihood_batch(ctxs[:2] + [broken])
+    assert e.value.code == epx.EPX_E_STATE
+    broken.close()
+    for c in ctxs:
+        c.close()
+
+
 @pytest.mark.parametrize("cid,kw,opts", [(2, {"N": 60, "L": 203}, ()), (2, {"N": 60, "L": 203}, ((6, 2),)), (2, {"N": 60, "L": 203}, ((3, 5),)),
                                          (2, {"N": 60, "L": 203}, ((3, 2),)), (2, {"N": 60, "L": 203}, ((3, 3),)),
                                          (2, {"N": 60, "L": 203}, ((3, 1), (1, 1))), (3, {"N": 9, "L": 40}, ()), (4, {"N": 40, "L": 3}, ())])
