@@ -126,6 +126,15 @@ def chain_flops(K: int, C: int, n_seg: np.ndarray) -> dict:
     return {"executed": executed, "straightforward": straightforward}
 
 
+def cached_chain_flops(K: int, C: int, M: int, n_seg: np.ndarray) -> dict:
+    """Executed useful flops with the cached products of consecutive full epochs (EPX_OPT_EPOCH_PRODUCTS):
+    a chain over >= 2 full epochs (n_seg >= 4) costs 3 products, the table costs a products for each (a, category), a = 1..M-2."""
+    nseg = n_seg.astype(np.int64)
+    chain = int(np.where(nseg >= 4, 3, nseg).sum()) * C * 2 * K ** 3
+    table = sum(range(1, M - 1)) * C * 2 * K ** 3
+    return {"chain": chain, "table": table, "executed": chain + table}
+
+
 def n_segments(prob) -> np.ndarray:
     """Segment count per matrix slot from the inputs (host integer arithmetic for the flop count only)."""
     ch, ph = prob.branch_heights()
@@ -442,6 +451,9 @@ def run_cuda(args) -> None:
         peaks = {"dfma": epx.measure_fp64_peak(0, 200.0, local), "dmma": epx.measure_fp64_peak(1, 200.0, local)}
     if rank == 0 and "matrices" in legs:
         line["matrices"] = bench_matrices(torch, epx, local, K, peaks)
+        # SURVEY.md 8(f) f1, reported separately (it changes the algorithmic flops; config 5's text asks for the full chain)
+        line["matrices_cached"] = bench_matrices(torch, epx, local, K, peaks, options=[(epx.EPX_OPT_EPOCH_PRODUCTS, 1)],
+                                                 label=", products of consecutive full epochs cached (SURVEY.md 8(f) f1)")
     if rank == 0 and "other" in legs:
         line["other_configs"] = bench_other_configs(torch, epx, local, K, peaks)
     if rank == 0 and "batch" in legs:
@@ -533,6 +545,10 @@ def bench_matrices(torch, epx, device: int, K: int, peaks: dict, options=(), lab
     prob = W.make_config(5)
     nseg = n_segments(prob)
     fl = chain_flops(prob.K, prob.C, nseg)
+    cached = dict(options).get(epx.EPX_OPT_EPOCH_PRODUCTS, 0) == 1
+    if cached:
+        cf = cached_chain_flops(prob.K, prob.C, prob.M, nseg)
+        fl = dict(fl, executed=cf["executed"], table=cf["table"])
     ctx = epx.from_problem(prob, device=device)
     for opt, val in options:
         ctx.set_option(opt, val)
@@ -558,12 +574,14 @@ def bench_matrices(torch, epx, device: int, K: int, peaks: dict, options=(), lab
     chain_ms = float(stage[2])
     achieved = fl["executed"] / (chain_ms * 1e-3) / 1e12
     n_mat = prob.n_br * prob.C
-    return {"metric": "epoch branch matrices/s (fp64)", "value": n_mat / (ms * 1e-3), "unit": "matrices/s",
+    kernel = ("epoch_product_table_kernel + chain_dmma64_kernel<1, 4> (a3+a4 fused; chains over >= 2 full epochs multiply by the "
+              "tabulated product of those epochs: 3 products per branch at most)" if cached else
+              "chain_dmma64_kernel<1, 4> (a3+a4 fused, mma.sync m8n8k4 f64, one product per segment)")
+    return {"metric": "epoch branch matrices/s (fp64)" + label, "value": n_mat / (ms * 1e-3), "unit": "matrices/s",
             "ms_per_step": ms, "steps": steps, "gpu_launches": int(launches), "clocks": clk,
             "config": dict(workload_config(prob, 5, 1), segments=int(nseg.sum())),
             "whole_step_useful_tflops": fl["executed"] / (ms * 1e-3) / 1e12,
-            "roofline": {"bound": "alu", "kernel": "chain_dmma64_kernel (a3+a4 fused, mma.sync m8n8k4 f64)",
-                         "tensor_pipe_active_ncu": 0.795,   # sm__pipe_tensor_subpipe_dmma_cycles_active, profiles/r1_chain_dmma64_ncu.md
+            "roofline": {"bound": "alu", "kernel": kernel,
                          "achieved": achieved, "peak": dmma, "unit": "TFLOP/s", "frac": achieved / dmma,
                          "traffic": None, "peak_source": "measured in this run by epx_measure_fp64_peak "
                                                          "(register-only DMMA m8n8k4 loop); DFMA peak beside it",

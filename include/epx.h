@@ -192,9 +192,10 @@ int epx_get_stage_ms(epx_ctx* ctx, float* ms, int* launches);
  * compiler from deleting the arithmetic).  Synchronises the stream. */
 int epx_measure_fp64_peak(int device, int kind, double ms_target, void* dev_scratch, void* cuda_stream, double* tflops);
 
-/* ---- tuning / test hooks (options 1-3, 6-8, 10 have no effect on results; 9 only within rounding) ---- */
+/* ---- tuning / test hooks (options 1-3, 6-8, 10 have no effect on results; 9 and 11 only within rounding) ---- */
 enum {
-    EPX_OPT_CHAIN_KERNEL = 1, /* 0 auto (default); 1 force the generic shared-memory chain kernel */
+    EPX_OPT_CHAIN_KERNEL = 1, /* 0 auto (default); 1 force the generic shared-memory chain kernel; 2 (32 < K <= 64) round 1's
+                                 tensor-pipe layout, two categories per CTA, instead of one category per CTA (four warps of 16 rows) */
     EPX_OPT_USE_GRAPH = 2,    /* 1 (default) replay the kernel sequence from a CUDA graph on non-default streams; 0 launch directly */
     EPX_OPT_PRUNE_KERNEL = 3, /* 0 auto (default).  K == 4: depth-first walk, one lane per site pattern, partials never
                                  re-read from HBM.  8 < K <= 64: level kernel on the FP64 tensor pipe, matrices staged by TMA in
@@ -216,8 +217,13 @@ enum {
                                  different warps + the part above them); 0 (default) auto */
     EPX_OPT_MMA_CHUNK = 8,    /* 8 < K <= 64 tensor-pipe level kernel: site patterns per CTA (rounded up to 8); 0 (default) auto */
     EPX_OPT_JACOBI_KERNEL = 9, /* a2: 0 (default) the one-barrier-per-round Jacobi for K <= 62; 1 round 1's two-barrier kernel */
-    EPX_OPT_SHARE_PROCESSES = 10 /* 1 (default) one eigensystem / full-epoch exponential per distinct process (epx_epoch_processes);
+    EPX_OPT_SHARE_PROCESSES = 10, /* 1 (default) one eigensystem / full-epoch exponential per distinct process (epx_epoch_processes);
                                  0 one per epoch */
+    EPX_OPT_EPOCH_PRODUCTS = 11 /* SURVEY.md 8(f) f1.  0 (default): every branch multiplies its whole chain, one product per
+                                 segment.  1 (reversible models with 32 < K <= 64, M >= 4, no branch rates): the products of
+                                 consecutive full epochs, D_a W_a ... D_b W_b per category, are tabulated once per call
+                                 ((M-2)(M-1)/2 C matrices) and a branch that crosses >= 2 full epochs does 3 products
+                                 whatever its length.  Same P within rounding (the association order changes) */
 };
 int epx_set_option(epx_ctx* ctx, int option, int value);
 /* Device status word of the last compute call (0 = all numeric checks passed); synchronises. */

@@ -19,7 +19,7 @@ LIB_PATH = os.path.join(_HERE, "libepx.so")
 EPX_OK, EPX_E_ARG, EPX_E_STATE, EPX_E_TREE, EPX_E_MODEL, EPX_E_WORKSPACE, EPX_E_CUDA, EPX_E_NUMERIC = 0, -1, -2, -3, -4, -5, -6, -7
 EPX_OPT_CHAIN_KERNEL, EPX_OPT_USE_GRAPH, EPX_OPT_PRUNE_KERNEL, EPX_OPT_EXP_METHOD = 1, 2, 3, 4
 EPX_OPT_STAGE_EVENTS, EPX_OPT_DFS_PPL, EPX_OPT_DFS_PIECES, EPX_OPT_MMA_CHUNK, EPX_OPT_JACOBI_KERNEL = 5, 6, 7, 8, 9
-EPX_OPT_SHARE_PROCESSES = 10
+EPX_OPT_SHARE_PROCESSES, EPX_OPT_EPOCH_PRODUCTS = 10, 11
 STAGE_NAMES = ("segment", "eigen", "chain", "prune", "root")
 
 _lib = None

@@ -83,6 +83,7 @@ size_t plan_workspace(const epx_ctx* c, char* base, DevBuffers* d)
     t.isp = (double*)take(8 * M * Kp);
     t.WB = (double*)take(Kp == 64 ? 8 * M * 4096 : 0);
     t.UTB = (double*)take(Kp == 64 ? 8 * M * 4096 : 0);
+    t.GB = (double*)take(Kp == 64 && M >= 4 ? 8 * ((M - 2) * (M - 1) / 2) * C * 4096 : 0);
     t.Efull = (double*)take(8 * M * C * K * K);
     t.P = (double*)take(8 * S * C * K * K);
     if (c->tree_mode) {
@@ -395,6 +396,7 @@ int epx_set_option(epx_ctx* c, int option, int value)
             c->dfs_ppl = value;
             if (c->has_tree) { int rc = build_plan(c); if (rc) return rc; c->tree_dirty = true; }
             break;
+        case 11: c->epoch_products = value ? 1 : 0; break;
         case 10: c->dedup = value ? 1 : 0; c->model_dirty = true; break;
         case 9: c->jacobi_kernel = value ? 1 : 0; break;
         case 8:

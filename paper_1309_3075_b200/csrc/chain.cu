@@ -178,33 +178,78 @@ __device__ __forceinline__ void bulk_g2s(void* dst, const void* src, uint32_t by
                  ::"r"(smem_u32(dst)), "l"(src), "r"(bytes), "r"(smem_u32(bar)) : "memory");
 }
 
-constexpr int CPC = 2;                  // categories per CTA: 2 -> 128 threads, 66 KB, two CTAs per SM overlap each other's
-                                        // prologue (U fragments from L2) and epilogue (P store) with DMMA work
-constexpr int DT = 64 * CPC;            // warp w -> category (w>>1) of the CTA, rows 32*(w&1) .. +32
 constexpr int FRAG_DOUBLES = 4096;      // one 64x64 operand in fragment order
-struct DmmaSmem {
+
+// NCAT categories per CTA, WPC warps per category (a warp owns 64 / WPC rows of the running product).
+//   <1, 4>: 128 threads for ONE category (default): 32 accumulator registers per lane, no spill, three CTAs per SM; the only
+//           layout that can take a per-category operand (the cached products of consecutive full epochs).
+//   <2, 2>: round 1's layout (EPX_OPT_CHAIN_KERNEL = 2): one staged operand serves two categories, 64 accumulator registers
+//           per lane (255 registers, 72 B spilled), two CTAs per SM.
+template <int NCAT>
+struct DmmaSmemT {
     double B[2][FRAG_DOUBLES];          // TMA destination ring (2 x 32 KB)
-    double D[2][CPC][64];               // exp(lambda r d) per stage / category
+    double D[2][NCAT][64];              // exp(lambda r d) per stage / category
     uint64_t bar[2];
 };
 
-__global__ void __launch_bounds__(DT, 2) chain_dmma64_kernel(int K, int C, const int32_t* __restrict__ order,
+// index of the cached product of the full epochs a, a-1, ..., b  (1 <= b <= a <= M-2)
+__host__ __device__ inline int epoch_pair_index(int a, int b) { return (a - 1) * a / 2 + (b - 1); }
+
+// acc (MTW m-tiles x 8 n-tiles of C fragments) <- (acc * diag(D)) * B, B in fragment order in shared memory
+template <int MTW>
+__device__ __forceinline__ void dmma_stage(double (&acc)[MTW][8][2], const double2* __restrict__ Bs, const double2* __restrict__ Ds,
+                                           int lane, int q)
+{
+#pragma unroll
+    for (int mp = 0; mp < MTW / 2; mp++) {
+        double a[2][8][2];
+#pragma unroll
+        for (int kt = 0; kt < 8; kt++) {
+            const double2 dv = Ds[kt * 4 + q];       // D[8kt + 2q], D[8kt + 2q + 1]
+#pragma unroll
+            for (int mi = 0; mi < 2; mi++) {
+                a[mi][kt][0] = acc[2 * mp + mi][kt][0] * dv.x;
+                a[mi][kt][1] = acc[2 * mp + mi][kt][1] * dv.y;
+                acc[2 * mp + mi][kt][0] = 0.0;
+                acc[2 * mp + mi][kt][1] = 0.0;
+            }
+        }
+#pragma unroll
+        for (int kt = 0; kt < 8; kt++)
+#pragma unroll
+            for (int nt = 0; nt < 8; nt++) {
+                const double2 bv = Bs[(kt * 8 + nt) * 32 + lane];
+                // h outer, mi inner: two other DMMAs sit between the two that update the same accumulator tile
+#pragma unroll
+                for (int h = 0; h < 2; h++)
+#pragma unroll
+                    for (int mi = 0; mi < 2; mi++)
+                        dmma884(acc[2 * mp + mi][nt][0], acc[2 * mp + mi][nt][1], a[mi][kt][h], h ? bv.y : bv.x);
+            }
+    }
+}
+
+template <int NCAT, int WPC>
+__global__ void __launch_bounds__(32 * WPC * NCAT, NCAT == 2 ? 2 : 3) chain_dmma64_kernel(int K, int C, int M,
+    const int32_t* __restrict__ order,
     const int32_t* __restrict__ n_seg, const int32_t* __restrict__ seg_off, const int32_t* __restrict__ seg_epoch,
     const double* __restrict__ seg_dur, const double* __restrict__ rates, const double* __restrict__ lam,
-    const double* __restrict__ WB, const double* __restrict__ UTB, const double* __restrict__ sp,
+    const double* __restrict__ WB, const double* __restrict__ UTB, const double* __restrict__ GB, const double* __restrict__ sp,
     const double* __restrict__ isp, double* __restrict__ P, int32_t* __restrict__ status)
 {
+    constexpr int DT = 32 * WPC * NCAT, MTW = 8 / WPC;
     extern __shared__ __align__(128) unsigned char smraw[];
-    DmmaSmem& sm = *reinterpret_cast<DmmaSmem*>(smraw);
+    DmmaSmemT<NCAT>& sm = *reinterpret_cast<DmmaSmemT<NCAT>*>(smraw);
     const int tid = threadIdx.x, lane = tid & 31, w = tid >> 5;
     const int g = lane >> 2, q = lane & 3;
-    const int ncg = (C + CPC - 1) / CPC;
+    const int ncg = (C + NCAT - 1) / NCAT;
     const int b = order[blockIdx.x / ncg], cg = blockIdx.x % ncg;
-    const int c = cg * CPC + (w >> 1), half = w & 1;
+    const int wc = w / WPC, rb = w % WPC;          // category of the CTA this warp serves, its block of 8 * MTW rows
+    const int c = cg * NCAT + wc;
     const bool active = c < C;
     const int n = n_seg[b];
     if (n == 0) {
-        for (int cc = cg * CPC; cc < min(C, cg * CPC + CPC); cc++) {
+        for (int cc = cg * NCAT; cc < min(C, cg * NCAT + NCAT); cc++) {
             double* out = P + ((size_t)b * C + cc) * K * K;
             for (int idx = tid; idx < K * K; idx += DT) out[idx] = (idx / K == idx % K) ? 1.0 : 0.0;
         }
@@ -212,15 +257,25 @@ __global__ void __launch_bounds__(DT, 2) chain_dmma64_kernel(int K, int C, const
     }
     const int off = seg_off[b];
     const int e_hi = seg_epoch[off], e_lo = seg_epoch[off + n - 1];
+    // f1: a chain over >= 2 full epochs multiplies by their cached product instead (one operand per category: NCAT == 1)
+    const bool cached = NCAT == 1 && GB != nullptr && n >= 4;
+    const int ns = cached ? 3 : n;                 // products of this chain
 
-    // stage t (0..n-1): B operand = WB[epoch_t] for t < n-1 (boundary epoch_t -> epoch_t - 1), U^T of e_lo for the last
+    // stage t: B operand = WB[epoch_t] for a boundary epoch_t -> epoch_t - 1, U^T of e_lo for the last; with the cache the
+    // middle stage is the product of the full epochs e_hi - 1 .. e_lo + 1 (already scaled: its D is 1)
     auto stage_src = [&](int t) -> const double* {
+        if (cached)
+            return t == 0 ? WB + (size_t)e_hi * FRAG_DOUBLES
+                 : t == 1 ? GB + ((size_t)epoch_pair_index(e_hi - 1, e_lo + 1) * C + cg) * FRAG_DOUBLES
+                          : UTB + (size_t)e_lo * FRAG_DOUBLES;
         return (t < n - 1) ? WB + (size_t)seg_epoch[off + t] * FRAG_DOUBLES : UTB + (size_t)e_lo * FRAG_DOUBLES;
     };
     auto fill_D = [&](int t) {     // one value per thread: category tid>>6, eigen index tid&63
-        int cc = cg * CPC + (tid >> 6), k = tid & 63;
-        double r = cc < C ? rates[cc] : 0.0;
-        sm.D[t & 1][tid >> 6][k] = exp(lam[seg_epoch[off + t] * 64 + k] * (r * seg_dur[off + t]));
+        if (tid >= 64 * NCAT) return;
+        const int cc = cg * NCAT + (tid >> 6), k = tid & 63;
+        const double r = cc < C ? rates[cc] : 0.0;
+        const int s = cached ? (t == 0 ? 0 : n - 1) : t;
+        sm.D[t & 1][tid >> 6][k] = (cached && t == 1) ? 1.0 : exp(lam[seg_epoch[off + s] * 64 + k] * (r * seg_dur[off + s]));
     };
     if (tid == 0) {
         mbar_init(&sm.bar[0], 1);
@@ -234,25 +289,25 @@ __global__ void __launch_bounds__(DT, 2) chain_dmma64_kernel(int K, int C, const
     }
     fill_D(0);
 
-    // accumulator = the warp's 32x64 slab of the running product, as 4 (m) x 8 (n) C-fragments.
+    // accumulator = the warp's slab of the running product, as MTW (m) x 8 (n) C-fragments.
     // Start: rows of U_{e_hi}; U^T in B-fragment order doubles as U in A-fragment order (same index map).
-    double acc[4][8][2];
+    double acc[MTW][8][2];
     {
         const double2* src = reinterpret_cast<const double2*>(UTB + (size_t)e_hi * FRAG_DOUBLES);
 #pragma unroll
-        for (int mt = 0; mt < 4; mt++)
+        for (int mt = 0; mt < MTW; mt++)
 #pragma unroll
             for (int kt = 0; kt < 8; kt++) {
-                double2 v = __ldg(&src[(kt * 8 + (4 * half + mt)) * 32 + lane]);
+                double2 v = __ldg(&src[(kt * 8 + (MTW * rb + mt)) * 32 + lane]);
                 acc[mt][kt][0] = v.x;
                 acc[mt][kt][1] = v.y;
             }
     }
     __syncthreads();
 
-    for (int t = 0; t < n; t++) {
+    for (int t = 0; t < ns; t++) {
         const int st = t & 1;
-        if (t + 1 < n) {               // prefetch the next stage into the other buffer (freed at the end of t-1)
+        if (t + 1 < ns) {              // prefetch the next stage into the other buffer (freed at the end of t-1)
             if (tid == 0) {
                 mbar_expect_tx(&sm.bar[st ^ 1], FRAG_DOUBLES * 8);
                 bulk_g2s(sm.B[st ^ 1], stage_src(t + 1), FRAG_DOUBLES * 8, &sm.bar[st ^ 1]);
@@ -260,37 +315,8 @@ __global__ void __launch_bounds__(DT, 2) chain_dmma64_kernel(int K, int C, const
             fill_D(t + 1);
         }
         mbar_wait(&sm.bar[st], (t >> 1) & 1);
-        if (active) {
-            const double2* Bs = reinterpret_cast<const double2*>(sm.B[st]);
-            const double2* Ds = reinterpret_cast<const double2*>(sm.D[st][w >> 1]);
-#pragma unroll
-            for (int mp = 0; mp < 2; mp++) {
-                double a[2][8][2];
-#pragma unroll
-                for (int kt = 0; kt < 8; kt++) {
-                    double2 dv = Ds[kt * 4 + q];       // D[8kt + 2q], D[8kt + 2q + 1]
-#pragma unroll
-                    for (int mi = 0; mi < 2; mi++) {
-                        a[mi][kt][0] = acc[2 * mp + mi][kt][0] * dv.x;
-                        a[mi][kt][1] = acc[2 * mp + mi][kt][1] * dv.y;
-                        acc[2 * mp + mi][kt][0] = 0.0;
-                        acc[2 * mp + mi][kt][1] = 0.0;
-                    }
-                }
-#pragma unroll
-                for (int kt = 0; kt < 8; kt++)
-#pragma unroll
-                    for (int nt = 0; nt < 8; nt++) {
-                        const double2 bv = Bs[(kt * 8 + nt) * 32 + lane];
-                        // h outer, mi inner: two other DMMAs sit between the two that update the same accumulator tile
-#pragma unroll
-                        for (int h = 0; h < 2; h++)
-#pragma unroll
-                            for (int mi = 0; mi < 2; mi++)
-                                dmma884(acc[2 * mp + mi][nt][0], acc[2 * mp + mi][nt][1], a[mi][kt][h], h ? bv.y : bv.x);
-                    }
-            }
-        }
+        if (active)
+            dmma_stage<MTW>(acc, reinterpret_cast<const double2*>(sm.B[st]), reinterpret_cast<const double2*>(sm.D[st][wc]), lane, q);
         __syncthreads();
     }
 
@@ -298,8 +324,8 @@ __global__ void __launch_bounds__(DT, 2) chain_dmma64_kernel(int K, int C, const
     double* out = P + ((size_t)b * C + c) * K * K;
     bool bad = false;
 #pragma unroll
-    for (int mt = 0; mt < 4; mt++) {
-        const int i = 32 * half + 8 * mt + g;
+    for (int mt = 0; mt < MTW; mt++) {
+        const int i = 8 * MTW * rb + 8 * mt + g;
         if (i >= K) continue;
         const double si = isp[e_hi * 64 + i];
 #pragma unroll
@@ -317,13 +343,88 @@ __global__ void __launch_bounds__(DT, 2) chain_dmma64_kernel(int K, int C, const
     if (bad) atomicOr(status, EPX_ST_NONFINITE_P);
 }
 
+// f1, second half (the convolutions dominate when many branches cross many
+// boundaries).  Products of consecutive FULL epochs do not depend on the branch:
+//   G[a, b] = D_a W_a D_{a-1} W_{a-1} ... D_b W_b,   D_e = exp(Lambda_e r_c (tau_e - tau_{e-1})),   1 <= b <= a <= M-2
+// maps the eigenbasis of epoch a to that of epoch b - 1.  One CTA per (a, pair of categories) accumulates G[a, a], G[a, a-1],
+// ..., G[a, 1] with the chain kernel's own stage code, starting from the identity, and stores each in B-fragment order.
+__global__ void __launch_bounds__(128, 2) epoch_product_table_kernel(int C, int M, const double* __restrict__ tau,
+    const double* __restrict__ rates, const double* __restrict__ lam, const double* __restrict__ WB, double* __restrict__ GB)
+{
+    extern __shared__ __align__(128) unsigned char smraw[];
+    DmmaSmemT<2>& sm = *reinterpret_cast<DmmaSmemT<2>*>(smraw);
+    const int tid = threadIdx.x, lane = tid & 31, w = tid >> 5, g = lane >> 2, q = lane & 3;
+    const int ncg = (C + 1) / 2;
+    const int a = 1 + blockIdx.x / ncg, cg = blockIdx.x % ncg;
+    const int c = cg * 2 + (w >> 1), half = w & 1;
+    const bool active = c < C;
+    const int ns = a;                               // stages: epochs a, a-1, ..., 1
+    auto fill_D = [&](int t) {
+        const int cc = cg * 2 + (tid >> 6), k = tid & 63, e = a - t;
+        const double r = cc < C ? rates[cc] : 0.0;
+        sm.D[t & 1][tid >> 6][k] = exp(lam[e * 64 + k] * (r * (tau[e] - tau[e - 1])));
+    };
+    if (tid == 0) {
+        mbar_init(&sm.bar[0], 1);
+        mbar_init(&sm.bar[1], 1);
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    }
+    __syncthreads();
+    if (tid == 0) {
+        mbar_expect_tx(&sm.bar[0], FRAG_DOUBLES * 8);
+        bulk_g2s(sm.B[0], WB + (size_t)a * FRAG_DOUBLES, FRAG_DOUBLES * 8, &sm.bar[0]);
+    }
+    fill_D(0);
+    double acc[4][8][2];                            // identity: row 32 half + 8 mt + g, columns 8 nt + 2 q + h
+#pragma unroll
+    for (int mt = 0; mt < 4; mt++)
+#pragma unroll
+        for (int nt = 0; nt < 8; nt++)
+#pragma unroll
+            for (int h = 0; h < 2; h++) acc[mt][nt][h] = (32 * half + 8 * mt + g == 8 * nt + 2 * q + h) ? 1.0 : 0.0;
+    __syncthreads();
+    for (int t = 0; t < ns; t++) {
+        const int st = t & 1;
+        if (t + 1 < ns) {
+            if (tid == 0) {
+                mbar_expect_tx(&sm.bar[st ^ 1], FRAG_DOUBLES * 8);
+                bulk_g2s(sm.B[st ^ 1], WB + (size_t)(a - t - 1) * FRAG_DOUBLES, FRAG_DOUBLES * 8, &sm.bar[st ^ 1]);
+            }
+            fill_D(t + 1);
+        }
+        mbar_wait(&sm.bar[st], (t >> 1) & 1);
+        if (active) {
+            dmma_stage<4>(acc, reinterpret_cast<const double2*>(sm.B[st]), reinterpret_cast<const double2*>(sm.D[st][w >> 1]), lane, q);
+            // G[a, a - t] in B-fragment order: element X[kappa][col] sits at ((kappa/8 * 8 + col/8) * 32 + 4 (col%8) + (kappa%8)/2) * 2 + kappa%2
+            double* out = GB + ((size_t)epoch_pair_index(a, a - t) * C + c) * FRAG_DOUBLES;
+#pragma unroll
+            for (int mt = 0; mt < 4; mt++)
+#pragma unroll
+                for (int nt = 0; nt < 8; nt++)
+#pragma unroll
+                    for (int h = 0; h < 2; h++)
+                        out[(((4 * half + mt) * 8 + nt) * 32 + 4 * (2 * q + h) + (g >> 1)) * 2 + (g & 1)] = acc[mt][nt][h];
+        }
+        __syncthreads();
+    }
+}
+
 }  // namespace
 
 int chain_init_attributes()
 {
     if (cudaFuncSetAttribute(chain_generic_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, 112 * 1024) != cudaSuccess) return -1;
-    if (cudaFuncSetAttribute(chain_dmma64_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(DmmaSmem)) != cudaSuccess) return -1;
+    if (cudaFuncSetAttribute(chain_dmma64_kernel<2, 2>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(DmmaSmemT<2>)) != cudaSuccess) return -1;
+    if (cudaFuncSetAttribute(chain_dmma64_kernel<1, 4>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(DmmaSmemT<1>)) != cudaSuccess) return -1;
+    if (cudaFuncSetAttribute(epoch_product_table_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(DmmaSmemT<2>)) != cudaSuccess) return -1;
     return 0;
+}
+
+// f1: the chain kernels multiply by cached products of consecutive full epochs (option on, 64-padded reversible models,
+// durations not rescaled per branch, at least two interior epochs)
+bool chain_uses_epoch_products(const epx_ctx* c)
+{
+    return c->epoch_products && c->Kp == 64 && c->chain_kernel != 1 && !c->has_brates && c->M >= 4;
 }
 
 int launch_chain_reversible(const epx_ctx* c, cudaStream_t s)
@@ -340,10 +441,29 @@ int launch_chain_reversible(const epx_ctx* c, cudaStream_t s)
         chain_rows_kernel<4><<<blocks, 256, 0, s>>>(n, C, c->sub_list, d.n_seg, d.seg_off, d.seg_epoch, d.seg_dur, d.rates,
                                                     d.lam, d.U, d.W, d.sp, d.isp, d.P, d.status);
     } else if (Kp == 64 && c->chain_kernel != 1) {
-        int ncg = (C + CPC - 1) / CPC;
-        chain_dmma64_kernel<<<n * ncg, DT, sizeof(DmmaSmem), s>>>(K, C, order, d.n_seg, d.seg_off, d.seg_epoch,
-                                                                 d.seg_dur, d.rates, d.lam, d.WB, d.UTB, d.sp, d.isp,
-                                                                 d.P, d.status);
+        int launched = 0;
+        if (chain_uses_epoch_products(c)) {
+            // (an incremental call keeps the table: it depends on the boundaries, the models and the category rates only)
+            if (!c->sub_list) {
+                epoch_product_table_kernel<<<(c->M - 2) * ((C + 1) / 2), 128, sizeof(DmmaSmemT<2>), s>>>(C, c->M, d.tau, d.rates, d.lam,
+                                                                                                       d.WB, d.GB);
+                launched++;
+            }
+            chain_dmma64_kernel<1, 4><<<n * C, 128, sizeof(DmmaSmemT<1>), s>>>(K, C, c->M, order, d.n_seg, d.seg_off, d.seg_epoch,
+                                                                               d.seg_dur, d.rates, d.lam, d.WB, d.UTB, d.GB, d.sp,
+                                                                               d.isp, d.P, d.status);
+        } else if (c->chain_kernel != 2) {       // default: one category per CTA, four warps of 16 rows (162 registers, no spill,
+                                                 // three CTAs per SM: measured 4.74 ms on config 5 against 5.02 ms for <2, 2>)
+            chain_dmma64_kernel<1, 4><<<n * C, 128, sizeof(DmmaSmemT<1>), s>>>(K, C, c->M, order, d.n_seg, d.seg_off, d.seg_epoch,
+                                                                               d.seg_dur, d.rates, d.lam, d.WB, d.UTB, nullptr, d.sp,
+                                                                               d.isp, d.P, d.status);
+        } else {                                 // round 1's layout: two categories per CTA share one staged operand
+            const int ncg = (C + 1) / 2;
+            chain_dmma64_kernel<2, 2><<<n * ncg, 128, sizeof(DmmaSmemT<2>), s>>>(K, C, c->M, order, d.n_seg, d.seg_off, d.seg_epoch,
+                                                                                 d.seg_dur, d.rates, d.lam, d.WB, d.UTB, nullptr,
+                                                                                 d.sp, d.isp, d.P, d.status);
+        }
+        return cudaGetLastError() == cudaSuccess ? launched + 1 : -1;
     } else {
         size_t smem = sizeof(double) * (2 * (size_t)Kp * (Kp + 1) + (size_t)Kp * Kp + Kp);
         chain_generic_kernel<<<n * C, GT, smem, s>>>(K, Kp, C, order, d.n_seg, d.seg_off, d.seg_epoch, d.seg_dur,

@@ -88,6 +88,7 @@ struct DevBuffers {
     double* isp;          // [M][Kp] 1/sqrt(pi)
     double* WB;           // [M][64*64] W in DMMA B-fragment order   (Kp == 64 only)
     double* UTB;          // [M][64*64] U^T in DMMA B-fragment order == U in A-fragment order (Kp == 64 only)
+    double* GB;           // [(M-2)(M-1)/2][C][64*64] f1: products of consecutive full epochs, B-fragment order (Kp == 64 only)
     // a2' (asymmetric)
     double* Efull;        // [M][C][K][K] exp(Q_e r_c (tau_e - tau_{e-1})) for interior epochs 1..M-2
     // a3/a4 output
@@ -120,6 +121,7 @@ struct epx_ctx {
     int prune_kernel = 0;  // EPX_OPT_PRUNE_KERNEL: 0 auto, 1 force the generic shared-memory kernel
     int dfs_ppl = 0;       // EPX_OPT_DFS_PPL: patterns per lane of the depth-first pruning walk (0 auto, 1, 2, 4)
     int dfs_want = 0;      // EPX_OPT_DFS_PIECES: pieces the tree is cut into for the depth-first walks (0 auto)
+    int epoch_products = 0; // EPX_OPT_EPOCH_PRODUCTS: 1 = chains over >= 2 full epochs use their cached product (f1); 0 (default) off
     int dedup = 1;         // EPX_OPT_SHARE_PROCESSES: 1 (default) one eigensystem / table entry per distinct process, 0 one per epoch
     std::vector<int32_t> eproc, fproc;   // host copies of the maps above (rebuilt when a model or a boundary changes)
     int jacobi_kernel = 0; // EPX_OPT_JACOBI_KERNEL: 0 auto (K <= 62: one barrier per round), 1 round 1's two-barrier kernel
@@ -210,6 +212,7 @@ struct epx_ctx {
 int launch_segmenter(const epx_ctx* c, cudaStream_t s);
 int launch_eigensystems(const epx_ctx* c, cudaStream_t s);
 int launch_chain_reversible(const epx_ctx* c, cudaStream_t s);
+bool chain_uses_epoch_products(const epx_ctx* c);
 int launch_pade_chain(const epx_ctx* c, cudaStream_t s);
 int launch_taylor_chain(const epx_ctx* c, cudaStream_t s);   // same kernels, shifted non-negative Taylor exponential
 int launch_pruning(const epx_ctx* c, cudaStream_t s);

@@ -254,10 +254,13 @@ def test_config6_amino_acid_full_size(epx, orc_ld):
 
 def test_config5_reduced_every_branch(epx, orc_ld):
     prob = W.make_config(5, n_br=300)
-    for kernel, jacobi in ((0, 0), (1, 0), (0, 1)):        # DMMA / generic chain kernel; one-barrier / round-1 Jacobi
+    # DMMA (two categories / one category per CTA) / generic chain kernel; one-barrier / round-1 Jacobi; f1: cached products
+    # of consecutive full epochs (Eq. 7 re-associated: same matrices within the same 1e-12)
+    for kernel, jacobi, cache in ((0, 0, 0), (1, 0, 0), (0, 1, 0), (2, 0, 0), (0, 0, 1)):
         ctx = epx.from_problem(prob)
         ctx.set_option(epx.EPX_OPT_CHAIN_KERNEL, kernel)
         ctx.set_option(epx.EPX_OPT_JACOBI_KERNEL, jacobi)
+        ctx.set_option(epx.EPX_OPT_EPOCH_PRODUCTS, cache)
         ctx.update_matrices()
         ref = orc_ld.evaluate(prob)
         check_segments(ctx, ref)
@@ -266,11 +269,14 @@ def test_config5_reduced_every_branch(epx, orc_ld):
         ctx.close()
 
 
-def test_config5_full_size_sampled(epx, orc_ld):
+@pytest.mark.parametrize("cache", [0, 1])
+def test_config5_full_size_sampled(epx, orc_ld, cache):
     # full launch configuration (20 000 branches); segments checked for every branch, matrices for a seeded sample
-    # that always includes the longest chains, plus row sums / non-negativity for every matrix
+    # that always includes the longest chains, plus row sums / non-negativity for every matrix.  cache = 1: SURVEY.md 8(f) f1,
+    # chains over >= 2 full epochs multiply by the tabulated product of those epochs
     prob = W.make_config(5)
     ctx = epx.from_problem(prob)
+    ctx.set_option(epx.EPX_OPT_EPOCH_PRODUCTS, cache)
     ctx.update_matrices()
     off_ref, ep_ref, du_ref = orc_ld.segments(prob.child_height, prob.parent_height, prob.tau)
     off = check_segments(ctx, {"seg_off": off_ref, "seg_epoch": ep_ref, "seg_dur": du_ref})
