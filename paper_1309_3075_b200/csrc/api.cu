@@ -597,29 +597,34 @@ static int set_tips_impl(epx_ctx* c, const T* states)
     }
     const unsigned K = (unsigned)c->K;
     uint8_t* const base = c->tips;
-    auto convert_rows = [=](size_t t0, size_t t1) {
+    // rows [t0, t1): everything the inner loops read is a by-value local (a byte store may alias any object in memory, so
+    // values reached through a closure or the ctx would be re-read every iteration and the loops would not vectorise)
+    auto convert_rows = [](const T* states, uint8_t* base, size_t L, size_t Lp, unsigned K, size_t t0, size_t t1) {
         for (size_t t = t0; t < t1; t++) {
             const T* __restrict__ src = states + t * L;
             uint8_t* __restrict__ dst = base + t * Lp;
             if (sizeof(T) == 1) {
                 const uint8_t k8 = (uint8_t)K;                // K <= 64
                 const uint8_t* __restrict__ s8 = reinterpret_cast<const uint8_t*>(src);
-                for (size_t p = 0; p < L; p++) dst[p] = (uint8_t)(s8[p] | (uint8_t)(0 - (uint8_t)(s8[p] >= k8)));   // byte-wide, vectorises
+                for (size_t p = 0; p < L; p++) dst[p] = (uint8_t)(s8[p] | (uint8_t)(0 - (uint8_t)(s8[p] >= k8)));   // byte-wide
             } else {
+                const uint32_t* __restrict__ s32 = reinterpret_cast<const uint32_t*>(src);
                 for (size_t p = 0; p < L; p++) {
-                    const unsigned s = (unsigned)src[p];      // negative int32 -> huge -> missing
-                    dst[p] = s < K ? (uint8_t)s : (uint8_t)255;
+                    const uint32_t s = s32[p];                // negative int32 -> huge -> missing
+                    dst[p] = (uint8_t)(s < K ? s : 255u);
                 }
             }
             for (size_t p = L; p < Lp; p++) dst[p] = 255;
         }
     };
-    size_t nthreads = std::min<size_t>(std::min<size_t>(16, std::max(1u, std::thread::hardware_concurrency())), (N * L) >> 20);
+    const size_t nthreads = std::min<size_t>(std::min<size_t>(16, std::max(1u, std::thread::hardware_concurrency())), (N * L) >> 21);
     if (nthreads <= 1) {
-        convert_rows(0, N);
+        convert_rows(states, base, L, Lp, K, 0, N);
     } else {
         std::vector<std::thread> pool;
-        for (size_t w = 0; w < nthreads; w++) pool.emplace_back(convert_rows, N * w / nthreads, N * (w + 1) / nthreads);
+        for (size_t w = 1; w < nthreads; w++)
+            pool.emplace_back(convert_rows, states, base, L, Lp, K, N * w / nthreads, N * (w + 1) / nthreads);
+        convert_rows(states, base, L, Lp, K, 0, N / nthreads);      // the calling thread takes the first share
         for (auto& th : pool) th.join();
     }
     c->has_tips = true; c->tips_dirty = true;
