@@ -343,16 +343,19 @@ def set_problem(ctx: Epx, prob, tip_states_u8=None) -> None:
     """Call every setter of `ctx` from a problem object (attributes as in workloads.EpochProblem; read by
     attribute, nothing is imported).  `tip_states_u8`: the tip states as a host uint8 array, passed through
     epx_set_tip_states_u8 instead of the int32 form."""
+    if prob.N > 0:
+        # the largest input first: on a bound ctx its host -> device copy is pipelined with the repacking and then runs
+        # behind the host work of the other setters (validation, pruning plan)
+        if tip_states_u8 is not None:
+            ctx.set_tip_states_u8(tip_states_u8)
+        else:
+            ctx.set_tip_states(prob.tip_states)
     ctx.set_epoch_boundaries(prob.tau)
     for e in range(prob.M):
         ctx.set_epoch_model(e, prob.Q[e], prob.freqs[e], prob.reversible)
     ctx.set_category_rates(prob.rates, prob.weights)
     if prob.N > 0:
         ctx.set_tree(prob.parent, prob.height)
-        if tip_states_u8 is not None:
-            ctx.set_tip_states_u8(tip_states_u8)
-        else:
-            ctx.set_tip_states(prob.tip_states)
         ctx.set_pattern_weights(prob.pattern_weights)
         ctx.set_root_frequencies(prob.root_freqs)
     else:

@@ -6,6 +6,7 @@
 #include "epx_internal.h"
 
 #include <algorithm>
+#include <atomic>
 #include <cmath>
 #include <cstdarg>
 #include <cstdio>
@@ -620,12 +621,42 @@ static int set_tips_impl(epx_ctx* c, const T* states)
     const size_t nthreads = std::min<size_t>(std::min<size_t>(16, std::max(1u, std::thread::hardware_concurrency())), (N * L) >> 21);
     if (nthreads <= 1) {
         convert_rows(states, base, L, Lp, K, 0, N);
-    } else {
+    } else if (!(c->bound && c->tips_pinned)) {
         std::vector<std::thread> pool;
         for (size_t w = 1; w < nthreads; w++)
             pool.emplace_back(convert_rows, states, base, L, Lp, K, N * w / nthreads, N * (w + 1) / nthreads);
         convert_rows(states, base, L, Lp, K, 0, N / nthreads);      // the calling thread takes the first share
         for (auto& th : pool) th.join();
+    } else {
+        // Bound ctx: the host -> device copy is pipelined with the repacking.  Workers take chunks of rows in order; the
+        // calling thread enqueues the copy of chunk k on the ctx's stream as soon as chunk k is complete, so the DMA of one
+        // chunk runs while the next ones are still being repacked (page-locked source, stream-ordered after the last
+        // evaluation that read the tips).
+        CUDA_TRY(c, cudaSetDevice(c->device));
+        const size_t nchunks = std::min<size_t>(N, 4 * nthreads);
+        std::atomic<size_t> next{0};
+        std::vector<std::atomic<int>> done(nchunks);
+        for (auto& f : done) f.store(0, std::memory_order_relaxed);
+        auto worker = [&]() {
+            for (size_t k; (k = next.fetch_add(1)) < nchunks;) {
+                convert_rows(states, base, L, Lp, K, N * k / nchunks, N * (k + 1) / nchunks);
+                done[k].store(1, std::memory_order_release);
+            }
+        };
+        std::vector<std::thread> pool;
+        for (size_t w = 1; w < nthreads; w++) pool.emplace_back(worker);
+        cudaError_t err = cudaSuccess;
+        for (size_t k = 0; k < nchunks; k++) {
+            while (!done[k].load(std::memory_order_acquire)) std::this_thread::yield();
+            const size_t r0 = N * k / nchunks, r1 = N * (k + 1) / nchunks;
+            if (err == cudaSuccess)
+                err = cudaMemcpyAsync(c->d.tips + r0 * Lp, base + r0 * Lp, (r1 - r0) * Lp, cudaMemcpyHostToDevice, c->stream);
+        }
+        for (auto& th : pool) th.join();
+        if (err != cudaSuccess) return fail(c, EPX_E_CUDA, "cudaMemcpyAsync (tip states): %s", cudaGetErrorString(err));
+        c->has_tips = true; c->tips_dirty = false;     // already on its way to the device
+        c->inc_valid = false;
+        return EPX_OK;
     }
     c->has_tips = true; c->tips_dirty = true;
     return EPX_OK;
