@@ -90,7 +90,7 @@ size_t plan_workspace(const epx_ctx* c, char* base, DevBuffers* d)
     if (c->tree_mode) {
         // sized for every layout an option can select later: states padded to 8 and one exponent per category when K > 8
         const size_t Kalloc = K > 8 ? (size_t)prune_kp(c) : K;
-        t.PB = (double*)take(K > 8 ? 8 * S * C * Kalloc * Kalloc : 0);
+        t.PB = (double*)take(K != 4 ? 8 * S * C * Kalloc * Kalloc : 0);     // fragment-ordered / transposed copies of P
         t.partials = (double*)take(8 * (N - 1 + (size_t)c->tip_cap) * C * L * Kalloc);
         t.scale_exp = (int32_t*)take(4 * (N - 1 + (size_t)c->tip_cap) * L * (K > 8 ? C : 1));
         t.site_lnl = (double*)take(8 * L);

@@ -14,7 +14,10 @@
 
 namespace {
 
-constexpr int PT = 256;
+constexpr int PT_MAX = 512;  // threads per CTA: 512 for K > 32 (a 61 x 61 product is 8 row tiles x 2 groups of 4 column tiles = one
+                             // item per warp; config 3 chain 0.264 -> 0.224 ms), 256 otherwise (K = 24 is barrier-bound in the
+                             // Gauss-Jordan sweep: 512 threads measured 0.81 ms against 0.33 ms on config 4)
+__host__ __device__ inline int pade_threads(int K) { return K > 32 ? 512 : 256; }
 
 __device__ __forceinline__ void dmma884(double& d0, double& d1, double a, double b)
 {
@@ -24,15 +27,17 @@ __device__ __forceinline__ void dmma884(double& d0, double& d1, double a, double
 // C = A B for dense K x K matrices in shared memory (row stride K).  The K^3 products of the scaling-and-squaring
 // exponentials are where this file spends its time; they run on the FP64 tensor pipe: warp w owns the 8-row tiles w,
 // w + 8, ..., all column tiles of a row tile accumulate in registers, fragments outside the matrix are zero.
+template <int PT>
 __device__ __forceinline__ void mm(int K, const double* __restrict__ A, const double* __restrict__ B,
                                    double* __restrict__ Cm)
 {
     const int lane = threadIdx.x & 31, w = threadIdx.x >> 5, g = lane >> 2, q = lane & 3;
-    const int nt_n = (K + 7) >> 3, nk = (K + 3) >> 2;
-    for (int mt = w; mt < nt_n; mt += PT / 32) {
+    const int nt_n = (K + 7) >> 3, nk = (K + 3) >> 2, ngrp = (nt_n + 3) >> 2;
+    for (int item = w; item < nt_n * ngrp; item += PT / 32) {      // item = (row tile, group of four column tiles)
+        const int mt = item / ngrp, n0 = 4 * (item - mt * ngrp);
         const int row = 8 * mt + g;
         const bool row_ok = row < K;
-        for (int n0 = 0; n0 < nt_n; n0 += 4) {                  // four column tiles at a time: 8 accumulator registers
+        {
             double acc[4][2] = {{0.0, 0.0}, {0.0, 0.0}, {0.0, 0.0}, {0.0, 0.0}};
             for (int kt = 0; kt < nk; kt++) {
                 const int k = 4 * kt + q;
@@ -58,10 +63,11 @@ __device__ __forceinline__ void mm(int K, const double* __restrict__ A, const do
 
 struct PadeBufs {
     double *A, *A2, *A4, *A6, *T1, *T2, *col;
-    double* red;   // [PT/32 + 2]
+    double* red;   // [PT_MAX/32 + 2]
 };
 
 // In: b.A holds the (unscaled) matrix.  Returns the buffer (b.T1 or b.T2) that holds exp(A).  All threads call.
+template <int PT>
 __device__ double* pade13(int K, PadeBufs& b, int32_t* status)
 {
     const double c[14] = {64764752532480000.0, 32382376266240000.0, 7771770303897600.0, 1187353796428800.0,
@@ -87,21 +93,21 @@ __device__ double* pade13(int K, PadeBufs& b, int32_t* status)
     __syncthreads();
     for (int idx = tid; idx < KK; idx += PT) b.A[idx] *= sc;
     __syncthreads();
-    mm(K, b.A, b.A, b.A2);
-    mm(K, b.A2, b.A2, b.A4);
-    mm(K, b.A4, b.A2, b.A6);
+    mm<PT>(K, b.A, b.A, b.A2);
+    mm<PT>(K, b.A2, b.A2, b.A4);
+    mm<PT>(K, b.A4, b.A2, b.A6);
     for (int idx = tid; idx < KK; idx += PT) b.T1[idx] = c[13] * b.A6[idx] + c[11] * b.A4[idx] + c[9] * b.A2[idx];
     __syncthreads();
-    mm(K, b.A6, b.T1, b.T2);
+    mm<PT>(K, b.A6, b.T1, b.T2);
     for (int idx = tid; idx < KK; idx += PT) {
         double d = (idx / K == idx % K) ? c[1] : 0.0;
         b.T2[idx] += c[7] * b.A6[idx] + c[5] * b.A4[idx] + c[3] * b.A2[idx] + d;
     }
     __syncthreads();
-    mm(K, b.A, b.T2, b.T1);                                 // T1 = U
+    mm<PT>(K, b.A, b.T2, b.T1);                                 // T1 = U
     for (int idx = tid; idx < KK; idx += PT) b.T2[idx] = c[12] * b.A6[idx] + c[10] * b.A4[idx] + c[8] * b.A2[idx];
     __syncthreads();
-    mm(K, b.A6, b.T2, b.A);                                 // A = A6 * (...)
+    mm<PT>(K, b.A6, b.T2, b.A);                                 // A = A6 * (...)
     for (int idx = tid; idx < KK; idx += PT) {
         double d = (idx / K == idx % K) ? c[0] : 0.0;
         double v = b.A[idx] + c[6] * b.A6[idx] + c[4] * b.A4[idx] + c[2] * b.A2[idx] + d;   // V
@@ -110,10 +116,15 @@ __device__ double* pade13(int K, PadeBufs& b, int32_t* status)
         b.T1[idx] = v + u;                                  // right-hand side, becomes R
     }
     __syncthreads();
-    // Gauss-Jordan with partial pivoting on [A2 | T1]
+    // Gauss-Jordan with partial pivoting on [A2 | T1].  Thread (r0, j) owns column j of the augmented matrix for the rows
+    // r0, r0 + nr, ...: no index arithmetic inside the sweep (the K = 24 case is bound by instruction issue and barriers).
     double* Lh = b.A2;
     double* Rh = b.T1;
-    int* piv = reinterpret_cast<int*>(b.red + PT / 32);
+    int* piv = reinterpret_cast<int*>(b.red + PT_MAX / 32);
+    double* prow = b.col + K;                          // [2K] the scaled pivot row
+    const int K2 = 2 * K, nr = PT / K2, r0 = tid / K2, j = tid - r0 * K2;
+    const bool on = nr > 0 ? r0 < nr : tid < K2;       // (a CTA narrower than 2K columns is not launched: PT >= 256 >= 2K)
+    double* const Mj = j < K ? Lh + j : Rh + (j - K);  // column j, row stride K
     for (int k = 0; k < K; k++) {
         if (tid < 32) {
             double best = -1.0; int bi = k;
@@ -130,31 +141,24 @@ __device__ double* pade13(int K, PadeBufs& b, int32_t* status)
         }
         __syncthreads();
         const int p = *piv;
-        if (p != k)
-            for (int j = tid; j < 2 * K; j += PT) {
-                double* Mx = j < K ? Lh : Rh; int jj = j < K ? j : j - K;
-                double t = Mx[k * K + jj]; Mx[k * K + jj] = Mx[p * K + jj]; Mx[p * K + jj] = t;
-            }
-        __syncthreads();
-        const double pinv = 1.0 / Lh[k * K + k];
-        for (int i = tid; i < K; i += PT) b.col[i] = (i == k) ? 0.0 : Lh[i * K + k];
-        __syncthreads();
-        for (int j = tid; j < 2 * K; j += PT) {
-            double* Mx = j < K ? Lh : Rh; int jj = j < K ? j : j - K;
-            Mx[k * K + jj] *= pinv;
+        if (p != k) {                                  // (uniform)
+            if (tid < K2) { const double t = Mj[k * K]; Mj[k * K] = Mj[p * K]; Mj[p * K] = t; }
+            __syncthreads();
         }
+        const double pinv = 1.0 / Lh[k * K + k];
+        if (tid < K) b.col[tid] = (tid == k) ? 0.0 : Lh[tid * K + k];
+        if (tid < K2) prow[tid] = Mj[k * K] * pinv;
         __syncthreads();
-        for (int idx = tid; idx < 2 * KK; idx += PT) {
-            int i = idx / (2 * K), j = idx % (2 * K);
-            double* Mx = j < K ? Lh : Rh; int jj = j < K ? j : j - K;
-            Mx[i * K + jj] = fma(-b.col[i], Mx[k * K + jj], Mx[i * K + jj]);
+        if (on) {
+            const double pk = prow[j];
+            for (int i = r0; i < K; i += nr) Mj[i * K] = (i == k) ? pk : fma(-b.col[i], pk, Mj[i * K]);
         }
         __syncthreads();
     }
     double* R = b.T1;
     double* O = b.T2;
     for (int q = 0; q < s; q++) {
-        mm(K, R, R, O);
+        mm<PT>(K, R, R, O);
         double* t = R; R = O; O = t;
     }
     return R;
@@ -169,6 +173,7 @@ __device__ double* pade13(int K, PadeBufs& b, int32_t* status)
 //   M = (A + mu I) / 2^s, ||M||_inf = mu / 2^s <= 1;  degree-16 Taylor by Paterson-Stockmeyer (powers M^2..M^4, three
 //   Horner steps: 6 products);  R = e^{-mu/2^s} * poly(M) (stochastic);  R <- R^2 s times.
 // In: b.A holds A.  Returns the buffer that holds exp(A).  All threads call.
+template <int PT>
 __device__ double* expm_shifted_taylor(int K, PadeBufs& b, int32_t* status)
 {
     const double c[17] = {1.0, 1.0, 1.0 / 2, 1.0 / 6, 1.0 / 24, 1.0 / 120, 1.0 / 720, 1.0 / 5040, 1.0 / 40320,
@@ -194,9 +199,9 @@ __device__ double* expm_shifted_taylor(int K, PadeBufs& b, int32_t* status)
         M1[idx] = v * sc;
     }
     __syncthreads();
-    mm(K, M1, M1, M2);
-    mm(K, M2, M1, M3);
-    mm(K, M2, M2, M4);
+    mm<PT>(K, M1, M1, M2);
+    mm<PT>(K, M2, M1, M3);
+    mm<PT>(K, M2, M2, M4);
     auto block = [&](int k, int idx) -> double {   // B_k = c[4k] I + c[4k+1] M + c[4k+2] M^2 + c[4k+3] M^3
         double d = (idx / K == idx % K) ? c[4 * k] : 0.0;
         return d + c[4 * k + 1] * M1[idx] + c[4 * k + 2] * M2[idx] + c[4 * k + 3] * M3[idx];
@@ -206,7 +211,7 @@ __device__ double* expm_shifted_taylor(int K, PadeBufs& b, int32_t* status)
     for (int idx = tid; idx < KK; idx += PT) R[idx] = block(3, idx) + c[16] * M4[idx];
     __syncthreads();
     for (int k = 2; k >= 0; k--) {
-        mm(K, R, M4, O);
+        mm<PT>(K, R, M4, O);
         for (int idx = tid; idx < KK; idx += PT) O[idx] += block(k, idx);
         __syncthreads();
         double* t = R; R = O; O = t;
@@ -215,16 +220,16 @@ __device__ double* expm_shifted_taylor(int K, PadeBufs& b, int32_t* status)
     for (int idx = tid; idx < KK; idx += PT) R[idx] *= damp;
     __syncthreads();
     for (int q = 0; q < s; q++) {
-        mm(K, R, R, O);
+        mm<PT>(K, R, R, O);
         double* t = R; R = O; O = t;
     }
     return R;
 }
 
-template <int METHOD>
+template <int METHOD, int PT>
 __device__ __forceinline__ double* expm_dense(int K, PadeBufs& b, int32_t* status)
 {
-    return METHOD == 0 ? pade13(K, b, status) : expm_shifted_taylor(K, b, status);
+    return METHOD == 0 ? pade13<PT>(K, b, status) : expm_shifted_taylor<PT>(K, b, status);
 }
 
 __device__ __forceinline__ void carve(int K, double* sm, PadeBufs& b, double*& acc)
@@ -232,11 +237,11 @@ __device__ __forceinline__ void carve(int K, double* sm, PadeBufs& b, double*& a
     const size_t KK = (size_t)K * K;
     b.A = sm; b.A2 = sm + KK; b.A4 = sm + 2 * KK; b.A6 = sm + 3 * KK; b.T1 = sm + 4 * KK; b.T2 = sm + 5 * KK;
     acc = sm + 6 * KK;
-    b.col = sm + 7 * KK;
-    b.red = b.col + K;
+    b.col = sm + 7 * KK;          // [K] pivot column + [2K] scaled pivot row
+    b.red = b.col + 3 * K;
 }
 
-template <int METHOD>
+template <int METHOD, int PT>
 __global__ void __launch_bounds__(PT) pade_full_epoch_kernel(int K, int M, int C, const double* __restrict__ Q,
     const double* __restrict__ tau, const double* __restrict__ rates, double* __restrict__ Efull,
     int32_t* __restrict__ status, const int32_t* __restrict__ fproc)
@@ -250,7 +255,7 @@ __global__ void __launch_bounds__(PT) pade_full_epoch_kernel(int K, int M, int C
     const double* Qe = Q + (size_t)e * K * K;
     for (int idx = threadIdx.x; idx < K * K; idx += PT) b.A[idx] = Qe[idx] * scale;
     __syncthreads();
-    double* R = expm_dense<METHOD>(K, b, status);
+    double* R = expm_dense<METHOD, PT>(K, b, status);
     for (int f = e; f <= M - 2; f++) {                       // every epoch that shares this entry
         if (fproc[f] != e) continue;
         double* out = Efull + ((size_t)f * C + c) * K * K;
@@ -258,7 +263,7 @@ __global__ void __launch_bounds__(PT) pade_full_epoch_kernel(int K, int M, int C
     }
 }
 
-template <int METHOD>
+template <int METHOD, int PT>
 __global__ void __launch_bounds__(PT) pade_chain_kernel(int K, int C, int use_table, const int32_t* __restrict__ order,
     const int32_t* __restrict__ n_seg, const int32_t* __restrict__ seg_off, const int32_t* __restrict__ seg_epoch,
     const double* __restrict__ seg_dur, const double* __restrict__ rates, const double* __restrict__ Q,
@@ -291,14 +296,14 @@ __global__ void __launch_bounds__(PT) pade_chain_kernel(int K, int C, int use_ta
             const double* Qe = Q + (size_t)e * KK;
             for (int idx = tid; idx < KK; idx += PT) b.A[idx] = Qe[idx] * scale;
             __syncthreads();
-            E = expm_dense<METHOD>(K, b, status);
+            E = expm_dense<METHOD, PT>(K, b, status);
         }
         if (!cur) {
             for (int idx = tid; idx < KK; idx += PT) acc[idx] = E[idx];
             __syncthreads();
             cur = acc;
         } else {
-            mm(K, cur, E, b.A);      // b.A is free once E is known; the old product buffer becomes the new b.A
+            mm<PT>(K, cur, E, b.A);      // b.A is free once E is known; the old product buffer becomes the new b.A
             double* t = cur; cur = b.A; b.A = t;
         }
     }
@@ -315,19 +320,23 @@ __global__ void __launch_bounds__(PT) pade_chain_kernel(int K, int C, int use_ta
 
 size_t pade_smem_bytes(int K)
 {
-    return sizeof(double) * (7 * (size_t)K * K + K + PT / 32 + 2);
+    return sizeof(double) * (7 * (size_t)K * K + 3 * K + PT_MAX / 32 + 2);
+}
+
+template <int METHOD, int PT>
+static int pade_attr()
+{
+    if (cudaFuncSetAttribute(pade_full_epoch_kernel<METHOD, PT>, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024) != cudaSuccess) return -1;
+    if (cudaFuncSetAttribute(pade_chain_kernel<METHOD, PT>, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024) != cudaSuccess) return -1;
+    return 0;
 }
 
 int pade_init_attributes()
 {
-    if (cudaFuncSetAttribute(pade_full_epoch_kernel<0>, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024) != cudaSuccess) return -1;
-    if (cudaFuncSetAttribute(pade_chain_kernel<0>, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024) != cudaSuccess) return -1;
-    if (cudaFuncSetAttribute(pade_full_epoch_kernel<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024) != cudaSuccess) return -1;
-    if (cudaFuncSetAttribute(pade_chain_kernel<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024) != cudaSuccess) return -1;
-    return 0;
+    return pade_attr<0, 256>() | pade_attr<0, 512>() | pade_attr<1, 256>() | pade_attr<1, 512>();
 }
 
-template <int METHOD>
+template <int METHOD, int PT>
 static int launch_dense(const epx_ctx* c, cudaStream_t s)
 {
     const DevBuffers& d = c->d;
@@ -339,14 +348,14 @@ static int launch_dense(const epx_ctx* c, cudaStream_t s)
     const int32_t* order = c->sub_list ? c->sub_list : d.order;      // depends on tau, Q and the rates only and is kept
     if (n == 0) return 0;
     if (M >= 3 && use_table && !c->sub_list) {
-        pade_full_epoch_kernel<METHOD><<<(M - 2) * C, PT, smem, s>>>(K, M, C, d.Q, d.tau, d.rates, d.Efull, d.status, d.fproc);
+        pade_full_epoch_kernel<METHOD, PT><<<(M - 2) * C, PT, smem, s>>>(K, M, C, d.Q, d.tau, d.rates, d.Efull, d.status, d.fproc);
         launched++;
     }
-    pade_chain_kernel<METHOD><<<n * C, PT, smem, s>>>(K, C, use_table, order, d.n_seg, d.seg_off, d.seg_epoch, d.seg_dur,
-                                                       d.rates, d.Q, d.Efull, d.P, d.status);
+    pade_chain_kernel<METHOD, PT><<<n * C, PT, smem, s>>>(K, C, use_table, order, d.n_seg, d.seg_off, d.seg_epoch, d.seg_dur,
+                                                           d.rates, d.Q, d.Efull, d.P, d.status);
     launched++;
     return cudaGetLastError() == cudaSuccess ? launched : -1;
 }
 
-int launch_pade_chain(const epx_ctx* c, cudaStream_t s) { return launch_dense<0>(c, s); }
-int launch_taylor_chain(const epx_ctx* c, cudaStream_t s) { return launch_dense<1>(c, s); }
+int launch_pade_chain(const epx_ctx* c, cudaStream_t s) { return pade_threads(c->K) == 512 ? launch_dense<0, 512>(c, s) : launch_dense<0, 256>(c, s); }
+int launch_taylor_chain(const epx_ctx* c, cudaStream_t s) { return pade_threads(c->K) == 512 ? launch_dense<1, 512>(c, s) : launch_dense<1, 256>(c, s); }

@@ -599,6 +599,43 @@ __device__ __forceinline__ double dot4(const double* __restrict__ row, const dou
     return (a0 + a1) + (a2 + a3);
 }
 
+// the same sum with the matrix row read at a stride (column i of the transposed copy): same chains, same bits
+__device__ __forceinline__ double dot4s(const double* __restrict__ col, int stride, const double* __restrict__ v, int K)
+{
+    double a0 = 0.0, a1 = 0.0, a2 = 0.0, a3 = 0.0;
+    int j = 0;
+    for (; j + 4 <= K; j += 4) {
+        a0 = fma(col[j * stride], v[j], a0);
+        a1 = fma(col[(j + 1) * stride], v[j + 1], a1);
+        a2 = fma(col[(j + 2) * stride], v[j + 2], a2);
+        a3 = fma(col[(j + 3) * stride], v[j + 3], a3);
+    }
+    if (j < K) a0 = fma(col[j * stride], v[j], a0);
+    if (j + 1 < K) a1 = fma(col[(j + 1) * stride], v[j + 1], a1);
+    if (j + 2 < K) a2 = fma(col[(j + 2) * stride], v[j + 2], a2);
+    return (a0 + a1) + (a2 + a3);
+}
+
+// PT[slot][c][j][i] = P[slot][c][i][j]: transposed copies for the few-pattern walk below, whose lane i reads row i of P -- from
+// the row-major matrix that is a stride of K doubles between lanes (16-way bank conflicts at K = 24); from the transposed
+// copy the lanes read consecutive words.
+__global__ void __launch_bounds__(256) pt_copy_kernel(int K, const double* __restrict__ P, double* __restrict__ PT)
+{
+    __shared__ double tile[32][33];
+    const double* src = P + (size_t)blockIdx.x * K * K;
+    double* dst = PT + (size_t)blockIdx.x * K * K;
+    const int tx = threadIdx.x & 31, ty = threadIdx.x >> 5;
+    for (int i0 = 0; i0 < K; i0 += 32)
+        for (int j0 = 0; j0 < K; j0 += 32) {
+            for (int r = ty; r < 32; r += 8)
+                tile[r][tx] = (i0 + r < K && j0 + tx < K) ? src[(i0 + r) * K + j0 + tx] : 0.0;
+            __syncthreads();
+            for (int r = ty; r < 32; r += 8)
+                if (j0 + r < K && i0 + tx < K) dst[(j0 + r) * K + i0 + tx] = tile[tx][r];
+            __syncthreads();
+        }
+}
+
 constexpr int GT = 256;
 
 __global__ void __launch_bounds__(GT) prune_generic_kernel(const PruneOp* __restrict__ ops, int tiles, int tile_p,
@@ -946,8 +983,8 @@ __device__ __forceinline__ void cp_async8(void* dst, const void* src)
 constexpr int KD_STAGES = 3;
 
 __global__ void __launch_bounds__(32) pruneK_dfs_kernel(const DfsOp* __restrict__ ops, const DfsPiece* __restrict__ pieces,
-    int K, int C, int L, int Lp, int depth, const double* __restrict__ P, const uint8_t* __restrict__ tips,
-    double* __restrict__ partials, int32_t* __restrict__ scale_exp)
+    int K, int C, int L, int Lp, int depth, const double* __restrict__ P /* transposed copies, pt_copy_kernel */,
+    const uint8_t* __restrict__ tips, double* __restrict__ partials, int32_t* __restrict__ scale_exp)
 {
     extern __shared__ double kd_sm[];
     const int CK = C * K, KK = K * K, CKK = C * KK;
@@ -1020,12 +1057,12 @@ __global__ void __launch_bounds__(32) pruneK_dfs_kernel(const DfsOp* __restrict_
         int ex = 0;
         for (int ch = 0; ch < 2; ch++) {
             const int src = srcs[ch];
-            const double* Pm = st + ch * CKK + (size_t)i * K;          // row i of category 0
+            const double* Pm = st + ch * CKK + i;                      // row i of P = column i of the staged transpose, category 0
             if (src == EPX_DFS_TIP) {
                 const int s = aux[ch];
 #pragma unroll
                 for (int c = 0; c < KD_MAXC; c++)
-                    if (c < C) f[c] *= s < K ? Pm[c * KK + s] : 1.0;
+                    if (c < C) f[c] *= s < K ? Pm[c * KK + s * K] : 1.0;
                 continue;
             }
             const double* v;
@@ -1042,7 +1079,7 @@ __global__ void __launch_bounds__(32) pruneK_dfs_kernel(const DfsOp* __restrict_
                 if (c >= C) break;
                 const double* row = Pm + c * KK;
                 const double* vc = v + c * K;
-                f[c] *= dot4(row, vc, K);              // the level kernel's summation order: incremental re-evaluation is bit-identical
+                f[c] *= dot4s(row, K, vc, K);          // the level kernel's summation order: incremental re-evaluation is bit-identical
             }
         }
         double m = 0.0;
@@ -1375,12 +1412,13 @@ int launch_pruning(const epx_ctx* c, cudaStream_t s)
         const DevBuffers& d = c->d;
         const int total = (int)c->dfs_pieces.size();
         const size_t smem = kdfs_smem(c->K, c->C, c->dfs_depth);
-        int n = 0;
+        int n = 1;
+        pt_copy_kernel<<<c->n_slots * c->C, 256, 0, s>>>(c->K, d.P, d.PB);
         for (int pass = 0; pass < 2; pass++) {
             const int first = pass == 0 ? 0 : c->dfs_bottom, count = pass == 0 ? c->dfs_bottom : total - c->dfs_bottom;
             if (count <= 0) continue;
             pruneK_dfs_kernel<<<count * c->L, 32, smem, s>>>(d.dfs_ops, d.dfs_pieces + first, c->K, c->C, c->L, c->Lp, c->dfs_depth,
-                                                           d.P, d.tips, d.partials, d.scale_exp);
+                                                           d.PB, d.tips, d.partials, d.scale_exp);
             n++;
         }
         return cudaGetLastError() == cudaSuccess ? n : -1;
