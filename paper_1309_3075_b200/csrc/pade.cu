@@ -17,7 +17,7 @@ namespace {
 constexpr int PT_MAX = 512;  // threads per CTA: 512 for K > 32 (a 61 x 61 product is 8 row tiles x 2 groups of 4 column tiles = one
                              // item per warp; config 3 chain 0.264 -> 0.224 ms), 256 otherwise (K = 24 is barrier-bound in the
                              // Gauss-Jordan sweep: 512 threads measured 0.81 ms against 0.33 ms on config 4)
-__host__ __device__ inline int pade_threads(int K) { return K > 32 ? 512 : 256; }
+__host__ __device__ inline int pade_threads(int K) { return K > 32 ? 512 : 128; }
 
 __device__ __forceinline__ void dmma884(double& d0, double& d1, double a, double b)
 {
@@ -333,7 +333,7 @@ static int pade_attr()
 
 int pade_init_attributes()
 {
-    return pade_attr<0, 256>() | pade_attr<0, 512>() | pade_attr<1, 256>() | pade_attr<1, 512>();
+    return pade_attr<0, 128>() | pade_attr<0, 512>() | pade_attr<1, 128>() | pade_attr<1, 512>();
 }
 
 template <int METHOD, int PT>
@@ -357,5 +357,5 @@ static int launch_dense(const epx_ctx* c, cudaStream_t s)
     return cudaGetLastError() == cudaSuccess ? launched : -1;
 }
 
-int launch_pade_chain(const epx_ctx* c, cudaStream_t s) { return pade_threads(c->K) == 512 ? launch_dense<0, 512>(c, s) : launch_dense<0, 256>(c, s); }
-int launch_taylor_chain(const epx_ctx* c, cudaStream_t s) { return pade_threads(c->K) == 512 ? launch_dense<1, 512>(c, s) : launch_dense<1, 256>(c, s); }
+int launch_pade_chain(const epx_ctx* c, cudaStream_t s) { return pade_threads(c->K) == 512 ? launch_dense<0, 512>(c, s) : launch_dense<0, 128>(c, s); }
+int launch_taylor_chain(const epx_ctx* c, cudaStream_t s) { return pade_threads(c->K) == 512 ? launch_dense<1, 512>(c, s) : launch_dense<1, 128>(c, s); }
