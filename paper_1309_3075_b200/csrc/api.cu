@@ -103,7 +103,7 @@ size_t plan_workspace(const epx_ctx* c, char* base, DevBuffers* d)
         t.inc_pops = (PruneOp*)take(sizeof(PruneOp) * (N - 1));
     }
     t.lnl = (double*)take(8);
-    t.status = (int32_t*)take(4);
+    t.status = (int32_t*)take(8);      // [0] status word, [1] arrival counter of the root reduction
     if (d) *d = t;
     return off;
 }

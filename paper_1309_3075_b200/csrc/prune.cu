@@ -1111,11 +1111,39 @@ size_t kdfs_smem(int K, int C, int depth)
 }
 
 // ------------------------------------------------------------------------------------------------ a6
+// Last-block-done final sum: every CTA publishes its partial sum, the CTA that arrives last adds them up in index order
+// (deterministic: the order does not depend on which CTA is last) and re-arms the counter.  Saves the final_sum launch.
+__device__ __forceinline__ void finish_sum(double block_total, int n_blocks, double* __restrict__ block_sums,
+                                           double* __restrict__ lnl, int32_t* __restrict__ counter, double* red)
+{
+    __shared__ bool last;
+    if (threadIdx.x == 0) {
+        block_sums[blockIdx.x] = block_total;
+        __threadfence();
+        last = atomicAdd(counter, 1) == n_blocks - 1;
+    }
+    __syncthreads();
+    if (!last) return;
+    __threadfence();
+    double t = 0.0;
+    for (int i = threadIdx.x; i < n_blocks; i += 256) t += __ldcg(block_sums + i);
+    for (int o = 16; o > 0; o >>= 1) t += __shfl_xor_sync(0xffffffffu, t, o);
+    __syncthreads();
+    if ((threadIdx.x & 31) == 0) red[threadIdx.x >> 5] = t;
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        double s = 0.0;
+        for (int w = 0; w < 8; w++) s += red[w];
+        *lnl = s;
+        *counter = 0;
+    }
+}
+
 __global__ void __launch_bounds__(256) root_site_kernel(int K, int C, int L, size_t sc, size_t sp, int root_pidx, int root_node,
     const double* __restrict__ partials, const int32_t* __restrict__ scale_exp, const double* __restrict__ freqs,
     const int32_t* __restrict__ e_hi, const double* __restrict__ root_freqs, const double* __restrict__ weights,
     const double* __restrict__ pattern_wt, double* __restrict__ site_lnl, double* __restrict__ block_sums,
-    int32_t* __restrict__ status)
+    int32_t* __restrict__ status, double* __restrict__ lnl)
 {
     __shared__ double red[8];
     const int tid = threadIdx.x;
@@ -1138,11 +1166,11 @@ __global__ void __launch_bounds__(256) root_site_kernel(int K, int C, int L, siz
     for (int o = 16; o > 0; o >>= 1) contrib += __shfl_xor_sync(0xffffffffu, contrib, o);
     if ((tid & 31) == 0) red[tid >> 5] = contrib;
     __syncthreads();
-    if (tid == 0) {
-        double t = 0.0;
+    double t = 0.0;
+    if (tid == 0)
         for (int w = 0; w < 8; w++) t += red[w];
-        block_sums[blockIdx.x] = t;
-    }
+    __syncthreads();
+    finish_sum(t, gridDim.x, block_sums, lnl, status + 1, red);
 }
 
 // K > 8: one warp per pattern, lanes over the states (coalesced reads of the root vectors), eight patterns per CTA.
@@ -1153,7 +1181,7 @@ __global__ void __launch_bounds__(256) root_site_warp_kernel(int K, int C, int L
     const double* __restrict__ partials, const int32_t* __restrict__ scale_exp, const double* __restrict__ freqs,
     const int32_t* __restrict__ e_hi, const double* __restrict__ root_freqs, const double* __restrict__ weights,
     const double* __restrict__ pattern_wt, double* __restrict__ site_lnl, double* __restrict__ block_sums,
-    int32_t* __restrict__ status)
+    int32_t* __restrict__ status, double* __restrict__ lnl)
 {
     __shared__ double red[8];
     const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
@@ -1186,28 +1214,11 @@ __global__ void __launch_bounds__(256) root_site_warp_kernel(int K, int C, int L
     }
     if (lane == 0) red[w] = contrib;
     __syncthreads();
-    if (threadIdx.x == 0) {
-        double t = 0.0;
-        for (int k = 0; k < 8; k++) t += red[k];
-        block_sums[blockIdx.x] = t;
-    }
-}
-
-__global__ void __launch_bounds__(256) final_sum_kernel(int n, const double* __restrict__ block_sums,
-                                                        double* __restrict__ lnl)
-{
-    __shared__ double red[8];
-    const int tid = threadIdx.x;
     double t = 0.0;
-    for (int i = tid; i < n; i += 256) t += block_sums[i];
-    for (int o = 16; o > 0; o >>= 1) t += __shfl_xor_sync(0xffffffffu, t, o);
-    if ((tid & 31) == 0) red[tid >> 5] = t;
+    if (threadIdx.x == 0)
+        for (int k = 0; k < 8; k++) t += red[k];
     __syncthreads();
-    if (tid == 0) {
-        double s = 0.0;
-        for (int w = 0; w < 8; w++) s += red[w];
-        *lnl = s;
-    }
+    finish_sum(t, gridDim.x, block_sums, lnl, status + 1, red);
 }
 
 size_t generic_smem(int K, int C, int tile_p)
@@ -1466,11 +1477,10 @@ int launch_root_reduction(const epx_ctx* c, cudaStream_t s)
         root_site_warp_kernel<<<blocks, 256, 0, s>>>(c->K, c->C, c->L, (size_t)root_pidx * lay.node, lay.sc, lay.sp, lay.exp_per_cat ? 1 : 0,
                                                      root_pidx, c->root, d.partials, d.scale_exp, d.freqs,
                                                      d.e_hi, c->has_root_freqs ? d.root_freqs : nullptr, d.weights,
-                                                     d.pattern_wt, d.site_lnl, d.block_sums, d.status);
+                                                     d.pattern_wt, d.site_lnl, d.block_sums, d.status, d.lnl);
     else
     root_site_kernel<<<blocks, 256, 0, s>>>(c->K, c->C, c->L, lay.sc, lay.sp, root_pidx, c->root, d.partials, d.scale_exp, d.freqs,
                                             d.e_hi, c->has_root_freqs ? d.root_freqs : nullptr, d.weights,
-                                            d.pattern_wt, d.site_lnl, d.block_sums, d.status);
-    final_sum_kernel<<<1, 256, 0, s>>>(blocks, d.block_sums, d.lnl);
-    return cudaGetLastError() == cudaSuccess ? 2 : -1;
+                                            d.pattern_wt, d.site_lnl, d.block_sums, d.status, d.lnl);
+    return cudaGetLastError() == cudaSuccess ? 1 : -1;
 }

@@ -128,6 +128,83 @@ __global__ void seg_fill_kernel(int n_br, int M, const double* __restrict__ tau,
     }
 }
 
+// All three steps in ONE CTA for small problems (configs 1 and 3; many small instances batched): three dependent launches
+// of a few microseconds each cost more in launch gaps than in work.  Pass 1 per chunk of 1024 slots: binary searches, block
+// scan of the segment counts, each thread fills its own branch's segments.  Pass 2: counting sort by chain length.
+constexpr int SEG_FUSED_MAX = 2048;     // beyond two chunks the single CTA loses to three parallel launches (cfg 2: 20 vs 18 us; cfg 5: 113 vs 33 us)
+
+__global__ void __launch_bounds__(1024) seg_fused_kernel(int n_br, int M, const double* __restrict__ tau,
+    const int32_t* __restrict__ parent, const double* __restrict__ height, const double* __restrict__ child_h,
+    const double* __restrict__ parent_h, const double* __restrict__ brate, int32_t* __restrict__ n_seg,
+    int32_t* __restrict__ e_hi_out, int32_t* __restrict__ seg_off, int32_t* __restrict__ seg_epoch,
+    double* __restrict__ seg_dur, int32_t* __restrict__ order)
+{
+    __shared__ int warp_tot[32];
+    __shared__ int carry;
+    __shared__ int hist[EPX_SORT_BINS];
+    __shared__ int bin_base[EPX_SORT_BINS];
+    const int tid = threadIdx.x, lane = tid & 31, wid = tid >> 5;
+    if (tid == 0) carry = 0;
+    if (tid < EPX_SORT_BINS) hist[tid] = 0;
+    __syncthreads();
+    for (int base = 0; base < n_br; base += 1024) {
+        const int b = base + tid;
+        int v = 0, e_hi = 0;
+        double hc = 0.0, hp = 0.0;
+        if (b < n_br) {
+            branch_ends(b, parent, height, child_h, parent_h, hc, hp);
+            const int e_lo = count_less(tau, M - 1, hc, true);
+            e_hi = count_less(tau, M - 1, hp, false);
+            v = (hp > hc) ? (e_hi - e_lo + 1) : 0;
+            e_hi_out[b] = e_hi;
+            n_seg[b] = v;
+            atomicAdd(&hist[min(v, EPX_SORT_BINS - 1)], 1);
+        }
+        int x = v;
+        for (int o = 1; o < 32; o <<= 1) {
+            const int y = __shfl_up_sync(0xffffffffu, x, o);
+            if (lane >= o) x += y;
+        }
+        if (lane == 31) warp_tot[wid] = x;
+        __syncthreads();
+        if (wid == 0) {
+            int w = warp_tot[lane];
+            for (int o = 1; o < 32; o <<= 1) {
+                const int y = __shfl_up_sync(0xffffffffu, w, o);
+                if (lane >= o) w += y;
+            }
+            warp_tot[lane] = w;   // inclusive over warps
+        }
+        __syncthreads();
+        const int off = carry + (wid ? warp_tot[wid - 1] : 0) + x - v;   // exclusive prefix
+        if (b < n_br) {
+            seg_off[b] = off;
+            const double rv = brate ? brate[b] : 1.0;
+            double upper = hp;
+            int e = e_hi;
+            for (int i = 0; i < v; i++, e--) {
+                const double lower = (i == v - 1) ? hc : tau[e - 1];
+                seg_epoch[off + i] = e;
+                seg_dur[off + i] = brate ? (upper - lower) * rv : upper - lower;
+                upper = lower;
+            }
+        }
+        __syncthreads();
+        if (tid == 1023) carry = off + v;
+        __syncthreads();
+    }
+    if (tid == 0) {
+        seg_off[n_br] = carry;
+        int acc = 0;
+        for (int k = EPX_SORT_BINS - 1; k >= 0; k--) { bin_base[k] = acc; acc += hist[k]; }
+    }
+    __syncthreads();
+    for (int i = tid; i < n_br; i += 1024) {
+        const int k = min(n_seg[i], EPX_SORT_BINS - 1);
+        order[atomicAdd(&bin_base[k], 1)] = i;
+    }
+}
+
 }  // namespace
 
 int launch_segmenter(const epx_ctx* c, cudaStream_t s)
@@ -136,6 +213,11 @@ int launch_segmenter(const epx_ctx* c, cudaStream_t s)
     int n = c->n_slots;
     int blocks = (n + 255) / 256;
     const int32_t* parent = c->tree_mode ? d.parent : nullptr;
+    if (n <= SEG_FUSED_MAX) {
+        seg_fused_kernel<<<1, 1024, 0, s>>>(n, c->M, d.tau, parent, d.height, d.child_h, d.parent_h, c->has_brates ? d.brate : nullptr,
+                                            d.n_seg, d.e_hi, d.seg_off, d.seg_epoch, d.seg_dur, d.order);
+        return cudaGetLastError() == cudaSuccess ? 1 : -1;
+    }
     seg_count_kernel<<<blocks, 256, 0, s>>>(n, c->M, d.tau, parent, d.height, d.child_h, d.parent_h, d.n_seg, d.e_hi);
     seg_scan_sort_kernel<<<1, 1024, 0, s>>>(n, d.n_seg, d.seg_off, d.order);
     seg_fill_kernel<<<blocks, 256, 0, s>>>(n, c->M, d.tau, parent, d.height, d.child_h, d.parent_h, d.n_seg, d.e_hi,
