@@ -164,38 +164,61 @@ __global__ void __launch_bounds__(JT_MAX) jacobi_kernel(int K, int Kp, const dou
 }
 
 // ------------------------------------------------------------------------------------------------ K <= 62: one barrier per round
-// The same two-sided round-robin Jacobi, reorganised so that a round costs ONE barrier and no index arithmetic (the kernel
-// above spends 221 instructions per warp and round, half of them on indices, and its 16 CTAs were 15 % of config 5's step):
-//   * the players are kept physically in pairing order: pair a = rows / columns 2a, 2a+1.  After a round the tournament
-//     rotates by a FIXED permutation (player at position p moves to newpos(p)), so thread (a, b) always reads the 2x2 block
-//     at the same addresses of the current buffer and writes its rotated block to the same four addresses of the other
-//     buffer (ping-pong): every address is a per-thread constant.  V's columns travel with the players.
+// The same two-sided round-robin Jacobi, reorganised so that a round costs ONE barrier, no index arithmetic and conflict-free
+// shared-memory traffic (the kernel above spends 221 instructions per warp and round, half of them on indices; its 16 CTAs
+// were 15 % of config 5's step):
+//   * the players of the tournament sit in two rows, tops T_0..T_{m-1} at positions 0..m-1 and bottoms B_0..B_{m-1} at
+//     positions m..2m-1; pair k = (T_k, B_k).  S and V are stored in position order.  After a round the tournament rotates by
+//     a FIXED permutation (T_0 stays, tops move right, bottoms move left, the ends change rows), so thread (a, b) always reads
+//     the 2x2 block {a, m+a} x {b, m+b} at the same addresses of the current buffer and writes its rotated block to the same
+//     four addresses of the other buffer (ping-pong): every address is a per-thread constant, and a warp's consecutive b are
+//     consecutive words on the read AND on the write side (64-bit accesses, no bank conflicts -- a first version with the
+//     pair in adjacent positions scattered its stores and was bound by shared-memory wavefronts, 2 130 per round).
+//   * the same thread rotates V's block (rows a, m+a; columns of pair b) with the rotation of pair b it already holds.
 //   * the rotation of a NEW pair j needs three entries of the updated matrix (two diagonal ones, the new pivot).  A spare
 //     warp computes them directly from the OLD matrix and the OLD rotations (closed forms of the 2x2 updates) while the
 //     other warps update S and V, so the next round's rotations are ready at the same barrier.
-//   * an odd K gets a dummy player whose row and column stay zero (its rotations are the identity).
-// After every sweep (n - 1 rounds) the players are back in their original order.
+//   * an odd K gets a dummy player (position 2m-1) whose row and column stay zero (its rotations are the identity).
+// After every sweep (n - 1 rounds) the players are back in their original positions, position = state index.
 __device__ __forceinline__ int jac_newpos(int pos, int m)
 {
     if (pos == 0 || m == 1) return pos;
-    const int k = pos >> 1;
-    if ((pos & 1) == 0) return k <= m - 2 ? 2 * k + 2 : 2 * m - 1;       // top row moves right, its last player drops down
-    return k == 0 ? 2 : 2 * k - 1;                                       // bottom row moves left, its first player goes up
+    if (pos < m) return pos <= m - 2 ? pos + 1 : 2 * m - 1;      // tops move right, the last one drops to the bottom row
+    return pos == m ? 1 : pos - 1;                               // bottoms move left, the first one rises to the top row
 }
 
+// 1/sqrt(x) and 1/x for normal x > 0: hardware seed (MUFU.RSQ64H / RCP64H, ~2^-22) + Newton-type corrections in FMAs.
+// The rotation of the next round is the critical path of a round (one warp computes it while 31 update S and V), and
+// CUDA's correctly-rounded rsqrt() / division are ~20 dependent instructions each.
+__device__ __forceinline__ double fast_rsqrt(double x)
+{
+    double y;
+    asm("rsqrt.approx.ftz.f64 %0, %1;" : "=d"(y) : "d"(x));
+    const double e = fma(-x * y, y, 1.0);                        // 1 - x y^2  ~ 2^-22
+    return fma(y * e, fma(0.375, e, 0.5), y);                    // y (1 + e/2 + 3 e^2 / 8): error O(e^3) ~ 2^-66 + rounding
+}
+__device__ __forceinline__ double fast_rcp(double x)
+{
+    double y;
+    asm("rcp.approx.ftz.f64 %0, %1;" : "=d"(y) : "d"(x));
+    double e = fma(-x, y, 1.0);
+    y = fma(y, e, y);                                            // 2^-44
+    e = fma(-x, y, 1.0);
+    return fma(y, e, y);                                         // 2^-88 + rounding
+}
+
+// Rotation (c, s) that annihilates the pivot apq of the pair with diagonal entries (spp, sqq).  t = tan of the angle, the root
+// of smaller magnitude of t^2 + 2 theta t - 1 = 0 with theta = d / h.  t only has to be accurate enough to annihilate the pivot
+// to rounding; c^2 + s^2 = 1 holds to rounding because c = rsqrt(1 + t^2) is accurate to ~1 ulp and s = t c.
 __device__ __forceinline__ double2 jac_rotation(double spp, double sqq, double apq)
 {
-    double c = 1.0, s = 0.0;
-    if (fabs(apq) > 1e-300) {
-        // t = tan of the rotation angle, the root of smaller magnitude of t^2 + 2 theta t - 1 = 0 with theta = d / h
-        const double d = sqq - spp, h = 2.0 * apq;
-        const double r2 = fma(d, d, h * h);
-        const double r = r2 * rsqrt(r2);
-        const double t = (d < 0 ? -h : h) / (fabs(d) + r);
-        c = rsqrt(fma(t, t, 1.0));
-        s = t * c;
-    }
-    return make_double2(c, s);
+    const double d = sqq - spp, h = 2.0 * apq;
+    const double r2 = fma(d, d, h * h);
+    if (!(r2 > 1e-280) || !(fabs(apq) > 1e-300)) return make_double2(1.0, 0.0);
+    const double r = r2 * fast_rsqrt(r2);
+    const double t = (d < 0 ? -h : h) * fast_rcp(fabs(d) + r);
+    const double c = fast_rsqrt(fma(t, t, 1.0));
+    return make_double2(c, t * c);
 }
 
 __global__ void __launch_bounds__(1024) jacobi1_kernel(int K, int Kp, const double* __restrict__ Qall,
@@ -207,17 +230,17 @@ __global__ void __launch_bounds__(1024) jacobi1_kernel(int K, int Kp, const doub
     extern __shared__ __align__(16) double sm[];
     if (eproc[blockIdx.x] != (int)blockIdx.x) return;   // f2: this epoch shares the process of an earlier one
     const int m = (K + 1) >> 1, n = 2 * m;              // pairs, players
-    const int NB = blockDim.x - 32;                     // block / V threads; the last warp prepares the rotations
+    const int NB = blockDim.x - 32;                     // block threads; the last warp prepares the rotations
     const int nn = n * n, kn = K * n;
-    double* const S0 = sm;                              // [2][n][n] ping-pong
-    double* const V0 = S0 + 2 * nn;                     // [2][K][n] ping-pong
+    double* const S0 = sm;                              // [2][n][n] ping-pong, position order
+    double* const V0 = S0 + 2 * nn;                     // [2][K][n] ping-pong, columns in position order
     double2* const R0 = reinterpret_cast<double2*>(V0 + 2 * kn);                          // [2][m] (cos, sin)
     double* const red = reinterpret_cast<double*>(R0 + 2 * m);                            // [33]
     const int e = blockIdx.x, tid = threadIdx.x, T = blockDim.x;
     const double* Q = Qall + (size_t)e * K * K;
     const double* pi = freqs + (size_t)e * K;
 
-    for (int idx = tid; idx < n * n; idx += T) {
+    for (int idx = tid; idx < n * n; idx += T) {        // position = state index at the start of every sweep
         const int i = idx / n, j = idx - i * n;
         double v = 0.0;
         if (i < K && j < K) {
@@ -245,36 +268,26 @@ __global__ void __launch_bounds__(1024) jacobi1_kernel(int K, int Kp, const doub
         tot2 = block_sum(t);
     }
 
-    // per-thread constants
+    // per-thread constants: block (a, b) = rows {a, m+a} x columns {b, m+b}
     const bool is_blk = tid < m * m;
     const int a = is_blk ? tid / m : 0, b = is_blk ? tid - a * m : 0;
-    const int rd0 = (2 * a) * n + 2 * b, rd1 = rd0 + n;
-    const int na0 = jac_newpos(2 * a, m) * n, na1 = jac_newpos(2 * a + 1, m) * n;
-    const int nb0 = jac_newpos(2 * b, m), nb1 = jac_newpos(2 * b + 1, m);
-    int v_rd[2], v_w0[2], v_w1[2], v_k[2];
-#pragma unroll
-    for (int u = 0; u < 2; u++) {
-        const int t = tid + u * NB;
-        const bool on = tid < NB && t < K * m;
-        const int i = on ? t / m : 0, k = on ? t - i * m : 0;
-        v_k[u] = on ? k : -1;
-        v_rd[u] = i * n + 2 * k;
-        v_w0[u] = i * n + jac_newpos(2 * k, m);
-        v_w1[u] = i * n + jac_newpos(2 * k + 1, m);
-    }
-    // rotation warp, lane j < m: the players that form NEW pair j sit at old positions x (top) and y (bottom)
+    const int rt = a * n, rb = (m + a) * n, ct = b, cb = m + b;                           // read
+    const int wrt = jac_newpos(a, m) * n, wrb = jac_newpos(m + a, m) * n;                 // write rows (S)
+    const int wct = jac_newpos(b, m), wcb = jac_newpos(m + b, m);                         // write columns (S and V)
+    const bool v0_on = is_blk && a < K, v1_on = is_blk && m + a < K;                      // V rows a and m + a
+    // rotation warp, lane j < m: the players that form NEW pair j sit at old positions x (-> T_j) and y (-> B_j)
     const int j = tid - NB;
     const bool is_rot = j >= 0 && j < m;
-    int x = 0, y = 1;
+    int x = 0, y = m;
     if (is_rot)
         for (int p = 0; p < n; p++) {
             const int q = jac_newpos(p, m);
-            if (q == 2 * j) x = p;
-            if (q == 2 * j + 1) y = p;
+            if (q == j) x = p;
+            if (q == m + j) y = p;
         }
-    const int ax = x >> 1, ay = y >> 1, px = x & 1, py = y & 1;
+    const int ax = x % m, ay = y % m, px = x / m, py = y / m;
 
-    if (is_rot) R0[j] = jac_rotation(S0[(2 * j) * n + 2 * j], S0[(2 * j + 1) * n + 2 * j + 1], S0[(2 * j) * n + 2 * j + 1]);
+    if (is_rot) R0[j] = jac_rotation(S0[j * n + j], S0[(m + j) * n + m + j], S0[j * n + m + j]);
     __syncthreads();
 
     int cur = 0;
@@ -287,44 +300,44 @@ __global__ void __launch_bounds__(1024) jacobi1_kernel(int K, int Kp, const doub
             double* Sn = S0 + (cur ^ 1) * nn;
             const double2* R = R0 + cur * m;
             if (is_blk) {
-                const double2 ra = R[a], rb = R[b];
-                const double2 x0 = *reinterpret_cast<const double2*>(S + rd0), x1 = *reinterpret_cast<const double2*>(S + rd1);
+                const double2 ra = R[a], rbb = R[b];
+                const double x00 = S[rt + ct], x01 = S[rt + cb], x10 = S[rb + ct], x11 = S[rb + cb];
                 // columns (pair b), then rows (pair a): S <- J^T S J on this 2x2 block
-                const double t00 = rb.x * x0.x - rb.y * x0.y, t01 = rb.y * x0.x + rb.x * x0.y;
-                const double t10 = rb.x * x1.x - rb.y * x1.y, t11 = rb.y * x1.x + rb.x * x1.y;
+                const double t00 = rbb.x * x00 - rbb.y * x01, t01 = rbb.y * x00 + rbb.x * x01;
+                const double t10 = rbb.x * x10 - rbb.y * x11, t11 = rbb.y * x10 + rbb.x * x11;
                 double y00 = ra.x * t00 - ra.y * t10, y01 = ra.x * t01 - ra.y * t11;
                 double y10 = ra.y * t00 + ra.x * t10, y11 = ra.y * t01 + ra.x * t11;
                 if (a == b) { y01 = 0.0; y10 = 0.0; }            // the pivot pair is annihilated exactly
-                Sn[na0 + nb0] = y00; Sn[na0 + nb1] = y01; Sn[na1 + nb0] = y10; Sn[na1 + nb1] = y11;
+                Sn[wrt + wct] = y00; Sn[wrt + wcb] = y01; Sn[wrb + wct] = y10; Sn[wrb + wcb] = y11;
                 if (r == n - 2) my_off = a == b ? 0.0 : fma(y00, y00, fma(y01, y01, fma(y10, y10, y11 * y11)));
-            }
-            if (tid < NB) {
+                // V <- V J: rows a and m + a, the columns of pair b
                 const double* V = V0 + cur * kn;
                 double* Vn = V0 + (cur ^ 1) * kn;
-#pragma unroll
-                for (int u = 0; u < 2; u++)
-                    if (v_k[u] >= 0) {
-                        const double2 rk = R[v_k[u]];
-                        const double2 v = *reinterpret_cast<const double2*>(V + v_rd[u]);
-                        Vn[v_w0[u]] = rk.x * v.x - rk.y * v.y;
-                        Vn[v_w1[u]] = rk.y * v.x + rk.x * v.y;
-                    }
+                if (v0_on) {
+                    const double v0 = V[rt + ct], v1 = V[rt + cb];
+                    Vn[rt + wct] = rbb.x * v0 - rbb.y * v1;
+                    Vn[rt + wcb] = rbb.y * v0 + rbb.x * v1;
+                }
+                if (v1_on) {
+                    const double v0 = V[rb + ct], v1 = V[rb + cb];
+                    Vn[rb + wct] = rbb.x * v0 - rbb.y * v1;
+                    Vn[rb + wcb] = rbb.y * v0 + rbb.x * v1;
+                }
             } else if (is_rot) {
                 double2 nr = make_double2(1.0, 0.0);
                 if (ax != ay) {
-                    const double2 ra = R[ax], rb = R[ay];
-                    const double app = S[(2 * ax) * n + 2 * ax], apq = S[(2 * ax) * n + 2 * ax + 1], aqq = S[(2 * ax + 1) * n + 2 * ax + 1];
-                    const double bpp = S[(2 * ay) * n + 2 * ay], bpq = S[(2 * ay) * n + 2 * ay + 1], bqq = S[(2 * ay + 1) * n + 2 * ay + 1];
-                    const double2 x0 = *reinterpret_cast<const double2*>(S + (2 * ax) * n + 2 * ay);
-                    const double2 x1 = *reinterpret_cast<const double2*>(S + (2 * ax + 1) * n + 2 * ay);
+                    const double2 ra = R[ax], rbb = R[ay];
+                    const double app = S[ax * n + ax], apq = S[ax * n + m + ax], aqq = S[(m + ax) * n + m + ax];
+                    const double bpp = S[ay * n + ay], bpq = S[ay * n + m + ay], bqq = S[(m + ay) * n + m + ay];
+                    const double x00 = S[ax * n + ay], x01 = S[ax * n + m + ay], x10 = S[(m + ax) * n + ay], x11 = S[(m + ax) * n + m + ay];
                     // the player's updated diagonal entry: (J^T S J)_pp = c^2 Spp - 2 c s Spq + s^2 Sqq, _qq = s^2 Spp + 2 c s Spq + c^2 Sqq
                     const double ca2 = ra.x * ra.x, sa2 = ra.y * ra.y, csa = 2.0 * ra.x * ra.y;
-                    const double cb2 = rb.x * rb.x, sb2 = rb.y * rb.y, csb = 2.0 * rb.x * rb.y;
+                    const double cb2 = rbb.x * rbb.x, sb2 = rbb.y * rbb.y, csb = 2.0 * rbb.x * rbb.y;
                     const double dx = px ? fma(sa2, app, fma(csa, apq, ca2 * aqq)) : fma(ca2, app, fma(-csa, apq, sa2 * aqq));
                     const double dy = py ? fma(sb2, bpp, fma(csb, bpq, cb2 * bqq)) : fma(cb2, bpp, fma(-csb, bpq, sb2 * bqq));
                     // the new pivot = entry (px, py) of the updated block (ax, ay)
-                    const double t0 = py ? rb.y * x0.x + rb.x * x0.y : rb.x * x0.x - rb.y * x0.y;
-                    const double t1 = py ? rb.y * x1.x + rb.x * x1.y : rb.x * x1.x - rb.y * x1.y;
+                    const double t0 = py ? rbb.y * x00 + rbb.x * x01 : rbb.x * x00 - rbb.y * x01;
+                    const double t1 = py ? rbb.y * x10 + rbb.x * x11 : rbb.x * x10 - rbb.y * x11;
                     const double piv = px ? ra.y * t0 + ra.x * t1 : ra.x * t0 - ra.y * t1;
                     nr = jac_rotation(dx, dy, piv);
                 }
