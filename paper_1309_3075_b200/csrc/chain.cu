@@ -44,36 +44,45 @@ __global__ void __launch_bounds__(256) chain_rows_kernel(int n_slots, int C, con
     }
     const int off = seg_off[b];
     const double r = rates[c];
-    int e = seg_epoch[off];
-    const double scale_i = isp[e * K + i];
-    double x[K];
-    {
-        const double rd = r * seg_dur[off];
+    // Deviation form: the thread carries a = (row i of the running product) - e_i and multiplies by
+    //   P_s = I + Pi^{-1/2} U expm1(L r d) U^T Pi^{1/2}
+    // segment by segment.  On a short segment every entry of P_s - I is O(r d) and is computed to a few ulp of ITSELF
+    // (U exp(L t) U^T instead leaves the orthogonality residual of U, ~1e-16 absolute, on off-diagonal entries of
+    // 1e-6 .. 1e-9: the 1e-12 bound on P holds either way, but a cherry's partial is a product of two such entries and
+    // config 2's per-node partials drifted to 1e-10 relative).  Same algebra as Eq. (7); W is not needed.
+    double a[K];
 #pragma unroll
-        for (int k = 0; k < K; k++) x[k] = U[(e * K + i) * K + k] * exp(lam[e * K + k] * rd);
-    }
-    for (int s = 1; s < n; s++) {
-        const double* Wm = W + (size_t)e * K * K;     // boundary between epoch e and e-1
-        e = seg_epoch[off + s];
+    for (int j = 0; j < K; j++) a[j] = 0.0;
+    for (int s = 0; s < n; s++) {
+        const int e = seg_epoch[off + s];
         const double rd = r * seg_dur[off + s];
-        double y[K];
+        const double* Ue = U + (size_t)e * K * K;
+        double z[K];
+        const double si = isp[e * K + i];
 #pragma unroll
-        for (int j = 0; j < K; j++) {
-            double a = 0.0;
+        for (int k = 0; k < K; k++) z[k] = si * Ue[i * K + k];
+        if (s > 0) {
 #pragma unroll
-            for (int k = 0; k < K; k++) a = fma(x[k], Wm[k * K + j], a);
-            y[j] = a * exp(lam[e * K + j] * rd);
+            for (int j = 0; j < K; j++) {
+                const double aj = a[j] * isp[e * K + j];
+#pragma unroll
+                for (int k = 0; k < K; k++) z[k] = fma(aj, Ue[j * K + k], z[k]);
+            }
         }
 #pragma unroll
-        for (int j = 0; j < K; j++) x[j] = y[j];
+        for (int k = 0; k < K; k++) z[k] *= expm1(lam[e * K + k] * rd);
+#pragma unroll
+        for (int j = 0; j < K; j++) {
+            double t = 0.0;
+#pragma unroll
+            for (int k = 0; k < K; k++) t = fma(z[k], Ue[j * K + k], t);
+            a[j] = fma(t, sp[e * K + j], a[j]);
+        }
     }
     bool bad = false;
 #pragma unroll
     for (int j = 0; j < K; j++) {
-        double a = 0.0;
-#pragma unroll
-        for (int k = 0; k < K; k++) a = fma(x[k], U[(e * K + j) * K + k], a);
-        double v = scale_i * a * sp[e * K + j];
+        const double v = (i == j ? 1.0 : 0.0) + a[j];
         bad |= !isfinite(v);
         out[j] = fmax(v, 0.0);      // reading A18: rounding can leave -1e-17; P is a probability
     }

@@ -169,6 +169,20 @@ def test_k4_extreme_tree_shapes(epx, orc_ld, shape, N):
     run_tree(epx, orc_ld, prob, options=[(epx.EPX_OPT_PRUNE_KERNEL, 3)])
 
 
+def test_k4_matrices_relative_accuracy(epx, orc_ld):
+    # K = 4 chain kernel in deviation form (P = I + ...): every entry is good to a few ulp of ITSELF, not only to 1e-12
+    # absolute -- on config 2's short branches off-diagonal entries are 1e-6 .. 1e-9 and a cherry's partial is a product of
+    # two of them (Eq. 4), so the per-node partials inherit the RELATIVE error of P.
+    prob = W.make_config(2, N=400, L=8)
+    ctx = epx.from_problem(prob)
+    ctx.update_matrices()
+    ref = orc_ld.evaluate(prob)
+    P = ctx.get_all_matrices().astype(np.longdouble)
+    rel = np.abs(P - ref["P"]) / np.abs(ref["P"])
+    assert float(np.max(rel)) <= 1e-12, float(np.max(rel))
+    ctx.close()
+
+
 def test_config2_full_size(epx, orc_ld):
     # the configuration bench.py times; the oracle's naive recursion takes ~1 min here
     import dataclasses
