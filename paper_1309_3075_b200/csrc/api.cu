@@ -399,7 +399,11 @@ int epx_set_option(epx_ctx* c, int option, int value)
             break;
         case 11: c->epoch_products = value ? 1 : 0; break;
         case 10: c->dedup = value ? 1 : 0; c->model_dirty = true; break;
-        case 9: c->jacobi_kernel = value ? 1 : 0; break;
+        case 9:
+            if (value != 0 && value != 1 && value != 2 && value != 14 && value != 18) return fail(c, EPX_E_ARG, "jacobi kernel %d", value);
+            
+            c->jacobi_kernel = value;
+            break;
         case 8:
             if (value < 0 || value > (1 << 20)) return fail(c, EPX_E_ARG, "chunk %d", value);
             c->mma_chunk = value;

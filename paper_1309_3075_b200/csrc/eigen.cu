@@ -221,6 +221,22 @@ __device__ __forceinline__ double2 jac_rotation(double spp, double sqq, double a
     return make_double2(c, t * c);
 }
 
+// The same rotation as a normalised direction: (c, s) = (|d| + r, sgn(d) h) / norm, r = sqrt(d^2 + h^2).  r only fixes the ANGLE
+// (seed + one Newton step, 2^-43), the normalisation is accurate, so c^2 + s^2 = 1 to rounding whatever the angle's error:
+// 17 dependent operations instead of 23.  For kernels that store the rotated pivot as computed.
+__device__ __forceinline__ double2 jac_rotation_n(double spp, double sqq, double apq)
+{
+    const double d = sqq - spp, h = 2.0 * apq;
+    const double r2 = fma(d, d, h * h);
+    if (!(r2 > 1e-280)) return make_double2(1.0, 0.0);
+    double y;
+    asm("rsqrt.approx.ftz.f64 %0, %1;" : "=d"(y) : "d"(r2));
+    y = fma(0.5 * y, fma(-r2 * y, y, 1.0), y);
+    const double cc = fabs(d) + r2 * y, ss = d < 0 ? -h : h;
+    const double wi = fast_rsqrt(fma(cc, cc, ss * ss));
+    return make_double2(cc * wi, ss * wi);
+}
+
 __global__ void __launch_bounds__(1024) jacobi1_kernel(int K, int Kp, const double* __restrict__ Qall,
                                                        const double* __restrict__ freqs, double* __restrict__ lam,
                                                        double* __restrict__ Uout, double* __restrict__ sp_out,
@@ -368,6 +384,325 @@ __global__ void __launch_bounds__(1024) jacobi1_kernel(int K, int Kp, const doub
     }
 }
 
+// ------------------------------------------------------------------------------------------------ 32 < K <= 62: a cluster per process
+// jacobi1_kernel is bound by the shared-memory bandwidth of ONE SM per process (config 5: 16 of 148 SMs busy for 0.52 ms, a
+// serial prefix of the chain kernel).  Here a thread-block cluster of 1 + NV CTAs shares a process:
+//   * CTA 0 owns S and is the only one on the critical path.  S is symmetric, so it keeps the entries (p, q) with p <= q only
+//     and runs one thread per block (a, b) with a <= b: 496 threads instead of 961, half the shared-memory traffic.  As in
+//     jacobi1_kernel every address is a per-thread constant (positions are fixed, the players rotate), the buffers ping-pong
+//     and a round costs one CTA barrier; the row stride is odd so that the transposed accesses are conflict free.
+//   * V <- V J touches V's rows independently and never feeds back into S: CTAs 1..NV own K / NV rows of V each and apply the
+//     rotations CTA 0's rotation warp pushes into a ring in THEIR shared memory (st.async: a 16-byte store whose
+//     completion is counted on the V CTA's mbarrier -- no fence anywhere in the iteration).  They run behind CTA 0 at their own pace; the ring's flow control (a progress word each V CTA stores
+//     back) never stalls CTA 0 in practice because a V CTA has less work per round.  After every sweep CTA 0 sends its
+//     verdict (converged or not); a sweep's rounds are the only thing the V CTAs wait for.
+// No cluster barrier inside the iteration (one at the start, one at the end).
+__device__ __forceinline__ uint32_t jc_smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
+__device__ __forceinline__ uint32_t jc_mapa(uint32_t addr, uint32_t rank)
+{
+    uint32_t r;
+    asm volatile("mapa.shared::cluster.u32 %0, %1, %2;" : "=r"(r) : "r"(addr), "r"(rank));
+    return r;
+}
+// 16 bytes into a peer's shared memory, completion counted on the peer's mbarrier (no fence: the store and its
+// complete_tx are ordered by the hardware, the consumer's try_wait makes the data visible)
+__device__ __forceinline__ void jc_st_async2(uint32_t addr, double2 v, uint32_t mbar)
+{
+    asm volatile("st.async.weak.shared::cluster.mbarrier::complete_tx::bytes.v2.f64 [%0], {%1, %2}, [%3];"
+                 ::"r"(addr), "d"(v.x), "d"(v.y), "r"(mbar) : "memory");
+}
+// progress words: relaxed cluster-scope accesses (no MEMBAR.GPU / CCTL.IVALL, which release / acquire at cluster scope cost).
+// They carry no data: a V CTA posts a round after its CTA barrier, when every load of the ring slot has been consumed.
+__device__ __forceinline__ void jc_st_relaxed_u32(uint32_t addr, uint32_t v)
+{
+    asm volatile("st.relaxed.cluster.shared::cluster.u32 [%0], %1;" ::"r"(addr), "r"(v) : "memory");
+}
+__device__ __forceinline__ uint32_t jc_ld_relaxed_u32(const uint32_t* p)
+{
+    uint32_t v;
+    asm volatile("ld.relaxed.cluster.shared::cta.u32 %0, [%1];" : "=r"(v) : "r"(jc_smem_u32(p)) : "memory");
+    return v;
+}
+__device__ __forceinline__ void jc_mbar_init(uint64_t* bar, int count)
+{
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(jc_smem_u32(bar)), "r"(count) : "memory");
+}
+__device__ __forceinline__ void jc_mbar_expect(uint64_t* bar, uint32_t bytes)
+{
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(jc_smem_u32(bar)), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void jc_mbar_wait(uint64_t* bar, uint32_t parity)
+{
+    const uint32_t addr = jc_smem_u32(bar);
+    uint32_t ok;
+    do {
+        asm volatile("{\n\t.reg .pred p;\n\tmbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n\tselp.u32 %0, 1, 0, p;\n\t}"
+                     : "=r"(ok) : "r"(addr), "r"(parity) : "memory");
+    } while (!ok);
+}
+__device__ __forceinline__ void jc_cluster_barrier()
+{
+    asm volatile("barrier.cluster.arrive.release.aligned;" ::: "memory");
+    asm volatile("barrier.cluster.wait.acquire.aligned;" ::: "memory");
+}
+
+constexpr int JSV_NS = 8;          // ring slots of rotations in a V CTA
+
+struct JsvHeader {                 // at the start of every CTA's dynamic shared memory (same offsets: mapa)
+    uint64_t full[JSV_NS];         // V CTAs: slot filled (the V CTA's own arrive + 16 m bytes stored by CTA 0's rotation lanes)
+    uint32_t vprog[8];             // CTA 0: rounds V CTA v has finished
+    uint32_t verdict;              // V CTAs: 2 * (sweeps decided) + converged
+    uint32_t pad[7];
+};
+
+template <int NV>
+__global__ void __launch_bounds__(1024) jacobi_sv_kernel(int K, int Kp, const double* __restrict__ Qall,
+                                                         const double* __restrict__ freqs, double* __restrict__ lam,
+                                                         double* __restrict__ Uout, double* __restrict__ sp_out,
+                                                         double* __restrict__ isp_out, int32_t* __restrict__ status,
+                                                         int M, const int32_t* __restrict__ eproc)
+{
+    extern __shared__ __align__(16) double sm[];
+    constexpr int G = NV + 1, NS = JSV_NS;
+    const int e = blockIdx.x / G;                       // the whole cluster serves (or skips) one process
+    if (eproc[e] != e) return;
+    uint32_t g;
+    asm volatile("mov.u32 %0, %%cluster_ctarank;" : "=r"(g));
+    const int m = (K + 1) >> 1, n = 2 * m;
+    const int tid = threadIdx.x, T = blockDim.x;
+    JsvHeader* const hd = reinterpret_cast<JsvHeader*>(sm);
+    double2* const ring = reinterpret_cast<double2*>(hd + 1);                             // [NS][m] (V CTAs)
+    double* const body = reinterpret_cast<double*>(ring + NS * m);
+    const double* Q = Qall + (size_t)e * K * K;
+    const double* pi = freqs + (size_t)e * K;
+
+    if (tid == 0) {
+        for (int q = 0; q < NS; q++) { jc_mbar_init(&hd->full[q], 1); if (g != 0) jc_mbar_expect(&hd->full[q], 16u * (uint32_t)m); }
+        for (int q = 0; q < 8; q++) hd->vprog[q] = 0;
+        hd->verdict = 0;
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    }
+
+    if (g == 0) {
+        // ------------------------------------------------------------------------------------------ CTA 0: S and the rotations
+        const int ld = n, nn = n * ld;      // even stride: the rotation lanes' diagonal walks (stride ld + 1) are conflict free
+        double* const S0 = body;                                                          // [2][n][ld], entries p <= q
+        double2* const R0 = reinterpret_cast<double2*>(S0 + 2 * nn);                      // [2][m] (cos, sin)
+        double* const red = reinterpret_cast<double*>(R0 + 2 * m);                        // [33]
+        auto sidx = [&](int p, int q) { return min(p, q) * ld + max(p, q); };
+        for (int idx = tid; idx < n * n; idx += T) {    // position = state index at the start of every sweep
+            const int i = idx / n, j = idx - i * n;
+            if (i > j) continue;
+            double v = 0.0;
+            if (i < K && j < K) {
+                const double a = sqrt(pi[i]) * Q[i * K + j] / sqrt(pi[j]);
+                const double b = sqrt(pi[j]) * Q[j * K + i] / sqrt(pi[i]);
+                v = 0.5 * (a + b);
+            }
+            S0[i * ld + j] = v;
+        }
+        __syncthreads();
+        auto block_sum = [&](double v) -> double {      // all threads call
+            for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
+            if ((tid & 31) == 0) red[tid >> 5] = v;
+            __syncthreads();
+            double t = 0;
+            for (int w = 0; w < T / 32; w++) t += red[w];
+            __syncthreads();
+            return t;
+        };
+        double tot2;
+        {
+            double t = 0;
+            for (int idx = tid; idx < n * n; idx += T) {
+                const int i = idx / n, j = idx - i * n;
+                if (i <= j) { const double x = S0[i * ld + j]; t += i == j ? x * x : 2.0 * x * x; }
+            }
+            tot2 = block_sum(t);
+        }
+        // per-thread constants: block (a, b), a <= b = rows {a, m+a} x columns {b, m+b}; row a of the triangle has m - a blocks
+        // Warp w runs on scheduler w % 4.  The rotations are the serial chain of a round (~25 dependent fp64 operations),
+        // so the rotation warp (warp 3) gets a scheduler and its fp64 lanes to itself: the block threads use the warps
+        // with w % 4 != 3 only, the other warps of scheduler 3 idle at the barrier.
+        const int nblk = m * (m + 1) / 2;
+        const int wid = tid >> 5;
+        const int bt = (wid & 3) == 3 ? -1 : ((wid - (wid >> 2)) << 5) + (tid & 31);
+        const bool is_blk = bt >= 0 && bt < nblk;
+        int a = 0, b = 0;
+        if (is_blk) {
+            int rem = bt;
+            while (rem >= m - a) { rem -= m - a; a++; }
+            b = a + rem;
+        }
+        const bool diag = a == b;
+        const int r00 = sidx(a, b), r01 = sidx(a, m + b), r10 = sidx(m + a, b), r11 = sidx(m + a, m + b);
+        const int pt = jac_newpos(a, m), pb = jac_newpos(m + a, m), qt = jac_newpos(b, m), qb = jac_newpos(m + b, m);
+        const int w00 = sidx(pt, qt), w01 = sidx(pt, qb), w10 = sidx(pb, qt), w11 = sidx(pb, qb);
+        // rotation warp, lane j < m: the players that form NEW pair j sit at old positions x (-> T_j) and y (-> B_j)
+        const int j = tid - 96;
+        const bool is_rot = j >= 0 && j < m;
+        int x = 0, y = m;
+        if (is_rot)
+            for (int p = 0; p < n; p++) {
+                const int q = jac_newpos(p, m);
+                if (q == j) x = p;
+                if (q == m + j) y = p;
+            }
+        const int ax = x % m, ay = y % m, px = x / m, py = y / m;
+        const int i_app = sidx(ax, ax), i_apq = sidx(ax, m + ax), i_aqq = sidx(m + ax, m + ax);
+        const int i_bpp = sidx(ay, ay), i_bpq = sidx(ay, m + ay), i_bqq = sidx(m + ay, m + ay);
+        // block (ax, ay) by position (sidx picks the stored copy of a symmetric entry)
+        const int i_x00 = sidx(ax, ay), i_x01 = sidx(ax, m + ay), i_x10 = sidx(m + ax, ay), i_x11 = sidx(m + ax, m + ay);
+        const uint32_t ring_u32 = jc_smem_u32(ring), full_u32 = jc_smem_u32(&hd->full[0]);
+        uint32_t ring_v[NV], full_v[NV];
+#pragma unroll
+        for (int v = 0; v < NV; v++) { ring_v[v] = jc_mapa(ring_u32, v + 1); full_v[v] = jc_mapa(full_u32, v + 1); }
+        auto push = [&](int t, double2 nr, const uint32_t* seen) {   // rotation lane: rotation j of global round t to every V CTA
+            const int slot = t % NS;
+#pragma unroll
+            for (int v = 0; v < NV; v++) {
+                if ((int)seen[v] < t + 1 - NS)
+                    while ((int)jc_ld_relaxed_u32(&hd->vprog[v]) < t + 1 - NS) { }        // slot free (never waits in practice)
+                jc_st_async2(ring_v[v] + 16u * (uint32_t)(slot * m + j), nr, full_v[v] + 8u * (uint32_t)slot);
+            }
+        };
+        jc_cluster_barrier();                           // every CTA of the cluster is running, its barriers initialised
+        if (is_rot) {
+            const double2 nr = jac_rotation_n(S0[sidx(j, j)], S0[sidx(m + j, m + j)], S0[sidx(j, m + j)]);
+            R0[j] = nr;
+            uint32_t seen[NV];
+#pragma unroll
+            for (int v = 0; v < NV; v++) seen[v] = 0;
+            push(0, nr, seen);
+        }
+        __syncthreads();
+
+        int cur = 0, t = 0;
+        bool converged = false;
+        double off2 = 0.0;
+        for (int sweep = 0; sweep < 40 && !converged; sweep++) {
+            double my_off = 0.0;
+            for (int r = 0; r < n - 1; r++, t++) {
+                const double* S = S0 + cur * nn;
+                double* Sn = S0 + (cur ^ 1) * nn;
+                const double2* R = R0 + cur * m;
+                if (is_blk) {
+                    const double2 ra = R[a], rbb = R[b];
+                    const double x00 = S[r00], x01 = S[r01], x10 = S[r10], x11 = S[r11];
+                    // columns (pair b), then rows (pair a): S <- J^T S J on this 2x2 block
+                    const double t00 = rbb.x * x00 - rbb.y * x01, t01 = rbb.y * x00 + rbb.x * x01;
+                    const double t10 = rbb.x * x10 - rbb.y * x11, t11 = rbb.y * x10 + rbb.x * x11;
+                    const double y00 = ra.x * t00 - ra.y * t10, y01 = ra.x * t01 - ra.y * t11;
+                    const double y10 = ra.y * t00 + ra.x * t10, y11 = ra.y * t01 + ra.x * t11;
+                    // (the rotated pivot of a diagonal block is stored as computed, not forced to zero: (c, s) is a rotation to
+                    // rounding whatever the accuracy of its angle, so the iteration stays an orthogonal similarity)
+                    Sn[w00] = y00; Sn[w01] = y01; Sn[w11] = y11;
+                    if (!diag) Sn[w10] = y10;                    // (a diagonal block's w10 is its w01)
+                    if (r == n - 2) my_off = diag ? 2.0 * y01 * y01 : 2.0 * fma(y00, y00, fma(y01, y01, fma(y10, y10, y11 * y11)));
+                } else if (is_rot) {
+                    double2 nr = make_double2(1.0, 0.0);
+                    uint32_t seen[NV];                           // the V CTAs' progress, read beside the operands
+#pragma unroll
+                    for (int v = 0; v < NV; v++) seen[v] = jc_ld_relaxed_u32(&hd->vprog[v]);
+                    if (ax != ay) {
+                        const double2 ra = R[ax], rbb = R[ay];
+                        const double app = S[i_app], apq = S[i_apq], aqq = S[i_aqq];
+                        const double bpp = S[i_bpp], bpq = S[i_bpq], bqq = S[i_bqq];
+                        const double x00 = S[i_x00], x01 = S[i_x01], x10 = S[i_x10], x11 = S[i_x11];
+                        // the player's updated diagonal entry: (J^T S J)_pp = c^2 Spp - 2 c s Spq + s^2 Sqq, _qq = s^2 Spp + 2 c s Spq + c^2 Sqq
+                        const double ca2 = ra.x * ra.x, sa2 = ra.y * ra.y, csa = 2.0 * ra.x * ra.y;
+                        const double cb2 = rbb.x * rbb.x, sb2 = rbb.y * rbb.y, csb = 2.0 * rbb.x * rbb.y;
+                        const double dx = px ? fma(sa2, app, fma(csa, apq, ca2 * aqq)) : fma(ca2, app, fma(-csa, apq, sa2 * aqq));
+                        const double dy = py ? fma(sb2, bpp, fma(csb, bpq, cb2 * bqq)) : fma(cb2, bpp, fma(-csb, bpq, sb2 * bqq));
+                        // the new pivot = entry (px, py) of the updated block (ax, ay)
+                        const double t0 = py ? rbb.y * x00 + rbb.x * x01 : rbb.x * x00 - rbb.y * x01;
+                        const double t1 = py ? rbb.y * x10 + rbb.x * x11 : rbb.x * x10 - rbb.y * x11;
+                        const double piv = px ? ra.y * t0 + ra.x * t1 : ra.x * t0 - ra.y * t1;
+                        nr = jac_rotation_n(dx, dy, piv);
+                    }
+                    R0[(cur ^ 1) * m + j] = nr;
+                    push(t + 1, nr, seen);
+                }
+                __syncthreads();
+                cur ^= 1;
+            }
+            off2 = block_sum(my_off);
+            converged = off2 <= 0.25 * 2.220446049250313e-16 * 2.220446049250313e-16 * tot2;
+            if (tid < NV) jc_st_relaxed_u32(jc_mapa(jc_smem_u32(&hd->verdict), tid + 1), 2u * (uint32_t)(sweep + 1) + (converged || sweep == 39 ? 1u : 0u));
+        }
+        if (tid == 0 && !(off2 <= 1e-28 * tot2)) atomicOr(status, EPX_ST_JACOBI_NOCONV);
+        const double* S = S0 + cur * nn;
+        for (int f = e; f < M; f++) {             // every epoch of this process gets the eigensystem
+            if (eproc[f] != e) continue;
+            for (int i = tid; i < Kp; i += T) {
+                lam[(size_t)f * Kp + i] = i < K ? S[i * ld + i] : 0.0;
+                sp_out[(size_t)f * Kp + i] = i < K ? sqrt(pi[i]) : 0.0;
+                isp_out[(size_t)f * Kp + i] = i < K ? 1.0 / sqrt(pi[i]) : 0.0;
+            }
+            double* U = Uout + (size_t)f * Kp * Kp;
+            for (int idx = K * Kp + tid; idx < Kp * Kp; idx += T) U[idx] = 0.0;          // padding rows
+        }
+    } else {
+        // ------------------------------------------------------------------------------------------ CTAs 1..NV: rows of V
+        const int rv = (K + NV - 1) / NV, i_lo = ((int)g - 1) * rv, rcnt = max(0, min(rv, K - i_lo));
+        double* const V0 = body;                                                          // [2][rv][n], columns in position order
+        const int vn = rv * n;
+        for (int idx = tid; idx < vn; idx += T) { const int i = idx / n, jj = idx - i * n; V0[idx] = (i_lo + i == jj) ? 1.0 : 0.0; }
+        const bool is_v = tid < rcnt * m;
+        const int il = is_v ? tid / m : 0, b = is_v ? tid % m : 0;
+        const int rt = il * n, ct = b, cb = m + b, wct = jac_newpos(b, m), wcb = jac_newpos(m + b, m);
+        const uint32_t vprog_remote = jc_mapa(jc_smem_u32(&hd->vprog[g - 1]), 0);
+        jc_cluster_barrier();
+        __syncthreads();
+        int cur = 0, t = 0;
+        bool done = false;
+        for (int sweep = 0; !done; sweep++) {
+            for (int r = 0; r < n - 1; r++, t++) {
+                const int slot = t % NS;
+                jc_mbar_wait(&hd->full[slot], (uint32_t)((t / NS) & 1));
+                if (is_v) {
+                    const double2 rbb = ring[slot * m + b];
+                    const double* V = V0 + cur * vn;
+                    double* Vn = V0 + (cur ^ 1) * vn;
+                    const double v0 = V[rt + ct], v1 = V[rt + cb];
+                    Vn[rt + wct] = rbb.x * v0 - rbb.y * v1;
+                    Vn[rt + wcb] = rbb.y * v0 + rbb.x * v1;
+                }
+                __syncthreads();
+                if (tid == 0) {
+                    jc_mbar_expect(&hd->full[slot], 16u * (uint32_t)m);          // arm the slot for round t + NS ...
+                    jc_st_relaxed_u32(vprog_remote, (uint32_t)(t + 1));          // ... and hand it back to CTA 0
+                }
+                cur ^= 1;
+            }
+            uint32_t vd;
+            while (((vd = jc_ld_relaxed_u32(&hd->verdict)) >> 1) <= (uint32_t)sweep) { }
+            done = vd & 1u;
+        }
+        const double* V = V0 + cur * vn;
+        for (int f = e; f < M; f++) {
+            if (eproc[f] != e) continue;
+            double* U = Uout + (size_t)f * Kp * Kp;
+            for (int idx = tid; idx < rcnt * Kp; idx += T) {
+                const int i = idx / Kp, jj = idx - i * Kp;
+                U[(size_t)(i_lo + i) * Kp + jj] = jj < K ? V[i * n + jj] : 0.0;
+            }
+        }
+    }
+    jc_cluster_barrier();                               // nobody leaves while a peer may still store into its shared memory
+}
+
+size_t jacobi_sv_smem(int K, int NV)
+{
+    const size_t m = (K + 1) / 2, n = 2 * m, rv = (K + NV - 1) / NV;
+    const size_t s_cta = sizeof(double) * (2 * n * n + 4 * m + 34);
+    const size_t v_cta = sizeof(double) * (2 * rv * n);
+    const size_t need = sizeof(JsvHeader) + 16 * JSV_NS * m + (s_cta > v_cta ? s_cta : v_cta) + 16;
+    // more than half of an SM's shared memory: the CTAs of a cluster must sit on different SMs (a V CTA beside CTA 0 would
+    // take the issue slots and shared-memory bandwidth the split is there to free)
+    return need > 120 * 1024 ? need : 120 * 1024;
+}
+
 size_t jacobi1_smem(int K)
 {
     const size_t m = (K + 1) / 2, n = 2 * m;
@@ -454,6 +789,8 @@ __global__ void __launch_bounds__(JT) prep64_kernel(const double* __restrict__ U
 int eigen_init_attributes()
 {
     if (cudaFuncSetAttribute(jacobi1_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)jacobi1_smem(62)) != cudaSuccess) return -1;
+    if (cudaFuncSetAttribute(jacobi_sv_kernel<3>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)jacobi_sv_smem(62, 3)) != cudaSuccess) return -1;
+    if (cudaFuncSetAttribute(jacobi_sv_kernel<7>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)jacobi_sv_smem(62, 7)) != cudaSuccess) return -1;
     return cudaFuncSetAttribute(jacobi_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, 96 * 1024) == cudaSuccess ? 0 : -1;
 }
 
@@ -463,7 +800,24 @@ int launch_eigensystems(const epx_ctx* c, cudaStream_t s)
     const int K = c->K, Kp = c->Kp;
     const int ld = K | 1;
     size_t smem = sizeof(double) * (2 * (size_t)K * ld + 2 * (K / 2 + 1) + 32) + sizeof(int) * 2 * (K / 2 + 1);
-    if (K <= 62 && c->jacobi_kernel == 0) {
+    const int jk = c->jacobi_kernel;           // 0 auto, 1 round-1 kernel, 2 one CTA per process, 14 / 18 clusters of 4 / 8
+    const int G = (jk == 14 || jk == 18) ? jk - 10 : (jk == 0 && K > 32 && K <= 62) ? 4 : 1;
+    if (K <= 62 && K >= 16 && G > 1) {
+        const int m = (K + 1) / 2, NV = G - 1, rv = (K + NV - 1) / NV;
+        int warps = 4, bw = (m * (m + 1) / 2 + 31) / 32;   // CTA 0: block warps w % 4 != 3, the rotation warp is warp 3
+        while (warps - warps / 4 < bw) warps++;
+        warps = max(warps, (rv * m + 31) / 32);
+        cudaLaunchConfig_t cfg = {};
+        cfg.gridDim = dim3((unsigned)(c->M * G)); cfg.blockDim = dim3((unsigned)(32 * warps));
+        cfg.dynamicSmemBytes = jacobi_sv_smem(K, NV); cfg.stream = s;
+        cudaLaunchAttribute attr;
+        attr.id = cudaLaunchAttributeClusterDimension;
+        attr.val.clusterDim.x = (unsigned)G; attr.val.clusterDim.y = 1; attr.val.clusterDim.z = 1;
+        cfg.attrs = &attr; cfg.numAttrs = 1;
+        auto kern = G == 4 ? jacobi_sv_kernel<3> : jacobi_sv_kernel<7>;
+        cudaLaunchKernelEx(&cfg, kern, K, Kp, (const double*)d.Q, (const double*)d.freqs, d.lam, d.U, d.sp, d.isp, d.status, c->M,
+                           (const int32_t*)d.eproc);
+    } else if (K <= 62 && jk != 1) {
         const int m = (K + 1) / 2;
         jacobi1_kernel<<<c->M, ((m * m + 31) & ~31) + 32, jacobi1_smem(K), s>>>(K, Kp, d.Q, d.freqs, d.lam, d.U, d.sp, d.isp, d.status, c->M, d.eproc);
     } else {

@@ -124,7 +124,7 @@ struct epx_ctx {
     int epoch_products = 0; // EPX_OPT_EPOCH_PRODUCTS: 1 = chains over >= 2 full epochs use their cached product (f1); 0 (default) off
     int dedup = 1;         // EPX_OPT_SHARE_PROCESSES: 1 (default) one eigensystem / table entry per distinct process, 0 one per epoch
     std::vector<int32_t> eproc, fproc;   // host copies of the maps above (rebuilt when a model or a boundary changes)
-    int jacobi_kernel = 0; // EPX_OPT_JACOBI_KERNEL: 0 auto (K <= 62: one barrier per round), 1 round 1's two-barrier kernel
+    int jacobi_kernel = 0; // EPX_OPT_JACOBI_KERNEL: 0 auto, 1 round 1 kernel, 2 one CTA per process, 12 / 14 / 18 clusters of 2 / 4 / 8
     int mma_chunk = 0;     // EPX_OPT_MMA_CHUNK: site patterns per CTA of the tensor-pipe level kernel (0 auto)
     int exp_method = 0;    // EPX_OPT_EXP_METHOD: 0 auto, 1 spectral (Jacobi / Pade), 2 componentwise (shifted Taylor)
     std::vector<char> model_sparse;   // per epoch: Q has a structural zero off the diagonal
