@@ -382,8 +382,10 @@ def run_cuda(args) -> None:
     #     (device -> host read of logL and the status word) inside the timed region
     e2e = None
     if "e2e" in legs:
+        tips_u8 = np.ascontiguousarray(prob.tip_states, dtype=np.uint8)    # the alignment as host BYTES (epx_set_tip_states_u8)
+
         def e2e_step():
-            epx.set_problem(ctx, prob)
+            epx.set_problem(ctx, prob, tip_states_u8=tips_u8)
             return ctx.log_likelihood()
         Ke = max(3, min(K, 20))
         for _ in range(2):
@@ -399,7 +401,7 @@ def run_cuda(args) -> None:
                8 * prob.M * prob.K * prob.K + 8 * prob.M * prob.K + 8 * (prob.M - 1) + 16 * prob.C + 8 * prob.K)
         e2e = {"value": whole_job_value(unit_bytes, ms_e2e, world), "unit": UNIT, "h2d_bytes_per_step": h2d,
                "d2h_bytes_per_step": 12, "ms_per_step": ms_e2e, "steps": Ke,
-               "what": "all epx_set_* calls from host arrays + epx_log_likelihood (syncs, reads logL + status)"}
+               "what": "all epx_set_* calls from host arrays (tip states as host bytes through epx_set_tip_states_u8) + epx_log_likelihood (syncs, reads logL + status)"}
     # (4) SURVEY.md 8(f) f1, reported beside the headline: one MCMC-style move (one random internal node slides between its
     #     children and its parent) followed by an incremental re-evaluation, host call to host result
     inc = bench_incremental(torch, epx, ctx, prob, stream) if "incremental" in legs else None

@@ -12,7 +12,11 @@
 #include <cstdio>
 #include <cstring>
 #include <cstdlib>
+#include <condition_variable>
+#include <functional>
+#include <mutex>
 #include <thread>
+#include <pthread.h>
 
 namespace {
 
@@ -577,6 +581,66 @@ int epx_set_branch_rates(epx_ctx* c, const double* rates)
     return EPX_OK;
 }
 
+// Host worker threads for the tip-state repacking, created once per process and parked on a condition variable (spawning
+// 15 threads per call cost ~0.4 ms of a 1.4 ms call).  Never destroyed: the threads are detached and the object is leaked on
+// purpose, so there is no destruction-order hazard at exit; a forked child starts a fresh pool.
+namespace {
+struct HostPool {
+    std::mutex mu, busy;
+    std::condition_variable cv, cv_done;
+    std::function<void()> job;
+    int want = 0, started = 0, finished = 0, nthreads = 0;
+    unsigned long long gen = 0;
+    HostPool()
+    {
+        nthreads = (int)std::min<size_t>(15, std::max(1u, std::thread::hardware_concurrency()) - 1);
+        for (int i = 0; i < nthreads; i++) std::thread([this] { loop(); }).detach();
+    }
+    void loop()
+    {
+        unsigned long long seen = 0;
+        std::unique_lock<std::mutex> lk(mu);
+        for (;;) {
+            cv.wait(lk, [&] { return gen != seen; });
+            seen = gen;
+            if (started >= want) continue;
+            started++;
+            lk.unlock();
+            job();
+            lk.lock();
+            if (++finished == want) cv_done.notify_all();
+        }
+    }
+    // `k` workers run fn once each while the caller goes on; finish() waits for them.  One job at a time per process.
+    void start(int k, std::function<void()> fn)
+    {
+        busy.lock();
+        std::lock_guard<std::mutex> lk(mu);
+        job = std::move(fn); want = std::min(k, nthreads); started = finished = 0; gen++;
+        cv.notify_all();
+    }
+    void finish()
+    {
+        {
+            std::unique_lock<std::mutex> lk(mu);
+            cv_done.wait(lk, [&] { return finished == want; });
+            job = nullptr;
+        }
+        busy.unlock();
+    }
+};
+HostPool* g_pool = nullptr;
+std::once_flag g_pool_fork;
+HostPool& host_pool()
+{
+    std::call_once(g_pool_fork, [] { pthread_atfork(nullptr, nullptr, [] { g_pool = nullptr; }); });
+    static std::mutex m;
+    std::lock_guard<std::mutex> lk(m);
+    if (!g_pool) g_pool = new HostPool();
+    return *g_pool;
+}
+}  // namespace
+
 // Repack tip states (int32 or bytes) into the padded byte rows of the page-locked staging buffer.  Integer repacking,
 // split over host threads; no arithmetic of the method.
 extern "C++" {
@@ -622,15 +686,22 @@ static int set_tips_impl(epx_ctx* c, const T* states)
             for (size_t p = L; p < Lp; p++) dst[p] = 255;
         }
     };
-    const size_t nthreads = std::min<size_t>(std::min<size_t>(16, std::max(1u, std::thread::hardware_concurrency())), (N * L) >> 21);
+    // measured on a 16-core host: bytes -> bytes saturates the memory system at 5-6 threads (more are slower), the int32 form
+    // reads four times as much and keeps gaining up to 16
+    const size_t max_nt = sizeof(T) == 1 ? 6 : 16;
+    const size_t nthreads = std::min<size_t>(std::min<size_t>(max_nt, std::max(1u, std::thread::hardware_concurrency())), (N * L) >> 21);
     if (nthreads <= 1) {
         convert_rows(states, base, L, Lp, K, 0, N);
     } else if (!(c->bound && c->tips_pinned)) {
-        std::vector<std::thread> pool;
-        for (size_t w = 1; w < nthreads; w++)
-            pool.emplace_back(convert_rows, states, base, L, Lp, K, N * w / nthreads, N * (w + 1) / nthreads);
-        convert_rows(states, base, L, Lp, K, 0, N / nthreads);      // the calling thread takes the first share
-        for (auto& th : pool) th.join();
+        HostPool& pool = host_pool();
+        const size_t nw = std::min<size_t>(nthreads, (size_t)pool.nthreads + 1);
+        std::atomic<size_t> share{1};
+        pool.start((int)nw - 1, [&] {
+            const size_t w = share.fetch_add(1);
+            convert_rows(states, base, L, Lp, K, N * w / nw, N * (w + 1) / nw);
+        });
+        convert_rows(states, base, L, Lp, K, 0, N / nw);            // the calling thread takes the first share
+        pool.finish();
     } else {
         // Bound ctx: the host -> device copy is pipelined with the repacking.  Workers take chunks of rows in order; the
         // calling thread enqueues the copy of chunk k on the ctx's stream as soon as chunk k is complete, so the DMA of one
@@ -638,6 +709,9 @@ static int set_tips_impl(epx_ctx* c, const T* states)
         // evaluation that read the tips).
         CUDA_TRY(c, cudaSetDevice(c->device));
         const size_t nchunks = std::min<size_t>(N, 4 * nthreads);
+        // copies of >= 4 MB: a host -> device copy has tens of microseconds of fixed cost (64 copies of 0.3 MB took 1.6 ms
+        // where 5 of 4 MB take 0.5)
+        const size_t per_copy = std::max<size_t>(1, std::min(nchunks, ((size_t)4 << 20) * nchunks / (N * Lp) + 1));
         std::atomic<size_t> next{0};
         std::vector<std::atomic<int>> done(nchunks);
         for (auto& f : done) f.store(0, std::memory_order_relaxed);
@@ -647,16 +721,20 @@ static int set_tips_impl(epx_ctx* c, const T* states)
                 done[k].store(1, std::memory_order_release);
             }
         };
-        std::vector<std::thread> pool;
-        for (size_t w = 1; w < nthreads; w++) pool.emplace_back(worker);
+        HostPool& pool = host_pool();
+        pool.start((int)nthreads - 1, worker);
+
+        if (pool.nthreads == 0) worker();
         cudaError_t err = cudaSuccess;
-        for (size_t k = 0; k < nchunks; k++) {
-            while (!done[k].load(std::memory_order_acquire)) std::this_thread::yield();
-            const size_t r0 = N * k / nchunks, r1 = N * (k + 1) / nchunks;
+        for (size_t k0 = 0; k0 < nchunks; k0 += per_copy) {
+            const size_t k1 = std::min(nchunks, k0 + per_copy);
+            for (size_t k = k0; k < k1; k++)
+                while (!done[k].load(std::memory_order_acquire)) std::this_thread::yield();
+            const size_t r0 = N * k0 / nchunks, r1 = N * k1 / nchunks;
             if (err == cudaSuccess)
                 err = cudaMemcpyAsync(c->d.tips + r0 * Lp, base + r0 * Lp, (r1 - r0) * Lp, cudaMemcpyHostToDevice, c->stream);
         }
-        for (auto& th : pool) th.join();
+        pool.finish();
         if (err != cudaSuccess) return fail(c, EPX_E_CUDA, "cudaMemcpyAsync (tip states): %s", cudaGetErrorString(err));
         c->has_tips = true; c->tips_dirty = false;     // already on its way to the device
         c->inc_valid = false;
