@@ -10,6 +10,7 @@
 // U^T in DMMA B-fragment order for the 64-wide tensor-core chain kernel.
 #include "epx_internal.h"
 #include <cstdio>
+#include <type_traits>
 
 namespace {
 
@@ -423,6 +424,12 @@ __device__ __forceinline__ uint32_t jc_ld_relaxed_u32(const uint32_t* p)
     asm volatile("ld.relaxed.cluster.shared::cta.u32 %0, [%1];" : "=r"(v) : "r"(jc_smem_u32(p)) : "memory");
     return v;
 }
+__device__ __forceinline__ uint32_t jc_ld_relaxed_u32a(uint32_t addr)
+{
+    uint32_t v;
+    asm volatile("ld.relaxed.cluster.shared::cta.u32 %0, [%1];" : "=r"(v) : "r"(addr) : "memory");
+    return v;
+}
 __device__ __forceinline__ void jc_mbar_init(uint64_t* bar, int count)
 {
     asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(jc_smem_u32(bar)), "r"(count) : "memory");
@@ -446,7 +453,36 @@ __device__ __forceinline__ void jc_cluster_barrier()
     asm volatile("barrier.cluster.wait.acquire.aligned;" ::: "memory");
 }
 
+// shared-memory accesses at a 32-bit shared address + compile-time byte offset (the generic pointers of a cluster launch make
+// the compiler rebuild the shared window base from SR_CgaCtaId inside the loop)
+template <int OFF> __device__ __forceinline__ double jc_lds(uint32_t a)
+{
+    double v;
+    asm volatile("ld.shared.f64 %0, [%1+%2];" : "=d"(v) : "r"(a), "n"(OFF) : "memory");
+    return v;
+}
+template <int OFF> __device__ __forceinline__ double2 jc_lds2(uint32_t a)
+{
+    double2 v;
+    asm volatile("ld.shared.v2.f64 {%0, %1}, [%2+%3];" : "=d"(v.x), "=d"(v.y) : "r"(a), "n"(OFF) : "memory");
+    return v;
+}
+template <int OFF> __device__ __forceinline__ void jc_sts(uint32_t a, double v)
+{
+    asm volatile("st.shared.f64 [%0+%1], %2;" ::"r"(a), "n"(OFF), "d"(v) : "memory");
+}
+template <int OFF> __device__ __forceinline__ void jc_sts2(uint32_t a, double2 v)
+{
+    asm volatile("st.shared.v2.f64 [%0+%1], {%2, %3};" ::"r"(a), "n"(OFF), "d"(v.x), "d"(v.y) : "memory");
+}
+
+// Launders a per-thread constant through an empty asm: the compiler keeps it in a register instead of re-deriving it from
+// special registers / the constant bank inside the round loops (S2R + LDC chains were ~200 cycles of every round).
+#define JC_PIN(x) asm volatile("" : "+r"(x))
+
 constexpr int JSV_NS = 8;          // ring slots of rotations in a V CTA
+constexpr int JSV_SBUF = 62 * 62;  // doubles per ping-pong buffer of S / of a V CTA's rows (compile-time: the buffer switch is an immediate offset)
+constexpr int JSV_RBUF = 32;       // rotations per ping-pong buffer
 
 struct JsvHeader {                 // at the start of every CTA's dynamic shared memory (same offsets: mapa)
     uint64_t full[JSV_NS];         // V CTAs: slot filled (the V CTA's own arrive + 16 m bytes stored by CTA 0's rotation lanes)
@@ -456,7 +492,7 @@ struct JsvHeader {                 // at the start of every CTA's dynamic shared
 };
 
 template <int NV>
-__global__ void __launch_bounds__(1024) jacobi_sv_kernel(int K, int Kp, const double* __restrict__ Qall,
+__global__ void __launch_bounds__(704) jacobi_sv_kernel(int K, int Kp, const double* __restrict__ Qall,
                                                          const double* __restrict__ freqs, double* __restrict__ lam,
                                                          double* __restrict__ Uout, double* __restrict__ sp_out,
                                                          double* __restrict__ isp_out, int32_t* __restrict__ status,
@@ -485,10 +521,10 @@ __global__ void __launch_bounds__(1024) jacobi_sv_kernel(int K, int Kp, const do
 
     if (g == 0) {
         // ------------------------------------------------------------------------------------------ CTA 0: S and the rotations
-        const int ld = n, nn = n * ld;      // even stride: the rotation lanes' diagonal walks (stride ld + 1) are conflict free
-        double* const S0 = body;                                                          // [2][n][ld], entries p <= q
-        double2* const R0 = reinterpret_cast<double2*>(S0 + 2 * nn);                      // [2][m] (cos, sin)
-        double* const red = reinterpret_cast<double*>(R0 + 2 * m);                        // [33]
+        const int ld = n;                   // even stride: the rotation lanes' diagonal walks (stride ld + 1) are conflict free
+        double* const S0 = body;                                                          // [2][JSV_SBUF] = [2][n][ld], entries p <= q
+        double2* const R0 = reinterpret_cast<double2*>(S0 + 2 * JSV_SBUF);                // [2][JSV_RBUF] (cos, sin)
+        double* const red = reinterpret_cast<double*>(R0 + 2 * JSV_RBUF);                 // [33]
         auto sidx = [&](int p, int q) { return min(p, q) * ld + max(p, q); };
         for (int idx = tid; idx < n * n; idx += T) {    // position = state index at the start of every sweep
             const int i = idx / n, j = idx - i * n;
@@ -553,85 +589,130 @@ __global__ void __launch_bounds__(1024) jacobi_sv_kernel(int K, int Kp, const do
         const int i_bpp = sidx(ay, ay), i_bpq = sidx(ay, m + ay), i_bqq = sidx(m + ay, m + ay);
         // block (ax, ay) by position (sidx picks the stored copy of a symmetric entry)
         const int i_x00 = sidx(ax, ay), i_x01 = sidx(ax, m + ay), i_x10 = sidx(m + ax, ay), i_x11 = sidx(m + ax, m + ay);
-        const uint32_t ring_u32 = jc_smem_u32(ring), full_u32 = jc_smem_u32(&hd->full[0]);
+        const uint32_t ring_u32 = jc_smem_u32(ring), full_u32 = jc_smem_u32(&hd->full[0]), vprog_u32 = jc_smem_u32(&hd->vprog[0]);
         uint32_t ring_v[NV], full_v[NV];
 #pragma unroll
         for (int v = 0; v < NV; v++) { ring_v[v] = jc_mapa(ring_u32, v + 1); full_v[v] = jc_mapa(full_u32, v + 1); }
-        auto push = [&](int t, double2 nr, const uint32_t* seen) {   // rotation lane: rotation j of global round t to every V CTA
-            const int slot = t % NS;
+        auto push0 = [&](double2 nr) {                  // the first rotations (round 0): every slot is free
 #pragma unroll
-            for (int v = 0; v < NV; v++) {
-                if ((int)seen[v] < t + 1 - NS)
-                    while ((int)jc_ld_relaxed_u32(&hd->vprog[v]) < t + 1 - NS) { }        // slot free (never waits in practice)
-                jc_st_async2(ring_v[v] + 16u * (uint32_t)(slot * m + j), nr, full_v[v] + 8u * (uint32_t)slot);
-            }
+            for (int v = 0; v < NV; v++) jc_st_async2(ring_v[v] + 16u * (uint32_t)j, nr, full_v[v]);
         };
         jc_cluster_barrier();                           // every CTA of the cluster is running, its barriers initialised
         if (is_rot) {
             const double2 nr = jac_rotation_n(S0[sidx(j, j)], S0[sidx(m + j, m + j)], S0[sidx(j, m + j)]);
             R0[j] = nr;
-            uint32_t seen[NV];
-#pragma unroll
-            for (int v = 0; v < NV; v++) seen[v] = 0;
-            push(0, nr, seen);
+            push0(nr);
         }
         __syncthreads();
 
-        int cur = 0, t = 0;
+        // Per-thread base pointers; the buffer of a round is a compile-time offset (the round body is instantiated for both
+        // parities), so a round is loads / stores at register + immediate and no address arithmetic: the block warps issue
+        // 27 instructions per round instead of 58, and the rotation lanes' operand loads leave at once.
+        const uint32_t s_u32 = jc_smem_u32(S0), r_u32 = jc_smem_u32(R0);
+        uint32_t p00 = s_u32 + 8 * r00, p01 = s_u32 + 8 * r01, p10 = s_u32 + 8 * r10, p11 = s_u32 + 8 * r11;
+        uint32_t q00 = s_u32 + 8 * w00, q01 = s_u32 + 8 * w01, q10 = s_u32 + 8 * w10, q11 = s_u32 + 8 * w11;
+        uint32_t Ra = r_u32 + 16 * a, Rb = r_u32 + 16 * b;
+        uint32_t o_app = s_u32 + 8 * i_app, o_apq = s_u32 + 8 * i_apq, o_aqq = s_u32 + 8 * i_aqq, o_bpp = s_u32 + 8 * i_bpp,
+                 o_bpq = s_u32 + 8 * i_bpq, o_bqq = s_u32 + 8 * i_bqq, o_x00 = s_u32 + 8 * i_x00, o_x01 = s_u32 + 8 * i_x01,
+                 o_x10 = s_u32 + 8 * i_x10, o_x11 = s_u32 + 8 * i_x11;
+        uint32_t Rax = r_u32 + 16 * ax, Ray = r_u32 + 16 * ay, Rj = r_u32 + 16 * (is_rot ? j : 0);
+        JC_PIN(p00); JC_PIN(p01); JC_PIN(p10); JC_PIN(p11); JC_PIN(q00); JC_PIN(q01); JC_PIN(q10); JC_PIN(q11); JC_PIN(Ra); JC_PIN(Rb);
+        JC_PIN(o_app); JC_PIN(o_apq); JC_PIN(o_aqq); JC_PIN(o_bpp); JC_PIN(o_bpq); JC_PIN(o_bqq);
+        JC_PIN(o_x00); JC_PIN(o_x01); JC_PIN(o_x10); JC_PIN(o_x11); JC_PIN(Rax); JC_PIN(Ray); JC_PIN(Rj);
+        int f_blk = is_blk, f_diag = diag, f_rot = is_rot, f_px = px, f_py = py, f_axy = ax != ay, rounds = n - 1;
+        JC_PIN(f_blk); JC_PIN(f_diag); JC_PIN(f_rot); JC_PIN(f_px); JC_PIN(f_py); JC_PIN(f_axy); JC_PIN(rounds);
+        uint32_t vprog_a = vprog_u32, ring_lane[NV], full_a[NV], slot_stride = 16u * (uint32_t)m;
+#pragma unroll
+        for (int v = 0; v < NV; v++) { ring_lane[v] = ring_v[v] + 16u * (uint32_t)(is_rot ? j : 0); full_a[v] = full_v[v]; JC_PIN(ring_lane[v]); JC_PIN(full_a[v]); }
+        JC_PIN(vprog_a); JC_PIN(slot_stride);
+        auto push = [&](int t, double2 nr, const uint32_t* seen) {   // rotation lane: rotation j of global round t to every V CTA
+            const uint32_t slot = (uint32_t)t % NS;
+#pragma unroll
+            for (int v = 0; v < NV; v++) {
+                if ((int)seen[v] < t + 1 - NS)
+                    while ((int)jc_ld_relaxed_u32a(vprog_a + 4 * v) < t + 1 - NS) { }     // slot free (never waits in practice)
+                jc_st_async2(ring_lane[v] + slot * slot_stride, nr, full_a[v] + 8u * slot);
+            }
+        };
+        // Warp-specialised rounds: the block warps and the rotation warp run their own small loops (each scheduler's
+        // instruction cache holds one of them) and meet at a named barrier that only they join; the other warps of
+        // scheduler 3 sleep until the end of the sweep.
+        const int nbw = (nblk + 31) >> 5;                                   // block warps
+        const bool blk_warp = (wid & 3) != 3 && (wid - (wid >> 2)) < nbw;
+        const bool rot_warp = wid == 3;
+        int nbar = 32 * (nbw + 1);
+        JC_PIN(nbar);
+        auto round_barrier = [&]() { asm volatile("bar.sync 1, %0;" ::"r"(nbar) : "memory"); };
+        int t = 0;
+        double my_off = 0.0;
+        auto blk_round = [&](auto CURC, bool last) {
+            constexpr int CUR = decltype(CURC)::value, SO = 8 * CUR * JSV_SBUF, SN = 8 * (CUR ^ 1) * JSV_SBUF, RO = 16 * CUR * JSV_RBUF;
+            if (f_blk) {
+                const double2 ra = jc_lds2<RO>(Ra), rbb = jc_lds2<RO>(Rb);
+                const double x00 = jc_lds<SO>(p00), x01 = jc_lds<SO>(p01), x10 = jc_lds<SO>(p10), x11 = jc_lds<SO>(p11);
+                // columns (pair b), then rows (pair a): S <- J^T S J on this 2x2 block
+                const double t00 = rbb.x * x00 - rbb.y * x01, t01 = rbb.y * x00 + rbb.x * x01;
+                const double t10 = rbb.x * x10 - rbb.y * x11, t11 = rbb.y * x10 + rbb.x * x11;
+                const double y00 = ra.x * t00 - ra.y * t10, y01 = ra.x * t01 - ra.y * t11;
+                const double y10 = ra.y * t00 + ra.x * t10, y11 = ra.y * t01 + ra.x * t11;
+                // (the rotated pivot of a diagonal block is stored as computed, not forced to zero: (c, s) is a rotation to
+                // rounding whatever the accuracy of its angle, so the iteration stays an orthogonal similarity)
+                jc_sts<SN>(q00, y00); jc_sts<SN>(q01, y01); jc_sts<SN>(q11, y11);
+                if (!f_diag) jc_sts<SN>(q10, y10);                    // (a diagonal block's w10 is its w01)
+                if (last) my_off = f_diag ? 2.0 * y01 * y01 : 2.0 * fma(y00, y00, fma(y01, y01, fma(y10, y10, y11 * y11)));
+            }
+            round_barrier();
+        };
+        auto rot_round = [&](auto CURC) {
+            constexpr int CUR = decltype(CURC)::value, SO = 8 * CUR * JSV_SBUF, RO = 16 * CUR * JSV_RBUF, RN = 16 * (CUR ^ 1) * JSV_RBUF;
+            if (f_rot) {
+                double2 nr = make_double2(1.0, 0.0);
+                uint32_t seen[NV];                           // the V CTAs' progress, read beside the operands
+#pragma unroll
+                for (int v = 0; v < NV; v++) seen[v] = jc_ld_relaxed_u32a(vprog_a + 4 * v);
+                if (f_axy) {
+                    const double2 ra = jc_lds2<RO>(Rax), rbb = jc_lds2<RO>(Ray);
+                    const double app = jc_lds<SO>(o_app), apq = jc_lds<SO>(o_apq), aqq = jc_lds<SO>(o_aqq);
+                    const double bpp = jc_lds<SO>(o_bpp), bpq = jc_lds<SO>(o_bpq), bqq = jc_lds<SO>(o_bqq);
+                    const double x00 = jc_lds<SO>(o_x00), x01 = jc_lds<SO>(o_x01), x10 = jc_lds<SO>(o_x10), x11 = jc_lds<SO>(o_x11);
+                    // the player's updated diagonal entry: (J^T S J)_pp = c^2 Spp - 2 c s Spq + s^2 Sqq, _qq = s^2 Spp + 2 c s Spq + c^2 Sqq
+                    const double ca2 = ra.x * ra.x, sa2 = ra.y * ra.y, csa = 2.0 * ra.x * ra.y;
+                    const double cb2 = rbb.x * rbb.x, sb2 = rbb.y * rbb.y, csb = 2.0 * rbb.x * rbb.y;
+                    const double dx = f_px ? fma(sa2, app, fma(csa, apq, ca2 * aqq)) : fma(ca2, app, fma(-csa, apq, sa2 * aqq));
+                    const double dy = f_py ? fma(sb2, bpp, fma(csb, bpq, cb2 * bqq)) : fma(cb2, bpp, fma(-csb, bpq, sb2 * bqq));
+                    // the new pivot = entry (px, py) of the updated block (ax, ay)
+                    const double t0 = f_py ? rbb.y * x00 + rbb.x * x01 : rbb.x * x00 - rbb.y * x01;
+                    const double t1 = f_py ? rbb.y * x10 + rbb.x * x11 : rbb.x * x10 - rbb.y * x11;
+                    const double piv = f_px ? ra.y * t0 + ra.x * t1 : ra.x * t0 - ra.y * t1;
+                    nr = jac_rotation_n(dx, dy, piv);
+                }
+                jc_sts2<RN>(Rj, nr);
+                push(t + 1, nr, seen);
+            }
+            round_barrier();
+        };
+        int cur = 0;
         bool converged = false;
         double off2 = 0.0;
         for (int sweep = 0; sweep < 40 && !converged; sweep++) {
-            double my_off = 0.0;
-            for (int r = 0; r < n - 1; r++, t++) {
-                const double* S = S0 + cur * nn;
-                double* Sn = S0 + (cur ^ 1) * nn;
-                const double2* R = R0 + cur * m;
-                if (is_blk) {
-                    const double2 ra = R[a], rbb = R[b];
-                    const double x00 = S[r00], x01 = S[r01], x10 = S[r10], x11 = S[r11];
-                    // columns (pair b), then rows (pair a): S <- J^T S J on this 2x2 block
-                    const double t00 = rbb.x * x00 - rbb.y * x01, t01 = rbb.y * x00 + rbb.x * x01;
-                    const double t10 = rbb.x * x10 - rbb.y * x11, t11 = rbb.y * x10 + rbb.x * x11;
-                    const double y00 = ra.x * t00 - ra.y * t10, y01 = ra.x * t01 - ra.y * t11;
-                    const double y10 = ra.y * t00 + ra.x * t10, y11 = ra.y * t01 + ra.x * t11;
-                    // (the rotated pivot of a diagonal block is stored as computed, not forced to zero: (c, s) is a rotation to
-                    // rounding whatever the accuracy of its angle, so the iteration stays an orthogonal similarity)
-                    Sn[w00] = y00; Sn[w01] = y01; Sn[w11] = y11;
-                    if (!diag) Sn[w10] = y10;                    // (a diagonal block's w10 is its w01)
-                    if (r == n - 2) my_off = diag ? 2.0 * y01 * y01 : 2.0 * fma(y00, y00, fma(y01, y01, fma(y10, y10, y11 * y11)));
-                } else if (is_rot) {
-                    double2 nr = make_double2(1.0, 0.0);
-                    uint32_t seen[NV];                           // the V CTAs' progress, read beside the operands
-#pragma unroll
-                    for (int v = 0; v < NV; v++) seen[v] = jc_ld_relaxed_u32(&hd->vprog[v]);
-                    if (ax != ay) {
-                        const double2 ra = R[ax], rbb = R[ay];
-                        const double app = S[i_app], apq = S[i_apq], aqq = S[i_aqq];
-                        const double bpp = S[i_bpp], bpq = S[i_bpq], bqq = S[i_bqq];
-                        const double x00 = S[i_x00], x01 = S[i_x01], x10 = S[i_x10], x11 = S[i_x11];
-                        // the player's updated diagonal entry: (J^T S J)_pp = c^2 Spp - 2 c s Spq + s^2 Sqq, _qq = s^2 Spp + 2 c s Spq + c^2 Sqq
-                        const double ca2 = ra.x * ra.x, sa2 = ra.y * ra.y, csa = 2.0 * ra.x * ra.y;
-                        const double cb2 = rbb.x * rbb.x, sb2 = rbb.y * rbb.y, csb = 2.0 * rbb.x * rbb.y;
-                        const double dx = px ? fma(sa2, app, fma(csa, apq, ca2 * aqq)) : fma(ca2, app, fma(-csa, apq, sa2 * aqq));
-                        const double dy = py ? fma(sb2, bpp, fma(csb, bpq, cb2 * bqq)) : fma(cb2, bpp, fma(-csb, bpq, sb2 * bqq));
-                        // the new pivot = entry (px, py) of the updated block (ax, ay)
-                        const double t0 = py ? rbb.y * x00 + rbb.x * x01 : rbb.x * x00 - rbb.y * x01;
-                        const double t1 = py ? rbb.y * x10 + rbb.x * x11 : rbb.x * x10 - rbb.y * x11;
-                        const double piv = px ? ra.y * t0 + ra.x * t1 : ra.x * t0 - ra.y * t1;
-                        nr = jac_rotation_n(dx, dy, piv);
-                    }
-                    R0[(cur ^ 1) * m + j] = nr;
-                    push(t + 1, nr, seen);
+            if (blk_warp) {
+                for (int r = 0; r < rounds; r++) {
+                    if (((cur + r) & 1) == 0) blk_round(std::integral_constant<int, 0>{}, r == rounds - 1);
+                    else blk_round(std::integral_constant<int, 1>{}, r == rounds - 1);
                 }
-                __syncthreads();
-                cur ^= 1;
+            } else if (rot_warp) {
+                for (int r = 0; r < rounds; r++, t++) {
+                    if (((cur + r) & 1) == 0) rot_round(std::integral_constant<int, 0>{});
+                    else rot_round(std::integral_constant<int, 1>{});
+                }
             }
+            cur = (cur + n - 1) & 1;
             off2 = block_sum(my_off);
             converged = off2 <= 0.25 * 2.220446049250313e-16 * 2.220446049250313e-16 * tot2;
             if (tid < NV) jc_st_relaxed_u32(jc_mapa(jc_smem_u32(&hd->verdict), tid + 1), 2u * (uint32_t)(sweep + 1) + (converged || sweep == 39 ? 1u : 0u));
         }
         if (tid == 0 && !(off2 <= 1e-28 * tot2)) atomicOr(status, EPX_ST_JACOBI_NOCONV);
-        const double* S = S0 + cur * nn;
+        const double* S = S0 + cur * JSV_SBUF;
         for (int f = e; f < M; f++) {             // every epoch of this process gets the eigensystem
             if (eproc[f] != e) continue;
             for (int i = tid; i < Kp; i += T) {
@@ -645,41 +726,45 @@ __global__ void __launch_bounds__(1024) jacobi_sv_kernel(int K, int Kp, const do
     } else {
         // ------------------------------------------------------------------------------------------ CTAs 1..NV: rows of V
         const int rv = (K + NV - 1) / NV, i_lo = ((int)g - 1) * rv, rcnt = max(0, min(rv, K - i_lo));
-        double* const V0 = body;                                                          // [2][rv][n], columns in position order
+        double* const V0 = body;                                                          // [2][JSV_SBUF] = [2][rv][n], columns in position order
         const int vn = rv * n;
         for (int idx = tid; idx < vn; idx += T) { const int i = idx / n, jj = idx - i * n; V0[idx] = (i_lo + i == jj) ? 1.0 : 0.0; }
         const bool is_v = tid < rcnt * m;
         const int il = is_v ? tid / m : 0, b = is_v ? tid % m : 0;
-        const int rt = il * n, ct = b, cb = m + b, wct = jac_newpos(b, m), wcb = jac_newpos(m + b, m);
+        const double *vr0 = V0 + il * n + b, *vr1 = V0 + il * n + m + b;
+        double *vw0 = V0 + il * n + jac_newpos(b, m), *vw1 = V0 + il * n + jac_newpos(m + b, m);
         const uint32_t vprog_remote = jc_mapa(jc_smem_u32(&hd->vprog[g - 1]), 0);
         jc_cluster_barrier();
         __syncthreads();
         int cur = 0, t = 0;
+        auto round = [&](auto CURC) {
+            constexpr int CUR = decltype(CURC)::value, VO = CUR * JSV_SBUF, VN = (CUR ^ 1) * JSV_SBUF;
+            const int slot = t % NS;
+            jc_mbar_wait(&hd->full[slot], (uint32_t)((t / NS) & 1));
+            if (is_v) {
+                const double2 rbb = ring[slot * m + b];
+                const double v0 = vr0[VO], v1 = vr1[VO];
+                vw0[VN] = rbb.x * v0 - rbb.y * v1;
+                vw1[VN] = rbb.y * v0 + rbb.x * v1;
+            }
+            __syncthreads();
+            if (tid == 0) {
+                jc_mbar_expect(&hd->full[slot], 16u * (uint32_t)m);          // arm the slot for round t + NS ...
+                jc_st_relaxed_u32(vprog_remote, (uint32_t)(t + 1));          // ... and hand it back to CTA 0
+            }
+        };
         bool done = false;
         for (int sweep = 0; !done; sweep++) {
             for (int r = 0; r < n - 1; r++, t++) {
-                const int slot = t % NS;
-                jc_mbar_wait(&hd->full[slot], (uint32_t)((t / NS) & 1));
-                if (is_v) {
-                    const double2 rbb = ring[slot * m + b];
-                    const double* V = V0 + cur * vn;
-                    double* Vn = V0 + (cur ^ 1) * vn;
-                    const double v0 = V[rt + ct], v1 = V[rt + cb];
-                    Vn[rt + wct] = rbb.x * v0 - rbb.y * v1;
-                    Vn[rt + wcb] = rbb.y * v0 + rbb.x * v1;
-                }
-                __syncthreads();
-                if (tid == 0) {
-                    jc_mbar_expect(&hd->full[slot], 16u * (uint32_t)m);          // arm the slot for round t + NS ...
-                    jc_st_relaxed_u32(vprog_remote, (uint32_t)(t + 1));          // ... and hand it back to CTA 0
-                }
+                if (cur == 0) round(std::integral_constant<int, 0>{});
+                else round(std::integral_constant<int, 1>{});
                 cur ^= 1;
             }
             uint32_t vd;
             while (((vd = jc_ld_relaxed_u32(&hd->verdict)) >> 1) <= (uint32_t)sweep) { }
             done = vd & 1u;
         }
-        const double* V = V0 + cur * vn;
+        const double* V = V0 + cur * JSV_SBUF;
         for (int f = e; f < M; f++) {
             if (eproc[f] != e) continue;
             double* U = Uout + (size_t)f * Kp * Kp;
@@ -695,8 +780,8 @@ __global__ void __launch_bounds__(1024) jacobi_sv_kernel(int K, int Kp, const do
 size_t jacobi_sv_smem(int K, int NV)
 {
     const size_t m = (K + 1) / 2, n = 2 * m, rv = (K + NV - 1) / NV;
-    const size_t s_cta = sizeof(double) * (2 * n * n + 4 * m + 34);
-    const size_t v_cta = sizeof(double) * (2 * rv * n);
+    const size_t s_cta = sizeof(double) * (2 * JSV_SBUF + 4 * JSV_RBUF + 34);
+    const size_t v_cta = sizeof(double) * (JSV_SBUF + rv * n);
     const size_t need = sizeof(JsvHeader) + 16 * JSV_NS * m + (s_cta > v_cta ? s_cta : v_cta) + 16;
     // more than half of an SM's shared memory: the CTAs of a cluster must sit on different SMs (a V CTA beside CTA 0 would
     // take the issue slots and shared-memory bandwidth the split is there to free)
