@@ -181,6 +181,10 @@ __global__ void __launch_bounds__(JT_MAX) jacobi_kernel(int K, int Kp, const dou
 //     other warps update S and V, so the next round's rotations are ready at the same barrier.
 //   * an odd K gets a dummy player (position 2m-1) whose row and column stay zero (its rotations are the identity).
 // After every sweep (n - 1 rounds) the players are back in their original positions, position = state index.
+// Launders a per-thread constant through an empty asm: the compiler keeps it in a register instead of re-deriving it from
+// special registers / the constant bank inside the round loops (S2R + LDC chains were ~200 cycles of every round).
+#define JC_PIN(x) asm volatile("" : "+r"(x))
+
 __device__ __forceinline__ int jac_newpos(int pos, int m)
 {
     if (pos == 0 || m == 1) return pos;
@@ -307,58 +311,69 @@ __global__ void __launch_bounds__(1024) jacobi1_kernel(int K, int Kp, const doub
     if (is_rot) R0[j] = jac_rotation(S0[j * n + j], S0[(m + j) * n + m + j], S0[j * n + m + j]);
     __syncthreads();
 
+    // (everything the round loop reads is pinned in a register: see JC_PIN)
+    int p_rt = rt, p_rb = rb, p_ct = ct, p_cb = cb, p_wrt = wrt, p_wrb = wrb, p_wct = wct, p_wcb = wcb, p_a = a, p_b = b;
+    int p_blk = is_blk, p_v0 = v0_on, p_v1 = v1_on, p_rot = is_rot, p_j = is_rot ? j : 0, p_rounds = n - 1, p_nn = nn, p_kn = kn, p_m = m;
+    int i_app = ax * n + ax, i_apq = ax * n + m + ax, i_aqq = (m + ax) * n + m + ax, i_bpp = ay * n + ay, i_bpq = ay * n + m + ay,
+        i_bqq = (m + ay) * n + m + ay, i_x00 = ax * n + ay, i_x01 = ax * n + m + ay, i_x10 = (m + ax) * n + ay, i_x11 = (m + ax) * n + m + ay;
+    int p_ax = ax, p_ay = ay, p_px = px, p_py = py;
+    JC_PIN(p_rt); JC_PIN(p_rb); JC_PIN(p_ct); JC_PIN(p_cb); JC_PIN(p_wrt); JC_PIN(p_wrb); JC_PIN(p_wct); JC_PIN(p_wcb); JC_PIN(p_a); JC_PIN(p_b);
+    JC_PIN(p_blk); JC_PIN(p_v0); JC_PIN(p_v1); JC_PIN(p_rot); JC_PIN(p_j); JC_PIN(p_rounds); JC_PIN(p_nn); JC_PIN(p_kn); JC_PIN(p_m);
+    JC_PIN(i_app); JC_PIN(i_apq); JC_PIN(i_aqq); JC_PIN(i_bpp); JC_PIN(i_bpq); JC_PIN(i_bqq); JC_PIN(i_x00); JC_PIN(i_x01); JC_PIN(i_x10); JC_PIN(i_x11);
+    JC_PIN(p_ax); JC_PIN(p_ay); JC_PIN(p_px); JC_PIN(p_py);
+
     int cur = 0;
     bool converged = false;
     double off2 = 0.0;
     for (int sweep = 0; sweep < 40 && !converged; sweep++) {
         double my_off = 0.0;
-        for (int r = 0; r < n - 1; r++) {
-            const double* S = S0 + cur * nn;
-            double* Sn = S0 + (cur ^ 1) * nn;
-            const double2* R = R0 + cur * m;
-            if (is_blk) {
-                const double2 ra = R[a], rbb = R[b];
-                const double x00 = S[rt + ct], x01 = S[rt + cb], x10 = S[rb + ct], x11 = S[rb + cb];
+        for (int r = 0; r < p_rounds; r++) {
+            const double* S = S0 + cur * p_nn;
+            double* Sn = S0 + (cur ^ 1) * p_nn;
+            const double2* R = R0 + cur * p_m;
+            if (p_blk) {
+                const double2 ra = R[p_a], rbb = R[p_b];
+                const double x00 = S[p_rt + p_ct], x01 = S[p_rt + p_cb], x10 = S[p_rb + p_ct], x11 = S[p_rb + p_cb];
                 // columns (pair b), then rows (pair a): S <- J^T S J on this 2x2 block
                 const double t00 = rbb.x * x00 - rbb.y * x01, t01 = rbb.y * x00 + rbb.x * x01;
                 const double t10 = rbb.x * x10 - rbb.y * x11, t11 = rbb.y * x10 + rbb.x * x11;
                 double y00 = ra.x * t00 - ra.y * t10, y01 = ra.x * t01 - ra.y * t11;
                 double y10 = ra.y * t00 + ra.x * t10, y11 = ra.y * t01 + ra.x * t11;
-                if (a == b) { y01 = 0.0; y10 = 0.0; }            // the pivot pair is annihilated exactly
-                Sn[wrt + wct] = y00; Sn[wrt + wcb] = y01; Sn[wrb + wct] = y10; Sn[wrb + wcb] = y11;
-                if (r == n - 2) my_off = a == b ? 0.0 : fma(y00, y00, fma(y01, y01, fma(y10, y10, y11 * y11)));
+                if (p_a == p_b) { y01 = 0.0; y10 = 0.0; }            // the pivot pair is annihilated exactly
+                Sn[p_wrt + p_wct] = y00; Sn[p_wrt + p_wcb] = y01; Sn[p_wrb + p_wct] = y10; Sn[p_wrb + p_wcb] = y11;
+                if (r == p_rounds - 1) my_off = p_a == p_b ? 0.0 : fma(y00, y00, fma(y01, y01, fma(y10, y10, y11 * y11)));
                 // V <- V J: rows a and m + a, the columns of pair b
-                const double* V = V0 + cur * kn;
-                double* Vn = V0 + (cur ^ 1) * kn;
-                if (v0_on) {
-                    const double v0 = V[rt + ct], v1 = V[rt + cb];
-                    Vn[rt + wct] = rbb.x * v0 - rbb.y * v1;
-                    Vn[rt + wcb] = rbb.y * v0 + rbb.x * v1;
+                const double* V = V0 + cur * p_kn;
+                double* Vn = V0 + (cur ^ 1) * p_kn;
+                if (p_v0) {
+                    const double v0 = V[p_rt + p_ct], v1 = V[p_rt + p_cb];
+                    Vn[p_rt + p_wct] = rbb.x * v0 - rbb.y * v1;
+                    Vn[p_rt + p_wcb] = rbb.y * v0 + rbb.x * v1;
                 }
-                if (v1_on) {
-                    const double v0 = V[rb + ct], v1 = V[rb + cb];
-                    Vn[rb + wct] = rbb.x * v0 - rbb.y * v1;
-                    Vn[rb + wcb] = rbb.y * v0 + rbb.x * v1;
+                if (p_v1) {
+                    const double v0 = V[p_rb + p_ct], v1 = V[p_rb + p_cb];
+                    Vn[p_rb + p_wct] = rbb.x * v0 - rbb.y * v1;
+                    Vn[p_rb + p_wcb] = rbb.y * v0 + rbb.x * v1;
                 }
-            } else if (is_rot) {
+            } else if (p_rot) {
                 double2 nr = make_double2(1.0, 0.0);
-                if (ax != ay) {
-                    const double2 ra = R[ax], rbb = R[ay];
-                    const double app = S[ax * n + ax], apq = S[ax * n + m + ax], aqq = S[(m + ax) * n + m + ax];
-                    const double bpp = S[ay * n + ay], bpq = S[ay * n + m + ay], bqq = S[(m + ay) * n + m + ay];
-                    const double x00 = S[ax * n + ay], x01 = S[ax * n + m + ay], x10 = S[(m + ax) * n + ay], x11 = S[(m + ax) * n + m + ay];
+                if (p_ax != p_ay) {
+                    const double2 ra = R[p_ax], rbb = R[p_ay];
+                    const double app = S[i_app], apq = S[i_apq], aqq = S[i_aqq];
+                    const double bpp = S[i_bpp], bpq = S[i_bpq], bqq = S[i_bqq];
+                    const double x00 = S[i_x00], x01 = S[i_x01], x10 = S[i_x10], x11 = S[i_x11];
                     // the player's updated diagonal entry: (J^T S J)_pp = c^2 Spp - 2 c s Spq + s^2 Sqq, _qq = s^2 Spp + 2 c s Spq + c^2 Sqq
                     const double ca2 = ra.x * ra.x, sa2 = ra.y * ra.y, csa = 2.0 * ra.x * ra.y;
                     const double cb2 = rbb.x * rbb.x, sb2 = rbb.y * rbb.y, csb = 2.0 * rbb.x * rbb.y;
-                    const double dx = px ? fma(sa2, app, fma(csa, apq, ca2 * aqq)) : fma(ca2, app, fma(-csa, apq, sa2 * aqq));
-                    const double dy = py ? fma(sb2, bpp, fma(csb, bpq, cb2 * bqq)) : fma(cb2, bpp, fma(-csb, bpq, sb2 * bqq));
+                    const double dx = p_px ? fma(sa2, app, fma(csa, apq, ca2 * aqq)) : fma(ca2, app, fma(-csa, apq, sa2 * aqq));
+                    const double dy = p_py ? fma(sb2, bpp, fma(csb, bpq, cb2 * bqq)) : fma(cb2, bpp, fma(-csb, bpq, sb2 * bqq));
                     // the new pivot = entry (px, py) of the updated block (ax, ay)
-                    const double t0 = py ? rbb.y * x00 + rbb.x * x01 : rbb.x * x00 - rbb.y * x01;
-                    const double t1 = py ? rbb.y * x10 + rbb.x * x11 : rbb.x * x10 - rbb.y * x11;
-                    const double piv = px ? ra.y * t0 + ra.x * t1 : ra.x * t0 - ra.y * t1;
+                    const double t0 = p_py ? rbb.y * x00 + rbb.x * x01 : rbb.x * x00 - rbb.y * x01;
+                    const double t1 = p_py ? rbb.y * x10 + rbb.x * x11 : rbb.x * x10 - rbb.y * x11;
+                    const double piv = p_px ? ra.y * t0 + ra.x * t1 : ra.x * t0 - ra.y * t1;
                     nr = jac_rotation(dx, dy, piv);
                 }
-                R0[(cur ^ 1) * m + j] = nr;
+                R0[(cur ^ 1) * p_m + p_j] = nr;
             }
             __syncthreads();
             cur ^= 1;
@@ -475,10 +490,6 @@ template <int OFF> __device__ __forceinline__ void jc_sts2(uint32_t a, double2 v
 {
     asm volatile("st.shared.v2.f64 [%0+%1], {%2, %3};" ::"r"(a), "n"(OFF), "d"(v.x), "d"(v.y) : "memory");
 }
-
-// Launders a per-thread constant through an empty asm: the compiler keeps it in a register instead of re-deriving it from
-// special registers / the constant bank inside the round loops (S2R + LDC chains were ~200 cycles of every round).
-#define JC_PIN(x) asm volatile("" : "+r"(x))
 
 constexpr int JSV_NS = 8;          // ring slots of rotations in a V CTA
 constexpr int JSV_SBUF = 62 * 62;  // doubles per ping-pong buffer of S / of a V CTA's rows (compile-time: the buffer switch is an immediate offset)
@@ -807,7 +818,25 @@ __global__ void __launch_bounds__(JT) prep_kernel(int Kp, const double* __restri
     const int e = blockIdx.x, tid = threadIdx.x;
     const double* Ue = U + (size_t)e * Kp * Kp;
     double* We = W + (size_t)e * Kp * Kp;
-    if (e >= 1) {
+    if (e >= 1 && Kp <= 32) {
+        // both operands staged in shared memory once (the loop below was a chain of dependent global loads: 19 us for K = 20)
+        __shared__ double ue[32 * 33], um[32 * 32];
+        const double* Um = U + (size_t)(e - 1) * Kp * Kp;
+        const double* spe = sp + (size_t)e * Kp;
+        const double* ispm = isp + (size_t)(e - 1) * Kp;
+        for (int idx = tid; idx < Kp * Kp; idx += JT) {
+            const int k = idx / Kp, a = idx % Kp;
+            ue[a * 33 + k] = Ue[idx] * (spe[k] * ispm[k]);      // transposed: thread (a, b) walks its row
+            um[idx] = Um[idx];
+        }
+        __syncthreads();
+        for (int idx = tid; idx < Kp * Kp; idx += JT) {
+            const int a = idx / Kp, b = idx % Kp;
+            double acc = 0.0;
+            for (int k = 0; k < Kp; k++) acc = fma(ue[a * 33 + k], um[k * Kp + b], acc);
+            We[idx] = acc;
+        }
+    } else if (e >= 1) {
         const double* Um = U + (size_t)(e - 1) * Kp * Kp;
         const double* spe = sp + (size_t)e * Kp;
         const double* ispm = isp + (size_t)(e - 1) * Kp;
