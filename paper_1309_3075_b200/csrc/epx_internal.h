@@ -239,7 +239,7 @@ inline int prune_kp(const epx_ctx* c) { return (c->K + 7) & ~7; }
 bool prune_uses_mma(const epx_ctx* c);
 int prune_mma_chunk(const epx_ctx* c, int nops);
 int prune_mma_init_attributes();
-void launch_prune_mma_level(const epx_ctx* c, const PruneOp* ops, int nops, cudaStream_t s);
+void launch_prune_mma_level(const epx_ctx* c, const PruneOp* ops, int nops, cudaStream_t s, bool pdl);
 void launch_pb_swizzle(const epx_ctx* c, cudaStream_t s);
 
 // Where the pruning kernels of this ctx keep partials and scale exponents.  Element (node block n, category c, pattern p,

@@ -1372,7 +1372,7 @@ static int launch_pruning_dfs(const epx_ctx* c, cudaStream_t s)
 }
 
 // one level of the level-by-level kernels: `nops` operations whose children are complete
-static void launch_level(const epx_ctx* c, const PruneOp* ops, int nops, cudaStream_t s)
+static void launch_level(const epx_ctx* c, const PruneOp* ops, int nops, cudaStream_t s, bool after_level = false)
 {
     const DevBuffers& d = c->d;
     const int K = c->K, C = c->C, L = c->L;
@@ -1388,7 +1388,7 @@ static void launch_level(const epx_ctx* c, const PruneOp* ops, int nops, cudaStr
             default: launch_prune4<8>(ops, nops, L, d, s); break;
         }
     } else if (prune_uses_mma(c)) {
-        launch_prune_mma_level(c, ops, nops, s);
+        launch_prune_mma_level(c, ops, nops, s, after_level);
     } else if (K > 32 && (c->prune_kernel == 4 || c->prune_kernel == 6) && mma64_smem(K, C) <= 227 * 1024) {
         const int tiles = (L + M_TP - 1) / M_TP;
         if (c->prune_kernel == 6) {              // round 1: one CTA per category, clusters of C
@@ -1440,7 +1440,7 @@ int launch_pruning(const epx_ctx* c, cudaStream_t s)
     for (int l = 0; l < n_levels; l++) {
         const int first = c->level_off[l], nops = c->level_off[l + 1] - first;
         if (nops == 0) continue;
-        launch_level(c, c->d.ops + first, nops, s);
+        launch_level(c, c->d.ops + first, nops, s, launched > 1);      // (launch 0 is the swizzle, 1 the first level)
         launched++;
     }
     return cudaGetLastError() == cudaSuccess ? launched : -1;
@@ -1460,7 +1460,7 @@ int launch_pruning_incremental(const epx_ctx* c, const std::vector<int>& group_o
     } else {
         if (prune_uses_mma(c)) { launch_pb_swizzle(c, s); launched++; }  // (the slots of c->sub_list)
         for (size_t g = 0; g + 1 < group_off.size(); g++) {
-            launch_level(c, c->d.inc_pops + group_off[g], group_off[g + 1] - group_off[g], s);
+            launch_level(c, c->d.inc_pops + group_off[g], group_off[g + 1] - group_off[g], s, g > 0);
             launched++;
         }
     }

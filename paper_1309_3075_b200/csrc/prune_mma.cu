@@ -100,6 +100,11 @@ __global__ void __launch_bounds__(MMA_T, KP > 48 ? 2 : 3) prune_mma_kernel(const
             }
     }
     __syncthreads();                                                    // the barriers are initialised
+    // Programmatic dependent launch: a level's CTAs become resident, initialise their barriers and stage their matrices (PB
+    // is complete before the first level starts) while the level below is still running, and wait HERE for its partials.
+    // The trigger comes after the wait, so by induction every earlier level is complete when a CTA passes this point.
+    asm volatile("griddepcontrol.wait;" ::: "memory");
+    asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
 
     const size_t LK = (size_t)L * KP;
     for (int p8 = p_begin + 8 * w; p8 < p_end; p8 += 8 * (MMA_T / 32)) {
@@ -190,12 +195,21 @@ int mma_attr()
 }
 
 template <int KP>
-void mma_launch(const epx_ctx* c, const PruneOp* ops, int nops, cudaStream_t s)
+void mma_launch(const epx_ctx* c, const PruneOp* ops, int nops, cudaStream_t s, bool pdl)
 {
     const DevBuffers& d = c->d;
     const int chunk_p = prune_mma_chunk(c, nops), chunks = (c->L + chunk_p - 1) / chunk_p;
-    prune_mma_kernel<KP><<<nops * c->C * chunks, MMA_T, mma_smem<KP>(), s>>>(ops, chunks, chunk_p, c->K, c->C, c->L, c->Lp, d.PB,
-                                                                             d.tips, d.partials, d.scale_exp);
+    cudaLaunchConfig_t cfg{};
+    cfg.gridDim = dim3((unsigned)(nops * c->C * chunks));
+    cfg.blockDim = dim3(MMA_T);
+    cfg.dynamicSmemBytes = mma_smem<KP>();
+    cfg.stream = s;
+    cudaLaunchAttribute attr{};
+    attr.id = cudaLaunchAttributeProgrammaticStreamSerialization;
+    attr.val.programmaticStreamSerializationAllowed = 1;
+    cfg.attrs = &attr; cfg.numAttrs = pdl ? 1 : 0;          // (the level below is an mma level too: it triggers early)
+    cudaLaunchKernelEx(&cfg, prune_mma_kernel<KP>, ops, chunks, chunk_p, c->K, c->C, c->L, c->Lp, (const double*)d.PB,
+                       (const uint8_t*)d.tips, d.partials, d.scale_exp);
 }
 
 template <int KP>
@@ -222,16 +236,16 @@ int prune_mma_init_attributes()
 }
 
 // One post-order level: `nops` operations whose children are complete.
-void launch_prune_mma_level(const epx_ctx* c, const PruneOp* ops, int nops, cudaStream_t s)
+void launch_prune_mma_level(const epx_ctx* c, const PruneOp* ops, int nops, cudaStream_t s, bool pdl)
 {
     switch (prune_kp(c)) {
-        case 16: mma_launch<16>(c, ops, nops, s); break;
-        case 24: mma_launch<24>(c, ops, nops, s); break;
-        case 32: mma_launch<32>(c, ops, nops, s); break;
-        case 40: mma_launch<40>(c, ops, nops, s); break;
-        case 48: mma_launch<48>(c, ops, nops, s); break;
-        case 56: mma_launch<56>(c, ops, nops, s); break;
-        default: mma_launch<64>(c, ops, nops, s); break;
+        case 16: mma_launch<16>(c, ops, nops, s, pdl); break;
+        case 24: mma_launch<24>(c, ops, nops, s, pdl); break;
+        case 32: mma_launch<32>(c, ops, nops, s, pdl); break;
+        case 40: mma_launch<40>(c, ops, nops, s, pdl); break;
+        case 48: mma_launch<48>(c, ops, nops, s, pdl); break;
+        case 56: mma_launch<56>(c, ops, nops, s, pdl); break;
+        default: mma_launch<64>(c, ops, nops, s, pdl); break;
     }
 }
 
