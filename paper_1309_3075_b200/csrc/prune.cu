@@ -616,6 +616,26 @@ __device__ __forceinline__ double dot4s(const double* __restrict__ col, int stri
     return (a0 + a1) + (a2 + a3);
 }
 
+// dot4s at a compile-time K (KT > 0): the same four chains in the same order, fully unrolled, every load at an immediate offset
+template <int KT>
+__device__ __forceinline__ double dot4t(const double* __restrict__ col, const double* __restrict__ v, int K)
+{
+    if (KT == 0) return dot4s(col, K, v, K);
+    double a0 = 0.0, a1 = 0.0, a2 = 0.0, a3 = 0.0;
+#pragma unroll
+    for (int j = 0; j + 4 <= KT; j += 4) {
+        a0 = fma(col[j * KT], v[j], a0);
+        a1 = fma(col[(j + 1) * KT], v[j + 1], a1);
+        a2 = fma(col[(j + 2) * KT], v[j + 2], a2);
+        a3 = fma(col[(j + 3) * KT], v[j + 3], a3);
+    }
+    constexpr int j = KT & ~3;
+    if (j < KT) a0 = fma(col[j * KT], v[j], a0);
+    if (j + 1 < KT) a1 = fma(col[(j + 1) * KT], v[j + 1], a1);
+    if (j + 2 < KT) a2 = fma(col[(j + 2) * KT], v[j + 2], a2);
+    return (a0 + a1) + (a2 + a3);
+}
+
 // PT[slot][c][j][i] = P[slot][c][i][j]: transposed copies for the few-pattern walk below, whose lane i reads row i of P -- from
 // the row-major matrix that is a stride of K doubles between lanes (16-way bank conflicts at K = 24); from the transposed
 // copy the lanes read consecutive words.
@@ -980,18 +1000,47 @@ __device__ __forceinline__ void cp_async8(void* dst, const void* src)
     asm volatile("cp.async.ca.shared.global [%0], [%1], 8;" ::"r"(smem_addr(dst)), "l"(src) : "memory");
 }
 
+// mbarrier + TMA 1-D bulk copy global -> shared for the staging ring of pruneK_dfs_kernel
+__device__ __forceinline__ void kd_mbar_init(uint64_t* bar, int count)
+{
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_addr(bar)), "r"(count) : "memory");
+}
+__device__ __forceinline__ void kd_mbar_expect_tx(uint64_t* bar, uint32_t bytes)
+{
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_addr(bar)), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void kd_mbar_wait(uint64_t* bar, uint32_t parity)
+{
+    uint32_t ok;
+    do {
+        asm volatile("{\n\t.reg .pred p;\n\tmbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n\tselp.u32 %0, 1, 0, p;\n\t}"
+                     : "=r"(ok) : "r"(smem_addr(bar)), "r"(parity) : "memory");
+    } while (!ok);
+}
+__device__ __forceinline__ void kd_bulk_g2s(void* dst, const void* src, uint32_t bytes, uint64_t* bar)
+{
+    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
+                 ::"r"(smem_addr(dst)), "l"(src), "r"(bytes), "r"(smem_addr(bar)) : "memory");
+}
+
 constexpr int KD_STAGES = 3;
 
+template <int KT, int CT>
 __global__ void __launch_bounds__(32) pruneK_dfs_kernel(const DfsOp* __restrict__ ops, const DfsPiece* __restrict__ pieces,
-    int K, int C, int L, int Lp, int depth, const double* __restrict__ P /* transposed copies, pt_copy_kernel */,
+    int K_rt, int C_rt, int L, int Lp, int depth, const double* __restrict__ P /* transposed copies, pt_copy_kernel */,
     const uint8_t* __restrict__ tips, double* __restrict__ partials, int32_t* __restrict__ scale_exp)
 {
     extern __shared__ double kd_sm[];
+    const int K = KT ? KT : K_rt;                                    // KT > 0: compile-time state count (unrolled dot products)
+    const int C = CT ? CT : C_rt;                                    // CT > 0: compile-time category count (no loops over 8 predicated categories)
+    constexpr int NCAT = CT ? CT : KD_MAXC;
     const int CK = C * K, KK = K * K, CKK = C * KK;
     const int stage_d = 2 * CKK + 2 * CK;                            // doubles per stage: both children's matrices + HBM vectors
     double* ring = kd_sm;                                            // [KD_STAGES][stage_d]
     double* slots = ring + (size_t)KD_STAGES * stage_d;              // [depth + 2][C * K]: stack + 2 hand-over slots
     int* slot_ex = reinterpret_cast<int*>(slots + (size_t)(depth + 2) * CK);    // [depth + 2]
+    uint64_t* kbar = reinterpret_cast<uint64_t*>(slots + (size_t)(depth + 2) * CK + ((depth + 4 + 1) >> 1));   // [KD_STAGES]
+    const bool bulk = ((CKK * 8) & 15) == 0;                         // matrices by TMA bulk copies (16-byte sizes and addresses)
     const int lane = threadIdx.x, i = min(lane, K - 1);
     const bool on = lane < K;
     const int piece = blockIdx.x / L, p = blockIdx.x - piece * L;
@@ -1013,8 +1062,13 @@ __global__ void __launch_bounds__(32) pruneK_dfs_kernel(const DfsOp* __restrict_
             const int srcA = (d.w & 0xff) - 3, srcB = ((d.w >> 8) & 0xff) - 3;
             const double* pa = P + (size_t)d.x * CKK;
             const double* pb = P + (size_t)d.y * CKK;
-            if ((CKK & 1) == 0) {                        // C K^2 even: 16-byte copies (matrices are 16-byte aligned then)
-                for (int o = 2 * lane; o < CKK; o += 64) { cp_async16(st + o, pa + o); cp_async16(st + CKK + o, pb + o); }
+            if (bulk) {                                  // one lane, two bulk copies, completion on the stage's mbarrier
+                if (lane == 0) {
+                    asm volatile("fence.proxy.async.shared::cta;" ::: "memory");       // the stage was read through the generic proxy
+                    kd_mbar_expect_tx(&kbar[k % KD_STAGES], 2 * CKK * 8);
+                    kd_bulk_g2s(st, pa, CKK * 8, &kbar[k % KD_STAGES]);
+                    kd_bulk_g2s(st + CKK, pb, CKK * 8, &kbar[k % KD_STAGES]);
+                }
             } else {
                 for (int o = lane; o < CKK; o += 32) { cp_async8(st + o, pa + o); cp_async8(st + CKK + o, pb + o); }
             }
@@ -1033,6 +1087,11 @@ __global__ void __launch_bounds__(32) pruneK_dfs_kernel(const DfsOp* __restrict_
         }
         cp_async_commit();
     };
+    if (lane == 0) {
+        for (int q = 0; q < KD_STAGES; q++) kd_mbar_init(&kbar[q], 1);
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    }
+    __syncwarp();
     int4 d0, h0, d1, h1, d2, h2, d3, h3;
     load_desc(0, d0, h0); load_desc(1, d1, h1); load_desc(2, d2, h2); load_desc(3, d3, h3);
     int ta0, tb0, ta1, tb1;
@@ -1049,11 +1108,12 @@ __global__ void __launch_bounds__(32) pruneK_dfs_kernel(const DfsOp* __restrict_
         const int out_slot = ((d.w >> 16) & 0xff) - 1;
         const int prev_slot = depth + ((k + 1) & 1), dst = out_slot >= 0 ? out_slot : depth + (k & 1);
         cp_async_wait<2>();
+        if (bulk) kd_mbar_wait(&kbar[k % KD_STAGES], (uint32_t)((k / KD_STAGES) & 1));
         __syncwarp();                                   // stage k has landed; the slot written by operation k-1 is visible
         const double* st = ring + (size_t)(k % KD_STAGES) * stage_d;
-        double f[KD_MAXC];
+        double f[NCAT];
 #pragma unroll
-        for (int c = 0; c < KD_MAXC; c++) f[c] = 1.0;
+        for (int c = 0; c < NCAT; c++) f[c] = 1.0;
         int ex = 0;
         for (int ch = 0; ch < 2; ch++) {
             const int src = srcs[ch];
@@ -1061,7 +1121,7 @@ __global__ void __launch_bounds__(32) pruneK_dfs_kernel(const DfsOp* __restrict_
             if (src == EPX_DFS_TIP) {
                 const int s = aux[ch];
 #pragma unroll
-                for (int c = 0; c < KD_MAXC; c++)
+                for (int c = 0; c < NCAT; c++)
                     if (c < C) f[c] *= s < K ? Pm[c * KK + s * K] : 1.0;
                 continue;
             }
@@ -1075,16 +1135,16 @@ __global__ void __launch_bounds__(32) pruneK_dfs_kernel(const DfsOp* __restrict_
                 ex += slot_ex[sl];
             }
 #pragma unroll
-            for (int c = 0; c < KD_MAXC; c++) {
+            for (int c = 0; c < NCAT; c++) {
                 if (c >= C) break;
                 const double* row = Pm + c * KK;
                 const double* vc = v + c * K;
-                f[c] *= dot4s(row, K, vc, K);          // the level kernel's summation order: incremental re-evaluation is bit-identical
+                f[c] *= dot4t<KT>(row, vc, K);         // the level kernel's summation order: incremental re-evaluation is bit-identical
             }
         }
         double m = 0.0;
 #pragma unroll
-        for (int c = 0; c < KD_MAXC; c++)
+        for (int c = 0; c < NCAT; c++)
             if (c < C && on) m = fmax(m, f[c]);
         for (int o = 16; o > 0; o >>= 1) m = fmax(m, __shfl_xor_sync(0xffffffffu, m, o));
         double sc = 1.0;
@@ -1095,7 +1155,7 @@ __global__ void __launch_bounds__(32) pruneK_dfs_kernel(const DfsOp* __restrict_
         __syncwarp();                                   // every lane has read its operands (dst may be a slot just consumed)
         double* S = slots + (size_t)dst * CK;
 #pragma unroll
-        for (int c = 0; c < KD_MAXC; c++)
+        for (int c = 0; c < NCAT; c++)
             if (c < C && on) {
                 const double val = f[c] * sc;
                 S[c * K + lane] = val;
@@ -1107,7 +1167,8 @@ __global__ void __launch_bounds__(32) pruneK_dfs_kernel(const DfsOp* __restrict_
 
 size_t kdfs_smem(int K, int C, int depth)
 {
-    return sizeof(double) * ((size_t)KD_STAGES * (2 * C * K * K + 2 * C * K) + (size_t)(depth + 2) * C * K) + sizeof(int) * (depth + 4);
+    return sizeof(double) * ((size_t)KD_STAGES * (2 * C * K * K + 2 * C * K) + (size_t)(depth + 2) * C * K) + sizeof(int) * (depth + 6) +
+           sizeof(uint64_t) * KD_STAGES;
 }
 
 // ------------------------------------------------------------------------------------------------ a6
@@ -1259,7 +1320,10 @@ int prune_init_attributes()
         dfs_set_attr<6>() || dfs_set_attr<7>() || dfs_set_attr<8>()) return -1;
     if (prune_lane_init_attributes()) return -1;
     if (cudaFuncSetAttribute(prune64_mma_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024) != cudaSuccess) return -1;
-    if (cudaFuncSetAttribute(pruneK_dfs_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, 100 * 1024) != cudaSuccess) return -1;
+    if (cudaFuncSetAttribute(pruneK_dfs_kernel<0, 0>, cudaFuncAttributeMaxDynamicSharedMemorySize, 100 * 1024) != cudaSuccess) return -1;
+    if (cudaFuncSetAttribute(pruneK_dfs_kernel<0, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, 100 * 1024) != cudaSuccess) return -1;
+    if (cudaFuncSetAttribute(pruneK_dfs_kernel<24, 0>, cudaFuncAttributeMaxDynamicSharedMemorySize, 100 * 1024) != cudaSuccess) return -1;
+    if (cudaFuncSetAttribute(pruneK_dfs_kernel<24, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, 100 * 1024) != cudaSuccess) return -1;
     if (cudaFuncSetAttribute(prune64_cluster_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024) != cudaSuccess) return -1;
     return cudaFuncSetAttribute(prune_generic_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024) == cudaSuccess ? 0 : -1;
 }
@@ -1428,8 +1492,10 @@ int launch_pruning(const epx_ctx* c, cudaStream_t s)
         for (int pass = 0; pass < 2; pass++) {
             const int first = pass == 0 ? 0 : c->dfs_bottom, count = pass == 0 ? c->dfs_bottom : total - c->dfs_bottom;
             if (count <= 0) continue;
-            pruneK_dfs_kernel<<<count * c->L, 32, smem, s>>>(d.dfs_ops, d.dfs_pieces + first, c->K, c->C, c->L, c->Lp, c->dfs_depth,
-                                                           d.PB, d.tips, d.partials, d.scale_exp);
+            auto kern = c->K == 24 ? (c->C == 1 ? pruneK_dfs_kernel<24, 1> : pruneK_dfs_kernel<24, 0>)
+                                   : (c->C == 1 ? pruneK_dfs_kernel<0, 1> : pruneK_dfs_kernel<0, 0>);
+            kern<<<count * c->L, 32, smem, s>>>(d.dfs_ops, d.dfs_pieces + first, c->K, c->C, c->L, c->Lp, c->dfs_depth,
+                                               d.PB, d.tips, d.partials, d.scale_exp);
             n++;
         }
         return cudaGetLastError() == cudaSuccess ? n : -1;
