@@ -241,12 +241,13 @@ __device__ __forceinline__ void carve(int K, double* sm, PadeBufs& b, double*& a
     b.red = b.col + 3 * K;
 }
 
-template <int METHOD, int PT>
-__global__ void __launch_bounds__(PT) pade_full_epoch_kernel(int K, int M, int C, const double* __restrict__ Q,
+template <int METHOD, int PT, int KT>
+__global__ void __launch_bounds__(PT) pade_full_epoch_kernel(int K_rt, int M, int C, const double* __restrict__ Q,
     const double* __restrict__ tau, const double* __restrict__ rates, double* __restrict__ Efull,
     int32_t* __restrict__ status, const int32_t* __restrict__ fproc)
 {
     extern __shared__ double sm[];
+    const int K = KT ? KT : K_rt;          // KT > 0: compile-time state count (full tiles, unrolled products and sweeps)
     PadeBufs b; double* acc;
     carve(K, sm, b, acc);
     const int e = 1 + blockIdx.x / C, c = blockIdx.x % C;    // interior epochs 1 .. M-2
@@ -263,13 +264,14 @@ __global__ void __launch_bounds__(PT) pade_full_epoch_kernel(int K, int M, int C
     }
 }
 
-template <int METHOD, int PT>
-__global__ void __launch_bounds__(PT) pade_chain_kernel(int K, int C, int use_table, const int32_t* __restrict__ order,
+template <int METHOD, int PT, int KT>
+__global__ void __launch_bounds__(PT) pade_chain_kernel(int K_rt, int C, int use_table, const int32_t* __restrict__ order,
     const int32_t* __restrict__ n_seg, const int32_t* __restrict__ seg_off, const int32_t* __restrict__ seg_epoch,
     const double* __restrict__ seg_dur, const double* __restrict__ rates, const double* __restrict__ Q,
     const double* __restrict__ Efull, double* __restrict__ P, int32_t* __restrict__ status)
 {
     extern __shared__ double sm[];
+    const int K = KT ? KT : K_rt;
     PadeBufs b; double* acc;
     carve(K, sm, b, acc);
     const int tid = threadIdx.x, KK = K * K;
@@ -323,20 +325,20 @@ size_t pade_smem_bytes(int K)
     return sizeof(double) * (7 * (size_t)K * K + 3 * K + PT_MAX / 32 + 2);
 }
 
-template <int METHOD, int PT>
+template <int METHOD, int PT, int KT>
 static int pade_attr()
 {
-    if (cudaFuncSetAttribute(pade_full_epoch_kernel<METHOD, PT>, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024) != cudaSuccess) return -1;
-    if (cudaFuncSetAttribute(pade_chain_kernel<METHOD, PT>, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024) != cudaSuccess) return -1;
+    if (cudaFuncSetAttribute(pade_full_epoch_kernel<METHOD, PT, KT>, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024) != cudaSuccess) return -1;
+    if (cudaFuncSetAttribute(pade_chain_kernel<METHOD, PT, KT>, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024) != cudaSuccess) return -1;
     return 0;
 }
 
 int pade_init_attributes()
 {
-    return pade_attr<0, 128>() | pade_attr<0, 512>() | pade_attr<1, 128>() | pade_attr<1, 512>();
+    return pade_attr<0, 128, 0>() | pade_attr<0, 128, 24>() | pade_attr<0, 512, 0>() | pade_attr<1, 128, 0>() | pade_attr<1, 512, 0>();
 }
 
-template <int METHOD, int PT>
+template <int METHOD, int PT, int KT = 0>
 static int launch_dense(const epx_ctx* c, cudaStream_t s)
 {
     const DevBuffers& d = c->d;
@@ -348,14 +350,18 @@ static int launch_dense(const epx_ctx* c, cudaStream_t s)
     const int32_t* order = c->sub_list ? c->sub_list : d.order;      // depends on tau, Q and the rates only and is kept
     if (n == 0) return 0;
     if (M >= 3 && use_table && !c->sub_list) {
-        pade_full_epoch_kernel<METHOD, PT><<<(M - 2) * C, PT, smem, s>>>(K, M, C, d.Q, d.tau, d.rates, d.Efull, d.status, d.fproc);
+        pade_full_epoch_kernel<METHOD, PT, KT><<<(M - 2) * C, PT, smem, s>>>(K, M, C, d.Q, d.tau, d.rates, d.Efull, d.status, d.fproc);
         launched++;
     }
-    pade_chain_kernel<METHOD, PT><<<n * C, PT, smem, s>>>(K, C, use_table, order, d.n_seg, d.seg_off, d.seg_epoch, d.seg_dur,
+    pade_chain_kernel<METHOD, PT, KT><<<n * C, PT, smem, s>>>(K, C, use_table, order, d.n_seg, d.seg_off, d.seg_epoch, d.seg_dur,
                                                            d.rates, d.Q, d.Efull, d.P, d.status);
     launched++;
     return cudaGetLastError() == cudaSuccess ? launched : -1;
 }
 
-int launch_pade_chain(const epx_ctx* c, cudaStream_t s) { return pade_threads(c->K) == 512 ? launch_dense<0, 512>(c, s) : launch_dense<0, 128>(c, s); }
+int launch_pade_chain(const epx_ctx* c, cudaStream_t s)
+{
+    if (c->K == 24) return launch_dense<0, 128, 24>(c, s);       // the trait-model size of config 4 at compile time
+    return pade_threads(c->K) == 512 ? launch_dense<0, 512>(c, s) : launch_dense<0, 128>(c, s);
+}
 int launch_taylor_chain(const epx_ctx* c, cudaStream_t s) { return pade_threads(c->K) == 512 ? launch_dense<1, 512>(c, s) : launch_dense<1, 128>(c, s); }
