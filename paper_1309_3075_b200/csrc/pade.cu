@@ -335,7 +335,7 @@ static int pade_attr()
 
 int pade_init_attributes()
 {
-    return pade_attr<0, 128, 0>() | pade_attr<0, 128, 24>() | pade_attr<0, 512, 0>() | pade_attr<1, 128, 0>() | pade_attr<1, 512, 0>();
+    return pade_attr<0, 128, 0>() | pade_attr<0, 128, 24>() | pade_attr<0, 512, 0>() | pade_attr<1, 128, 0>() | pade_attr<1, 512, 0>() | pade_attr<1, 512, 61>();
 }
 
 template <int METHOD, int PT, int KT = 0>
@@ -364,4 +364,8 @@ int launch_pade_chain(const epx_ctx* c, cudaStream_t s)
     if (c->K == 24) return launch_dense<0, 128, 24>(c, s);       // the trait-model size of config 4 at compile time
     return pade_threads(c->K) == 512 ? launch_dense<0, 512>(c, s) : launch_dense<0, 128>(c, s);
 }
-int launch_taylor_chain(const epx_ctx* c, cudaStream_t s) { return pade_threads(c->K) == 512 ? launch_dense<1, 512>(c, s) : launch_dense<1, 128>(c, s); }
+int launch_taylor_chain(const epx_ctx* c, cudaStream_t s)
+{
+    if (c->K == 61) return launch_dense<1, 512, 61>(c, s);       // the codon models of config 3 at compile time
+    return pade_threads(c->K) == 512 ? launch_dense<1, 512>(c, s) : launch_dense<1, 128>(c, s);
+}
