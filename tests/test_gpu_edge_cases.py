@@ -41,6 +41,27 @@ def test_state_counts_across_kernel_families(epx, orc_ld, K, C, L, reversible):
     run_tree(epx, orc_ld, prob, options=[(epx.EPX_OPT_CHAIN_KERNEL, 1), (epx.EPX_OPT_PRUNE_KERNEL, 1)])
 
 
+@pytest.mark.parametrize("K,C,L,reversible", [(24, 1, 5, False), (24, 3, 7, True), (9, 3, 4, True), (16, 1, 2, True), (31, 2, 3, True)])
+def test_few_pattern_walk_instances(epx, orc_ld, K, C, L, reversible):
+    # pruneK_dfs_kernel (L C <= 64, N >= 8): the compile-time instances K = 24 with C = 1 / runtime C, the generic ones,
+    # matrices staged by TMA bulk copies (C K^2 even) and by cp.async (K = 9, C = 3: odd), several pieces + a top piece;
+    # every node's partials against the oracle, then the level kernels on the same problem
+    rng = np.random.default_rng(2000 + 10 * K + C)
+    prob = _small_problem(rng, K=K, M=3, C=C, N=41, L=L, reversible=reversible, tip_h=rng.uniform(0, 0.2, 41))
+    tips = prob.tip_states.copy()
+    tips[::7, 0] = -1
+    prob = dataclasses.replace(prob, tip_states=tips)
+    if not reversible:
+        prob = dataclasses.replace(prob, root_freqs=prob.freqs[-1].copy())
+    # (reversible models: componentwise exponential, so that every node's partials meet the RELATIVE bound -- DESIGN.md A21)
+    exp_opt = [(epx.EPX_OPT_EXP_METHOD, 2)] if reversible else []
+    lnl, _ = run_tree(epx, orc_ld, prob, options=exp_opt)
+    info = epx.from_problem(prob).plan_info()
+    assert info["depth_first"] == 1 and info["bottom_pieces"] >= 2
+    lnl_level, _ = run_tree(epx, orc_ld, prob, options=exp_opt + [(epx.EPX_OPT_PRUNE_KERNEL, 1)])
+    assert lnl == lnl_level                  # same summation order: bit-identical
+
+
 def test_single_epoch_and_boundaries_outside_the_tree(epx, orc_ld):
     rng = np.random.default_rng(7)
     one = _small_problem(rng, K=4, M=1, C=2, N=10, L=50)                    # M = 1: no boundary at all (homogeneous model)
