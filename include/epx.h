@@ -83,7 +83,10 @@ int epx_epoch_processes(epx_ctx* ctx, int32_t* phi, int* n_processes);
 int epx_set_category_rates(epx_ctx* ctx, const double* rates, const double* weights);
 
 /* ---- tree mode (N tips, 2N-1 nodes, bifurcating) ---- */
-/* parent: 2N-1 entries, tips are 0..N-1, the root has -1.  height: 2N-1, height[parent] >= height[child]. */
+/* parent: 2N-1 entries, tips are 0..N-1, the root has -1.  height: 2N-1, height[parent] >= height[child].
+ * EPX_E_TREE on anything else.  A call whose parent array equals the current one only validates and replaces the heights (the
+ * pruning plans and launch graphs depend on the topology alone) and, if it fails, leaves the current tree in place; a new
+ * topology that fails validation leaves the context without a tree. */
 int epx_set_tree(epx_ctx* ctx, const int32_t* parent, const double* height);
 /* states: [N][L] row-major; 0..K-1 = observed state, anything else = missing (all-ones tip vector, A10). */
 int epx_set_tip_states(epx_ctx* ctx, const int32_t* states);

@@ -512,6 +512,20 @@ int epx_set_tree(epx_ctx* c, const int32_t* parent, const double* height)
 {
     if (!c || !parent || !height) return EPX_E_ARG;
     if (!c->tree_mode) return fail(c, EPX_E_STATE, "ctx is in branch-list mode");
+    if (c->has_tree && (int)c->parent.size() == c->n_nodes && std::memcmp(c->parent.data(), parent, sizeof(int32_t) * c->n_nodes) == 0) {
+        // Same topology (an MCMC chain mostly moves heights): the pruning plans, the launch shapes and the CUDA graphs depend
+        // on the topology only, so only the heights are validated and replaced (the plans cost 0.2 ms for 2 000 tips).
+        for (int i = 0; i < c->n_nodes; i++) {
+            if (!std::isfinite(height[i])) return fail(c, EPX_E_TREE, "height[%d] is not finite", i);
+            const int p = parent[i];
+            if (p >= 0 && height[p] < height[i]) return fail(c, EPX_E_TREE, "node %d is above its parent %d", i, p);
+        }
+        c->height.assign(height, height + c->n_nodes);
+        c->heights_dirty = true;
+        c->inc_valid = false;              // every branch may have changed: the next evaluation is a full one
+        c->dirty_nodes.clear();
+        return EPX_OK;
+    }
     std::vector<int32_t> old_parent = c->parent;
     c->parent.assign(parent, parent + c->n_nodes);
     c->height.assign(height, height + c->n_nodes);

@@ -62,6 +62,32 @@ def test_few_pattern_walk_instances(epx, orc_ld, K, C, L, reversible):
     assert lnl == lnl_level                  # same summation order: bit-identical
 
 
+def test_set_tree_same_topology_fast_path(epx, orc_ld):
+    # epx_set_tree with an unchanged parent array keeps the pruning plans and the CUDA graphs and only replaces the heights:
+    # the result must be that of a fresh context, bad heights must be rejected and leave the context usable
+    prob = W.make_config(2, N=60, L=70)
+    ctx = epx.from_problem(prob)
+    ctx.log_likelihood()
+    rng = np.random.default_rng(3)
+    h2 = prob.height.copy()
+    h2[prob.N:] *= 1.0 + 0.05 * rng.random(prob.n_nodes - prob.N).cumsum() / (prob.n_nodes - prob.N)   # monotone stretch: order kept
+    order_ok = all(h2[prob.parent[i]] >= h2[i] for i in range(prob.n_nodes) if prob.parent[i] >= 0)
+    assert order_ok
+    ctx.set_tree(prob.parent, h2)
+    lnl = ctx.log_likelihood_incremental()          # no complete evaluation of these heights: falls back to a full one
+    prob2 = dataclasses.replace(prob, height=h2)
+    fresh = epx.from_problem(prob2)
+    assert lnl == fresh.log_likelihood()
+    ref = orc_ld.evaluate(prob2)
+    assert abs(np.longdouble(lnl) - ref["lnl"]) <= LNL_RTOL * abs(ref["lnl"])
+    bad = h2.copy()
+    bad[prob.N] = h2.max() + 1.0                    # an internal node above the root
+    with pytest.raises(Exception):
+        ctx.set_tree(prob.parent, bad)
+    assert ctx.log_likelihood() == lnl              # the old tree is still in place
+    ctx.close(); fresh.close()
+
+
 def test_single_epoch_and_boundaries_outside_the_tree(epx, orc_ld):
     rng = np.random.default_rng(7)
     one = _small_problem(rng, K=4, M=1, C=2, N=10, L=50)                    # M = 1: no boundary at all (homogeneous model)
