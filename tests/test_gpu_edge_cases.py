@@ -26,9 +26,11 @@ def epx():
 
 
 @pytest.mark.parametrize("K,C,L,reversible", [(2, 1, 5, True), (7, 3, 45, True), (24, 2, 33, True), (33, 1, 40, True),
-                                              (40, 3, 45, True), (64, 2, 37, True), (7, 2, 9, False), (20, 1, 3, False)])
+                                              (34, 2, 11, True), (40, 3, 45, True), (62, 1, 9, True), (64, 2, 37, True),
+                                              (7, 2, 9, False), (20, 1, 3, False)])
 def test_state_counts_across_kernel_families(epx, orc_ld, K, C, L, reversible):
-    # K = 2, 7, 24: generic shared-memory kernels; 33, 40, 64: DMMA chain + DMMA pruning with 31 / 24 / 0 padding columns;
+    # K = 2, 7, 24: generic shared-memory kernels; 33 .. 64: DMMA chain + DMMA pruning with padding columns; 33 .. 62 take the
+    # cluster Jacobi (odd K: a dummy player; 62: the largest it serves), 64 round 1's kernel;
     # asymmetric: Pade.  L is never a multiple of the pattern tile; some tips are missing.
     rng = np.random.default_rng(1000 + K)
     prob = _small_problem(rng, K=K, M=4, C=C, N=9, L=L, reversible=reversible, tip_h=rng.uniform(0, 0.3, 9))
