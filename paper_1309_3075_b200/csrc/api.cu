@@ -17,6 +17,9 @@
 #include <mutex>
 #include <thread>
 #include <pthread.h>
+#if defined(__SSE2__)
+#include <emmintrin.h>
+#endif
 
 namespace {
 
@@ -689,16 +692,50 @@ static int set_tips_impl(epx_ctx* c, const T* states)
             if (sizeof(T) == 1) {
                 const uint8_t k8 = (uint8_t)K;                // K <= 64
                 const uint8_t* __restrict__ s8 = reinterpret_cast<const uint8_t*>(src);
-                for (size_t p = 0; p < L; p++) dst[p] = (uint8_t)(s8[p] | (uint8_t)(0 - (uint8_t)(s8[p] >= k8)));   // byte-wide
+                size_t p = 0;
+#if defined(__SSE2__)
+                // Streaming (non-temporal) stores: the staging buffer is only read by the DMA engine, and lines left dirty in
+                // the caches of six cores halved the host -> device rate (20 MB: 0.8 - 1.0 ms against 0.4 ms).  Rows of the
+                // page-locked buffer start on 32-byte boundaries (Lp is a multiple of 32).
+                if ((reinterpret_cast<uintptr_t>(dst) & 15) == 0) {
+                    const __m128i kv = _mm_set1_epi8((char)k8);
+                    for (; p + 16 <= L; p += 16) {
+                        const __m128i v = _mm_loadu_si128(reinterpret_cast<const __m128i*>(s8 + p));
+                        const __m128i ge = _mm_cmpeq_epi8(_mm_max_epu8(v, kv), v);          // v >= K (unsigned): 0xff
+                        _mm_stream_si128(reinterpret_cast<__m128i*>(dst + p), _mm_or_si128(v, ge));
+                    }
+                }
+#endif
+                for (; p < L; p++) dst[p] = (uint8_t)(s8[p] | (uint8_t)(0 - (uint8_t)(s8[p] >= k8)));   // byte-wide
             } else {
                 const uint32_t* __restrict__ s32 = reinterpret_cast<const uint32_t*>(src);
-                for (size_t p = 0; p < L; p++) {
+                size_t p = 0;
+#if defined(__SSE2__)
+                if ((reinterpret_cast<uintptr_t>(dst) & 15) == 0) {         // 16 states per streamed store (see the byte form)
+                    const __m128i bias = _mm_set1_epi32((int)0x80000000u), kk = _mm_set1_epi32((int)(K ^ 0x80000000u));
+                    const __m128i miss = _mm_set1_epi32(255);
+                    for (; p + 16 <= L; p += 16) {
+                        __m128i r[4];
+                        for (int q = 0; q < 4; q++) {
+                            const __m128i u = _mm_loadu_si128(reinterpret_cast<const __m128i*>(s32 + p + 4 * q));
+                            const __m128i lt = _mm_cmplt_epi32(_mm_xor_si128(u, bias), kk);              // u < K, unsigned
+                            r[q] = _mm_or_si128(_mm_and_si128(lt, u), _mm_andnot_si128(lt, miss));
+                        }
+                        _mm_stream_si128(reinterpret_cast<__m128i*>(dst + p),
+                                         _mm_packus_epi16(_mm_packs_epi32(r[0], r[1]), _mm_packs_epi32(r[2], r[3])));
+                    }
+                }
+#endif
+                for (; p < L; p++) {
                     const uint32_t s = s32[p];                // negative int32 -> huge -> missing
                     dst[p] = (uint8_t)(s < K ? s : 255u);
                 }
             }
             for (size_t p = L; p < Lp; p++) dst[p] = 255;
         }
+#if defined(__SSE2__)
+        _mm_sfence();                                         // the streamed rows are globally visible before the chunk is reported
+#endif
     };
     // measured on a 16-core host: bytes -> bytes saturates the memory system at 5-6 threads (more are slower), the int32 form
     // reads four times as much and keeps gaining up to 16
