@@ -32,29 +32,46 @@ __device__ __forceinline__ void mm(int K, const double* __restrict__ A, const do
                                    double* __restrict__ Cm)
 {
     const int lane = threadIdx.x & 31, w = threadIdx.x >> 5, g = lane >> 2, q = lane & 3;
-    const int nt_n = (K + 7) >> 3, nk = (K + 3) >> 2, ngrp = (nt_n + 3) >> 2;
+    // Which matrix rows / columns form an 8-wide tile is free (the same map on the A rows, the B columns and the D entries).
+    // Odd K (row stride odd): tile t of a 16-group takes {0, 4, 8, 12, 1, 5, 9, 13} + 2 (t & 1), so the half-warp that makes
+    // one shared-memory wavefront (rows / columns g = 0..3 or 4..7, k = q) hits 16 different 8-byte banks; with consecutive rows
+    // the stride-61 walks of the codon models were 2-way conflicts on every operand load (l1tex 84 %, the limiter of the kernel).
+    const bool perm = K & 1;
+    const int nt_n = perm ? 2 * ((K + 15) >> 4) : (K + 7) >> 3, nk = (K + 3) >> 2, ngrp = (nt_n + 3) >> 2;
+    auto index = [&](int t, int gg) { return perm ? 16 * (t >> 1) + 2 * (t & 1) + 4 * (gg & 3) + (gg >> 2) : 8 * t + gg; };
     for (int item = w; item < nt_n * ngrp; item += PT / 32) {      // item = (row tile, group of four column tiles)
         const int mt = item / ngrp, n0 = 4 * (item - mt * ngrp);
-        const int row = 8 * mt + g;
+        const int row = index(mt, g);
         const bool row_ok = row < K;
         {
             double acc[4][2] = {{0.0, 0.0}, {0.0, 0.0}, {0.0, 0.0}, {0.0, 0.0}};
+            int colB[4];
+#pragma unroll
+            for (int t = 0; t < 4; t++) colB[t] = index(n0 + t, g);
+            // (operands outside the matrix: the load is unconditional at a clamped index and the VALUE is selected -- a guarded
+            //  load may compile to a branch, and mma.sync needs the whole warp converged)
+            const double* Arow = A + min(row, K - 1) * K;
+            int colC[4];
+#pragma unroll
+            for (int t = 0; t < 4; t++) colC[t] = min(colB[t], K - 1);
             for (int kt = 0; kt < nk; kt++) {
-                const int k = 4 * kt + q;
+                const int k = 4 * kt + q, kc = min(k, K - 1);
                 const bool k_ok = k < K;
-                const double a = (row_ok && k_ok) ? A[row * K + k] : 0.0;
+                const double av = Arow[kc];
+                const double a = (row_ok && k_ok) ? av : 0.0;
+                const double* Bk = B + kc * K;
 #pragma unroll
                 for (int t = 0; t < 4; t++) {
-                    const int col = 8 * (n0 + t) + g;
-                    const double b = (k_ok && col < K) ? B[k * K + col] : 0.0;
+                    const double bv = Bk[colC[t]];
+                    const double b = (k_ok && colB[t] < K) ? bv : 0.0;
                     dmma884(acc[t][0], acc[t][1], a, b);
                 }
             }
 #pragma unroll
             for (int t = 0; t < 4; t++) {
-                const int col = 8 * (n0 + t) + 2 * q;
-                if (row_ok && col < K) Cm[row * K + col] = acc[t][0];
-                if (row_ok && col + 1 < K) Cm[row * K + col + 1] = acc[t][1];
+                const int c0 = index(n0 + t, 2 * q), c1 = index(n0 + t, 2 * q + 1);
+                if (row_ok && c0 < K) Cm[row * K + c0] = acc[t][0];
+                if (row_ok && c1 < K) Cm[row * K + c1] = acc[t][1];
             }
         }
     }
