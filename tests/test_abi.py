@@ -100,6 +100,17 @@ def test_host_validation_rules(L):
         with pytest.raises(epx.EpxError) as ei:
             c.set_tree(parent, h)
         assert ei.value.code == epx.EPX_E_TREE
+    # a call with the CURRENT topology only replaces the heights; if it is refused the tree stays in place
+    c.set_tree(good_parent, good_h)
+    c.set_tree(good_parent, [0.0, 0.0, 0.1, 0.4, 2.0])
+    with pytest.raises(epx.EpxError) as ei:
+        c.set_tree(good_parent, [0.0, 0.0, 0.1, 2.4, 2.0])
+    assert ei.value.code == epx.EPX_E_TREE
+    assert c.plan_info()["operations"] == 2          # still planned: the refused call changed nothing
+    with pytest.raises(epx.EpxError):
+        c.set_tree([3, 3, 3, 4, -1], good_h)         # a NEW topology that fails leaves the context without a tree ...
+    with pytest.raises(epx.EpxError):
+        c.plan_info()                                # ... (EPX_E_STATE)
     # moving nodes (f1): a node must stay between its children and its parent; a refused move changes nothing
     c.set_tree(good_parent, good_h)
     c.set_node_heights([3], [0.5])
