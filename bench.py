@@ -646,7 +646,7 @@ def bench_other_configs(torch, epx, device: int, K: int, peaks: dict) -> dict:
                                    "flops": tf["flops"], "dense_products": tf["chain_products"] + tf["table_products"],
                                    "launches": int(sl[2])}
         else:
-            o["bound"] = ("latency: %d dependent operations (largest subtree piece + top piece) of %d, %d tree levels"
+            o["bound"] = ("latency: %d dependent operations (the largest piece of every tier of the walk, one launch per tier) of %d, %d tree levels"
                           % (plan["largest_piece_ops"] + plan["top_piece_ops"], plan["operations"], plan["levels"])
                           if plan["depth_first"] else "latency: %d tree levels, one launch each" % plan["levels"])
             o["us_per_step"] = ms * 1e3

@@ -241,9 +241,11 @@ int epx_tree_levels(const epx_ctx* ctx, int* n_levels);
 /* Shape of the pruning plan of the current tree (host integers; tree mode, after epx_set_tree; EPX_E_STATE otherwise):
  * info[0] post-order levels; [1] pruning operations (internal nodes); [2] 1 if this ctx prunes with a depth-first walk
  * (pieces of the tree walked by independent warps), 0 if level by level; [3] bottom pieces (independent subtrees, one
- * launch); [4] operations of the largest bottom piece; [5] operations of the top piece (second launch; 0 = none);
- * [6] stack slots a walk needs; [7] pruning kernel launches per full evaluation.  [4] + [5] is the dependent-operation
- * chain that bounds the walk when there are few site patterns (PAPER.md L224 workload A, config 4). */
+ * launch); [4] operations of the largest bottom piece; [5] operations above the bottom pieces that depend on each other:
+ * the top piece (second launch; 0 = none), or, when a deep tree is cut into several tiers of pieces (few-pattern walk: level
+ * bands, one launch per tier), the sum over the higher tiers of their largest piece; [6] stack slots a walk needs;
+ * [7] pruning kernel launches per full evaluation.  [4] + [5] is the dependent-operation chain that bounds the walk when
+ * there are few site patterns (PAPER.md L224 workload A, config 4). */
 int epx_plan_info(const epx_ctx* ctx, int32_t info[8]);
 
 #ifdef __cplusplus

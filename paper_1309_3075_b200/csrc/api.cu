@@ -232,20 +232,47 @@ int build_plan(epx_ctx* c)
         for (int u : cuts) is_cut[u] = 1;
     }
     const bool has_top = !(cuts.size() == 1 && cuts[0] == root);
+    // Tiers of pieces, one launch each: the bottom pieces, then what reads their roots from HBM, and so on.
+    std::vector<std::vector<int>> tier_roots;
+    tier_roots.push_back(cuts);
+    if (has_top) tier_roots.push_back({root});
+    // Few-pattern walk (K != 4, one warp per pattern) on a DEEP tree: the time is the chain of dependent operations, largest
+    // bottom piece + top piece (322 of config 4's 1499).  Level bands cut that chain to about the depth of the tree: a piece =
+    // a connected set of nodes whose level (height above the tips in operations) falls into one band, bands widening
+    // like (k / T)^2.5 towards the root (the upper tree is a caterpillar: a band of width w there is a chain of ~w operations,
+    // while near the tips many small subtrees run side by side).  Config 4: 6 bands, 186 dependent operations.
+    if (prune_wants_kdfs(c) && c->dfs_want == 0 && max_level >= 48) {
+        const int T = std::min(8, std::max(3, (max_level + 14) / 28));
+        std::vector<int> th(T);
+        for (int k = 0; k < T; k++) th[k] = std::max(k + 1, (int)std::lround(max_level * std::pow((k + 1.0) / T, 2.5)));    // (exponents 1.5 .. 3 measured: 2.5 gives the shortest chain on config 4)
+        th[T - 1] = max_level;
+        std::vector<int> band(n, -1);
+        for (int u : internal) { int k = 0; while (level[u] > th[k]) k++; band[u] = k; }
+        std::fill(is_cut.begin(), is_cut.end(), 0);
+        tier_roots.assign(T, {});
+        std::vector<int> comp(n, 0);              // operations of the piece below (and including) u
+        for (int k = n - 1; k >= 0; k--) {
+            const int u = order[k];
+            if (left[u] < 0) continue;
+            comp[u] = 1;
+            for (int ch : {left[u], right[u]}) if (left[ch] >= 0 && band[ch] == band[u]) comp[u] += comp[ch];
+        }
+        for (int u : internal)
+            if (c->parent[u] < 0 || band[c->parent[u]] != band[u]) { tier_roots[band[u]].push_back(u); is_cut[u] = 1; }
+        for (auto& r : tier_roots) std::sort(r.begin(), r.end(), [&](int x, int y) { return comp[x] != comp[y] ? comp[x] > comp[y] : x < y; });
+        tier_roots.erase(std::remove_if(tier_roots.begin(), tier_roots.end(), [](const std::vector<int>& r) { return r.empty(); }), tier_roots.end());
+    }
     // kind of a child as seen from the piece being walked: 0 tip, 1 internal (walk into it), 2 root of a bottom piece
     // (a tip with a partial vector is read from HBM like the root of another piece)
-    auto kind = [&](int v, bool top) { return left[v] < 0 ? (c->tip_slot[v] >= 0 ? 2 : 0) : (top && is_cut[v]) ? 2 : 1; };
-    for (int pass = 0; pass < 2; pass++) {     // need[] below the cuts, then above them
-        for (int k = n - 1; k >= 0; k--) {
-            int u = order[k];
-            if (left[u] < 0) continue;
-            int ka = kind(left[u], pass == 1), kb = kind(right[u], pass == 1);
-            int na = ka == 1 ? need[left[u]] : 0, nb = kb == 1 ? need[right[u]] : 0;
-            if (pass == 1 && is_cut[u]) continue;             // keep the bottom value
-            if (ka == 1 && kb == 1) need[u] = std::max(std::max(na, nb), std::min(na, nb) + 1);
-            else need[u] = std::max(1, std::max(na, nb));
-        }
-        if (!has_top) break;
+    // (a piece never contains the root of another piece except as an operand: inside a bottom piece there is none)
+    auto kind = [&](int v, bool) { return left[v] < 0 ? (c->tip_slot[v] >= 0 ? 2 : 0) : is_cut[v] ? 2 : 1; };
+    for (int k = n - 1; k >= 0; k--) {         // stack slots a walk of u's piece needs (Sethi-Ullman), children before parents
+        int u = order[k];
+        if (left[u] < 0) continue;
+        int ka = kind(left[u], true), kb = kind(right[u], true);
+        int na = ka == 1 ? need[left[u]] : 0, nb = kb == 1 ? need[right[u]] : 0;
+        if (ka == 1 && kb == 1) need[u] = std::max(std::max(na, nb), std::min(na, nb) + 1);
+        else need[u] = std::max(1, std::max(na, nb));
     }
     struct Frame { int u, first, second, stage, slot; };
     std::vector<Frame> fr;
@@ -300,9 +327,12 @@ int build_plan(epx_ctx* c)
         high = std::max(high, next_slot);
         c->dfs_pieces.push_back({begin, (int)c->dfs_ops.size()});
     };
-    for (int u : cuts) walk(u, false);
-    c->dfs_bottom = (int)cuts.size();
-    if (has_top) walk(root, true);
+    c->dfs_tier_end.clear();
+    for (const auto& roots : tier_roots) {
+        for (int u : roots) walk(u, true);
+        c->dfs_tier_end.push_back((int)c->dfs_pieces.size());
+    }
+    c->dfs_bottom = c->dfs_tier_end[0];
     c->dfs_depth = std::max(high, 1);
     if (high > 250) return fail(c, EPX_E_TREE, "tree needs %d pruning stack slots (limit 250)", high);
     return EPX_OK;

@@ -165,6 +165,7 @@ struct epx_ctx {
     std::vector<DfsOp> dfs_ops;        // depth-first post-order walk with its stack-slot allocation
     std::vector<DfsPiece> dfs_pieces;  // bottom pieces (independent subtrees, largest first), then the top piece if any
     int dfs_bottom = 0;                // number of bottom pieces (launch 1); the rest (0 or 1) is launch 2
+    std::vector<int> dfs_tier_end;     // pieces up to and including tier t (one launch per tier; K = 4 walks: at most two tiers)
     int dfs_depth = 0;                 // stack slots the walk needs
     int Lp = 0;                        // L rounded up to a multiple of 32 (row stride of the tip-state array)
     int root = -1;
@@ -225,6 +226,7 @@ int eigen_init_attributes();
 int prune_init_attributes();
 int prune_tile(int K, int C);   // patterns per CTA of the generic pruning kernel
 int dfs_tiles(const epx_ctx* c);         // warps per piece of the depth-first walk
+bool prune_wants_kdfs(const epx_ctx* c); // the same without the shared-memory check (which needs the plan)
 bool prune_uses_kdfs(const epx_ctx* c);  // K != 4 depth-first walk for few patterns (generic partials layout)
 bool prune_uses_lane(const epx_ctx* c);  // K == 4 depth-first walk, one lane per pattern (default; generic partials layout)
 bool prune_uses_dfs(const epx_ctx* c);   // K == 4 depth-first walk, lane = (pattern, category): partials are laid out [node][L][C][4]

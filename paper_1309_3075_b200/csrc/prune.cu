@@ -1339,10 +1339,13 @@ int dfs_patterns_per_lane(const epx_ctx* c)
 }
 
 // walk for few patterns and K <= 32 (pruneK_dfs_kernel); generic partials layout
+bool prune_wants_kdfs(const epx_ctx* c)
+{
+    return c->tree_mode && c->K != 4 && c->K <= 32 && c->C <= KD_MAXC && c->prune_kernel == 0 && (long)c->L * c->C <= 64 && c->N >= 8;
+}
 bool prune_uses_kdfs(const epx_ctx* c)
 {
-    return c->tree_mode && c->K != 4 && c->K <= 32 && c->C <= KD_MAXC && c->prune_kernel == 0 && (long)c->L * c->C <= 64 &&
-           c->N >= 8 && kdfs_smem(c->K, c->C, c->dfs_depth > 0 ? c->dfs_depth : 1) <= 100 * 1024;
+    return prune_wants_kdfs(c) && kdfs_smem(c->K, c->C, c->dfs_depth > 0 ? c->dfs_depth : 1) <= 100 * 1024;
 }
 
 // 8 < K <= 64 with enough patterns for 8-pattern tensor tiles: level kernel of prune_mma.cu
@@ -1489,8 +1492,9 @@ int launch_pruning(const epx_ctx* c, cudaStream_t s)
         const size_t smem = kdfs_smem(c->K, c->C, c->dfs_depth);
         int n = 1;
         pt_copy_kernel<<<c->n_slots * c->C, 256, 0, s>>>(c->K, d.P, d.PB);
-        for (int pass = 0; pass < 2; pass++) {
-            const int first = pass == 0 ? 0 : c->dfs_bottom, count = pass == 0 ? c->dfs_bottom : total - c->dfs_bottom;
+        (void)total;
+        for (size_t t = 0; t < c->dfs_tier_end.size(); t++) {           // one launch per tier of pieces
+            const int first = t ? c->dfs_tier_end[t - 1] : 0, count = c->dfs_tier_end[t] - first;
             if (count <= 0) continue;
             auto kern = c->K == 24 ? (c->C == 1 ? pruneK_dfs_kernel<24, 1> : pruneK_dfs_kernel<24, 0>)
                                    : (c->C == 1 ? pruneK_dfs_kernel<0, 1> : pruneK_dfs_kernel<0, 0>);
