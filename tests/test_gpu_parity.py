@@ -169,6 +169,26 @@ def test_k4_extreme_tree_shapes(epx, orc_ld, shape, N):
     run_tree(epx, orc_ld, prob, options=[(epx.EPX_OPT_PRUNE_KERNEL, 3)])
 
 
+@pytest.mark.parametrize("shape,N", [("caterpillar", 130), ("balanced", 128)])
+def test_few_pattern_walk_tiers_on_deep_and_flat_trees(epx, orc_ld, shape, N):
+    # config 4's model (24 states, asymmetric, one site) on a ladder (129 levels: the walk is cut into tiers of pieces by
+    # level bands, one launch per tier, every piece above the first reads its operands from HBM) and on a balanced tree
+    # (7 levels: bottom pieces + one top piece); every node's partials, and bit-identical to the level kernels
+    import dataclasses
+    prob = W.make_config(4, N=N, L=2)
+    parent, height = _shaped_tree(shape, N)
+    height = height * (prob.height.max() / height.max())
+    prob = dataclasses.replace(prob, parent=parent, height=height)
+    ctx = epx.from_problem(prob)
+    info = ctx.plan_info()
+    ctx.close()
+    assert info["depth_first"] == 1
+    assert (info["prune_launches"] >= 5) == (shape == "caterpillar"), info
+    lnl, _ = run_tree(epx, orc_ld, prob)
+    lnl_level, _ = run_tree(epx, orc_ld, prob, options=[(epx.EPX_OPT_PRUNE_KERNEL, 1)])
+    assert lnl == lnl_level
+
+
 def test_k4_matrices_relative_accuracy(epx, orc_ld):
     # K = 4 chain kernel in deviation form (P = I + ...): every entry is good to a few ulp of ITSELF, not only to 1e-12
     # absolute -- on config 2's short branches off-diagonal entries are 1e-6 .. 1e-9 and a cherry's partial is a product of
