@@ -621,10 +621,24 @@ def bench_other_configs(torch, epx, device: int, K: int, peaks: dict) -> dict:
             stage += m
         stage /= steps
         plan = ctx.plan_info()
+        alt = None
+        if cid == 4:
+            # the same step with the asymmetric exponentials by the componentwise-accurate shifted Taylor series instead of Pade 13
+            # (EPX_OPT_EXP_METHOD = 2: no Gauss-Jordan solve; north_star names Pade for asymmetric Q, so it stays the default)
+            ctx.set_option(epx.EPX_OPT_EXP_METHOD, 2)
+            for _ in range(3):
+                lnl_alt = ctx.log_likelihood()
+            ms_alt = bracket(torch, ctx.stream, ctx.enqueue_log_likelihood, steps) / steps
+            ctx.enqueue_log_likelihood()
+            m_alt, _ = ctx.get_stage_ms()
+            alt = {"exp_method": "componentwise shifted Taylor (EPX_OPT_EXP_METHOD = 2)", "ms_per_step": ms_alt,
+                   "chain_ms": float(m_alt[2]), "log_likelihood": lnl_alt}
         ctx.close()
         o = {"config": workload_config(prob, cid, 1), "ms_per_step": ms, "steps": steps, "gpu_launches_per_step": int(launches),
              "log_likelihood": lnl, "stage_ms": {n: float(v) for n, v in zip(epx.STAGE_NAMES, stage)},
              "stage_launches": {n: int(v) for n, v in zip(epx.STAGE_NAMES, sl)}, "plan": plan}
+        if alt is not None:
+            o["alternative"] = alt
         if cid in (3, 6):
             Kc, C, L, n_int = prob.K, prob.C, prob.L, prob.N - 1
             pf = n_int * C * L * (4 * Kc * Kc + Kc)              # O(K^2 N C L) with both children counted
