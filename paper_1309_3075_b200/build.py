@@ -14,7 +14,7 @@ _HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(_HERE, "csrc")
 LIB_PATH = os.path.join(_HERE, "libepx.so")
 SOURCES = ["api.cu", "segmenter.cu", "eigen.cu", "chain.cu", "pade.cu", "prune.cu", "prune_lane.cu", "prune_mma.cu", "peaks.cu"]
-DEPS = ["epx_internal.h", "prune_common.cuh", "api_compute.inc", os.path.join("..", "..", "include", "epx.h")]
+DEPS = ["epx_internal.h", "prune_common.cuh", "seg_common.cuh", "api_compute.inc", os.path.join("..", "..", "include", "epx.h")]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",
               "-Xcompiler", "-fPIC"] + os.environ.get("EPX_NVCC_EXTRA", "").split()
 

@@ -378,6 +378,7 @@ void epx_destroy(epx_ctx* c)
     for (cudaEvent_t e : c->ev) if (e) cudaEventDestroy(e);
     if (c->ev_fork) cudaEventDestroy(c->ev_fork);
     if (c->ev_join) cudaEventDestroy(c->ev_join);
+    if (c->ev_seg) cudaEventDestroy(c->ev_seg);
     if (c->side) cudaStreamDestroy(c->side);
     if (c->tips) { if (c->tips_pinned) cudaFreeHost(c->tips); else free(c->tips); }
     delete c;

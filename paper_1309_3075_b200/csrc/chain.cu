@@ -17,14 +17,15 @@
 //                         mma.sync m8n8k4 f64 (DMMA) tiles, B operands pre-swizzled in fragment order and staged by
 //                         TMA bulk copies (cp.async.bulk + mbarrier) into a double-buffered shared-memory ring
 #include "epx_internal.h"
+#include "seg_common.cuh"
 
 namespace {
 
 // ------------------------------------------------------------------------------------------------ K == 4
 template <int K>
 __global__ void __launch_bounds__(256) chain_rows_kernel(int n_slots, int C, const int32_t* __restrict__ list,
-    const int32_t* __restrict__ n_seg,
-    const int32_t* __restrict__ seg_off, const int32_t* __restrict__ seg_epoch, const double* __restrict__ seg_dur,
+    int M, const double* __restrict__ tau, const int32_t* __restrict__ parent, const double* __restrict__ height,
+    const double* __restrict__ child_h, const double* __restrict__ parent_h, const double* __restrict__ brate,
     const double* __restrict__ rates, const double* __restrict__ lam, const double* __restrict__ U,
     const double* __restrict__ W, const double* __restrict__ sp, const double* __restrict__ isp,
     double* __restrict__ P, int32_t* __restrict__ status)
@@ -36,14 +37,20 @@ __global__ void __launch_bounds__(256) chain_rows_kernel(int n_slots, int C, con
     const int bi = (int)(idx / ((long long)K * C));
     const int b = list ? list[bi] : bi;            // f1: only the listed slots
     double* out = P + (((size_t)b * C + c) * K + i) * K;
-    const int n = n_seg[b];
+    // The branch is segmented HERE (a1's expressions: same epochs, same durations bit for bit), so this kernel depends on the
+    // eigensystems only and the segmenter kernels -- whose arrays remain API outputs -- run beside it in the graph.
+    double hc, hp;
+    epxseg::branch_ends(b, parent, height, child_h, parent_h, hc, hp);
+    const int e_lo = epxseg::count_less(tau, M - 1, hc, true), e_hi = epxseg::count_less(tau, M - 1, hp, false);
+    const int n = (hp > hc) ? (e_hi - e_lo + 1) : 0;
     if (n == 0) {
 #pragma unroll
         for (int j = 0; j < K; j++) out[j] = (i == j) ? 1.0 : 0.0;
         return;
     }
-    const int off = seg_off[b];
+    const double rv = brate ? brate[b] : 1.0;
     const double r = rates[c];
+    double upper = hp;
     // Deviation form: the thread carries a = (row i of the running product) - e_i and multiplies by
     //   P_s = I + Pi^{-1/2} U expm1(L r d) U^T Pi^{1/2}
     // segment by segment.  On a short segment every entry of P_s - I is O(r d) and is computed to a few ulp of ITSELF
@@ -54,8 +61,10 @@ __global__ void __launch_bounds__(256) chain_rows_kernel(int n_slots, int C, con
 #pragma unroll
     for (int j = 0; j < K; j++) a[j] = 0.0;
     for (int s = 0; s < n; s++) {
-        const int e = seg_epoch[off + s];
-        const double rd = r * seg_dur[off + s];
+        const int e = e_hi - s;
+        const double lower = (s == n - 1) ? hc : tau[e - 1];
+        const double rd = r * (brate ? (upper - lower) * rv : upper - lower);
+        upper = lower;
         const double* Ue = U + (size_t)e * K * K;
         double z[K];
         const double si = isp[e * K + i];
@@ -447,7 +456,8 @@ int launch_chain_reversible(const epx_ctx* c, cudaStream_t s)
     if (K == 4) {
         long long threads = (long long)n * C * 4;
         int blocks = (int)((threads + 255) / 256);
-        chain_rows_kernel<4><<<blocks, 256, 0, s>>>(n, C, c->sub_list, d.n_seg, d.seg_off, d.seg_epoch, d.seg_dur, d.rates,
+        chain_rows_kernel<4><<<blocks, 256, 0, s>>>(n, C, c->sub_list, c->M, d.tau, c->tree_mode ? d.parent : nullptr, d.height, d.child_h, d.parent_h,
+                                                    c->has_brates ? d.brate : nullptr, d.rates,
                                                     d.lam, d.U, d.W, d.sp, d.isp, d.P, d.status);
     } else if (Kp == 64 && c->chain_kernel != 1) {
         int launched = 0;

@@ -799,6 +799,62 @@ size_t jacobi_sv_smem(int K, int NV)
     return need > 120 * 1024 ? need : 120 * 1024;
 }
 
+// ------------------------------------------------------------------------------------------------ K == 4: one warp, no shared memory
+// The 4-state models sit on the critical path of every nucleotide evaluation (a3 / a4 wait for them; 13 us in jacobi1_kernel:
+// 20 rounds of a CTA barrier and a rotation chain through shared memory).  Here a warp holds everything in registers: lane
+// 4 i + j of the lower half owns S[i][j], of the upper half V[i][j].  The three rounds of a sweep pair index t with t ^ 1, t ^ 2,
+// t ^ 3, so a partner row / column is the lane with those bits flipped: a round is 6 shuffles for the two rotations (every lane
+// computes both), 3 for the 2x2 update and a dozen fp64 operations; no barrier anywhere.
+__global__ void __launch_bounds__(32) jacobi4_kernel(const double* __restrict__ Qall, const double* __restrict__ freqs,
+                                                     double* __restrict__ lam, double* __restrict__ Uout, double* __restrict__ sp_out,
+                                                     double* __restrict__ isp_out, int32_t* __restrict__ status, int M,
+                                                     const int32_t* __restrict__ eproc)
+{
+    constexpr unsigned FULL = 0xffffffffu;
+    const int e = blockIdx.x;
+    if (eproc[e] != e) return;                          // f2: this epoch shares the process of an earlier one
+    const int lane = threadIdx.x, i = (lane >> 2) & 3, j = lane & 3;
+    const bool is_s = lane < 16;
+    const double* Q = Qall + (size_t)e * 16;
+    const double* pi = freqs + (size_t)e * 4;
+    double x;
+    {
+        const double si = sqrt(pi[i]), sj = sqrt(pi[j]);
+        const double a = si * Q[i * 4 + j] / sj, b = sj * Q[j * 4 + i] / si;
+        x = is_s ? 0.5 * (a + b) : (i == j ? 1.0 : 0.0);
+    }
+    auto warp_sum = [&](double v) { for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(FULL, v, o); return v; };
+    const double tot2 = warp_sum(is_s ? x * x : 0.0);
+    double off2 = 0.0;
+    bool converged = false;
+    for (int sweep = 0; sweep < 40 && !converged; sweep++) {
+#pragma unroll
+        for (int m = 1; m <= 3; m++) {                  // pairs (t, t ^ m); p = the smaller index
+            const int ip = i ^ m, jp = j ^ m;
+            const int pi_ = min(i, ip), qi = max(i, ip), pj = min(j, jp), qj = max(j, jp);
+            // the two rotations this lane needs, from the S half (every lane computes them: no broadcast step)
+            const double2 ri = jac_rotation_n(__shfl_sync(FULL, x, 5 * pi_), __shfl_sync(FULL, x, 5 * qi), __shfl_sync(FULL, x, 4 * pi_ + qi));
+            const double2 rj = jac_rotation_n(__shfl_sync(FULL, x, 5 * pj), __shfl_sync(FULL, x, 5 * qj), __shfl_sync(FULL, x, 4 * pj + qj));
+            const double xj = __shfl_xor_sync(FULL, x, m);           // same row, partner column
+            const double xi = __shfl_xor_sync(FULL, x, m << 2);      // partner row, same column
+            const double xij = __shfl_xor_sync(FULL, x, m | (m << 2));
+            // new column p = c col_p - s col_q, new column q = s col_p + c col_q (and the same for rows): S <- J^T S J, V <- V J
+            const double bj = j < jp ? -rj.y : rj.y, bi = i < ip ? -ri.y : ri.y;
+            const double row_own = fma(bj, xj, rj.x * x), row_par = fma(bj, xij, rj.x * xi);
+            x = is_s ? fma(bi, row_par, ri.x * row_own) : row_own;
+        }
+        off2 = warp_sum(is_s && i != j ? x * x : 0.0);
+        converged = off2 <= 0.25 * 2.220446049250313e-16 * 2.220446049250313e-16 * tot2;
+    }
+    if (lane == 0 && !(off2 <= 1e-28 * tot2)) atomicOr(status, EPX_ST_JACOBI_NOCONV);
+    for (int f = e; f < M; f++) {                       // every epoch of this process gets the eigensystem (Kp == K == 4)
+        if (eproc[f] != e) continue;
+        if (!is_s) Uout[(size_t)f * 16 + 4 * i + j] = x;
+        else if (i == j) lam[(size_t)f * 4 + i] = x;
+        if (lane < 4) { sp_out[(size_t)f * 4 + lane] = sqrt(pi[lane]); isp_out[(size_t)f * 4 + lane] = 1.0 / sqrt(pi[lane]); }
+    }
+}
+
 size_t jacobi1_smem(int K)
 {
     const size_t m = (K + 1) / 2, n = 2 * m;
@@ -915,6 +971,12 @@ int launch_eigensystems(const epx_ctx* c, cudaStream_t s)
     const int ld = K | 1;
     size_t smem = sizeof(double) * (2 * (size_t)K * ld + 2 * (K / 2 + 1) + 32) + sizeof(int) * 2 * (K / 2 + 1);
     const int jk = c->jacobi_kernel;           // 0 auto, 1 round-1 kernel, 2 one CTA per process, 14 / 18 clusters of 4 / 8
+    if (K == 4 && jk == 0) {                   // one warp per process, everything in registers
+        jacobi4_kernel<<<c->M, 32, 0, s>>>(d.Q, d.freqs, d.lam, d.U, d.sp, d.isp, d.status, c->M, d.eproc);
+        if (c->chain_kernel == 0) return cudaGetLastError() == cudaSuccess ? 1 : -1;      // chain_rows_kernel<4> needs no W
+        prep_kernel<<<c->M, JT, 0, s>>>(Kp, d.U, d.sp, d.isp, d.W, d.WB, d.UTB);
+        return cudaGetLastError() == cudaSuccess ? 2 : -1;
+    }
     const int G = (jk == 14 || jk == 18) ? jk - 10 : (jk == 0 && K > 32 && K <= 62) ? 4 : 1;
     if (K <= 62 && K >= 16 && G > 1) {
         const int m = (K + 1) / 2, NV = G - 1, rv = (K + NV - 1) / NV;

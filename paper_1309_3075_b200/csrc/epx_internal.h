@@ -190,7 +190,7 @@ struct epx_ctx {
     bool capturing = false;   // enqueue_kernels is running under stream capture
     // graph mode only: a1 (segmenter) and a2 (eigensystems) are independent and run as two branches of the graph
     cudaStream_t side = nullptr;
-    cudaEvent_t ev_fork = nullptr, ev_join = nullptr;
+    cudaEvent_t ev_fork = nullptr, ev_join = nullptr, ev_seg = nullptr;
 
     long long launches = 0;
     bool have_result = false;
