@@ -28,8 +28,19 @@ __global__ void __launch_bounds__(256) chain_rows_kernel(int n_slots, int C, con
     const double* __restrict__ child_h, const double* __restrict__ parent_h, const double* __restrict__ brate,
     const double* __restrict__ rates, const double* __restrict__ lam, const double* __restrict__ U,
     const double* __restrict__ W, const double* __restrict__ sp, const double* __restrict__ isp,
-    double* __restrict__ P, int32_t* __restrict__ status)
+    double* __restrict__ P, int32_t* __restrict__ status, int staged)
 {
+    // The per-epoch inputs (boundaries, eigenvalues, eigenvectors, sqrt(pi)) are a few KB: one cooperative copy into shared
+    // memory replaces the chains of dependent global loads of the boundary search and of every segment.
+    extern __shared__ double cs[];
+    if (staged) {
+        double* s_tau = cs; double* s_lam = s_tau + (M - 1); double* s_U = s_lam + M * K; double* s_sp = s_U + M * K * K; double* s_isp = s_sp + M * K;
+        for (int t = threadIdx.x; t < M - 1; t += blockDim.x) s_tau[t] = tau[t];
+        for (int t = threadIdx.x; t < M * K; t += blockDim.x) { s_lam[t] = lam[t]; s_sp[t] = sp[t]; s_isp[t] = isp[t]; }
+        for (int t = threadIdx.x; t < M * K * K; t += blockDim.x) s_U[t] = U[t];
+        __syncthreads();
+        tau = s_tau; lam = s_lam; U = s_U; sp = s_sp; isp = s_isp;
+    }
     long long idx = (long long)blockIdx.x * blockDim.x + threadIdx.x;
     if (idx >= (long long)n_slots * C * K) return;
     const int i = (int)(idx % K);
@@ -456,9 +467,11 @@ int launch_chain_reversible(const epx_ctx* c, cudaStream_t s)
     if (K == 4) {
         long long threads = (long long)n * C * 4;
         int blocks = (int)((threads + 255) / 256);
-        chain_rows_kernel<4><<<blocks, 256, 0, s>>>(n, C, c->sub_list, c->M, d.tau, c->tree_mode ? d.parent : nullptr, d.height, d.child_h, d.parent_h,
-                                                    c->has_brates ? d.brate : nullptr, d.rates,
-                                                    d.lam, d.U, d.W, d.sp, d.isp, d.P, d.status);
+        const size_t stage_bytes = sizeof(double) * ((size_t)c->M - 1 + (size_t)c->M * (4 * 4 + 3 * 4));
+        const int staged = stage_bytes <= 16 * 1024;
+        chain_rows_kernel<4><<<blocks, 256, staged ? stage_bytes : 0, s>>>(n, C, c->sub_list, c->M, d.tau, c->tree_mode ? d.parent : nullptr, d.height,
+                                                    d.child_h, d.parent_h, c->has_brates ? d.brate : nullptr, d.rates,
+                                                    d.lam, d.U, d.W, d.sp, d.isp, d.P, d.status, staged);
     } else if (Kp == 64 && c->chain_kernel != 1) {
         int launched = 0;
         if (chain_uses_epoch_products(c)) {
