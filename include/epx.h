@@ -219,10 +219,11 @@ enum {
     EPX_OPT_DFS_PIECES = 7,   /* depth-first pruning: number of pieces the tree is cut into (independent subtrees walked by
                                  different warps + the part above them); 0 (default) auto */
     EPX_OPT_MMA_CHUNK = 8,    /* 8 < K <= 64 tensor-pipe level kernel: site patterns per CTA (rounded up to 8); 0 (default) auto */
-    EPX_OPT_JACOBI_KERNEL = 9, /* a2: 0 (default) auto: for 32 < K <= 62 a thread-block cluster of 4 CTAs per process (rows of S and V
-                                 split over the CTAs, one cluster barrier per round), for K <= 32 one CTA per process with one
-                                 barrier per round; 2 one CTA per process; 12 / 14 / 18 clusters of 2 / 4 / 8 CTAs (identical
-                                 bits to 2); 1 round 1's two-barrier kernel */
+    EPX_OPT_JACOBI_KERNEL = 9, /* a2: 0 (default) auto: K == 4 one warp per process (everything in registers); 32 < K <= 62 a
+                                 thread-block cluster of 4 CTAs per process (S in one CTA, V's rows in the three others, rotations
+                                 streamed through distributed shared memory); otherwise one CTA per process with one barrier per
+                                 round.  2 one CTA per process for any K <= 62; 14 / 18 clusters of 4 / 8 CTAs (16 <= K <= 62);
+                                 1 round 1's two-barrier kernel.  All meet the same bounds; their bits differ */
     EPX_OPT_SHARE_PROCESSES = 10, /* 1 (default) one eigensystem / full-epoch exponential per distinct process (epx_epoch_processes);
                                  0 one per epoch */
     EPX_OPT_EPOCH_PRODUCTS = 11 /* SURVEY.md 8(f) f1.  0 (default): every branch multiplies its whole chain, one product per
