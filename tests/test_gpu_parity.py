@@ -88,6 +88,9 @@ def test_config1_generic_kernels_and_no_graph(epx, orc_ld):
     prob = W.make_config(1)
     run_tree(epx, orc_ld, prob, options=[(epx.EPX_OPT_CHAIN_KERNEL, 1), (epx.EPX_OPT_PRUNE_KERNEL, 1)])
     run_tree(epx, orc_ld, prob, options=[(epx.EPX_OPT_USE_GRAPH, 0)])
+    # a2 for K = 4: the single-warp kernel is the default; the CTA kernels (one barrier per round, round 1's) stay selectable
+    run_tree(epx, orc_ld, prob, options=[(epx.EPX_OPT_JACOBI_KERNEL, 2)])
+    run_tree(epx, orc_ld, prob, options=[(epx.EPX_OPT_JACOBI_KERNEL, 1), (epx.EPX_OPT_CHAIN_KERNEL, 1)])
 
 
 def test_config2_reduced(epx, orc_ld):
