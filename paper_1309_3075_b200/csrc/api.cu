@@ -103,7 +103,7 @@ size_t plan_workspace(const epx_ctx* c, char* base, DevBuffers* d)
         t.site_lnl = (double*)take(8 * L);
         t.block_sums = (double*)take(8 * ((L + 7) / 8));
     }
-    t.inc_slots = (int32_t*)take(4 * S);
+    t.inc_slots = (int32_t*)take(4 * (S + 1));      // [S] = number of listed slots (read by the incremental graph's chain kernel)
     if (c->tree_mode) {
         t.inc_ops = (DfsOp*)take(sizeof(DfsOp) * (N - 1));
         t.inc_piece = (DfsPiece*)take(sizeof(DfsPiece));
@@ -120,6 +120,7 @@ void drop_graphs(epx_ctx* c)
     c->inc_valid = false;      // whatever invalidates the graphs also invalidates an incremental continuation
     c->tipp_dirty = true;      // ... and may change the partials layout the tip blocks were written in
     if (c->graph_mat) { cudaGraphExecDestroy(c->graph_mat); c->graph_mat = nullptr; }
+    if (c->graph_inc) { cudaGraphExecDestroy(c->graph_inc); c->graph_inc = nullptr; }
     if (c->graph_lik) { cudaGraphExecDestroy(c->graph_lik); c->graph_lik = nullptr; }
 }
 

@@ -28,8 +28,9 @@ __global__ void __launch_bounds__(256) chain_rows_kernel(int n_slots, int C, con
     const double* __restrict__ child_h, const double* __restrict__ parent_h, const double* __restrict__ brate,
     const double* __restrict__ rates, const double* __restrict__ lam, const double* __restrict__ U,
     const double* __restrict__ W, const double* __restrict__ sp, const double* __restrict__ isp,
-    double* __restrict__ P, int32_t* __restrict__ status, int staged)
+    double* __restrict__ P, int32_t* __restrict__ status, int staged, const int32_t* __restrict__ n_dev)
 {
+    if (n_dev) n_slots = *n_dev;                 // incremental graph: fixed grid, the slot count lives on the device
     // The per-epoch inputs (boundaries, eigenvalues, eigenvectors, sqrt(pi)) are a few KB: one cooperative copy into shared
     // memory replaces the chains of dependent global loads of the boundary search and of every segment.
     extern __shared__ double cs[];
@@ -469,9 +470,9 @@ int launch_chain_reversible(const epx_ctx* c, cudaStream_t s)
         int blocks = (int)((threads + 255) / 256);
         const size_t stage_bytes = sizeof(double) * ((size_t)c->M - 1 + (size_t)c->M * (4 * 4 + 3 * 4));
         const int staged = stage_bytes <= 16 * 1024;
-        chain_rows_kernel<4><<<blocks, 256, staged ? stage_bytes : 0, s>>>(n, C, c->sub_list, c->M, d.tau, c->tree_mode ? d.parent : nullptr, d.height,
+        chain_rows_kernel<4><<<c->sub_count_dev ? (EPX_INC_GRAPH_SLOTS * C * 4 + 255) / 256 : blocks, 256, staged ? stage_bytes : 0, s>>>(n, C, c->sub_list, c->M, d.tau, c->tree_mode ? d.parent : nullptr, d.height,
                                                     d.child_h, d.parent_h, c->has_brates ? d.brate : nullptr, d.rates,
-                                                    d.lam, d.U, d.W, d.sp, d.isp, d.P, d.status, staged);
+                                                    d.lam, d.U, d.W, d.sp, d.isp, d.P, d.status, staged, c->sub_count_dev);
     } else if (Kp == 64 && c->chain_kernel != 1) {
         int launched = 0;
         if (chain_uses_epoch_products(c)) {

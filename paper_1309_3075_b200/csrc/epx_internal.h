@@ -9,6 +9,7 @@
 #define EPX_MAX_K 64
 #define EPX_MAX_C 8
 #define EPX_MAX_M 4096
+#define EPX_INC_GRAPH_SLOTS 64     // matrix slots an incremental call may touch and still replay its CUDA graph
 #define EPX_SORT_BINS 64 /* counting-sort bins for n_seg (n_seg >= 63 share the top bin) */
 
 // Device-side status word bits (written by kernels, read back by the *log_likelihood calls).
@@ -179,7 +180,9 @@ struct epx_ctx {
     DevBuffers d{};
 
     // CUDA graphs (only with a non-default stream)
-    cudaGraphExec_t graph_mat = nullptr, graph_lik = nullptr;
+    cudaGraphExec_t graph_mat = nullptr, graph_lik = nullptr, graph_inc = nullptr;   // graph_inc: an incremental call at K = 4 (fixed launch shapes)
+    long long graph_inc_nodes = 0;
+    const int32_t* sub_count_dev = nullptr;   // when set (incremental graph): the chain kernel reads the number of listed slots from here
     long long graph_mat_nodes = 0, graph_lik_nodes = 0;
     bool graphs_valid = false;
 
@@ -187,6 +190,7 @@ struct epx_ctx {
     int stage_events = 0;
     cudaEvent_t ev[6] = {nullptr, nullptr, nullptr, nullptr, nullptr, nullptr};
     int stage_launches_mat[5] = {0, 0, 0, 0, 0}, stage_launches_lik[5] = {0, 0, 0, 0, 0};
+    int graph_lik_launches[5] = {0, 0, 0, 0, 0}, graph_inc_launches[5] = {0, 0, 0, 0, 0};   // per-stage counts of the captured sequences
     bool capturing = false;   // enqueue_kernels is running under stream capture
     // graph mode only: a1 (segmenter) and a2 (eigensystems) are independent and run as two branches of the graph
     cudaStream_t side = nullptr;
