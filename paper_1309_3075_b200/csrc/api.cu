@@ -103,10 +103,15 @@ size_t plan_workspace(const epx_ctx* c, char* base, DevBuffers* d)
         t.site_lnl = (double*)take(8 * L);
         t.block_sums = (double*)take(8 * ((L + 7) / 8));
     }
-    t.inc_slots = (int32_t*)take(4 * (S + 1));      // [S] = number of listed slots (read by the incremental graph's chain kernel)
+    // one block: the piece of an incremental walk (8 B), the number of listed slots (4 B, read by the incremental graph's chain
+    // kernel), 4 B of padding, the slot list -- so that a move uploads them with ONE copy
+    {
+        unsigned char* hdr = (unsigned char*)take(16 + 4 * S);
+        t.inc_piece = (DfsPiece*)hdr;
+        t.inc_slots = (int32_t*)(hdr ? hdr + 16 : nullptr);
+    }
     if (c->tree_mode) {
         t.inc_ops = (DfsOp*)take(sizeof(DfsOp) * (N - 1));
-        t.inc_piece = (DfsPiece*)take(sizeof(DfsPiece));
         t.inc_pops = (PruneOp*)take(sizeof(PruneOp) * (N - 1));
     }
     t.lnl = (double*)take(8);
