@@ -239,7 +239,9 @@ inline bool prune_walk4(const epx_ctx* c) { return prune_uses_lane(c) || prune_u
 int lane_patterns_per_lane(const epx_ctx* c);
 size_t lane_smem_bytes(const epx_ctx* c, int depth);
 int prune_lane_init_attributes();
-void launch_prune4_lane(const epx_ctx* c, const DfsOp* ops, const DfsPiece* pieces, int n_pieces, cudaStream_t s, bool hbm_operands);
+void launch_prune4_lane(const epx_ctx* c, const DfsOp* ops, const DfsPiece* pieces, int n_pieces, cudaStream_t s, bool hbm_operands,
+                        bool with_root = false);   // with_root: the LAST piece ends at the root; its warps also do a6
+bool prune_root_fused(const epx_ctx* c);   // a6 runs inside the K = 4 lane walk (no root kernel)
 // prune_mma.cu: level kernel on the FP64 tensor pipe for 8 < K <= 64
 inline int prune_kp(const epx_ctx* c) { return (c->K + 7) & ~7; }
 bool prune_uses_mma(const epx_ctx* c);

@@ -1431,7 +1431,8 @@ static int launch_pruning_dfs(const epx_ctx* c, cudaStream_t s)
     for (int pass = 0; pass < 2; pass++) {
         const int first = pass == 0 ? 0 : c->dfs_bottom, count = pass == 0 ? c->dfs_bottom : total - c->dfs_bottom;
         if (count <= 0) continue;
-        if (prune_uses_lane(c)) launch_prune4_lane(c, c->d.dfs_ops, c->d.dfs_pieces + first, count, s, pass == 1);
+        const bool last_launch = pass == 1 || total == c->dfs_bottom;                 // the root's piece is the last one of this launch
+        if (prune_uses_lane(c)) launch_prune4_lane(c, c->d.dfs_ops, c->d.dfs_pieces + first, count, s, pass == 1, last_launch && prune_root_fused(c));
         else launch_dfs_any(c, c->d.dfs_ops, c->d.dfs_pieces + first, count, s, pass == 1);
         launched++;
     }
@@ -1522,7 +1523,7 @@ int launch_pruning_incremental(const epx_ctx* c, const std::vector<int>& group_o
 {
     int launched = 0;
     if (prune_uses_lane(c)) {
-        launch_prune4_lane(c, c->d.inc_ops, c->d.inc_piece, 1, s, true);
+        launch_prune4_lane(c, c->d.inc_ops, c->d.inc_piece, 1, s, true, prune_root_fused(c));   // (a dirty path always ends at the root)
         launched = 1;
     } else if (prune_uses_dfs(c)) {
         launch_dfs_any(c, c->d.inc_ops, c->d.inc_piece, 1, s, true);
@@ -1537,8 +1538,12 @@ int launch_pruning_incremental(const epx_ctx* c, const std::vector<int>& group_o
     return cudaGetLastError() == cudaSuccess ? launched : -1;
 }
 
+// a6 inside the K = 4 lane walk (prune_lane.cu): no root kernel
+bool prune_root_fused(const epx_ctx* c) { return prune_uses_lane(c); }
+
 int launch_root_reduction(const epx_ctx* c, cudaStream_t s)
 {
+    if (prune_root_fused(c)) return 0;
     const DevBuffers& d = c->d;
     const int blocks = c->reduce_blocks;
     const int root_pidx = c->node_pidx[c->root];

@@ -32,10 +32,20 @@ size_t ln_smem(int C, int PPL, bool HB, int depth)
     return (size_t)LN_STAGES * ln_stage_bytes(C, PPL, HB) + (size_t)depth * PPL * (C * 1024 + 128);
 }
 
+// a6 inside the walk: the warps of the piece that ends at the root also reduce their patterns (PAPER.md L72:
+// l_p = sum_c w_c sum_i pi_i L_root(i), logL = sum_p wt_p ln l_p) -- the root's vectors are still in registers, and the
+// separate root kernel (9 us + a launch gap, a fifth of config 1's step) disappears.  site_lnl == nullptr: not fused.
+struct LaneRoot {
+    const double *freqs, *root_freqs, *weights, *pattern_wt, *tau, *height;
+    double *site_lnl, *block_sums, *lnl;
+    int32_t* status;         // [0] status word, [1] arrival counter
+    int root_node, M;
+};
+
 template <int C, int PPL, bool HB>
 __global__ void __launch_bounds__(32) prune4_lane_kernel(const DfsOp* __restrict__ ops, const DfsPiece* __restrict__ pieces,
     int tiles, int L, int Lp, int depth, const double* __restrict__ P, const uint8_t* __restrict__ tips,
-    double* __restrict__ partials, int32_t* __restrict__ scale_exp)
+    double* __restrict__ partials, int32_t* __restrict__ scale_exp, const LaneRoot root)
 {
     extern __shared__ __align__(16) unsigned char smraw[];
     constexpr int PW = 32 * PPL;                    // patterns per warp
@@ -53,6 +63,22 @@ __global__ void __launch_bounds__(32) prune4_lane_kernel(const DfsOp* __restrict
     const DfsPiece pc = pieces[piece];
     const int n_ops = pc.end - pc.begin;
     ops += pc.begin;
+    // a6 (fused): the root's frequency vector is located and the pattern weights are requested NOW, so that the walk hides the
+    // chain of dependent loads (boundary search) that would otherwise sit at the tail of the kernel
+    const bool do_root = root.site_lnl != nullptr && piece == (int)(gridDim.x / tiles) - 1;
+    const double* rf = nullptr;
+    if (do_root) {
+        rf = root.root_freqs;
+        if (!rf) {                                       // reading A9: the epoch that holds the root, #{k : tau_k < h_root}
+            const double h = root.height[root.root_node];
+            int lo = 0, hi = root.M - 1;
+            while (lo < hi) { const int mid = (lo + hi) >> 1; if (root.tau[mid] < h) lo = mid + 1; else hi = mid; }
+            rf = root.freqs + (size_t)lo * 4;
+        }
+        asm volatile("prefetch.global.L1 [%0];" ::"l"(rf));
+        asm volatile("prefetch.global.L1 [%0];" ::"l"(root.weights));
+        if (p0 + lane < L) asm volatile("prefetch.global.L1 [%0];" ::"l"(root.pattern_wt + p0 + lane));
+    }
 
     // 32-bit indexing in units of one state vector (32 B): (N-1 + tip blocks) C L < 2^32 is checked by prune_uses_dfs
     const unsigned uL = (unsigned)L, node_stride = uL * C;
@@ -260,6 +286,47 @@ __global__ void __launch_bounds__(32) prune4_lane_kernel(const DfsOp* __restrict
         }
         if (++buf == LN_STAGES) buf = 0;
     }
+    if (!do_root) return;
+    // ---- a6 for this warp's patterns: `cur` is the root's (rescaled) vector set, cur_ex its exponent.  The expressions per
+    // pattern are those of root_site_kernel (same site log-likelihoods bit for bit); the weighted sum is taken per warp, then
+    // over the warps in index order by whichever warp arrives last.
+    double contrib = 0.0;
+#pragma unroll
+    for (int u = 0; u < PPL; u++) {
+        if (!live[u]) continue;
+        double site = 0.0;
+#pragma unroll
+        for (int c = 0; c < C; c++) {
+            double sacc = 0.0;
+#pragma unroll
+            for (int i = 0; i < 4; i++) sacc = fma(rf[i], cur[u][c][i], sacc);
+            site = fma(root.weights[c], sacc, site);
+        }
+        if (!(site > 0.0) || !(site < 1.7e308)) atomicOr(root.status, EPX_ST_BAD_SITE);
+        const double ln = log(site) + (double)cur_ex[u] * 0.6931471805599453094;
+        root.site_lnl[pat[u]] = ln;
+        contrib += root.pattern_wt[pat[u]] * ln;
+    }
+    for (int o = 16; o > 0; o >>= 1) contrib += __shfl_xor_sync(FULL, contrib, o);
+    int last = 0;
+    if (lane == 0) {
+        root.block_sums[tile] = contrib;
+        __threadfence();
+        last = atomicAdd(root.status + 1, 1) == tiles - 1;
+    }
+    last = __shfl_sync(FULL, last, 0);
+    if (!last) return;
+    __threadfence();
+    double t = 0.0;
+    for (int i0 = 0; i0 < tiles; i0 += 128) {            // four loads in flight per lane; the order of the sum is fixed by the indices
+        double v[4];
+#pragma unroll
+        for (int q = 0; q < 4; q++) { const int i = i0 + 32 * q + lane; v[q] = i < tiles ? __ldcg(root.block_sums + i) : 0.0; }
+#pragma unroll
+        for (int q = 0; q < 4; q++) t += v[q];
+    }
+    for (int o = 16; o > 0; o >>= 1) t += __shfl_xor_sync(FULL, t, o);
+    if (lane == 0) { *root.lnl = t; root.status[1] = 0; }
 }
 
 template <int C, int PPL, bool HB>
@@ -272,20 +339,26 @@ template <int C>
 int ln_attr_c() { return ln_attr<C, 1, false>() | ln_attr<C, 2, false>() | ln_attr<C, 1, true>(); }
 
 template <int C, int PPL, bool HB>
-void ln_launch(const epx_ctx* c, const DfsOp* ops, const DfsPiece* pieces, int n_pieces, cudaStream_t s)
+void ln_launch(const epx_ctx* c, const DfsOp* ops, const DfsPiece* pieces, int n_pieces, cudaStream_t s, bool with_root)
 {
     const DevBuffers& d = c->d;
     const int tiles = (c->L + 32 * PPL - 1) / (32 * PPL);
+    LaneRoot root{};
+    if (with_root) {
+        root.freqs = d.freqs; root.root_freqs = c->has_root_freqs ? d.root_freqs : nullptr; root.weights = d.weights;
+        root.pattern_wt = d.pattern_wt; root.tau = d.tau; root.height = d.height; root.site_lnl = d.site_lnl;
+        root.block_sums = d.block_sums; root.lnl = d.lnl; root.status = d.status; root.root_node = c->root; root.M = c->M;
+    }
     prune4_lane_kernel<C, PPL, HB><<<n_pieces * tiles, 32, ln_smem(C, PPL, HB, c->dfs_depth), s>>>(ops, pieces, tiles, c->L, c->Lp,
-        c->dfs_depth, d.P, d.tips, d.partials, d.scale_exp);
+        c->dfs_depth, d.P, d.tips, d.partials, d.scale_exp, root);
 }
 
 template <int C>
-void ln_launch_c(const epx_ctx* c, const DfsOp* ops, const DfsPiece* pieces, int n_pieces, cudaStream_t s, bool hbm_operands)
+void ln_launch_c(const epx_ctx* c, const DfsOp* ops, const DfsPiece* pieces, int n_pieces, cudaStream_t s, bool hbm_operands, bool with_root)
 {
-    if (hbm_operands) { ln_launch<C, 1, true>(c, ops, pieces, n_pieces, s); return; }
-    if (lane_patterns_per_lane(c) == 2) ln_launch<C, 2, false>(c, ops, pieces, n_pieces, s);
-    else ln_launch<C, 1, false>(c, ops, pieces, n_pieces, s);
+    if (hbm_operands) { ln_launch<C, 1, true>(c, ops, pieces, n_pieces, s, with_root); return; }
+    if (lane_patterns_per_lane(c) == 2) ln_launch<C, 2, false>(c, ops, pieces, n_pieces, s, with_root);
+    else ln_launch<C, 1, false>(c, ops, pieces, n_pieces, s, with_root);
 }
 
 }  // namespace
@@ -309,16 +382,17 @@ int prune_lane_init_attributes()
 
 // `hbm_operands`: the piece reads most of its operands from partials written by an earlier launch (top piece, incremental
 // re-evaluation): one pattern per lane, operands streamed through the staging ring.
-void launch_prune4_lane(const epx_ctx* c, const DfsOp* ops, const DfsPiece* pieces, int n_pieces, cudaStream_t s, bool hbm_operands)
+void launch_prune4_lane(const epx_ctx* c, const DfsOp* ops, const DfsPiece* pieces, int n_pieces, cudaStream_t s, bool hbm_operands,
+                        bool with_root)
 {
     switch (c->C) {
-        case 1: ln_launch_c<1>(c, ops, pieces, n_pieces, s, hbm_operands); break;
-        case 2: ln_launch_c<2>(c, ops, pieces, n_pieces, s, hbm_operands); break;
-        case 3: ln_launch_c<3>(c, ops, pieces, n_pieces, s, hbm_operands); break;
-        case 4: ln_launch_c<4>(c, ops, pieces, n_pieces, s, hbm_operands); break;
-        case 5: ln_launch_c<5>(c, ops, pieces, n_pieces, s, hbm_operands); break;
-        case 6: ln_launch_c<6>(c, ops, pieces, n_pieces, s, hbm_operands); break;
-        case 7: ln_launch_c<7>(c, ops, pieces, n_pieces, s, hbm_operands); break;
-        default: ln_launch_c<8>(c, ops, pieces, n_pieces, s, hbm_operands); break;
+        case 1: ln_launch_c<1>(c, ops, pieces, n_pieces, s, hbm_operands, with_root); break;
+        case 2: ln_launch_c<2>(c, ops, pieces, n_pieces, s, hbm_operands, with_root); break;
+        case 3: ln_launch_c<3>(c, ops, pieces, n_pieces, s, hbm_operands, with_root); break;
+        case 4: ln_launch_c<4>(c, ops, pieces, n_pieces, s, hbm_operands, with_root); break;
+        case 5: ln_launch_c<5>(c, ops, pieces, n_pieces, s, hbm_operands, with_root); break;
+        case 6: ln_launch_c<6>(c, ops, pieces, n_pieces, s, hbm_operands, with_root); break;
+        case 7: ln_launch_c<7>(c, ops, pieces, n_pieces, s, hbm_operands, with_root); break;
+        default: ln_launch_c<8>(c, ops, pieces, n_pieces, s, hbm_operands, with_root); break;
     }
 }

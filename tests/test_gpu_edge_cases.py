@@ -233,7 +233,14 @@ def test_stage_events_and_launch_count(epx):
     ctx.log_likelihood()
     ms, launches = ctx.get_stage_ms()
     assert np.all(ms >= 0) and ms[3] > 0 and launches.sum() == ctx.launch_count() - n0
-    assert launches[0] == 1 and launches[4] == 1          # small problem: fused segmenter; root reduction with a last-block final sum
+    assert launches[0] == 1 and launches[4] == 0          # small problem: fused segmenter; K = 4: the root reduction runs inside the walk
+    ctx.set_option(epx.EPX_OPT_PRUNE_KERNEL, 2)           # level kernels: a root kernel of its own (last-block final sum)
+    lnl_walk = ctx.get_site_log_likelihoods().copy()
+    ctx.log_likelihood()
+    _, launches = ctx.get_stage_ms()
+    assert launches[4] == 1
+    assert np.allclose(ctx.get_site_log_likelihoods(), lnl_walk, rtol=1e-13, atol=0)   # the same quantities from either reduction
+    ctx.set_option(epx.EPX_OPT_PRUNE_KERNEL, 0)
     ctx.update_matrices()
     ms, launches = ctx.get_stage_ms()
     assert launches[3] == 0 and launches[4] == 0 and ms[3] == 0
@@ -330,7 +337,8 @@ def test_incremental_reevaluation(epx, orc_ld, cid, kw, opts):
         seg = 1 if prob.n_br <= 2048 else 3
         full_cost = seg + 6 if (prob.K == 4 and not opts) else seg + 2 + 2 + ctx.tree_levels() + 1     # (+1: fragment-order copies)
         if prob.K == 4 and (not opts or opts[0][0] == 6 or opts[0] == (3, 5)):
-            assert used == seg + 1 + 1 + 1          # segmenter, chain, ONE pruning walk over the dirty path, root
+            root = 1 if opts and opts[0] == (3, 5) else 0    # the lane walk does the root reduction itself
+            assert used == seg + 1 + 1 + root       # segmenter, chain, ONE pruning walk over the dirty path (, root kernel)
         else:
             assert used < full_cost                  # no eigensystems / tables, only the dirty levels
         fresh = epx.from_problem(prob)
