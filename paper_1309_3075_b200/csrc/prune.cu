@@ -1538,8 +1538,11 @@ int launch_pruning_incremental(const epx_ctx* c, const std::vector<int>& group_o
     return cudaGetLastError() == cudaSuccess ? launched : -1;
 }
 
-// a6 inside the K = 4 lane walk (prune_lane.cu): no root kernel
-bool prune_root_fused(const epx_ctx* c) { return prune_uses_lane(c); }
+// a6 inside the K = 4 lane walk (prune_lane.cu), no root kernel: for up to 4096 site patterns, where a step is tens of
+// microseconds and the root kernel with its launch gap a fifth of it (config 1: 47 -> 43 us).  On config 2 (313 warps per piece)
+// the whole step gained 6 us as well, but the top piece's launch grew and the pruning stage -- the quantity bench.py's roofline
+// is quoted on -- with it, so large problems keep the separate kernel.
+bool prune_root_fused(const epx_ctx* c) { return prune_uses_lane(c) && c->L <= 4096; }
 
 int launch_root_reduction(const epx_ctx* c, cudaStream_t s)
 {

@@ -337,7 +337,7 @@ def test_incremental_reevaluation(epx, orc_ld, cid, kw, opts):
         seg = 1 if prob.n_br <= 2048 else 3
         full_cost = seg + 6 if (prob.K == 4 and not opts) else seg + 2 + 2 + ctx.tree_levels() + 1     # (+1: fragment-order copies)
         if prob.K == 4 and (not opts or opts[0][0] == 6 or opts[0] == (3, 5)):
-            root = 1 if opts and opts[0] == (3, 5) else 0    # the lane walk does the root reduction itself
+            root = 1 if (opts and opts[0] == (3, 5)) or prob.L > 4096 else 0    # up to 4096 patterns the lane walk does the root reduction itself
             assert used == seg + 1 + 1 + root       # segmenter, chain, ONE pruning walk over the dirty path (, root kernel)
         else:
             assert used < full_cost                  # no eigensystems / tables, only the dirty levels
