@@ -226,22 +226,6 @@ __device__ __forceinline__ double2 jac_rotation(double spp, double sqq, double a
     return make_double2(c, t * c);
 }
 
-// The same rotation as a normalised direction: (c, s) = (|d| + r, sgn(d) h) / norm, r = sqrt(d^2 + h^2).  r only fixes the ANGLE
-// (seed + one Newton step, 2^-43), the normalisation is accurate, so c^2 + s^2 = 1 to rounding whatever the angle's error:
-// 17 dependent operations instead of 23.  For kernels that store the rotated pivot as computed.
-__device__ __forceinline__ double2 jac_rotation_n(double spp, double sqq, double apq)
-{
-    const double d = sqq - spp, h = 2.0 * apq;
-    const double r2 = fma(d, d, h * h);
-    if (!(r2 > 1e-280)) return make_double2(1.0, 0.0);
-    double y;
-    asm("rsqrt.approx.ftz.f64 %0, %1;" : "=d"(y) : "d"(r2));
-    y = fma(0.5 * y, fma(-r2 * y, y, 1.0), y);
-    const double cc = fabs(d) + r2 * y, ss = d < 0 ? -h : h;
-    const double wi = fast_rsqrt(fma(cc, cc, ss * ss));
-    return make_double2(cc * wi, ss * wi);
-}
-
 __global__ void __launch_bounds__(1024) jacobi1_kernel(int K, int Kp, const double* __restrict__ Qall,
                                                        const double* __restrict__ freqs, double* __restrict__ lam,
                                                        double* __restrict__ Uout, double* __restrict__ sp_out,
@@ -610,7 +594,7 @@ __global__ void __launch_bounds__(704) jacobi_sv_kernel(int K, int Kp, const dou
         };
         jc_cluster_barrier();                           // every CTA of the cluster is running, its barriers initialised
         if (is_rot) {
-            const double2 nr = jac_rotation_n(S0[sidx(j, j)], S0[sidx(m + j, m + j)], S0[sidx(j, m + j)]);
+            const double2 nr = jac_rotation(S0[sidx(j, j)], S0[sidx(m + j, m + j)], S0[sidx(j, m + j)]);
             R0[j] = nr;
             push0(nr);
         }
@@ -666,8 +650,8 @@ __global__ void __launch_bounds__(704) jacobi_sv_kernel(int K, int Kp, const dou
                 const double t10 = rbb.x * x10 - rbb.y * x11, t11 = rbb.y * x10 + rbb.x * x11;
                 const double y00 = ra.x * t00 - ra.y * t10, y01 = ra.x * t01 - ra.y * t11;
                 const double y10 = ra.y * t00 + ra.x * t10, y11 = ra.y * t01 + ra.x * t11;
-                // (the rotated pivot of a diagonal block is stored as computed, not forced to zero: (c, s) is a rotation to
-                // rounding whatever the accuracy of its angle, so the iteration stays an orthogonal similarity)
+                // (the rotated pivot of a diagonal block is stored as computed, not forced to zero: the iteration stays an
+                // orthogonal similarity to rounding)
                 jc_sts<SN>(q00, y00); jc_sts<SN>(q01, y01); jc_sts<SN>(q11, y11);
                 if (!f_diag) jc_sts<SN>(q10, y10);                    // (a diagonal block's w10 is its w01)
                 if (last) my_off = f_diag ? 2.0 * y01 * y01 : 2.0 * fma(y00, y00, fma(y01, y01, fma(y10, y10, y11 * y11)));
@@ -695,7 +679,7 @@ __global__ void __launch_bounds__(704) jacobi_sv_kernel(int K, int Kp, const dou
                     const double t0 = f_py ? rbb.y * x00 + rbb.x * x01 : rbb.x * x00 - rbb.y * x01;
                     const double t1 = f_py ? rbb.y * x10 + rbb.x * x11 : rbb.x * x10 - rbb.y * x11;
                     const double piv = f_px ? ra.y * t0 + ra.x * t1 : ra.x * t0 - ra.y * t1;
-                    nr = jac_rotation_n(dx, dy, piv);
+                    nr = jac_rotation(dx, dy, piv);
                 }
                 jc_sts2<RN>(Rj, nr);
                 push(t + 1, nr, seen);
@@ -833,8 +817,8 @@ __global__ void __launch_bounds__(32) jacobi4_kernel(const double* __restrict__ 
             const int ip = i ^ m, jp = j ^ m;
             const int pi_ = min(i, ip), qi = max(i, ip), pj = min(j, jp), qj = max(j, jp);
             // the two rotations this lane needs, from the S half (every lane computes them: no broadcast step)
-            const double2 ri = jac_rotation_n(__shfl_sync(FULL, x, 5 * pi_), __shfl_sync(FULL, x, 5 * qi), __shfl_sync(FULL, x, 4 * pi_ + qi));
-            const double2 rj = jac_rotation_n(__shfl_sync(FULL, x, 5 * pj), __shfl_sync(FULL, x, 5 * qj), __shfl_sync(FULL, x, 4 * pj + qj));
+            const double2 ri = jac_rotation(__shfl_sync(FULL, x, 5 * pi_), __shfl_sync(FULL, x, 5 * qi), __shfl_sync(FULL, x, 4 * pi_ + qi));
+            const double2 rj = jac_rotation(__shfl_sync(FULL, x, 5 * pj), __shfl_sync(FULL, x, 5 * qj), __shfl_sync(FULL, x, 4 * pj + qj));
             const double xj = __shfl_xor_sync(FULL, x, m);           // same row, partner column
             const double xi = __shfl_xor_sync(FULL, x, m << 2);      // partner row, same column
             const double xij = __shfl_xor_sync(FULL, x, m | (m << 2));
