@@ -37,7 +37,7 @@ import workloads as W  # noqa: E402  (input generators only; shared with the ora
 
 # dram__bytes_read.sum + dram__bytes_write.sum of the pruning launches of one config-2 step, from the committed
 # `ncu --set full` capture named here (re-captured whenever the pruning kernel changes; `--traffic` overrides it)
-NCU_TRAFFIC = {"bytes_per_step": 2.6018e9, "profile": "profiles/r2_prune4_lane_ncu.md", "commit": "00f37ea",
+NCU_TRAFFIC = {"bytes_per_step": 2.6034e9, "profile": "profiles/r2_prune4_lane_ncu.md", "commit": "0aeab7f",
                "kernel": "prune4_lane_kernel<4, 1, false> + <4, 1, true>"}
 
 METRIC = "pruning partials GB/s (fp64) over the whole a1..a6 log-likelihood step; epoch branch matrices/s in `matrices`"
