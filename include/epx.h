@@ -195,6 +195,45 @@ int epx_get_stage_ms(epx_ctx* ctx, float* ms, int* launches);
  * compiler from deleting the arithmetic).  Synchronises the stream. */
 int epx_measure_fp64_peak(int device, int kind, double ms_target, void* dev_scratch, void* cuda_stream, double* tflops);
 
+/* ---- a1 alone, for callers that may not allocate device memory (PAPER.md L78 change-point process, L117 the epochs a
+ * branch spans; readings A1-A3) ----
+ * Everything above borrows a workspace that somebody had to allocate.  Some callers cannot: a routine that runs inside
+ * another program's sampling loop under that program's fixed GPU memory budget, a callback on a path where cudaMalloc's
+ * device-wide synchronisation would stall other streams, a plug-in whose host hands it input and output buffers from its own
+ * arena and nothing more.  For them this one call splits a branch list into its per-epoch segments using only the buffers it
+ * is given: its intermediates (segment counts, parent-end epochs, a sort order; 12 bytes per branch) live in an array that
+ * is part of the library's device image -- 384 KiB on every GPU that loads the library, until the process exits.  The call
+ * makes no cudaMalloc / cudaFree and uses no allocating library routine.
+ *
+ *   device            CUDA device the pointers and the stream belong to; made current for the call, the previous one restored.
+ *   n_br              0 .. EPX_STATIC_MAX_BRANCHES branches.  More is refused with EPX_E_WORKSPACE and a message naming the
+ *                     limit (split the list, or use a bound context: epx_set_branches + epx_update_matrices).
+ *   M, dev_tau        M epochs (1 .. 4096) and their M-1 finite, strictly increasing boundary heights (DEVICE; may be NULL iff
+ *                     M == 1).  Not validated: the caller vouches for the order, as it does for the heights.
+ *   dev_child_height, dev_parent_height   [n_br] DEVICE, parent >= child (a branch of length 0 gets no segment).
+ *   dev_seg_off       [n_br + 1] DEVICE out: CSR offsets; dev_seg_off[n_br] = total number of segments.
+ *   dev_seg_epoch, dev_seg_dur, cap       DEVICE out with room for `cap` segments each: branch b's segments sit at
+ *                     [seg_off[b], seg_off[b+1]), parent end first (epoch numbers descending), unscaled durations -- the
+ *                     values epx_get_all_segments returns for the same branches, bit for bit.  Segments at positions >= cap are
+ *                     not stored (check dev_seg_off[n_br] <= cap; n_br * M always suffices).  May be NULL iff cap == 0.
+ *   cuda_stream       the three kernels are enqueued here; the call does not synchronise.  Inputs, outputs and the stream stay
+ *                     the caller's.
+ *   errbuf, errbuf_len   optional host buffer for a NUL-terminated message when the return code is not EPX_OK (there is no ctx
+ *                     to keep it); may be NULL / 0.
+ *
+ * First call on a device: looks up where that device keeps the built-in array (cudaGetSymbolAddress) and remembers it; this may
+ * make the CUDA runtime load the library's device code.  Make that first call during start-up, before the stream is put under
+ * stream capture.  Later calls on the same device only launch kernels.
+ * Sharing: every call on a device uses the same array, and the array keeps the previous call's contents.  Each call overwrites
+ * the part it reads before reading it, so calls that follow one another on the GPU (same stream, or ordered by events) are
+ * independent; two calls whose kernels can overlap on the GPU (different streams, different host threads) race on the array
+ * and may both return wrong segments.  Thread-safe on the host side otherwise.
+ * Returns EPX_OK, EPX_E_ARG (NULL pointer, range), EPX_E_WORKSPACE (n_br over the limit) or EPX_E_CUDA. */
+#define EPX_STATIC_MAX_BRANCHES 32768
+int epx_segment_branches_static(int device, int n_br, int M, const double* dev_tau, const double* dev_child_height,
+                                const double* dev_parent_height, int32_t* dev_seg_off, int32_t* dev_seg_epoch,
+                                double* dev_seg_dur, int cap, void* cuda_stream, char* errbuf, size_t errbuf_len);
+
 /* ---- tuning / test hooks (options 1-3, 6-8, 10 have no effect on results; 9 and 11 only within rounding) ---- */
 enum {
     EPX_OPT_CHAIN_KERNEL = 1, /* 0 auto (default); 1 force the generic shared-memory chain kernel; 2 (32 < K <= 64) round 1's

@@ -21,6 +21,7 @@ EPX_OPT_CHAIN_KERNEL, EPX_OPT_USE_GRAPH, EPX_OPT_PRUNE_KERNEL, EPX_OPT_EXP_METHO
 EPX_OPT_STAGE_EVENTS, EPX_OPT_DFS_PPL, EPX_OPT_DFS_PIECES, EPX_OPT_MMA_CHUNK, EPX_OPT_JACOBI_KERNEL = 5, 6, 7, 8, 9
 EPX_OPT_SHARE_PROCESSES, EPX_OPT_EPOCH_PRODUCTS = 10, 11
 STAGE_NAMES = ("segment", "eigen", "chain", "prune", "root")
+EPX_STATIC_MAX_BRANCHES = 32768   # epx.h: most branches one epx_segment_branches_static call takes
 
 _lib = None
 
@@ -85,6 +86,7 @@ def lib():
     _sig(L, "epx_set_option", i, vp, i, i)
     _sig(L, "epx_last_error", ct.c_char_p, vp)
     _sig(L, "epx_measure_fp64_peak", i, i, i, ct.c_double, vp, vp, ct.POINTER(ct.c_double))
+    _sig(L, "epx_segment_branches_static", i, i, i, i, dp, dp, dp, ip, ip, dp, i, vp, ct.c_char_p, ct.c_size_t)
     _lib = L
     return L
 
@@ -397,3 +399,37 @@ def measure_fp64_peak(kind: int, ms_target: float = 50.0, device: int = 0) -> fl
     if rc != EPX_OK:
         raise EpxError(rc, "epx_measure_fp64_peak")
     return v.value
+
+
+def segment_branches_static(tau, child_height, parent_height, seg_off, seg_epoch, seg_dur, stream=None) -> None:
+    """epx_segment_branches_static: split a branch list into per-epoch segments without allocating anything on the device.
+
+    For code that has device buffers for its inputs and results but may not ask CUDA for more memory (it runs under a host
+    program's fixed memory budget, or where an allocation's device-wide synchronisation is unwelcome).  Every argument is
+    a CUDA tensor the CALLER made, all on one device: ``tau`` float64 [M-1] (may be empty), ``child_height`` /
+    ``parent_height`` float64 [n_br], outputs ``seg_off`` int32 [n_br+1], ``seg_epoch`` int32 [cap], ``seg_dur`` float64
+    [cap].  This wrapper passes their addresses and sizes on and creates no tensor; the intermediates live in a fixed array
+    inside libepx.so, so n_br <= EPX_STATIC_MAX_BRANCHES (EpxError with code EPX_E_WORKSPACE otherwise).  Work is enqueued
+    on ``stream`` (default: the device's current torch stream) and not synchronised.  The first call on a device also looks
+    the array's address up: make it at start-up, outside stream capture.  Calls that can overlap on the GPU share that
+    array and race; calls that run one after the other are independent (see include/epx.h)."""
+    import torch
+    dev = child_height.device
+    for t, dt in ((tau, torch.float64), (child_height, torch.float64), (parent_height, torch.float64),
+                  (seg_off, torch.int32), (seg_epoch, torch.int32), (seg_dur, torch.float64)):
+        if not (t.is_cuda and t.device == dev and t.dtype == dt and t.is_contiguous() and t.dim() == 1):
+            raise ValueError("segment_branches_static takes contiguous 1-d CUDA tensors on one device (float64 / int32 as documented)")
+    n_br, M = child_height.numel(), tau.numel() + 1
+    if parent_height.numel() != n_br or seg_off.numel() != n_br + 1 or seg_epoch.numel() != seg_dur.numel():
+        raise ValueError("segment_branches_static: tensor sizes do not match")
+    cap = seg_epoch.numel()
+    if stream is None:
+        stream = torch.cuda.current_stream(dev)
+    msg = ct.create_string_buffer(256)
+    rc = lib().epx_segment_branches_static(
+        dev.index, n_br, M, ct.c_void_p(tau.data_ptr() if M > 1 else None),
+        ct.c_void_p(child_height.data_ptr() if n_br else None), ct.c_void_p(parent_height.data_ptr() if n_br else None),
+        ct.c_void_p(seg_off.data_ptr()), ct.c_void_p(seg_epoch.data_ptr() if cap else None),
+        ct.c_void_p(seg_dur.data_ptr() if cap else None), cap, ct.c_void_p(stream.cuda_stream), msg, len(msg))
+    if rc != EPX_OK:
+        raise EpxError(rc, msg.value.decode())

@@ -202,3 +202,123 @@ int launch_segmenter(const epx_ctx* c, cudaStream_t s)
                                            d.seg_off, c->has_brates ? d.brate : nullptr, d.seg_epoch, d.seg_dur);
     return cudaGetLastError() == cudaSuccess ? 3 : -1;
 }
+
+// ---------------------------------------------------------------------------------------------------------------------------
+// epx_segment_branches_static: a1 for callers that have no device memory to lend (include/epx.h has the contract).
+//
+// Every other path of the library carves its intermediates (n_seg, e_hi, order above) out of the workspace the caller binds.
+// Here the same three intermediates sit in ONE array that is part of the library's device image, so the call needs the
+// caller's inputs and outputs and nothing else: no cudaMalloc, no workspace, no context object.
+//
+// What is easy to get wrong, and is therefore kept in this one file:
+//   - In HOST code `g_static_seg_scratch` is only the handle the runtime registered for the symbol.  It is not a device
+//     address; a kernel handed `g_static_seg_scratch` from the host would fault (or, on a system where the GPU can reach host
+//     memory, quietly scribble somewhere else).  The device address is asked for with cudaGetSymbolAddress, once per device,
+//     while that device is current, and that pointer is what the kernels get.
+//   - Each device that loads the library has its own copy of the array at its own address, hence the per-device table.
+//   - The array outlives every call and keeps what the last call left in it.  Nothing below reads a word before the same call
+//     has written it (count writes n_seg / e_hi for [0, n_br), scan + sort writes order for [0, n_br), fill reads only those),
+//     so nothing has to be cleared -- a future user of this array that accumulates into it must clear its part first.
+// ---------------------------------------------------------------------------------------------------------------------------
+#include <mutex>
+#include <stdio.h>
+#include "../../include/epx.h"
+
+// n_seg | e_hi | order, EPX_STATIC_MAX_BRANCHES entries each: 3 * 32768 * 4 B = 384 KiB per device, held until the process exits.
+static __device__ __align__(256) int32_t g_static_seg_scratch[3 * EPX_STATIC_MAX_BRANCHES];
+
+namespace {
+
+constexpr int STATIC_MAX_DEVICES = 64;
+int32_t* g_static_scratch_addr[STATIC_MAX_DEVICES];   // device address of the array on device i; nullptr = not looked up yet
+std::mutex g_static_mu;
+
+// The fill step of a1 with the caller's capacity respected: segments whose position is >= cap are not stored (the caller
+// sees the shortfall in seg_off[n_br]).  Same expressions as seg_fill_kernel, so the stored values have the same bits.
+__global__ void seg_fill_capped_kernel(int n_br, const double* __restrict__ tau, const double* __restrict__ child_h,
+                                       const double* __restrict__ parent_h, const int32_t* __restrict__ n_seg,
+                                       const int32_t* __restrict__ e_hi_in, const int32_t* __restrict__ seg_off, int cap,
+                                       int32_t* __restrict__ seg_epoch, double* __restrict__ seg_dur)
+{
+    const int b = blockIdx.x * blockDim.x + threadIdx.x;
+    if (b >= n_br) return;
+    const int n = n_seg[b];
+    if (n == 0) return;
+    const double hc = child_h[b], hp = parent_h[b];
+    int e = e_hi_in[b];
+    const int off = seg_off[b];
+    double upper = hp;
+    for (int i = 0; i < n; i++, e--) {
+        const double lower = (i == n - 1) ? hc : tau[e - 1];
+        if (off + i < cap) {
+            seg_epoch[off + i] = e;
+            seg_dur[off + i] = upper - lower;
+        }
+        upper = lower;
+    }
+}
+
+int static_fail(char* errbuf, size_t errbuf_len, int code, const char* what, const char* detail = nullptr)
+{
+    if (errbuf && errbuf_len) snprintf(errbuf, errbuf_len, detail ? "epx_segment_branches_static: %s (%s)" : "epx_segment_branches_static: %s", what, detail);
+    return code;
+}
+
+}  // namespace
+
+extern "C" int epx_segment_branches_static(int device, int n_br, int M, const double* dev_tau, const double* dev_child_height,
+                                           const double* dev_parent_height, int32_t* dev_seg_off, int32_t* dev_seg_epoch,
+                                           double* dev_seg_dur, int cap, void* cuda_stream, char* errbuf, size_t errbuf_len)
+{
+    if (errbuf && errbuf_len) errbuf[0] = 0;
+    // argument checks first: none of them touches the CUDA runtime
+    if (n_br > EPX_STATIC_MAX_BRANCHES) {
+        char msg[160];
+        snprintf(msg, sizeof msg, "n_br = %d exceeds EPX_STATIC_MAX_BRANCHES = %d, the size of the built-in scratch array; "
+                 "split the branch list or use a bound context", n_br, EPX_STATIC_MAX_BRANCHES);
+        return static_fail(errbuf, errbuf_len, EPX_E_WORKSPACE, msg);
+    }
+    if (n_br < 0 || M < 1 || M > EPX_MAX_M || cap < 0 || device < 0 || device >= STATIC_MAX_DEVICES)
+        return static_fail(errbuf, errbuf_len, EPX_E_ARG, "n_br, M, cap or device out of range");
+    if (!dev_seg_off || (M > 1 && !dev_tau) || (n_br > 0 && (!dev_child_height || !dev_parent_height)) ||
+        (cap > 0 && (!dev_seg_epoch || !dev_seg_dur)))
+        return static_fail(errbuf, errbuf_len, EPX_E_ARG, "a required device pointer is NULL");
+
+    int prev = -1;
+    cudaError_t e = cudaGetDevice(&prev);
+    if (e == cudaSuccess && prev != device) e = cudaSetDevice(device);
+    if (e != cudaSuccess) return static_fail(errbuf, errbuf_len, EPX_E_CUDA, "cannot select the device", cudaGetErrorString(e));
+
+    // set-up, once per device, with that device current: where does this device keep the array?
+    int32_t* scratch = nullptr;
+    {
+        std::lock_guard<std::mutex> lock(g_static_mu);
+        if (!g_static_scratch_addr[device]) {
+            void* p = nullptr;
+            e = cudaGetSymbolAddress(&p, g_static_seg_scratch);
+            if (e == cudaSuccess && !p) e = cudaErrorInvalidSymbol;
+            if (e == cudaSuccess) g_static_scratch_addr[device] = static_cast<int32_t*>(p);
+        }
+        scratch = g_static_scratch_addr[device];
+    }
+    int rc = EPX_OK;
+    if (e != cudaSuccess) {
+        rc = static_fail(errbuf, errbuf_len, EPX_E_CUDA, "cudaGetSymbolAddress of the scratch array failed", cudaGetErrorString(e));
+    } else {
+        int32_t* n_seg = scratch;
+        int32_t* e_hi = scratch + EPX_STATIC_MAX_BRANCHES;
+        int32_t* order = scratch + 2 * EPX_STATIC_MAX_BRANCHES;
+        cudaStream_t s = static_cast<cudaStream_t>(cuda_stream);
+        const int blocks = (n_br + 255) / 256;
+        if (n_br > 0)
+            seg_count_kernel<<<blocks, 256, 0, s>>>(n_br, M, dev_tau, nullptr, nullptr, dev_child_height, dev_parent_height, n_seg, e_hi);
+        seg_scan_sort_kernel<<<1, 1024, 0, s>>>(n_br, n_seg, dev_seg_off, order);   // n_br == 0: writes seg_off[0] = 0 only
+        if (n_br > 0)
+            seg_fill_capped_kernel<<<blocks, 256, 0, s>>>(n_br, dev_tau, dev_child_height, dev_parent_height, n_seg, e_hi, dev_seg_off,
+                                                          cap, dev_seg_epoch, dev_seg_dur);
+        e = cudaGetLastError();
+        if (e != cudaSuccess) rc = static_fail(errbuf, errbuf_len, EPX_E_CUDA, "kernel launch failed", cudaGetErrorString(e));
+    }
+    if (prev >= 0 && prev != device) cudaSetDevice(prev);
+    return rc;
+}
