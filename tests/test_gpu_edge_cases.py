@@ -366,6 +366,51 @@ def test_incremental_reevaluation(epx, orc_ld, cid, kw, opts):
     ctx.close()
 
 
+@pytest.mark.parametrize("variant", ["taylor", "pade"])
+def test_incremental_k4_off_the_spectral_path(epx, orc_ld, variant):
+    """f1 at K = 4 when a3 is NOT done by eigensystems (EPX_OPT_EXP_METHOD = 2 on a reversible model; an asymmetric model on
+    the Pade path).  Those chain kernels read the segment lists and take their grid from the host-side slot count, so the
+    incremental call must neither replay a graph captured for another move's slot count nor run the segmenter beside them:
+    1-node, 4-node and root moves in one sequence (3 -> 12 -> 2 touched slots), each bit-identical to a fresh full evaluation."""
+    rng = np.random.default_rng(170)
+    prob = W.make_config(2, N=90, L=257)
+    opts = ()
+    if variant == "taylor":
+        opts = ((epx.EPX_OPT_EXP_METHOD, 2),)
+    else:
+        regimes = [models.asymmetric_trait(rng, 4, keep=0.9) for _ in range(2)]
+        Q = np.stack([regimes[e % 2] for e in range(prob.M)])
+        F = np.stack([models.stationary(regimes[e % 2]) for e in range(prob.M)])
+        prob = dataclasses.replace(prob, Q=Q, freqs=F, reversible=False, root_freqs=F[0].copy())
+    ctx = epx.from_problem(prob)
+    for o, v in opts:
+        ctx.set_option(o, v)
+    ctx.log_likelihood()
+    for it, k in enumerate((1, 4, 1, 4, 0, 1)):
+        if k == 0:
+            nodes, new_h = np.array([prob.n_nodes - 1], dtype=np.int32), np.array([prob.height.max() * 1.07])   # the root
+            h = prob.height.copy(); h[nodes[0]] = new_h[0]
+        else:
+            nodes, new_h, h = _move_nodes(rng, prob, k)
+        prob = dataclasses.replace(prob, height=h)
+        ctx.set_node_heights(nodes, new_h)
+        lnl = ctx.log_likelihood_incremental()
+        fresh = epx.from_problem(prob)
+        for o, v in opts:
+            fresh.set_option(o, v)
+        full = fresh.log_likelihood()
+        assert lnl == full, (variant, it, lnl, full)
+        assert np.array_equal(ctx.get_site_log_likelihoods(), fresh.get_site_log_likelihoods())
+        assert np.array_equal(ctx.get_all_matrices(), fresh.get_all_matrices())
+        for x, y in zip(ctx.get_all_segments(), fresh.get_all_segments()):
+            assert np.array_equal(x, y)
+        fresh.close()
+        ref = orc_ld.evaluate(prob)
+        assert abs(np.longdouble(lnl) - ref["lnl"]) <= LNL_RTOL * abs(ref["lnl"])
+        assert ctx.status() == 0
+    ctx.close()
+
+
 def test_tip_states_from_bytes_and_two_contexts_on_two_streams(epx, orc_ld):
     """epx_set_tip_states_u8 == epx_set_tip_states; two contexts on their own streams, interleaved call by call, do not
     disturb each other (independent instances are independent contexts)."""
