@@ -88,7 +88,9 @@ int epx_set_category_rates(epx_ctx* ctx, const double* rates, const double* weig
  * pruning plans and launch graphs depend on the topology alone) and, if it fails, leaves the current tree in place; a new
  * topology that fails validation leaves the context without a tree. */
 int epx_set_tree(epx_ctx* ctx, const int32_t* parent, const double* height);
-/* states: [N][L] row-major; 0..K-1 = observed state, anything else = missing (all-ones tip vector, A10). */
+/* states: [N][L] row-major; 0..K-1 = observed state, anything else = missing (all-ones tip vector, A10).  Large inputs
+ * (>= 4 M states) are repacked by a process-wide pool of host threads that serves ONE call at a time: tip-state setters of
+ * different contexts or threads queue behind each other for that part.  The pool survives fork() (the child starts its own). */
 int epx_set_tip_states(epx_ctx* ctx, const int32_t* states);
 /* The same from bytes ([N][L] row-major; 0..K-1 = observed state, anything else, e.g. 255, = missing): a quarter of the
  * host memory traffic of the int32 form -- sequence data are bytes to begin with. */

@@ -684,12 +684,32 @@ struct HostPool {
     }
 };
 HostPool* g_pool = nullptr;
+std::mutex g_pool_mu;             // guards g_pool
 std::once_flag g_pool_fork;
+// fork(): only the forking thread exists in the child, so a pool mutex that some other thread held at that moment would stay
+// locked there for ever (the child's first epx_set_tip_states would hang).  The prepare handler therefore takes all three locks
+// (in the order start() takes them: g_pool_mu, busy, mu -- an in-flight repacking job is waited for), both sides release them
+// again, and the child drops the pool (its worker threads do not exist there; a fresh one is made on first use).
+void pool_fork_prepare()
+{
+    g_pool_mu.lock();
+    if (g_pool) { g_pool->busy.lock(); g_pool->mu.lock(); }
+}
+void pool_fork_parent()
+{
+    if (g_pool) { g_pool->mu.unlock(); g_pool->busy.unlock(); }
+    g_pool_mu.unlock();
+}
+void pool_fork_child()
+{
+    if (g_pool) { g_pool->mu.unlock(); g_pool->busy.unlock(); }
+    g_pool = nullptr;             // (the old object is leaked on purpose: its condition variables belong to threads that are gone)
+    g_pool_mu.unlock();
+}
 HostPool& host_pool()
 {
-    std::call_once(g_pool_fork, [] { pthread_atfork(nullptr, nullptr, [] { g_pool = nullptr; }); });
-    static std::mutex m;
-    std::lock_guard<std::mutex> lk(m);
+    std::call_once(g_pool_fork, [] { pthread_atfork(pool_fork_prepare, pool_fork_parent, pool_fork_child); });
+    std::lock_guard<std::mutex> lk(g_pool_mu);
     if (!g_pool) g_pool = new HostPool();
     return *g_pool;
 }

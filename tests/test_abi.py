@@ -194,3 +194,51 @@ def test_shared_processes_are_detected(L):
     phi, S = c.epoch_processes()
     assert S == 9 and phi.tolist() == [0, 1, 2, 3, 4, 5, 6, 2, 7, 8]
     c.close()
+
+
+def test_tip_state_pool_survives_fork(L):
+    """The host thread pool behind epx_set_tip_states is process-wide.  A child forked while another thread is inside a
+    repacking job must still be able to set tip states (its own pool, no mutex left locked by a thread that does not exist
+    in the child); the parent's pool must keep working after the forks.  No GPU: an unbound ctx repacks into host memory."""
+    import signal
+    import threading
+    import time
+    import warnings
+    import paper_1309_3075_b200 as epx
+    N, Lp = 1100, 4000                       # 4.4 M states: above the 4 M threshold of the pooled path
+    rng = np.random.default_rng(5)
+    states = rng.integers(0, 4, size=(N, Lp), dtype=np.uint8)
+    a = epx.Epx(4, 1, 1, N, Lp)
+    a.set_tip_states_u8(states)              # creates the pool in the parent
+    stop = threading.Event()
+
+    def hammer():
+        while not stop.is_set():
+            a.set_tip_states_u8(states)
+
+    t = threading.Thread(target=hammer)
+    t.start()
+    try:
+        for k in range(6):
+            time.sleep(0.003 * k)
+            with warnings.catch_warnings():
+                warnings.simplefilter("ignore", DeprecationWarning)      # fork() in a multi-threaded process: the case under test
+                pid = os.fork()
+            if pid == 0:
+                code = 1
+                try:
+                    signal.alarm(20)         # a deadlocked child dies by SIGALRM instead of hanging the suite
+                    b = epx.Epx(4, 1, 1, N, Lp)
+                    b.set_tip_states_u8(states)
+                    b.set_tip_states(states.astype(np.int32))
+                    code = 0
+                finally:
+                    os._exit(code)
+            _, status = os.waitpid(pid, 0)
+            assert os.WIFEXITED(status) and os.WEXITSTATUS(status) == 0, f"forked child {k}: status {status:#x}"
+    finally:
+        stop.set()
+        t.join(30)
+    assert not t.is_alive()
+    a.set_tip_states_u8(states)              # the parent's pool still serves
+    a.close()
