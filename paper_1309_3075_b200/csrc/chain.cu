@@ -465,7 +465,7 @@ int launch_chain_reversible(const epx_ctx* c, cudaStream_t s)
     const int n = c->sub_list ? c->sub_count : c->n_slots;
     const int32_t* order = c->sub_list ? c->sub_list : d.order;
     if (n == 0) return 0;
-    if (K == 4) {
+    if (K == 4 && c->chain_kernel != 1) {      // (EPX_OPT_CHAIN_KERNEL = 1 forces the generic kernel at K = 4 too)
         long long threads = (long long)n * C * 4;
         int blocks = (int)((threads + 255) / 256);
         const size_t stage_bytes = sizeof(double) * ((size_t)c->M - 1 + (size_t)c->M * (4 * 4 + 3 * 4));
