@@ -3,7 +3,8 @@
 Only tests/, ``__graft_entry__.smoke()`` and bench.py's ``cpu_baseline`` / ``--impl reference`` legs may import
 this package.  It imports nothing from the CUDA product and nothing from ``workloads`` (problems are read by
 attribute).  Two builds of the one C source: ``"ld"`` (80-bit long double, the parity referee) and ``"d"``
-(double, the timed CPU baseline, "as it stands").
+(double, the timed CPU baseline, "as it stands"); a third, ``"q"`` (binary128), exists only to pin the referee's own
+rounding error (tests/test_oracle_pins.py).
 """
 from __future__ import annotations
 
@@ -16,7 +17,16 @@ import numpy as np
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
 _SRC = os.path.join(_HERE, "epoch_oracle.c")
-_LIBS = {"ld": os.path.join(_HERE, "liborc_ld.so"), "d": os.path.join(_HERE, "liborc_d.so")}
+_LIBS = {"ld": os.path.join(_HERE, "liborc_ld.so"), "d": os.path.join(_HERE, "liborc_d.so"), "q": os.path.join(_HERE, "liborc_q.so")}
+_FLAGS = {"ld": ["-DORC_LONG_DOUBLE"], "d": [], "q": ["-DORC_QUAD"]}
+_REAL_BYTES = {"ld": 16, "d": 8, "q": 16}
+# ORC_SANITIZE=1: separate builds with AddressSanitizer + UndefinedBehaviorSanitizer (the process must preload libasan;
+# tests/test_oracle_pins.py runs the pins' inputs through them in a subprocess).  Same source, same arithmetic.
+_SAN = os.environ.get("ORC_SANITIZE") == "1"
+if _SAN:
+    _LIBS = {k: v.replace(".so", "_san.so") for k, v in _LIBS.items()}
+    _FLAGS = {k: v + ["-fsanitize=address,undefined", "-fno-sanitize-recover=undefined", "-fno-omit-frame-pointer", "-g"]
+              for k, v in _FLAGS.items()}
 _lock = threading.Lock()
 _loaded: dict = {}
 
@@ -26,9 +36,9 @@ def build(force: bool = False) -> None:
     for prec, path in _LIBS.items():
         if not force and os.path.exists(path) and os.path.getmtime(path) >= os.path.getmtime(_SRC):
             continue
-        cmd = ["gcc", "-O2", "-fopenmp", "-fPIC", "-shared", "-o", path, _SRC, "-lm"]
-        if prec == "ld":
-            cmd.insert(1, "-DORC_LONG_DOUBLE")
+        cmd = ["gcc"] + _FLAGS[prec] + ["-O2", "-fopenmp", "-fPIC", "-shared", "-o", path, _SRC, "-lm"]
+        if prec == "q":
+            cmd.append("-lquadmath")
         subprocess.run(cmd, check=True)
 
 
@@ -38,7 +48,7 @@ def _lib(prec: str):
             build()
             lib = ct.CDLL(_LIBS[prec])
             lib.orc_real_bytes.restype = ct.c_int
-            want = 16 if prec == "ld" else 8
+            want = _REAL_BYTES[prec]
             if lib.orc_real_bytes() != want:
                 raise RuntimeError(f"oracle build {prec}: REAL is {lib.orc_real_bytes()} bytes, expected {want}")
             _loaded[prec] = lib
@@ -53,10 +63,21 @@ class Oracle:
     """One precision of the oracle. ``real`` is the numpy dtype its REAL arrays use."""
 
     def __init__(self, precision: str = "ld"):
-        assert precision in ("ld", "d")
+        assert precision in ("ld", "d", "q")
         self.precision = precision
         self.lib = _lib(precision)
-        self.real = np.longdouble if precision == "ld" else np.float64
+        # "q" (binary128): numpy has no such type, so REAL arrays are opaque 16-byte cells on the Python side and results are
+        # read back rounded to long double (_out); only evaluate() / branch_matrices / log_likelihood serve this build
+        self.real = {"ld": np.longdouble, "d": np.float64, "q": np.dtype("V16")}[precision]
+
+    def _out(self, a):
+        """A REAL array as numbers numpy can compute with (binary128 -> long double by orc_real_to_ld; others unchanged)."""
+        if self.precision != "q" or a is None:
+            return a
+        a = np.ascontiguousarray(a)
+        out = np.zeros(a.shape, dtype=np.longdouble)
+        self.lib.orc_real_to_ld(ct.c_size_t(a.size), _p(a), _p(out))
+        return out
 
     # ---- O2
     def segments(self, child_h, parent_h, tau):
@@ -93,7 +114,7 @@ class Oracle:
         return out
 
     # ---- O3 + O4
-    def branch_matrices(self, Q, rates, seg_off, seg_epoch, seg_dur):
+    def branch_matrices(self, Q, rates, seg_off, seg_epoch, seg_dur, raw: bool = False):
         Q = np.ascontiguousarray(Q, dtype=np.float64)
         rates = np.ascontiguousarray(rates, dtype=np.float64)
         seg_off = np.ascontiguousarray(seg_off, dtype=np.int32)
@@ -105,7 +126,7 @@ class Oracle:
         rc = self.lib.orc_branch_matrices(K, M, C, _p(Q), _p(rates), n_br, _p(seg_off), _p(seg_epoch), _p(seg_dur), _p(P))
         if rc != 0:
             raise RuntimeError(f"orc_branch_matrices rc={rc}")
-        return P
+        return P if raw else self._out(P)       # raw: REAL cells as the C side wrote them (input of log_likelihood)
 
     # ---- O5 + O6
     def log_likelihood(self, parent, P, tip_states, root_freqs, cat_weights, pattern_weights=None,
@@ -137,7 +158,7 @@ class Oracle:
                                             None if tp is None else _p(tp), None if has is None else _p(has))
         if rc != 0:
             raise RuntimeError(f"orc_log_likelihood rc={rc}")
-        return {"lnl": lnl[0], "site_lnl": site, "partials": partials}
+        return {"lnl": self._out(lnl)[0], "site_lnl": self._out(site), "partials": self._out(partials)}
 
     # ---- O1
     def validate_model(self, Q, freqs, reversible: bool) -> int:
@@ -165,8 +186,8 @@ class Oracle:
         if branches is not None:
             ch, ph = np.asarray(ch)[branches], np.asarray(ph)[branches]
         off, ep, du = self.segments(ch, ph, prob.tau)
-        P = self.branch_matrices(prob.Q, prob.rates, off, ep, du)
-        out = {"seg_off": off, "seg_epoch": ep, "seg_dur": du, "P": P}
+        P = self.branch_matrices(prob.Q, prob.rates, off, ep, du, raw=True)
+        out = {"seg_off": off, "seg_epoch": ep, "seg_dur": du, "P": self._out(P)}
         if prob.N > 0 and branches is None:
             if prob.root_freqs is not None:
                 rf = prob.root_freqs

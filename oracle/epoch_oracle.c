@@ -16,6 +16,7 @@
  * here converges to them to rounding.  Compiled twice from this one source:
  *   -DORC_LONG_DOUBLE : REAL = 80-bit long double (64-bit mantissa)  -> the parity referee
  *   (default)         : REAL = double                                -> the timed CPU baseline ("as it stands")
+ *   -DORC_QUAD        : REAL = __float128 (113-bit mantissa)         -> pins the referee's own rounding, nothing else
  * Pins (tests/test_oracle_pins.py): JC69 closed form, K-state equal-input multi-epoch closed form (fixes the
  * product ORDER), row sums, homogeneous collapse, redundant boundaries, scipy.linalg.expm, Taylor vs
  * uniformisation, detailed balance / stationarity, brute-force enumeration of ancestral states, two-tip
@@ -32,7 +33,18 @@
 #include <string.h>
 #include <float.h>
 
-#ifdef ORC_LONG_DOUBLE
+#if defined(ORC_QUAD)
+/* Third build, same source: REAL = IEEE binary128 (113-bit mantissa, libquadmath).  It exists for ONE pin (last
+ * row of the pin table; the series definition of exp at PAPER.md:L48): the long-double referee's own rounding error, measured
+ * against 49 more bits, must sit far inside the 1e-12 / 1e-9 parity gates.  Not used by any parity test or bench leg. */
+#include <quadmath.h>
+typedef __float128 REAL;
+#define R_EPS FLT128_EPSILON
+#define R_LOG logq
+#define R_EXP expq
+#define R_FABS fabsq
+#define R_LDEXP ldexpq
+#elif defined(ORC_LONG_DOUBLE)
 typedef long double REAL;
 #define R_EPS LDBL_EPSILON
 #define R_LOG logl
@@ -49,6 +61,9 @@ typedef double REAL;
 #endif
 
 int orc_real_bytes(void) { return (int)sizeof(REAL); }
+/* REAL -> long double, element by element (a rounding for the binary128 build, a copy or a widening otherwise): how the
+ * Python front-end reads results of a build whose REAL numpy cannot represent.  No arithmetic of the method. */
+void orc_real_to_ld(size_t n, const REAL *in, long double *out) { for (size_t i = 0; i < n; i++) out[i] = (long double)in[i]; }
 
 /* ---------------------------------------------------------------- O2: segmentation */
 /* Walk the boundaries linearly from the parent height down to the child height. Emits (epoch, duration) with

@@ -4,12 +4,15 @@ None of these re-types the oracle's own formula or re-calls its own routine: eve
 a closed form, a different algorithm (scipy's Pade, brute-force enumeration) or an invariant the paper fixes.
 """
 import itertools
+import os
 
 import numpy as np
 import pytest
 import scipy.linalg
 
 import workloads as W
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
 from workloads import models, trees
 
 LD = np.longdouble
@@ -394,6 +397,72 @@ def test_double_build_agrees_with_long_double(orc_ld, orc_d):
     assert np.max(np.abs(a["P"].astype(np.float64) - b["P"])) < 1e-14
     assert abs(float(a["lnl"]) - float(b["lnl"])) < 1e-11 * abs(float(a["lnl"]))
     assert np.array_equal(a["seg_epoch"], b["seg_epoch"]) and np.array_equal(a["seg_dur"], b["seg_dur"])
+
+
+def test_long_double_referee_against_binary128():
+    """The referee's own rounding (last row of the pin table; exp as its power series): the same
+    source built with REAL = __float128 (113-bit mantissa) on config 1, on a 61-state 3-taxon codon problem, on a reduced
+    config 2 (10 epochs) and on a reduced asymmetric config 4.  The 80-bit build must agree with it to 1e-17 on every P entry
+    and to 1e-16 relative on logL and on every site logL -- five and seven orders inside the 1e-12 / 1e-9 parity gates, so a
+    GPU result that passes or fails a gate does so on its own error, not on the referee's.  (Measured: 3e-18, < 2e-19, 3e-19.)"""
+    import oracle
+    q, ld = oracle.Oracle("q"), oracle.Oracle("ld")
+    for prob in (W.make_config(1), W.make_config(3, N=3, L=30), W.make_config(2, N=60, L=100), W.make_config(4, N=20, L=2)):
+        a, b = ld.evaluate(prob), q.evaluate(prob)
+        assert np.array_equal(a["seg_epoch"], b["seg_epoch"]) and np.array_equal(a["seg_dur"], b["seg_dur"])
+        assert b["P"].dtype == np.longdouble and np.all(np.isfinite(b["P"]))
+        assert float(np.max(np.abs(a["P"] - b["P"]))) <= 1e-17, prob.name
+        assert float(abs(a["lnl"] - b["lnl"])) <= 1e-16 * float(abs(b["lnl"])), prob.name
+        assert float(np.max(np.abs(a["site_lnl"] - b["site_lnl"]) / np.abs(b["site_lnl"]))) <= 1e-16, prob.name
+    # and the double build sits where its 53 bits put it: the quad build separates "ld is right" from "ld and d agree"
+    d = oracle.Oracle("d").evaluate(W.make_config(1))
+    b = q.evaluate(W.make_config(1))
+    assert 1e-18 < float(np.max(np.abs(d["P"] - b["P"]))) < 1e-14
+
+
+_SANITIZED_RUN = r"""
+import sys
+sys.path.insert(0, sys.argv[1])
+import numpy as np
+import oracle, workloads as W
+for prec in ("ld", "d"):
+    orc = oracle.Oracle(prec)
+    for prob in (W.make_config(1, L=64), W.make_config(3, N=4, L=6), W.make_config(4, N=20, L=2), W.make_config(5, n_br=24),
+                 W.make_config(6, N=8, L=20)):
+        out = orc.evaluate(prob, want_partials=prob.N > 0)
+        assert np.all(np.isfinite(out["P"].astype(np.float64)))
+    # segmentation edge cases: zero length, ends on boundaries, one epoch, capacity exactly met
+    tau = np.array([0.25, 0.5, 0.75])
+    orc.segments(np.array([0.0, 0.25, 0.3, 0.5, 0.1]), np.array([1.0, 0.75, 0.3, 0.5, 0.1000001]), tau)
+    orc.segments(np.array([0.0, 0.2]), np.array([1.0, 0.2]), np.array([]))
+    A = np.array([[-1.0, 1.0], [2.0, -2.0]])
+    orc.expm(A.astype(orc.real), "taylor"); orc.expm(A.astype(orc.real), "uniformisation")
+    pi = np.array([0.1, 0.2, 0.3, 0.4]); Q = W.models.hky(2.0, pi)
+    assert orc.validate_model(Q, pi, True) == 0
+print("SANITIZED-OK")
+"""
+
+
+def test_oracle_clean_under_address_and_undefined_behaviour_sanitizers(tmp_path):
+    """SURVEY.md section 5 (sanitizers): the oracle's C source built with -fsanitize=address,undefined runs the shapes the pins
+    and the parity tests use (every config family, tip partial output, segmentation edge cases) without a report."""
+    import shutil
+    import subprocess
+    import sys
+    if shutil.which("gcc") is None:
+        pytest.skip("no gcc")
+    asan = subprocess.run(["gcc", "-print-file-name=libasan.so"], capture_output=True, text=True).stdout.strip()
+    ubsan = subprocess.run(["gcc", "-print-file-name=libubsan.so"], capture_output=True, text=True).stdout.strip()
+    if not (os.path.isabs(asan) and os.path.exists(asan)):
+        pytest.skip("libasan not installed")
+    script = tmp_path / "san.py"
+    script.write_text(_SANITIZED_RUN)
+    env = dict(os.environ, ORC_SANITIZE="1", LD_PRELOAD=asan + (":" + ubsan if os.path.isabs(ubsan) and os.path.exists(ubsan) else ""),
+               ASAN_OPTIONS="detect_leaks=0:abort_on_error=0", UBSAN_OPTIONS="print_stacktrace=1", OMP_NUM_THREADS="4")
+    r = subprocess.run([sys.executable, str(script), ROOT], env=env, capture_output=True, text=True, timeout=600)
+    assert r.returncode == 0, r.stderr[-3000:]
+    assert "SANITIZED-OK" in r.stdout
+    assert "AddressSanitizer" not in r.stderr and "runtime error" not in r.stderr, r.stderr[-3000:]
 
 
 def test_validation_rules(orc_ld):
