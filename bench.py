@@ -431,7 +431,10 @@ def run_cuda(args) -> None:
                 "peak_source": peak_src, "launches_per_step": prune_launches,
                 "algorithmic_bytes_per_launch": comp["a5"] / prune_launches,
                 "avg_launch_ms": prune_ms / prune_launches, "share_of_step": prune_ms / float(stage_ms.sum()),
-                "stage_ms": {n: float(v) for n, v in zip(epx.STAGE_NAMES, stage_ms)}}
+                "stage_ms": {n: float(v) for n, v in zip(epx.STAGE_NAMES, stage_ms)},
+                "stage_ms_flat": "segment/eigen/chain/prune/root = " + "/".join("%.4f" % v for v in stage_ms),
+                # (K = 4, graph replay: a1 runs on a second branch beside a2..a5, so its stage reads ~0 ms: hidden, not measured)
+                "stage_note": "segment ~0: a1 overlaps a2-a5 on a second graph branch at K=4, its time is not measured"}
 
     cfg = workload_config(prob, 2, world)
     assert cfg["tree_levels"] == plan["levels"]
@@ -452,7 +455,7 @@ def run_cuda(args) -> None:
     if rank == 0 and ("matrices" in legs or "other" in legs):
         peaks = {"dfma": epx.measure_fp64_peak(0, 200.0, local), "dmma": epx.measure_fp64_peak(1, 200.0, local)}
     if rank == 0 and "matrices" in legs:
-        line["matrices"] = bench_matrices(torch, epx, local, K, peaks)
+        line["matrices"] = bench_matrices(torch, epx, local, K, peaks, sustain_s=args.sustain)
         # SURVEY.md 8(f) f1, reported separately (it changes the algorithmic flops; config 5's text asks for the full chain)
         line["matrices_cached"] = bench_matrices(torch, epx, local, K, peaks, options=[(epx.EPX_OPT_EPOCH_PRODUCTS, 1)],
                                                  label=", products of consecutive full epochs cached (SURVEY.md 8(f) f1)")
@@ -468,7 +471,89 @@ def run_cuda(args) -> None:
         dist.barrier()
         dist.destroy_process_group()
     if rank == 0:
-        print(json.dumps(line), flush=True)
+        print(json.dumps(finalise_line(line)), flush=True)
+
+
+def _r(x, digits: int = 4):
+    """Round to `digits` significant digits (the compact copies only; the full objects keep every digit)."""
+    if x is None:
+        return None
+    x = float(x)
+    return 0.0 if x == 0 else float(f"{x:.{digits}g}")
+
+
+def compact_numbers(line: dict) -> dict:
+    """The numbers of the optional legs that BASELINE.json's metric and north_star name -- config 5's matrices/s and its share of
+    the FP64 tensor peak, the rooflines of configs 3 and 6, the latencies of configs 1 and 4 -- as one flat dict of short keys
+    and scalars.  Missing legs leave their keys out."""
+    out = {}
+
+    def put(k, v, digits=4):
+        if v is not None:
+            if isinstance(v, (int, np.integer)) and not isinstance(v, bool):
+                out[k] = int(v)
+            else:
+                out[k] = _r(v, digits) if isinstance(v, (float, np.floating)) else v
+
+    for tag, key in (("cfg5", "matrices"), ("cfg5c", "matrices_cached")):     # cfg5c: products of consecutive full epochs cached (f1)
+        m = line.get(key)
+        if not m:
+            continue
+        rf = m["roofline"]
+        put(tag + "_ms", m["ms_per_step"]); put(tag + "_Mmat_per_s", m["value"] / 1e6)
+        put(tag + "_chain_ms", rf["stage_ms"]["chain"]); put(tag + "_eigen_ms", rf["stage_ms"]["eigen"])
+        put(tag + "_chain_tflops", rf["achieved"]); put(tag + "_dmma_peak", rf["peak"]); put(tag + "_chain_frac", rf["frac"])
+        put(tag + "_sm_mhz", m["clocks"].get("sm_mhz")); put(tag + "_reasons", ",".join(m["clocks"].get("reasons") or []) or "none")
+        su = m.get("sustained")
+        if su:
+            put(tag + "_sus_s", su["seconds"], 3); put(tag + "_sus_ms", su["ms_per_step"]); put(tag + "_sus_Mmat_per_s", su["matrices_per_s"] / 1e6)
+            put(tag + "_sus_tflops", su["whole_step_useful_tflops"]); put(tag + "_sus_dmma_peak", su["dmma_peak_sustained"])
+            put(tag + "_sus_frac", su["whole_step_frac_of_sustained_peak"]); put(tag + "_sus_sm_mhz", su["clocks"].get("sm_mhz"))
+            put(tag + "_sus_peak_sm_mhz", su["peak_probe_clocks"].get("sm_mhz"))
+            put(tag + "_sus_reasons", ",".join(su["clocks"].get("reasons") or []) or "none")
+    other = line.get("other_configs") or {}
+    for name, o in other.items():
+        if not isinstance(o, dict) or "config" not in o:
+            continue
+        tag = name.split("_")[0]                       # cfg1, cfg3, cfg4, cfg6
+        put(tag + "_ms", o["ms_per_step"]); put(tag + "_launches", o["gpu_launches_per_step"])
+        for leg in ("prune", "chain"):
+            rf = o.get("roofline_" + leg)
+            if rf:
+                put(f"{tag}_{leg}_ms", o["stage_ms"][leg]); put(f"{tag}_{leg}_tflops", rf["achieved"]); put(f"{tag}_{leg}_frac", rf["frac"])
+                put(f"{tag}_{leg}_launches", rf["launches"])
+        if "us_per_step" in o and "roofline_prune" not in o:
+            put(tag + "_dep_ops", o["plan"]["largest_piece_ops"] + o["plan"]["top_piece_ops"] if o["plan"]["depth_first"] else o["plan"]["levels"])
+        if "alternative" in o:
+            put(tag + "_taylor_ms", o["alternative"]["ms_per_step"])
+    inc = line.get("incremental")
+    if inc and "ms_per_move" in inc:
+        put("inc_ms_per_move", inc["ms_per_move"])
+    return out
+
+
+def finalise_line(line: dict) -> dict:
+    """What the driver keeps of the JSON line is `roofline` (scalars, strings cut at ~120 characters) and the last ~1 500
+    characters.  So the numbers of compact_numbers() go (a) as flat scalars into `roofline` and (b) into a `summary` object that is
+    the LAST key of the line and stays under 1 200 characters; the full objects stay where they were."""
+    nums = compact_numbers(line)
+    out = dict(line)
+    out["roofline"] = dict(line["roofline"], **nums)
+    head = {"cfg2_ms": _r(line["ms_per_step"]), "cfg2_GBps": _r(line["value"]), "cfg2_prune_frac": _r(line["roofline"]["frac"]),
+            "cfg2_prune_GBps": _r(line["roofline"]["achieved"]), "hbm_peak": _r(line["roofline"]["peak"])}
+    if line.get("e2e"):
+        head["cfg2_e2e_ms"] = _r(line["e2e"]["ms_per_step"])
+    summary = dict(head, **nums)
+    # shortest-first trimming if a future key pushes it over: drop the least important tails, never the cfg5 / cfg3 / cfg6 fractions
+    for k in ("cfg3_chain_launches", "cfg1_launches", "cfg4_launches", "cfg6_launches", "cfg3_launches", "cfg5c_dmma_peak", "cfg5c_eigen_ms",
+              "cfg4_taylor_ms", "cfg5c_chain_tflops", "cfg3_chain_tflops", "cfg3_prune_tflops", "cfg6_prune_tflops", "cfg5c_reasons",
+              "cfg5_sus_peak_sm_mhz", "cfg5_sus_tflops", "cfg5_reasons", "cfg5_sus_reasons"):
+        if len(json.dumps(summary)) <= 1200:
+            break
+        summary.pop(k, None)
+    out.pop("summary", None)
+    out["summary"] = summary
+    return out
 
 
 def prune_kernel_name(opts, L: int) -> str:
@@ -542,7 +627,7 @@ def bench_incremental(torch, epx, ctx, prob, stream, moves: int = 64) -> dict:
             "kernel_launches_per_move": launches, "moves": moves}
 
 
-def bench_matrices(torch, epx, device: int, K: int, peaks: dict, options=(), label: str = "") -> dict:
+def bench_matrices(torch, epx, device: int, K: int, peaks: dict, options=(), label: str = "", sustain_s: float = 0.0) -> dict:
     """Second half of the metric: config 5 (61-state matrix-convolution microbenchmark, a1..a4 only)."""
     prob = W.make_config(5)
     nseg = n_segments(prob)
@@ -571,6 +656,24 @@ def bench_matrices(torch, epx, device: int, K: int, peaks: dict, options=(), lab
         stage += m
     stage /= steps
     clk = clocks.stop()
+    sustained = None
+    if not cached and sustain_s > 0:
+        # the burst above is ~50 ms of work; a tensor-pipe load held for seconds drops this box's SM clock (MEASURED_PEAKS.json:
+        # 1 342 MHz median under a 4 s bf16 matmul), so the same step is also timed back to back for >= sustain_s seconds, with
+        # its own clock samples, against a DMMA peak probe that runs as long
+        n_s = max(steps, int(np.ceil(sustain_s * 1e3 / ms)))
+        cs = ClockSampler(device)
+        cs.start()
+        ms_s = bracket(torch, ctx.stream, ctx.update_matrices, n_s) / n_s
+        clk_s = cs.stop()
+        cs = ClockSampler(device)
+        cs.start()
+        dmma_s = epx.measure_fp64_peak(1, sustain_s * 1e3, device)
+        clk_p = cs.stop()
+        sustained = {"seconds": ms_s * n_s * 1e-3, "steps": n_s, "ms_per_step": ms_s, "matrices_per_s": prob.n_br * prob.C / (ms_s * 1e-3),
+                     "whole_step_useful_tflops": fl["executed"] / (ms_s * 1e-3) / 1e12, "dmma_peak_sustained": dmma_s,
+                     "whole_step_frac_of_sustained_peak": fl["executed"] / (ms_s * 1e-3) / 1e12 / dmma_s,
+                     "clocks": clk_s, "peak_probe_clocks": clk_p}
     ctx.close()
     dfma, dmma = peaks["dfma"], peaks["dmma"]
     chain_ms = float(stage[2])
@@ -580,7 +683,7 @@ def bench_matrices(torch, epx, device: int, K: int, peaks: dict, options=(), lab
               "tabulated product of those epochs: 3 products per branch at most)" if cached else
               "chain_dmma64_kernel<1, 4> (a3+a4 fused, mma.sync m8n8k4 f64, one product per segment)")
     return {"metric": "epoch branch matrices/s (fp64)" + label, "value": n_mat / (ms * 1e-3), "unit": "matrices/s",
-            "ms_per_step": ms, "steps": steps, "gpu_launches": int(launches), "clocks": clk,
+            "ms_per_step": ms, "steps": steps, "gpu_launches": int(launches), "clocks": clk, "sustained": sustained,
             "config": dict(workload_config(prob, 5, 1), segments=int(nseg.sum())),
             "whole_step_useful_tflops": fl["executed"] / (ms * 1e-3) / 1e12,
             "roofline": {"bound": "alu", "kernel": kernel,
@@ -728,6 +831,8 @@ def main() -> None:
     ap.add_argument("--no-matrices", action="store_true", help="skip the config-5 matrices/s leg")
     ap.add_argument("--no-cpu-baseline", action="store_true", help="skip timing the oracle on the host cores")
     ap.add_argument("--opt", type=parse_opts, default=[], help="EPX_OPT overrides for the config-2 context, e.g. 3=2,6=1")
+    ap.add_argument("--sustain", type=float, default=2.0,
+                    help="seconds of back-to-back config-5 steps (and of the DMMA peak probe) for the sustained matrices/s figure; 0 = skip")
     ap.add_argument("--traffic", type=float, default=None,
                     help="dram bytes per launch of the dominant kernel from the committed ncu capture (profiles/)")
     args = ap.parse_args()

@@ -188,6 +188,9 @@ enum {
  * after each stage (inside the CUDA graph when one is used).  This call synchronises the stream and writes the device
  * time of each stage of the LAST compute call to ms[EPX_N_STAGES] and the number of kernels each stage launched to
  * launches[EPX_N_STAGES] (either may be NULL).  Stages the call did not run report 0 ms / 0 launches.
+ * K == 4 on the eigensystem path with a non-default stream: the segmenter runs on a second stream beside a2..a5 (the chain
+ * kernel segments its own branches), so EPX_STAGE_SEGMENT reports ~0 ms with its launches counted -- its time is hidden, not
+ * measured, and these stage times are not comparable with a run where a1 sits in front (EPX_OPT_USE_GRAPH = 0).
  * EPX_E_STATE if the option is off or nothing has run. */
 int epx_get_stage_ms(epx_ctx* ctx, float* ms, int* launches);
 

@@ -139,3 +139,90 @@ def test_reference_arm_prints_the_contract_line():
     assert d["cpu_baseline"]["kind"] == "oracle" and d["cpu_baseline"]["value"] == d["value"] and d["cpu_baseline"]["cores"] >= 1
     assert d["e2e"] == {"value": d["value"], "unit": d["unit"], "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0}
     assert d["value"] > 0
+
+
+def _stub_line():
+    """A JSON line of the shape run_cuda() assembles, with made-up numbers and strings as long as the real ones."""
+    import bench
+    long = "x" * 150
+    clk = {"sm_mhz": 1965.0, "sm_max_mhz": 1965, "reasons": [], "samples": 6, "power_w_max": 480.0}
+    stage = {n: 0.1 * (i + 1) for i, n in enumerate(("segment", "eigen", "chain", "prune", "root"))}
+
+    def matrices(ms, cached):
+        return {"metric": long, "value": 8e4 / (ms * 1e-3), "unit": "matrices/s", "ms_per_step": ms, "steps": 10, "gpu_launches": 50,
+                "clocks": clk, "config": {"workload": long}, "whole_step_useful_tflops": 25.0,
+                "sustained": None if cached else {"seconds": 2.01, "steps": 400, "ms_per_step": ms * 1.2, "matrices_per_s": 8e4 / (ms * 1.2e-3),
+                                                  "whole_step_useful_tflops": 21.0, "dmma_peak_sustained": 30.0,
+                                                  "whole_step_frac_of_sustained_peak": 0.7, "clocks": dict(clk, reasons=["sw_power_cap"]),
+                                                  "peak_probe_clocks": clk},
+                "roofline": {"bound": "alu", "kernel": long, "achieved": 26.9, "peak": 37.05, "unit": "TFLOP/s", "frac": 0.726,
+                             "traffic": None, "peak_source": long, "stage_ms": dict(stage, chain=ms * 0.94, eigen=0.246)}}
+
+    def other(cid, K, rf):
+        o = {"config": {"workload": long}, "ms_per_step": 0.4, "steps": 20, "gpu_launches_per_step": 20, "log_likelihood": -1.0,
+             "stage_ms": stage, "stage_launches": {n: 1 for n in stage},
+             "plan": {"levels": 17, "operations": 199, "depth_first": 0, "bottom_pieces": 0, "largest_piece_ops": 0, "top_piece_ops": 0,
+                      "stack_slots": 0, "prune_launches": 18}}
+        for leg in rf:
+            o["roofline_" + leg] = {"bound": "alu", "kernel": long, "achieved": 12.6, "peak": 37.05, "unit": "TFLOP/s", "frac": 0.34,
+                                    "traffic": None, "flops": 2.5e9, "flops_definition": long, "peak_source": long, "launches": 18,
+                                    "avg_launch_ms": 0.011}
+        if not rf:
+            o["bound"] = long; o["us_per_step"] = 400.0
+        if cid == 4:
+            o["alternative"] = {"exp_method": long, "ms_per_step": 0.3, "chain_ms": 0.1, "log_likelihood": -1.0}
+        return o
+
+    line = {"metric": bench.METRIC, "value": 5139.0, "unit": "GB/s", "n_gpus": 1, "steps": 20, "warmup": 5, "ms_per_step": 0.5178,
+            "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "config": {"workload": long}, "value_definition": long, "workspace_bytes": 1, "plan": {},
+            "roofline": {"bound": "hbm", "kernel": long, "achieved": 5559.0, "peak": 6517.6, "unit": "GB/s", "frac": 0.853, "traffic": 1.3e9,
+                         "stage_ms": stage},
+            "gpu_launches": 100, "clocks": clk, "log_likelihood": -1.0,
+            "e2e": {"value": 2000.0, "unit": "GB/s", "h2d_bytes_per_step": 1, "d2h_bytes_per_step": 12, "ms_per_step": 1.18, "what": long},
+            "incremental": {"ms_per_move": 0.105, "what": long},
+            "matrices": matrices(5.02, False), "matrices_cached": matrices(3.53, True),
+            "other_configs": {W.CONFIG_NAMES[1]: other(1, 4, ()), W.CONFIG_NAMES[3]: other(3, 61, ("prune", "chain")),
+                              W.CONFIG_NAMES[4]: other(4, 24, ()), W.CONFIG_NAMES[6]: other(6, 20, ("prune",)), "clocks": clk},
+            "batch": {long: {"instances": 8, "speedup": 1.3}},
+            "cpu_baseline": {"value": 5.1, "unit": "GB/s", "cores": 16, "kind": "oracle", "sample": long * 2}}
+    return line
+
+
+def test_second_half_of_the_metric_stays_in_what_the_driver_keeps():
+    """The driver's record keeps `roofline` (scalars) and the last ~1 500 characters of the line.  Config 5's matrices/s and
+    tensor-peak fraction (the second half of BASELINE.json's metric), its sustained figure, and the rooflines of configs 3
+    and 6 must therefore sit inside `roofline` as flat scalars AND inside a trailing `summary` of at most 1 200 characters."""
+    import bench
+    out = bench.finalise_line(_stub_line())
+    text = json.dumps(out)
+    assert list(out.keys())[-1] == "summary" and len(json.dumps(out["summary"])) <= 1200
+    tail = text[-1500:]
+    need = ("cfg5_ms", "cfg5_Mmat_per_s", "cfg5_chain_ms", "cfg5_chain_tflops", "cfg5_dmma_peak", "cfg5_chain_frac", "cfg5_eigen_ms",
+            "cfg5_sm_mhz", "cfg5_sus_ms", "cfg5_sus_Mmat_per_s", "cfg5_sus_frac", "cfg5_sus_sm_mhz", "cfg5c_ms", "cfg5c_Mmat_per_s",
+            "cfg5c_chain_frac", "cfg3_prune_ms", "cfg3_prune_frac", "cfg3_chain_ms", "cfg3_chain_frac", "cfg6_prune_ms",
+            "cfg6_prune_frac", "cfg6_prune_launches", "cfg1_ms", "cfg4_ms", "cfg4_dep_ops", "inc_ms_per_move", "cfg5_sus_reasons")
+    for k in need:
+        assert k in out["roofline"], k
+        assert not isinstance(out["roofline"][k], (dict, list)), k
+        assert '"%s":' % k in tail, k
+    assert out["roofline"]["cfg5_Mmat_per_s"] == pytest.approx(8e4 / 5.02e-3 / 1e6, rel=1e-3)
+    assert out["summary"]["cfg2_prune_frac"] == pytest.approx(0.853)
+    # the full objects are still there, untouched
+    assert out["matrices"] == _stub_line()["matrices"] and out["roofline"]["frac"] == 0.853
+    # a line without the optional legs still finalises
+    bare = {k: v for k, v in _stub_line().items() if k not in ("matrices", "matrices_cached", "other_configs", "incremental", "e2e")}
+    assert "cfg5_ms" not in bench.finalise_line(bare)["summary"]
+
+
+def test_ncu_traffic_constant_is_the_number_in_the_profile_it_names():
+    """bench.py's NCU_TRAFFIC (bytes per step of the pruning launches) is a constant taken from a committed ncu capture: it must
+    be the figure that profile states, so that a re-capture that forgets one of the two cannot go unnoticed."""
+    import re
+    import bench
+    text = open(os.path.join(ROOT, bench.NCU_TRAFFIC["profile"])).read()
+    m = re.findall(r"DRAM bytes per step = \*\*([0-9 \u00a0\u202f.]+) MB\*\*", text)
+    assert m, "the profile no longer states 'DRAM bytes per step = **... MB**'"
+    mb = float(re.sub(r"[^0-9.]", "", m[-1]))
+    assert abs(mb * 1e6 - bench.NCU_TRAFFIC["bytes_per_step"]) <= 1e-4 * bench.NCU_TRAFFIC["bytes_per_step"]
+    assert bench.NCU_TRAFFIC["kernel"].split("<")[0] in text
