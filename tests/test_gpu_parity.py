@@ -43,7 +43,7 @@ def check_matrices(ctx, ref, slots=None):
     return float(err)
 
 
-def check_likelihood(ctx, prob, ref, lnl, partial_nodes=()):
+def check_likelihood(ctx, prob, ref, lnl, partial_nodes=(), partial_rtol=PARTIAL_RTOL):
     ref_lnl = ref["lnl"]
     assert abs(np.longdouble(lnl) - ref_lnl) <= LNL_RTOL * abs(ref_lnl), (lnl, float(ref_lnl))
     site = ctx.get_site_log_likelihoods()
@@ -54,10 +54,10 @@ def check_likelihood(ctx, prob, ref, lnl, partial_nodes=()):
         got = np.ldexp(out.astype(np.longdouble), ex[None, :, None])
         want = ref["partials"][node]
         scale = np.max(want, axis=(0, 2), keepdims=True)
-        assert np.max(np.abs(got - want) / scale) <= PARTIAL_RTOL, f"partials of node {node}"
+        assert np.max(np.abs(got - want) / scale) <= partial_rtol, f"partials of node {node}"
 
 
-def run_tree(epx, orc, prob, partial_nodes="all", options=(), likelihood=True):
+def run_tree(epx, orc, prob, partial_nodes="all", options=(), likelihood=True, partial_rtol=PARTIAL_RTOL):
     ctx = epx.from_problem(prob)
     for o, v in options:
         ctx.set_option(o, v)
@@ -69,7 +69,7 @@ def run_tree(epx, orc, prob, partial_nodes="all", options=(), likelihood=True):
     if partial_nodes == "all":
         partial_nodes = range(prob.n_nodes)
     if likelihood:
-        check_likelihood(ctx, prob, ref, lnl, partial_nodes or ())
+        check_likelihood(ctx, prob, ref, lnl, partial_nodes or (), partial_rtol)
     assert ctx.status() == 0
     assert ctx.launch_count() > 0
     # update_matrices alone reproduces the same matrices
@@ -283,12 +283,16 @@ def test_config6_amino_acid_reduced(epx, orc_ld):
 def test_config6_amino_acid_full_size(epx, orc_ld):
     prob = W.make_config(6)
     # default (spectral: Jacobi + eigenbasis chain) against north_star's two gates: 1e-12 absolute on P, 1e-9 relative on logL /
-    # site logL.  Node-by-node partials at PARTIAL_RTOL are compared on the componentwise exponential: a P entry of 1e-3 that
-    # is within 1e-13 ABSOLUTE is only good to 1e-10 RELATIVE, and a cherry's partial is a product of two such entries
-    # (measured 1.2e-10 here) -- the spectral path's contract is the absolute one (A21).
-    run_tree(epx, orc_ld, prob, partial_nodes=())
-    run_tree(epx, orc_ld, prob, options=[(epx.EPX_OPT_EXP_METHOD, 2)],
-             partial_nodes=[prob.N, prob.N + 57, prob.n_nodes - 2, prob.n_nodes - 1])
+    # site logL -- and node-by-node partials at the bound an ABSOLUTE contract on P implies (A21).  The spectral
+    # matrices are within 3e-15 absolute here, but between amino acids that are rarely exchanged the entries of a short
+    # branch's P are 1e-6 and smaller, so such an entry is only good to ~3e-9 RELATIVE, and where it is the term that decides a
+    # tip likelihood the partial inherits that: measured over all 199 internal nodes 5e-10 .. 6.2e-9 relative to the vector's
+    # maximum, not growing with the level.  Asserted: 2e-8 (3x the measured worst).  The logL gate is far looser: 1e-9 on
+    # ln l ~ -1000 per site allows 1e-6 on the site likelihood itself.  The componentwise exponential meets the suite's
+    # PARTIAL_RTOL = 1e-10 on the same nodes (measured 1e-14).
+    nodes = [prob.N, prob.N + 57, prob.n_nodes - 2, prob.n_nodes - 1]
+    run_tree(epx, orc_ld, prob, partial_nodes=nodes, partial_rtol=2e-8)
+    run_tree(epx, orc_ld, prob, options=[(epx.EPX_OPT_EXP_METHOD, 2)], partial_nodes=nodes)
 
 
 def test_config5_reduced_every_branch(epx, orc_ld):
@@ -309,27 +313,39 @@ def test_config5_reduced_every_branch(epx, orc_ld):
         ctx.close()
 
 
-@pytest.mark.parametrize("cache", [0, 1])
-def test_config5_full_size_sampled(epx, orc_ld, cache):
-    # full launch configuration (20 000 branches); segments checked for every branch, matrices for a seeded sample
-    # that always includes the longest chains, plus row sums / non-negativity for every matrix.  cache = 1: SURVEY.md 8(f) f1,
-    # chains over >= 2 full epochs multiply by the tabulated product of those epochs
+def test_config5_full_size_every_branch(epx, orc_ld):
+    """Config 5 in the launch configuration bench.py times (20 000 branches x 4 categories of 61-state matrices, Eq. 7):
+    segments of every branch, and EVERY matrix entry against the long-double oracle at 1e-12 -- for the default chain
+    (one product per segment) and for the cached products of consecutive full epochs from the same
+    oracle pass.  The oracle works through the branches in chunks of 2 000 (OpenMP over branches; a few minutes on the
+    box's host cores), so a wrong W_e, a wrong cached-product index or a stale D on a rare (e_hi, e_lo) shape cannot hide
+    behind a sample."""
     prob = W.make_config(5)
-    ctx = epx.from_problem(prob)
-    ctx.set_option(epx.EPX_OPT_EPOCH_PRODUCTS, cache)
-    ctx.update_matrices()
     off_ref, ep_ref, du_ref = orc_ld.segments(prob.child_height, prob.parent_height, prob.tau)
-    off = check_segments(ctx, {"seg_off": off_ref, "seg_epoch": ep_ref, "seg_dur": du_ref})
-    nseg = np.diff(off)
-    rng = np.random.default_rng(5)
-    # every 20th branch, the 8 longest and the 4 shortest chains, 48 random ones: > 1 000 of the 20 000 (Eq. 7 element-wise)
-    sample = np.unique(np.concatenate([np.arange(0, prob.n_br, 20), np.argsort(nseg)[-8:], np.argsort(nseg)[:4],
-                                       rng.choice(prob.n_br, 48, replace=False)]))
-    assert sample.size >= 1000
-    ref = orc_ld.evaluate(prob, branches=sample)
-    P = ctx.get_all_matrices()
-    err = np.max(np.abs(P[sample].astype(np.longdouble) - ref["P"]))
-    assert err <= P_TOL, float(err)
-    assert np.all(P >= 0) and np.max(np.abs(P.sum(-1) - 1.0)) < 1e-11
-    assert ctx.status() == 0
-    ctx.close()
+    Ps = []
+    for cache in (0, 1):
+        ctx = epx.from_problem(prob)
+        ctx.set_option(epx.EPX_OPT_EPOCH_PRODUCTS, cache)
+        ctx.update_matrices()
+        check_segments(ctx, {"seg_off": off_ref, "seg_epoch": ep_ref, "seg_dur": du_ref})
+        P = ctx.get_all_matrices()
+        assert ctx.status() == 0
+        ctx.close()
+        assert np.all(P >= 0) and np.max(np.abs(P.sum(-1) - 1.0)) < 1e-11
+        Ps.append(P)
+    shapes = set()
+    worst = [0.0, 0.0]
+    for lo in range(0, prob.n_br, 2000):
+        chunk = np.arange(lo, min(lo + 2000, prob.n_br))
+        ref = orc_ld.evaluate(prob, branches=chunk)["P"]
+        for k in (0, 1):
+            err = float(np.max(np.abs(Ps[k][chunk].astype(np.longdouble) - ref)))
+            worst[k] = max(worst[k], err)
+            assert err <= P_TOL, (k, lo, err)
+        for b in chunk:
+            if off_ref[b + 1] > off_ref[b]:
+                shapes.add((int(ep_ref[off_ref[b]]), int(ep_ref[off_ref[b + 1] - 1])))
+    # the workload reaches most (e_hi, e_lo) shapes of a 16-epoch model, the long ones included
+    assert len(shapes) >= 100 and max(hi - lo for hi, lo in shapes) >= prob.M - 3
+    print(f"config 5, every branch: max |P - P_oracle| = {worst[0]:.2e} (default), {worst[1]:.2e} (cached epoch products); "
+          f"{len(shapes)} distinct (e_hi, e_lo) shapes")
